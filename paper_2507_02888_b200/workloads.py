@@ -1,0 +1,124 @@
+"""Seeded synthetic inputs for the five BASELINE.json configurations.
+
+This module holds NO Ewald arithmetic: only cell sizes, cut-off parameters and random draws.  The same
+arrays are handed to the CPU oracle and to the CUDA path (neither imports the other).  The inputs stand in
+for the paper's CASINO VMC workloads (3D HEG N = 100-1630; 2D HEG; bulk
+solids), whose input decks are not available: uniform-random positions replace
+Metropolis-sampled ones (same shapes, sizes and costs).
+
+Every array is float64; the FP32 path receives these arrays rounded to float32 by the caller.
+Positions are arrays of points [n_walkers, n, dim]; the library's SoA layout is produced by the binding.
+"""
+import math
+from dataclasses import dataclass, field
+
+import numpy as np
+
+SEED0 = 250702888  # arxiv id; seed of config c is SEED0 + c
+
+
+@dataclass
+class Workload:
+    name: str
+    index: int            # 1..5, position in BASELINE.json "configs" (1-based)
+    dim: int
+    n: int                # mobile particles per walker
+    n_walkers: int
+    L: float              # cell side (bohr); all five cells are cubic / square
+    kappa: float          # splitting parameter, inverse bohr (paper's gamma = kappa^2)
+    n2_max: int           # keep integer G with n1^2+n2^2+n3^2 <= n2_max
+    r_cutoff: float       # real-space spherical cut-off (bohr)
+    precisions: tuple
+    n_steps: int = 0      # config 5: sequential single-electron moves per walker
+    step_sigma: float = 0.0
+    cell: np.ndarray = field(default=None, repr=False)
+    charges: np.ndarray = field(default=None, repr=False)
+    ion_pos: np.ndarray = field(default=None, repr=False)
+    ion_q: np.ndarray = field(default=None, repr=False)
+
+    @property
+    def g_cutoff(self):
+        # shell membership is decided by the integer n^2 <= n2_max; the next shell is >= 0.5 % away
+        return 2.0 * math.pi / self.L * math.sqrt(self.n2_max) * (1.0 + 1e-9)
+
+    @property
+    def n_max(self):
+        return int(math.isqrt(self.n2_max))
+
+    @property
+    def seed(self):
+        return SEED0 + self.index
+
+    def positions(self, n_walkers=None):
+        """[n_walkers, n, dim] float64; the first k walkers of a larger draw equal a draw of k walkers."""
+        nw = self.n_walkers if n_walkers is None else n_walkers
+        rng = np.random.Generator(np.random.PCG64(self.seed))
+        if self.ion_pos is None:
+            return rng.random((nw, self.n, self.dim)) * self.L
+        # config 4: electron 4I+m sits at ion I plus N(0,1) per component (reading R13)
+        per_ion = self.n // len(self.ion_pos)
+        base = np.repeat(self.ion_pos, per_ion, axis=0)
+        return base[None, :, :] + rng.standard_normal((nw, self.n, self.dim))
+
+    def moves(self, n_walkers=None, n_steps=None):
+        """Config 5 move stream (reading R14): electron [S, W] int32, displacement [S, W, dim] float64."""
+        nw = self.n_walkers if n_walkers is None else n_walkers
+        ns = self.n_steps if n_steps is None else n_steps
+        rng_e = np.random.Generator(np.random.PCG64(self.seed + 1000))
+        rng_d = np.random.Generator(np.random.PCG64(self.seed + 2000))
+        # drawn walker-major so that a walker subset / a step prefix is a prefix of the full stream
+        electron = rng_e.integers(0, self.n, size=(nw, self.n_steps or ns), dtype=np.int32)[:, :ns]
+        disp = rng_d.standard_normal((nw, self.n_steps or ns, self.dim))[:, :ns] * self.step_sigma
+        return np.ascontiguousarray(electron.T), np.ascontiguousarray(disp.transpose(1, 0, 2))
+
+
+def _cubic(L, dim):
+    return np.eye(dim) * L
+
+
+def _diamond_ions(a, reps):
+    """Conventional diamond cell (8 sites), reps^3 cells; order: cell loops (i,j,k) outer, basis inner."""
+    fcc = np.array([[0, 0, 0], [0, .5, .5], [.5, 0, .5], [.5, .5, 0]])
+    basis = np.concatenate([fcc, fcc + 0.25])
+    pts = []
+    for i in range(reps):
+        for j in range(reps):
+            for k in range(reps):
+                pts.append((basis + np.array([i, j, k])) * a)
+    return np.concatenate(pts)
+
+
+def config(index):
+    """Workload for BASELINE.json configs[index-1]; parameters of SURVEY.md section 8(d)."""
+    if index == 1:
+        n, rs = 54, 2.0
+        L = rs * (4.0 * math.pi * n / 3.0) ** (1.0 / 3.0)
+        return Workload("heg3d_n54", 1, 3, n, 8, L, 2.8 / L, 36, 2.2 * L, ("f64",),
+                        cell=_cubic(L, 3), charges=-np.ones(n))
+    if index == 2:
+        n, rs = 250, 1.0
+        L = rs * (4.0 * math.pi * n / 3.0) ** (1.0 / 3.0)
+        return Workload("heg3d_n250", 2, 3, n, 1024, L, 4.4 / L, 61, 1.3 * L, ("f64", "f32"),
+                        cell=_cubic(L, 3), charges=-np.ones(n))
+    if index == 3:
+        n, rs = 450, 5.0
+        L = rs * math.sqrt(math.pi * n)
+        return Workload("heg2d_n450", 3, 2, n, 1024, L, 12.0 / L, 484, 0.5 * L, ("f64", "f32"),
+                        cell=_cubic(L, 2), charges=-np.ones(n))
+    if index == 4:
+        a = 10.26
+        L = 2 * a
+        ions = _diamond_ions(a, 2)
+        return Workload("diamond_2x2x2", 4, 3, 256, 4096, L, 4.8 / L, 81, 1.2 * L, ("f64",),
+                        cell=_cubic(L, 3), charges=-np.ones(256), ion_pos=ions,
+                        ion_q=4.0 * np.ones(len(ions)))
+    if index == 5:
+        n, rs = 1000, 1.0
+        L = rs * (4.0 * math.pi * n / 3.0) ** (1.0 / 3.0)
+        return Workload("heg3d_n1000_moves", 5, 3, n, 4096, L, 5.4 / L, 97, 1.1 * L, ("f64", "f32"),
+                        n_steps=100, step_sigma=0.3 * rs, cell=_cubic(L, 3), charges=-np.ones(n))
+    raise ValueError("config index must be 1..5")
+
+
+def all_configs():
+    return [config(i) for i in range(1, 6)]
