@@ -1,0 +1,660 @@
+/* ewald_api.cu -- the C ABI of include/ewald.h: context, device tables, launches.
+ * No torch types; plain pointers and sizes.  No CPU fallback: every compute entry point launches
+ * the sm_100a kernels of ewald_kernels.cuh or fails with EWALD_ECUDA. */
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <string>
+#include <vector>
+
+#include "ewald.h"
+#include "ewald_internal.h"
+#include "ewald_kernels.cuh"
+
+using namespace ewald;
+
+struct DevBuf {
+    void *p = nullptr;
+    size_t cap = 0;
+};
+
+struct ProfRec {
+    int kind;
+    cudaEvent_t a, b;
+};
+
+struct ewald_ctx {
+    bool prof = false;
+    std::vector<ProfRec> recs;
+    long long launches = 0; /* kernels launched since setup */
+    HostTables t;
+    int device = 0;
+    cudaStream_t stream = nullptr;
+    std::string err;
+    int ngp = 0, ngp_pad = 0, nimg = 0;
+    int off[3] = {0, 0, 0}, rowlen = 0;
+
+    /* tables, FP64 and FP32 copies */
+    short4 *d_gn = nullptr;
+    double *d_w2 = nullptr; float *d_w2f = nullptr;
+    double *d_img = nullptr; float *d_imgf = nullptr;
+    double *d_ion_rho = nullptr; float *d_ion_rhof = nullptr;
+    double *d_ion_pos = nullptr; float *d_ion_posf = nullptr;
+    double *d_ion_q = nullptr; float *d_ion_qf = nullptr;
+
+    /* scratch */
+    DevBuf partial_recip, partial_real, qsums;
+    DevBuf stage_pos, stage_q, stage_e, stage_comp;           /* *_host entry points */
+    DevBuf mv_walker, mv_electron, mv_newr, mv_de;
+
+    /* stored walker population */
+    int st_walkers = 0, st_n = 0, st_npad = 0;
+    ewald_prec st_prec = EWALD_F64;
+    DevBuf st_pos, st_q, st_rho;
+    bool loaded = false;
+};
+
+static const char *kVersion = "ewald-b200 0.1 (sm_100a)";
+
+#define CU_TRY(ctx, expr)                                                                        \
+    do {                                                                                         \
+        cudaError_t e_ = (expr);                                                                 \
+        if (e_ != cudaSuccess) {                                                                 \
+            (ctx)->err = std::string(#expr) + ": " + cudaGetErrorString(e_);                     \
+            return e_ == cudaErrorMemoryAllocation ? EWALD_ENOMEM : EWALD_ECUDA;                 \
+        }                                                                                        \
+    } while (0)
+
+/* Brackets one kernel launch with events when profiling is on. */
+struct ProfScope {
+    ewald_ctx *c;
+    ProfRec r;
+    bool on;
+    ProfScope(ewald_ctx *ctx, int kind) : c(ctx), on(ctx->prof)
+    {
+        c->launches++;
+        if (!on) return;
+        r.kind = kind;
+        on = cudaEventCreate(&r.a) == cudaSuccess && cudaEventCreate(&r.b) == cudaSuccess &&
+             cudaEventRecord(r.a, c->stream) == cudaSuccess;
+    }
+    ~ProfScope()
+    {
+        if (on && cudaEventRecord(r.b, c->stream) == cudaSuccess) c->recs.push_back(r);
+    }
+};
+
+static ewald_status fail(ewald_ctx *c, ewald_status s, const char *msg)
+{
+    if (c) c->err = msg;
+    return s;
+}
+
+static ewald_status ensure(ewald_ctx *c, DevBuf *b, size_t bytes)
+{
+    if (bytes <= b->cap) return EWALD_OK;
+    if (b->p) { CU_TRY(c, cudaStreamSynchronize(c->stream)); CU_TRY(c, cudaFree(b->p)); b->p = nullptr; b->cap = 0; }
+    size_t want = bytes + bytes / 4 + 256;
+    CU_TRY(c, cudaMalloc(&b->p, want));
+    b->cap = want;
+    return EWALD_OK;
+}
+
+static void release(DevBuf *b)
+{
+    if (b->p) cudaFree(b->p);
+    b->p = nullptr;
+    b->cap = 0;
+}
+
+template <typename T>
+static ewald_status upload(ewald_ctx *c, T **dst, const std::vector<T> &src)
+{
+    if (*dst) { CU_TRY(c, cudaFree(*dst)); *dst = nullptr; }
+    if (src.empty()) return EWALD_OK;
+    CU_TRY(c, cudaMalloc((void **)dst, src.size() * sizeof(T)));
+    CU_TRY(c, cudaMemcpy(*dst, src.data(), src.size() * sizeof(T), cudaMemcpyHostToDevice));
+    return EWALD_OK;
+}
+
+static std::vector<float> to_f32(const std::vector<double> &v)
+{
+    std::vector<float> f(v.size());
+    for (size_t i = 0; i < v.size(); i++) f[i] = (float)v[i];
+    return f;
+}
+
+template <typename T> static void fill_cell(const HostTables &t, CellT<T> *c)
+{
+    for (int i = 0; i < 9; i++) { c->a[i] = (T)t.a[i]; c->binv[i] = (T)t.binv[i]; }
+    c->kappa = (T)t.kappa;
+    c->rcut2 = (T)(t.r_cutoff * t.r_cutoff);
+}
+
+extern "C" int ewald_padded_n(int n) { return n <= 0 ? 0 : (n + 3) & ~3; }
+extern "C" const char *ewald_version(void) { return kVersion; }
+extern "C" const char *ewald_last_error(const ewald_ctx *c) { return c ? c->err.c_str() : ""; }
+
+extern "C" ewald_status ewald_setup(ewald_ctx **out, int dim, const double *cell, double gamma,
+                                    double g_cutoff, const ewald_opts *opts)
+{
+    if (!out) return EWALD_EINVAL;
+    *out = nullptr;
+    ewald_ctx *c = new (std::nothrow) ewald_ctx;
+    if (!c) return EWALD_ENOMEM;
+    std::string err;
+    ewald_status st = build_tables(dim, cell, gamma, g_cutoff, opts ? opts->r_cutoff : 0.0, &c->t, &err);
+    if (st != EWALD_OK) { delete c; return st; }
+    c->device = opts ? opts->device : 0;
+    c->stream = opts ? (cudaStream_t)opts->stream : nullptr;
+    cudaError_t ce = cudaSetDevice(c->device);
+    if (ce != cudaSuccess) { delete c; return EWALD_ECUDA; }
+
+    const HostTables &t = c->t;
+    c->ngp = (int)t.g_w2.size();
+    c->ngp_pad = (c->ngp + 31) & ~31;
+    c->nimg = (int)(t.img.size() / 3);
+    int o = 0;
+    for (int k = 0; k < 3; k++) { c->off[k] = o; if (k < dim) o += t.n_max[k] + 1; }
+    c->rowlen = o;
+
+    std::vector<short4> gn(c->ngp);
+    for (int g = 0; g < c->ngp; g++)
+        gn[g] = make_short4((short)t.g_n[3 * g], (short)t.g_n[3 * g + 1], (short)t.g_n[3 * g + 2], 0);
+    st = upload(c, &c->d_gn, gn);
+    if (st == EWALD_OK) st = upload(c, &c->d_w2, t.g_w2);
+    if (st == EWALD_OK) st = upload(c, &c->d_w2f, to_f32(t.g_w2));
+    if (st == EWALD_OK) st = upload(c, &c->d_img, t.img);
+    if (st == EWALD_OK) st = upload(c, &c->d_imgf, to_f32(t.img));
+    if (st == EWALD_OK) st = ensure(c, &c->qsums, 2 * sizeof(double));
+    if (st != EWALD_OK) { ewald_destroy(c); return st; }
+    *out = c;
+    return EWALD_OK;
+}
+
+extern "C" ewald_status ewald_setup_summary(int dim, const double *cell, double gamma, double g_cutoff,
+                                            double r_cutoff, int *num_g, int *num_images, int *n_max,
+                                            double *xi_r, double *v_m)
+{
+    HostTables t;
+    std::string err;
+    ewald_status st = build_tables(dim, cell, gamma, g_cutoff, r_cutoff, &t, &err);
+    if (st != EWALD_OK) return st;
+    if (num_g) *num_g = 2 * (int)t.g_w2.size();
+    if (num_images) *num_images = (int)(t.img.size() / 3);
+    if (n_max) for (int k = 0; k < 3; k++) n_max[k] = t.n_max[k];
+    if (xi_r) *xi_r = t.xi_r;
+    if (v_m) *v_m = t.v_m;
+    return EWALD_OK;
+}
+
+extern "C" void ewald_destroy(ewald_ctx *c)
+{
+    if (!c) return;
+    cudaSetDevice(c->device);
+    cudaStreamSynchronize(c->stream);
+    cudaFree(c->d_gn); cudaFree(c->d_w2); cudaFree(c->d_w2f); cudaFree(c->d_img); cudaFree(c->d_imgf);
+    cudaFree(c->d_ion_rho); cudaFree(c->d_ion_rhof); cudaFree(c->d_ion_pos); cudaFree(c->d_ion_posf);
+    cudaFree(c->d_ion_q); cudaFree(c->d_ion_qf);
+    DevBuf *bufs[] = {&c->partial_recip, &c->partial_real, &c->qsums, &c->stage_pos, &c->stage_q,
+                      &c->stage_e, &c->stage_comp, &c->mv_walker, &c->mv_electron, &c->mv_newr,
+                      &c->mv_de, &c->st_pos, &c->st_q, &c->st_rho};
+    for (DevBuf *b : bufs) release(b);
+    delete c;
+}
+
+extern "C" ewald_status ewald_set_stream(ewald_ctx *c, void *stream)
+{
+    if (!c) return EWALD_EINVAL;
+    c->stream = (cudaStream_t)stream;
+    return EWALD_OK;
+}
+
+extern "C" ewald_status ewald_set_fixed_charges(ewald_ctx *c, int n_ion, const double *pos, const double *q)
+{
+    if (!c) return EWALD_EINVAL;
+    CU_TRY(c, cudaSetDevice(c->device));
+    std::string err;
+    ewald_status st = build_fixed_charges(&c->t, n_ion, pos, q, &err);
+    if (st != EWALD_OK) return fail(c, st, err.c_str());
+    CU_TRY(c, cudaStreamSynchronize(c->stream));
+    const HostTables &t = c->t;
+    st = upload(c, &c->d_ion_rho, n_ion ? t.ion_rho : std::vector<double>());
+    if (st == EWALD_OK) st = upload(c, &c->d_ion_rhof, n_ion ? to_f32(t.ion_rho) : std::vector<float>());
+    if (st == EWALD_OK) st = upload(c, &c->d_ion_pos, t.ion_pos);
+    if (st == EWALD_OK) st = upload(c, &c->d_ion_posf, to_f32(t.ion_pos));
+    if (st == EWALD_OK) st = upload(c, &c->d_ion_q, t.ion_q);
+    if (st == EWALD_OK) st = upload(c, &c->d_ion_qf, to_f32(t.ion_q));
+    c->loaded = false; /* a stored rho(G) would no longer match */
+    return st;
+}
+
+/* ---- launches ---------------------------------------------------------------------------- */
+
+template <typename T> struct Tabs;
+template <> struct Tabs<double> {
+    static const double *w2(const ewald_ctx *c) { return c->d_w2; }
+    static const double *img(const ewald_ctx *c) { return c->d_img; }
+    static const double *ion_rho(const ewald_ctx *c) { return c->d_ion_rho; }
+    static const double *ion_pos(const ewald_ctx *c) { return c->d_ion_pos; }
+    static const double *ion_q(const ewald_ctx *c) { return c->d_ion_q; }
+};
+template <> struct Tabs<float> {
+    static const float *w2(const ewald_ctx *c) { return c->d_w2f; }
+    static const float *img(const ewald_ctx *c) { return c->d_imgf; }
+    static const float *ion_rho(const ewald_ctx *c) { return c->d_ion_rhof; }
+    static const float *ion_pos(const ewald_ctx *c) { return c->d_ion_posf; }
+    static const float *ion_q(const ewald_ctx *c) { return c->d_ion_qf; }
+};
+
+template <typename K> static ewald_status allow_smem(ewald_ctx *c, K kernel, size_t bytes)
+{
+    if (bytes > 48 * 1024) {
+        if (bytes > 227 * 1024) return fail(c, EWALD_ERANGE, "problem too large for shared memory");
+        CU_TRY(c, cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes));
+    }
+    return EWALD_OK;
+}
+
+template <typename T>
+static ewald_status launch_recip(ewald_ctx *c, int W, int n, const T *pos, const T *q, T *rho_out,
+                                 int *n_slabs_out)
+{
+    typedef typename Num<T>::T2 T2;
+    const int per = RECIP_THREADS * RECIP_GPT;
+    const int n_slabs = (c->ngp + per - 1) / per;
+    ewald_status st = ensure(c, &c->partial_recip, (size_t)W * n_slabs * sizeof(double));
+    if (st != EWALD_OK) return st;
+    RecipArgs<T> A;
+    A.pos = pos; A.q = q; A.n = n; A.npad = ewald_padded_n(n);
+    A.gn = c->d_gn; A.w2 = Tabs<T>::w2(c); A.ion_rho = c->t.n_ion ? Tabs<T>::ion_rho(c) : nullptr;
+    A.ngp = c->ngp; A.ngp_pad = c->ngp_pad;
+    for (int k = 0; k < 3; k++) { A.nmax[k] = c->t.n_max[k]; A.off[k] = c->off[k]; }
+    A.rowlen = c->rowlen;
+    A.rho_out = rho_out;
+    A.partial = (double *)c->partial_recip.p;
+    A.n_slabs = n_slabs;
+    for (int i = 0; i < 9; i++) A.binv[i] = (T)c->t.binv[i];
+    const size_t smem = (size_t)RECIP_CHUNK * c->rowlen * sizeof(T2);
+    const long long grid = (long long)W * n_slabs;
+    if (grid > 0x7fffffffLL) return fail(c, EWALD_ERANGE, "grid too large");
+    if (c->t.dim == 3) {
+        st = allow_smem(c, recip_kernel<T, 3>, smem);
+        if (st != EWALD_OK) return st;
+        ProfScope ps(c, 0);
+        recip_kernel<T, 3><<<(unsigned)grid, RECIP_THREADS, smem, c->stream>>>(A);
+    } else {
+        st = allow_smem(c, recip_kernel<T, 2>, smem);
+        if (st != EWALD_OK) return st;
+        ProfScope ps(c, 0);
+        recip_kernel<T, 2><<<(unsigned)grid, RECIP_THREADS, smem, c->stream>>>(A);
+    }
+    CU_TRY(c, cudaGetLastError());
+    *n_slabs_out = n_slabs;
+    return EWALD_OK;
+}
+
+template <typename T>
+static ewald_status launch_real(ewald_ctx *c, int W, int n, const T *pos, const T *q, int *n_tiles_out)
+{
+    const long long H = (n - 1) / 2;
+    const long long total = (long long)n * H + ((n & 1) ? 0 : n / 2) + (long long)n * c->t.n_ion;
+    long long n_tiles = (4LL * 148 * 2 + W - 1) / W;
+    const long long max_tiles = (total + REAL_THREADS - 1) / REAL_THREADS;
+    if (n_tiles > max_tiles) n_tiles = max_tiles;
+    if (n_tiles < 1) n_tiles = 1;
+    ewald_status st = ensure(c, &c->partial_real, (size_t)W * n_tiles * sizeof(double));
+    if (st != EWALD_OK) return st;
+    RealArgs<T> A;
+    A.pos = pos; A.q = q; A.n = n; A.npad = ewald_padded_n(n);
+    A.img = Tabs<T>::img(c); A.nimg = c->nimg;
+    A.ion_pos = Tabs<T>::ion_pos(c); A.ion_q = Tabs<T>::ion_q(c); A.n_ion = c->t.n_ion;
+    A.partial = (double *)c->partial_real.p;
+    A.n_tiles = (int)n_tiles;
+    fill_cell(c->t, &A.cell);
+    const size_t smem = ((size_t)(c->t.dim + 1) * n + 3 * (size_t)c->nimg) * sizeof(T);
+    const long long grid = (long long)W * n_tiles;
+    if (grid > 0x7fffffffLL) return fail(c, EWALD_ERANGE, "grid too large");
+    if (c->t.dim == 3) {
+        st = allow_smem(c, real_kernel<T, 3>, smem);
+        if (st != EWALD_OK) return st;
+        ProfScope ps(c, 1);
+        real_kernel<T, 3><<<(unsigned)grid, REAL_THREADS, smem, c->stream>>>(A);
+    } else {
+        st = allow_smem(c, real_kernel<T, 2>, smem);
+        if (st != EWALD_OK) return st;
+        ProfScope ps(c, 1);
+        real_kernel<T, 2><<<(unsigned)grid, REAL_THREADS, smem, c->stream>>>(A);
+    }
+    CU_TRY(c, cudaGetLastError());
+    *n_tiles_out = (int)n_tiles;
+    return EWALD_OK;
+}
+
+template <typename T>
+static ewald_status energy_batch_t(ewald_ctx *c, int W, int n, const T *pos, const T *q,
+                                   double *energies, double *components)
+{
+    int n_slabs = 0, n_tiles = 0;
+    {
+        ProfScope ps(c, 2);
+        charge_sums_kernel<T><<<1, 256, 0, c->stream>>>(q, n, (double *)c->qsums.p);
+    }
+    CU_TRY(c, cudaGetLastError());
+    ewald_status st = launch_recip<T>(c, W, n, pos, q, nullptr, &n_slabs);
+    if (st != EWALD_OK) return st;
+    st = launch_real<T>(c, W, n, pos, q, &n_tiles);
+    if (st != EWALD_OK) return st;
+    CombineArgs A;
+    A.recip_partial = (const double *)c->partial_recip.p; A.n_recip = n_slabs;
+    A.real_partial = (const double *)c->partial_real.p; A.n_real = n_tiles;
+    A.qsums = (const double *)c->qsums.p;
+    A.ion_q2 = c->t.ion_q2; A.ion_qsum = c->t.ion_qsum; A.ion_real = c->t.ion_real;
+    A.xi_r = c->t.xi_r; A.self_coef = c->t.self_coef; A.bg_coef = c->t.bg_coef;
+    A.energies = energies; A.components = components; A.n_walkers = W;
+    {
+        ProfScope ps(c, 2);
+        combine_kernel<<<(W + 127) / 128, 128, 0, c->stream>>>(A);
+    }
+    CU_TRY(c, cudaGetLastError());
+    return EWALD_OK;
+}
+
+static ewald_status check_batch(ewald_ctx *c, int W, int n, ewald_prec prec, const void *pos, const void *q)
+{
+    if (!c) return EWALD_EINVAL;
+    if (W < 0 || n <= 0) return fail(c, EWALD_EINVAL, "n_walkers < 0 or n_particles <= 0");
+    if (prec != EWALD_F64 && prec != EWALD_F32) return fail(c, EWALD_EINVAL, "bad precision");
+    if (W > 0 && (!pos || !q)) return fail(c, EWALD_EINVAL, "null positions or charges");
+    return EWALD_OK;
+}
+
+extern "C" ewald_status ewald_energy_batch(ewald_ctx *c, int W, int n, ewald_prec prec, const void *pos,
+                                           const void *q, double *energies, double *components)
+{
+    ewald_status st = check_batch(c, W, n, prec, pos, q);
+    if (st != EWALD_OK) return st;
+    if (W == 0) return EWALD_OK;
+    if (!energies) return fail(c, EWALD_EINVAL, "null energies");
+    CU_TRY(c, cudaSetDevice(c->device));
+    if (prec == EWALD_F64)
+        return energy_batch_t<double>(c, W, n, (const double *)pos, (const double *)q, energies, components);
+    return energy_batch_t<float>(c, W, n, (const float *)pos, (const float *)q, energies, components);
+}
+
+extern "C" ewald_status ewald_energy_batch_host(ewald_ctx *c, int W, int n, ewald_prec prec,
+                                                const void *pos, const void *q, double *energies,
+                                                double *components)
+{
+    ewald_status st = check_batch(c, W, n, prec, pos, q);
+    if (st != EWALD_OK) return st;
+    if (W == 0) return EWALD_OK;
+    if (!energies) return fail(c, EWALD_EINVAL, "null energies");
+    CU_TRY(c, cudaSetDevice(c->device));
+    const size_t es = prec == EWALD_F64 ? 8 : 4;
+    const size_t pbytes = (size_t)W * c->t.dim * ewald_padded_n(n) * es, qbytes = (size_t)n * es;
+    if ((st = ensure(c, &c->stage_pos, pbytes)) != EWALD_OK) return st;
+    if ((st = ensure(c, &c->stage_q, qbytes)) != EWALD_OK) return st;
+    if ((st = ensure(c, &c->stage_e, (size_t)W * 8)) != EWALD_OK) return st;
+    if (components && (st = ensure(c, &c->stage_comp, (size_t)W * 32)) != EWALD_OK) return st;
+    CU_TRY(c, cudaMemcpyAsync(c->stage_pos.p, pos, pbytes, cudaMemcpyHostToDevice, c->stream));
+    CU_TRY(c, cudaMemcpyAsync(c->stage_q.p, q, qbytes, cudaMemcpyHostToDevice, c->stream));
+    st = ewald_energy_batch(c, W, n, prec, c->stage_pos.p, c->stage_q.p, (double *)c->stage_e.p,
+                            components ? (double *)c->stage_comp.p : nullptr);
+    if (st != EWALD_OK) return st;
+    CU_TRY(c, cudaMemcpyAsync(energies, c->stage_e.p, (size_t)W * 8, cudaMemcpyDeviceToHost, c->stream));
+    if (components)
+        CU_TRY(c, cudaMemcpyAsync(components, c->stage_comp.p, (size_t)W * 32, cudaMemcpyDeviceToHost, c->stream));
+    CU_TRY(c, cudaStreamSynchronize(c->stream));
+    return EWALD_OK;
+}
+
+extern "C" ewald_status ewald_load_walkers(ewald_ctx *c, int W, int n, ewald_prec prec, const void *pos,
+                                           const void *q)
+{
+    ewald_status st = check_batch(c, W, n, prec, pos, q);
+    if (st != EWALD_OK) return st;
+    if (W == 0) return fail(c, EWALD_EINVAL, "n_walkers must be > 0");
+    CU_TRY(c, cudaSetDevice(c->device));
+    const size_t es = prec == EWALD_F64 ? 8 : 4;
+    const int npad = ewald_padded_n(n);
+    const size_t pbytes = (size_t)W * c->t.dim * npad * es;
+    c->loaded = false;
+    if ((st = ensure(c, &c->st_pos, pbytes)) != EWALD_OK) return st;
+    if ((st = ensure(c, &c->st_q, (size_t)n * es)) != EWALD_OK) return st;
+    if ((st = ensure(c, &c->st_rho, (size_t)W * 2 * c->ngp_pad * es)) != EWALD_OK) return st;
+    CU_TRY(c, cudaMemcpyAsync(c->st_pos.p, pos, pbytes, cudaMemcpyDeviceToDevice, c->stream));
+    CU_TRY(c, cudaMemcpyAsync(c->st_q.p, q, (size_t)n * es, cudaMemcpyDeviceToDevice, c->stream));
+    CU_TRY(c, cudaMemsetAsync(c->st_rho.p, 0, (size_t)W * 2 * c->ngp_pad * es, c->stream));
+    int n_slabs = 0;
+    if (prec == EWALD_F64)
+        st = launch_recip<double>(c, W, n, (const double *)c->st_pos.p, (const double *)c->st_q.p,
+                                  (double *)c->st_rho.p, &n_slabs);
+    else
+        st = launch_recip<float>(c, W, n, (const float *)c->st_pos.p, (const float *)c->st_q.p,
+                                 (float *)c->st_rho.p, &n_slabs);
+    if (st != EWALD_OK) return st;
+    c->st_walkers = W; c->st_n = n; c->st_npad = npad; c->st_prec = prec;
+    c->loaded = true;
+    return EWALD_OK;
+}
+
+template <typename T>
+static ewald_status move_batch_t(ewald_ctx *c, int n_moves, const int *walker, const int *electron,
+                                 const T *new_r, int commit, double *delta_e)
+{
+    typedef typename Num<T>::T2 T2;
+    MoveArgs<T> A;
+    A.pos = (T *)c->st_pos.p; A.q = (const T *)c->st_q.p; A.rho = (T *)c->st_rho.p;
+    A.n = c->st_n; A.npad = c->st_npad; A.n_walkers = c->st_walkers;
+    A.gn = c->d_gn; A.w2 = Tabs<T>::w2(c); A.ngp = c->ngp; A.ngp_pad = c->ngp_pad;
+    for (int k = 0; k < 3; k++) { A.nmax[k] = c->t.n_max[k]; A.off[k] = c->off[k]; }
+    A.rowlen = c->rowlen;
+    A.img = Tabs<T>::img(c); A.nimg = c->nimg;
+    A.ion_pos = Tabs<T>::ion_pos(c); A.ion_q = Tabs<T>::ion_q(c); A.n_ion = c->t.n_ion;
+    A.walker = walker; A.electron = electron; A.new_r = new_r; A.commit = commit; A.delta_e = delta_e;
+    fill_cell(c->t, &A.cell);
+    const size_t smem = 2 * (size_t)c->rowlen * sizeof(T2) + 3 * (size_t)c->nimg * sizeof(T);
+    ewald_status st;
+    if (c->t.dim == 3) {
+        if ((st = allow_smem(c, move_kernel<T, 3>, smem)) != EWALD_OK) return st;
+        ProfScope ps(c, 3);
+        move_kernel<T, 3><<<n_moves, MOVE_THREADS, smem, c->stream>>>(A);
+    } else {
+        if ((st = allow_smem(c, move_kernel<T, 2>, smem)) != EWALD_OK) return st;
+        ProfScope ps(c, 3);
+        move_kernel<T, 2><<<n_moves, MOVE_THREADS, smem, c->stream>>>(A);
+    }
+    CU_TRY(c, cudaGetLastError());
+    return EWALD_OK;
+}
+
+extern "C" ewald_status ewald_move_delta_batch(ewald_ctx *c, int n_moves, const int *walker,
+                                               const int *electron, const void *new_r, int commit,
+                                               double *delta_e)
+{
+    if (!c) return EWALD_EINVAL;
+    if (!c->loaded) return fail(c, EWALD_ESTATE, "no walkers loaded (call ewald_load_walkers first)");
+    if (n_moves < 0) return fail(c, EWALD_EINVAL, "n_moves < 0");
+    if (n_moves == 0) return EWALD_OK;
+    if (!walker || !electron || !new_r || !delta_e) return fail(c, EWALD_EINVAL, "null move argument");
+    CU_TRY(c, cudaSetDevice(c->device));
+    if (c->st_prec == EWALD_F64)
+        return move_batch_t<double>(c, n_moves, walker, electron, (const double *)new_r, commit, delta_e);
+    return move_batch_t<float>(c, n_moves, walker, electron, (const float *)new_r, commit, delta_e);
+}
+
+extern "C" ewald_status ewald_move_delta_batch_host(ewald_ctx *c, int n_moves, const int *walker,
+                                                    const int *electron, const void *new_r, int commit,
+                                                    double *delta_e)
+{
+    if (!c) return EWALD_EINVAL;
+    if (!c->loaded) return fail(c, EWALD_ESTATE, "no walkers loaded (call ewald_load_walkers first)");
+    if (n_moves < 0) return fail(c, EWALD_EINVAL, "n_moves < 0");
+    if (n_moves == 0) return EWALD_OK;
+    if (!walker || !electron || !new_r || !delta_e) return fail(c, EWALD_EINVAL, "null move argument");
+    CU_TRY(c, cudaSetDevice(c->device));
+    const size_t es = c->st_prec == EWALD_F64 ? 8 : 4;
+    const size_t rbytes = (size_t)n_moves * c->t.dim * es;
+    ewald_status st;
+    if ((st = ensure(c, &c->mv_walker, (size_t)n_moves * 4)) != EWALD_OK) return st;
+    if ((st = ensure(c, &c->mv_electron, (size_t)n_moves * 4)) != EWALD_OK) return st;
+    if ((st = ensure(c, &c->mv_newr, rbytes)) != EWALD_OK) return st;
+    if ((st = ensure(c, &c->mv_de, (size_t)n_moves * 8)) != EWALD_OK) return st;
+    CU_TRY(c, cudaMemcpyAsync(c->mv_walker.p, walker, (size_t)n_moves * 4, cudaMemcpyHostToDevice, c->stream));
+    CU_TRY(c, cudaMemcpyAsync(c->mv_electron.p, electron, (size_t)n_moves * 4, cudaMemcpyHostToDevice, c->stream));
+    CU_TRY(c, cudaMemcpyAsync(c->mv_newr.p, new_r, rbytes, cudaMemcpyHostToDevice, c->stream));
+    st = ewald_move_delta_batch(c, n_moves, (const int *)c->mv_walker.p, (const int *)c->mv_electron.p,
+                                c->mv_newr.p, commit, (double *)c->mv_de.p);
+    if (st != EWALD_OK) return st;
+    CU_TRY(c, cudaMemcpyAsync(delta_e, c->mv_de.p, (size_t)n_moves * 8, cudaMemcpyDeviceToHost, c->stream));
+    CU_TRY(c, cudaStreamSynchronize(c->stream));
+    return EWALD_OK;
+}
+
+extern "C" ewald_status ewald_move_delta(ewald_ctx *c, int walker, int electron, const double *new_r,
+                                         int commit, double *delta_e)
+{
+    if (!c) return EWALD_EINVAL;
+    if (!c->loaded) return fail(c, EWALD_ESTATE, "no walkers loaded (call ewald_load_walkers first)");
+    if (!new_r || !delta_e) return fail(c, EWALD_EINVAL, "null move argument");
+    if (walker < 0 || walker >= c->st_walkers) return fail(c, EWALD_ESTATE, "walker index out of range");
+    if (electron < 0 || electron >= c->st_n) return fail(c, EWALD_ESTATE, "electron index out of range");
+    float rf[3];
+    for (int x = 0; x < c->t.dim; x++) rf[x] = (float)new_r[x];
+    const void *r = c->st_prec == EWALD_F64 ? (const void *)new_r : (const void *)rf;
+    return ewald_move_delta_batch_host(c, 1, &walker, &electron, r, commit, delta_e);
+}
+
+/* ---- per-kernel timers -------------------------------------------------------------------- */
+
+extern "C" ewald_status ewald_profile_enable(ewald_ctx *c, int on)
+{
+    if (!c) return EWALD_EINVAL;
+    c->prof = on != 0;
+    return EWALD_OK;
+}
+
+extern "C" ewald_status ewald_profile_read(ewald_ctx *c, double *ms, int *launches)
+{
+    if (!c || !ms || !launches) return EWALD_EINVAL;
+    CU_TRY(c, cudaSetDevice(c->device));
+    CU_TRY(c, cudaStreamSynchronize(c->stream));
+    for (int k = 0; k < 4; k++) { ms[k] = 0; launches[k] = 0; }
+    for (ProfRec &r : c->recs) {
+        float t = 0;
+        if (cudaEventElapsedTime(&t, r.a, r.b) == cudaSuccess && r.kind >= 0 && r.kind < 4) {
+            ms[r.kind] += t;
+            launches[r.kind]++;
+        }
+        cudaEventDestroy(r.a);
+        cudaEventDestroy(r.b);
+    }
+    c->recs.clear();
+    return EWALD_OK;
+}
+
+extern "C" long long ewald_launch_count(const ewald_ctx *c) { return c ? c->launches : -1; }
+
+/* ---- introspection ------------------------------------------------------------------------ */
+
+extern "C" int ewald_num_g(const ewald_ctx *c) { return c ? 2 * c->ngp : -1; }
+extern "C" int ewald_num_images(const ewald_ctx *c) { return c ? c->nimg : -1; }
+extern "C" double ewald_r_cutoff(const ewald_ctx *c) { return c ? c->t.r_cutoff : NAN; }
+
+extern "C" ewald_status ewald_get_g(const ewald_ctx *c, int *n_out)
+{
+    if (!c || !n_out) return EWALD_EINVAL;
+    memcpy(n_out, c->t.g_n.data(), c->t.g_n.size() * sizeof(int));
+    return EWALD_OK;
+}
+
+extern "C" ewald_status ewald_get_constants(const ewald_ctx *c, double *xi_r, double *v_m, double *e_fixed)
+{
+    if (!c) return EWALD_EINVAL;
+    if (xi_r) *xi_r = c->t.xi_r;
+    if (v_m) *v_m = c->t.v_m;
+    if (e_fixed) {
+        /* Eq. 2 restricted to the fixed charges: recip + real + self + background */
+        long double er = 0;
+        for (int g = 0; g < c->ngp && c->t.n_ion; g++)
+            er += (long double)c->t.g_w2[g] * ((long double)c->t.ion_rho[2 * g] * c->t.ion_rho[2 * g] +
+                                               (long double)c->t.ion_rho[2 * g + 1] * c->t.ion_rho[2 * g + 1]);
+        *e_fixed = (double)(er + c->t.ion_real + 0.5L * c->t.ion_q2 * c->t.xi_r -
+                            (long double)c->t.self_coef * c->t.ion_q2 -
+                            0.5L * c->t.bg_coef * c->t.ion_qsum * c->t.ion_qsum);
+    }
+    return EWALD_OK;
+}
+
+extern "C" ewald_status ewald_get_rho(ewald_ctx *c, int walker, double *re_im)
+{
+    if (!c || !re_im) return EWALD_EINVAL;
+    if (!c->loaded) return fail(c, EWALD_ESTATE, "no walkers loaded");
+    if (walker < 0 || walker >= c->st_walkers) return fail(c, EWALD_ESTATE, "walker index out of range");
+    CU_TRY(c, cudaSetDevice(c->device));
+    const size_t es = c->st_prec == EWALD_F64 ? 8 : 4;
+    std::vector<unsigned char> h((size_t)2 * c->ngp_pad * es);
+    CU_TRY(c, cudaMemcpyAsync(h.data(), (const char *)c->st_rho.p + (size_t)walker * h.size(), h.size(),
+                              cudaMemcpyDeviceToHost, c->stream));
+    CU_TRY(c, cudaStreamSynchronize(c->stream));
+    for (int g = 0; g < c->ngp; g++) {
+        if (es == 8) {
+            const double *d = (const double *)h.data();
+            re_im[2 * g] = d[g]; re_im[2 * g + 1] = d[c->ngp_pad + g];
+        } else {
+            const float *f = (const float *)h.data();
+            re_im[2 * g] = f[g]; re_im[2 * g + 1] = f[c->ngp_pad + g];
+        }
+    }
+    return EWALD_OK;
+}
+
+extern "C" ewald_status ewald_get_positions(ewald_ctx *c, int walker, double *pos)
+{
+    if (!c || !pos) return EWALD_EINVAL;
+    if (!c->loaded) return fail(c, EWALD_ESTATE, "no walkers loaded");
+    if (walker < 0 || walker >= c->st_walkers) return fail(c, EWALD_ESTATE, "walker index out of range");
+    CU_TRY(c, cudaSetDevice(c->device));
+    const size_t es = c->st_prec == EWALD_F64 ? 8 : 4;
+    const int dim = c->t.dim, npad = c->st_npad, n = c->st_n;
+    std::vector<unsigned char> h((size_t)dim * npad * es);
+    CU_TRY(c, cudaMemcpyAsync(h.data(), (const char *)c->st_pos.p + (size_t)walker * h.size(), h.size(),
+                              cudaMemcpyDeviceToHost, c->stream));
+    CU_TRY(c, cudaStreamSynchronize(c->stream));
+    for (int i = 0; i < n; i++)
+        for (int x = 0; x < dim; x++)
+            pos[(size_t)i * dim + x] = es == 8 ? ((const double *)h.data())[x * npad + i]
+                                               : (double)((const float *)h.data())[x * npad + i];
+    return EWALD_OK;
+}
+
+extern "C" ewald_status ewald_probe_fma(ewald_ctx *c, ewald_prec prec, int iters, double *flops)
+{
+    if (!c || !flops || iters <= 0) return EWALD_EINVAL;
+    CU_TRY(c, cudaSetDevice(c->device));
+    cudaDeviceProp prop;
+    CU_TRY(c, cudaGetDeviceProperties(&prop, c->device));
+    ewald_status st = ensure(c, &c->stage_e, 64);
+    if (st != EWALD_OK) return st;
+    const int blocks = prop.multiProcessorCount * 8, threads = 256;
+    cudaEvent_t e0, e1;
+    CU_TRY(c, cudaEventCreate(&e0));
+    CU_TRY(c, cudaEventCreate(&e1));
+    for (int rep = 0; rep < 2; rep++) { /* first pass warms up */
+        CU_TRY(c, cudaEventRecord(e0, c->stream));
+        if (prec == EWALD_F64)
+            fma_probe_kernel<double><<<blocks, threads, 0, c->stream>>>(iters, 1.0000001, 1e-9, (double *)c->stage_e.p);
+        else
+            fma_probe_kernel<float><<<blocks, threads, 0, c->stream>>>(iters, 1.0001f, 1e-6f, (float *)c->stage_e.p);
+        CU_TRY(c, cudaEventRecord(e1, c->stream));
+        CU_TRY(c, cudaEventSynchronize(e1));
+    }
+    float ms = 0;
+    CU_TRY(c, cudaEventElapsedTime(&ms, e0, e1));
+    cudaEventDestroy(e0);
+    cudaEventDestroy(e1);
+    *flops = 2.0 * 64.0 * iters * (double)blocks * threads / (ms * 1e-3);
+    return EWALD_OK;
+}

@@ -1,0 +1,48 @@
+/* ewald_internal.h -- shared between the host setup (ewald_setup.cpp) and the CUDA side
+ * (ewald_kernels.cu, ewald_api.cu).  Not part of the public boundary (include/ewald.h). */
+#ifndef EWALD_INTERNAL_H
+#define EWALD_INTERNAL_H
+
+#include <string>
+#include <vector>
+
+#include "ewald.h"
+
+namespace ewald {
+
+/* Everything ewald_setup computes on the host, in long double, before rounding (PAPER.md:359:
+ * "lookup tables for Ewald interactions ... always performed using DP arithmetic"). */
+struct HostTables {
+    int dim = 3;
+    double kappa = 0, g_cutoff = 0, r_cutoff = 0;
+    double a[9];     /* lattice vectors as rows (dim = 2 embedded with a3 = (0,0,1))            */
+    double binv[9];  /* rows b_k / 2pi : fractional coordinate s_k = r . binv[k]                 */
+    double volume = 0;
+    bool orthogonal = false; /* a_k along Cartesian axis k                                       */
+    int n_max[3] = {0, 0, 0};
+    /* canonical half set G+, lexicographic in (n1,n2,n3) */
+    std::vector<int> g_n;      /* [ngp][3]                                                      */
+    std::vector<double> g_w2;  /* [ngp]  2 w(G): E_recip = sum_{G+} g_w2 |rho|^2                */
+    /* lattice images scanned per (reduced) pair displacement */
+    std::vector<double> img;   /* [nimg][3] Cartesian R                                         */
+    std::vector<int> img_m;    /* [nimg][3] integer coefficients                                */
+    double xi_r = 0;       /* sum_{R != 0, R < rc} erfc(kappa R)/R                               */
+    double self_coef = 0;  /* E_self = -self_coef * sum q^2,  self_coef = kappa/sqrt(pi)          */
+    double bg_coef = 0;    /* E_bg = -bg_coef/2 * Q^2 ; pi/(Omega kappa^2) (3D), 2 sqrt(pi)/(A kappa) (2D) */
+    double v_m = 0;        /* Eq. 4 */
+    /* fixed charges */
+    int n_ion = 0;
+    std::vector<double> ion_pos; /* [n_ion][3] */
+    std::vector<double> ion_q;
+    std::vector<double> ion_rho; /* [ngp][2], sum_I q_I exp(iG.r_I)                              */
+    double ion_q2 = 0, ion_qsum = 0, ion_real = 0; /* sum q^2, sum q, sum_{I<J} q_I q_J psi(r_IJ) */
+};
+
+/* Returns EWALD_OK or an error status with a message. */
+ewald_status build_tables(int dim, const double *cell, double kappa, double g_cutoff,
+                          double r_cutoff, HostTables *out, std::string *err);
+ewald_status build_fixed_charges(HostTables *t, int n_ion, const double *pos, const double *q,
+                                 std::string *err);
+
+} // namespace ewald
+#endif

@@ -1,0 +1,472 @@
+/* ewald_kernels.cuh -- device code of the B200 Ewald library (sm_100a).
+ *
+ * Kernels (SURVEY.md section 8(a) step names in brackets):
+ *   recip_kernel   [S1-S4]  phase seeds exp(2 pi i s_k) by sincospi, power tables by complex
+ *                           recurrence in shared memory (Eq. 8: "powers of these
+ *                           exponentials are computed and buffered"), rho(G) on the half set,
+ *                           E_recip = sum_{G+} 2 w(G) |rho(G)|^2; optionally stores rho(G)
+ *   real_kernel    [S5]     sum_{i<j} q_i q_j sum_R erfc(kappa|r_ij-R|)/|r_ij-R| (real-lattice sum
+ *                           of Eq. 3) plus mobile-ion pairs
+ *   combine_kernel [S6]     adds partial sums and the constants of Eqs. 3-4
+ *   move_kernel    [S7a-d]  single-particle move: Delta E and patch of the stored rho(G)
+ * The paper's version-2 loop structure (real-lattice loop || reciprocal-lattice loop, then a
+ * combining loop) is kept as three kernels; everything inside them is new.
+ */
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace ewald {
+
+template <typename T> struct Num;
+template <> struct Num<double> {
+    typedef double2 T2;
+    static __device__ __forceinline__ void sincospi_(double x, double *s, double *c) { sincospi(x, s, c); }
+    static __device__ __forceinline__ double rint_(double x) { return rint(x); }
+    static __device__ __forceinline__ double erfc_(double x) { return erfc(x); }
+    static __device__ __forceinline__ double rsqrt_(double x) { return rsqrt(x); }
+};
+template <> struct Num<float> {
+    typedef float2 T2;
+    static __device__ __forceinline__ void sincospi_(float x, float *s, float *c) { sincospif(x, s, c); }
+    static __device__ __forceinline__ float rint_(float x) { return rintf(x); }
+    static __device__ __forceinline__ float erfc_(float x) { return erfcf(x); }
+    static __device__ __forceinline__ float rsqrt_(float x) { return rsqrtf(x); }
+};
+
+/* Cell geometry in the kernel's precision. */
+template <typename T> struct CellT {
+    T a[9];    /* lattice rows */
+    T binv[9]; /* s_k = r . binv[k] */
+    T kappa;
+    T rcut2;
+};
+
+__device__ __forceinline__ double warp_sum(double v)
+{
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    return v;
+}
+
+/* Sum over the block in FP64; result valid in thread 0.  `red` holds >= 32 doubles. */
+__device__ __forceinline__ double block_sum(double v, double *red)
+{
+    v = warp_sum(v);
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    __syncthreads();
+    if (lane == 0) red[wid] = v;
+    __syncthreads();
+    if (wid == 0) {
+        const int nw = (blockDim.x + 31) >> 5;
+        v = lane < nw ? red[lane] : 0.0;
+        v = warp_sum(v);
+    }
+    return v;
+}
+
+/* Power table of one point for one direction: tab[n] = scale * exp(2 pi i s)^n, n = 0..nmax. */
+template <typename T>
+__device__ __forceinline__ void power_row(T s, T scale, int nmax, typename Num<T>::T2 *tab)
+{
+    typedef typename Num<T>::T2 T2;
+    s -= Num<T>::rint_(s); /* exact: the phase is periodic in s */
+    T sn, cs;
+    Num<T>::sincospi_(2 * s, &sn, &cs);
+    T2 e; e.x = scale; e.y = 0;
+    tab[0] = e;
+    for (int n = 1; n <= nmax; n++) {
+        T2 f;
+        f.x = e.x * cs - e.y * sn;
+        f.y = e.x * sn + e.y * cs;
+        e = f;
+        tab[n] = e;
+    }
+}
+
+/* ------------------------------------------------------------------------------------------ */
+/* [S1-S4] rho(G) and E_recip.  grid = n_walkers * n_slabs; each thread owns GPT members of G+. */
+
+template <typename T> struct RecipArgs {
+    const T *pos;      /* [W][DIM][npad] */
+    const T *q;        /* [n] */
+    int n, npad;
+    const short4 *gn;  /* [ngp] (n1,n2,n3,0) */
+    const T *w2;       /* [ngp] */
+    const T *ion_rho;  /* [ngp][2] or null */
+    int ngp, ngp_pad;
+    int nmax[3];
+    int off[3], rowlen; /* table row: direction k starts at off[k] */
+    T *rho_out;        /* [W][2][ngp_pad] or null */
+    double *partial;   /* [W][n_slabs] */
+    int n_slabs;
+    T binv[9];
+};
+
+constexpr int RECIP_THREADS = 256;
+constexpr int RECIP_GPT = 4;
+constexpr int RECIP_CHUNK = 32;
+
+template <typename T, int DIM>
+__global__ void __launch_bounds__(RECIP_THREADS) recip_kernel(RecipArgs<T> A)
+{
+    typedef typename Num<T>::T2 T2;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    T2 *tab = reinterpret_cast<T2 *>(smem_raw); /* [RECIP_CHUNK][rowlen] */
+    __shared__ double red[32];
+
+    const int w = blockIdx.x / A.n_slabs, slab = blockIdx.x - w * A.n_slabs, tid = threadIdx.x;
+    const T *pw = A.pos + (size_t)w * DIM * A.npad;
+
+    int gi[RECIP_GPT];
+    int i1[RECIP_GPT], i2[RECIP_GPT], i3[RECIP_GPT];
+    T sg2[RECIP_GPT], sg3[RECIP_GPT];
+    T2 acc[RECIP_GPT];
+#pragma unroll
+    for (int u = 0; u < RECIP_GPT; u++) {
+        int g = (slab * RECIP_GPT + u) * RECIP_THREADS + tid;
+        gi[u] = g < A.ngp ? g : -1;
+        short4 nn = A.gn[g < A.ngp ? g : 0];
+        i1[u] = A.off[0] + nn.x;
+        i2[u] = A.off[1] + (nn.y < 0 ? -nn.y : nn.y);
+        i3[u] = DIM == 3 ? A.off[2] + (nn.z < 0 ? -nn.z : nn.z) : 0;
+        sg2[u] = nn.y < 0 ? T(-1) : T(1);
+        sg3[u] = nn.z < 0 ? T(-1) : T(1);
+        acc[u].x = 0; acc[u].y = 0;
+    }
+
+    for (int base = 0; base < A.n; base += RECIP_CHUNK) {
+        const int cnt = min(RECIP_CHUNK, A.n - base);
+        __syncthreads();
+        /* [S1,S2] one (particle, direction) per thread */
+        for (int t = tid; t < cnt * DIM; t += RECIP_THREADS) {
+            const int p = t / DIM, k = t - p * DIM;
+            T s = 0;
+#pragma unroll
+            for (int x = 0; x < DIM; x++) s += pw[x * A.npad + base + p] * A.binv[3 * k + x];
+            power_row<T>(s, k == 0 ? A.q[base + p] : T(1), A.nmax[k], tab + p * A.rowlen + A.off[k]);
+        }
+        __syncthreads();
+        /* [S3] rho(G) += q e1^n1 e2^n2 e3^n3 */
+        for (int p = 0; p < cnt; p++) {
+            const T2 *row = tab + p * A.rowlen;
+#pragma unroll
+            for (int u = 0; u < RECIP_GPT; u++) {
+                T2 e1 = row[i1[u]], e2 = row[i2[u]];
+                e2.y *= sg2[u];
+                T2 e12;
+                e12.x = e1.x * e2.x - e1.y * e2.y;
+                e12.y = e1.x * e2.y + e1.y * e2.x;
+                if (DIM == 3) {
+                    T2 e3 = row[i3[u]];
+                    e3.y *= sg3[u];
+                    acc[u].x += e12.x * e3.x - e12.y * e3.y;
+                    acc[u].y += e12.x * e3.y + e12.y * e3.x;
+                } else {
+                    acc[u].x += e12.x;
+                    acc[u].y += e12.y;
+                }
+            }
+        }
+    }
+
+    /* [S4] */
+    double e = 0;
+#pragma unroll
+    for (int u = 0; u < RECIP_GPT; u++) {
+        if (gi[u] < 0) continue;
+        T re = acc[u].x, im = acc[u].y;
+        if (A.ion_rho) { re += A.ion_rho[2 * gi[u]]; im += A.ion_rho[2 * gi[u] + 1]; }
+        if (A.rho_out) {
+            T *ro = A.rho_out + (size_t)w * 2 * A.ngp_pad;
+            ro[gi[u]] = re;
+            ro[A.ngp_pad + gi[u]] = im;
+        }
+        e += (double)(A.w2[gi[u]] * (re * re + im * im));
+    }
+    e = block_sum(e, red);
+    if (tid == 0) A.partial[(size_t)w * A.n_slabs + slab] = e;
+}
+
+/* ------------------------------------------------------------------------------------------ */
+/* [S5] real-space pair sum.  grid = n_walkers * n_tiles. */
+
+template <typename T> struct RealArgs {
+    const T *pos; const T *q;
+    int n, npad;
+    const T *img; int nimg;          /* [nimg][3] */
+    const T *ion_pos; const T *ion_q; int n_ion; /* [n_ion][3] */
+    double *partial;                 /* [W][n_tiles] */
+    int n_tiles;
+    CellT<T> cell;
+};
+
+constexpr int REAL_THREADS = 256;
+
+/* minimum-image style reduction to fractional coordinates in [-1/2,1/2] (reading R10) */
+template <typename T, int DIM>
+__device__ __forceinline__ void reduce_disp(const CellT<T> &c, T *d)
+{
+    T f[3];
+#pragma unroll
+    for (int k = 0; k < DIM; k++) {
+        T s = 0;
+#pragma unroll
+        for (int x = 0; x < DIM; x++) s += d[x] * c.binv[3 * k + x];
+        f[k] = Num<T>::rint_(s);
+    }
+#pragma unroll
+    for (int x = 0; x < DIM; x++) {
+        T v = d[x];
+#pragma unroll
+        for (int k = 0; k < DIM; k++) v -= f[k] * c.a[3 * k + x];
+        d[x] = v;
+    }
+}
+
+/* psi(d) = sum_R erfc(kappa|d-R|)/|d-R| over images within the cut-off; d already reduced */
+template <typename T, int DIM>
+__device__ __forceinline__ T psi_images(const CellT<T> &c, const T *img, int nimg, const T *d)
+{
+    T s = 0;
+    for (int m = 0; m < nimg; m++) {
+        T r2 = 0;
+#pragma unroll
+        for (int x = 0; x < DIM; x++) { T v = d[x] - img[3 * m + x]; r2 += v * v; }
+        if (r2 < c.rcut2) {
+            T ri = Num<T>::rsqrt_(r2);
+            s += Num<T>::erfc_(c.kappa * (r2 * ri)) * ri;
+        }
+    }
+    return s;
+}
+
+template <typename T, int DIM>
+__global__ void __launch_bounds__(REAL_THREADS) real_kernel(RealArgs<T> A)
+{
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    T *sp = reinterpret_cast<T *>(smem_raw);        /* [DIM][n] positions, then [n] charges */
+    T *sq = sp + DIM * A.n;
+    T *simg = sq + A.n;                              /* [nimg][3] */
+    __shared__ double red[32];
+    const int w = blockIdx.x / A.n_tiles, tile = blockIdx.x - w * A.n_tiles, tid = threadIdx.x;
+    const T *pw = A.pos + (size_t)w * DIM * A.npad;
+    for (int t = tid; t < A.n; t += REAL_THREADS) {
+#pragma unroll
+        for (int x = 0; x < DIM; x++) sp[x * A.n + t] = pw[x * A.npad + t];
+        sq[t] = A.q[t];
+    }
+    for (int t = tid; t < 3 * A.nimg; t += REAL_THREADS) simg[t] = A.img[t];
+    __syncthreads();
+
+    const int n = A.n;
+    const int H = (n - 1) / 2;
+    const long long n_mm = (long long)n * H + ((n & 1) ? 0 : n / 2);
+    const long long total = n_mm + (long long)n * A.n_ion;
+    const long long per = (total + A.n_tiles - 1) / A.n_tiles;
+    const long long lo = per * tile, hi = min(total, lo + per);
+
+    double acc = 0;
+    for (long long p = lo + tid; p < hi; p += REAL_THREADS) {
+        T d[3] = {0, 0, 0};
+        T qq;
+        if (p < n_mm) {
+            int i, j;
+            if (p < (long long)n * H) { i = (int)(p % n); j = i + (int)(p / n) + 1; }
+            else { i = (int)(p - (long long)n * H); j = i + n / 2; }
+            if (j >= n) j -= n;
+#pragma unroll
+            for (int x = 0; x < DIM; x++) d[x] = sp[x * n + i] - sp[x * n + j];
+            qq = sq[i] * sq[j];
+        } else {
+            const long long e = p - n_mm;
+            const int i = (int)(e % n), I = (int)(e / n);
+#pragma unroll
+            for (int x = 0; x < DIM; x++) d[x] = sp[x * n + i] - A.ion_pos[3 * I + x];
+            qq = sq[i] * A.ion_q[I];
+        }
+        reduce_disp<T, DIM>(A.cell, d);
+        acc += (double)(qq * psi_images<T, DIM>(A.cell, simg, A.nimg, d));
+    }
+    acc = block_sum(acc, red);
+    if (tid == 0) A.partial[(size_t)w * A.n_tiles + tile] = acc;
+}
+
+/* ------------------------------------------------------------------------------------------ */
+/* [S6] combine.  One thread per walker. */
+
+struct CombineArgs {
+    const double *recip_partial; int n_recip;
+    const double *real_partial; int n_real;
+    const double *qsums;   /* [2] = sum q^2, sum q of the mobile particles */
+    double ion_q2, ion_qsum, ion_real;
+    double xi_r, self_coef, bg_coef;
+    double *energies; double *components; int n_walkers;
+};
+
+__global__ void combine_kernel(CombineArgs A)
+{
+    const int w = blockIdx.x * blockDim.x + threadIdx.x;
+    if (w >= A.n_walkers) return;
+    double er = 0, ep = 0;
+    for (int k = 0; k < A.n_recip; k++) er += A.recip_partial[(size_t)w * A.n_recip + k];
+    for (int k = 0; k < A.n_real; k++) ep += A.real_partial[(size_t)w * A.n_real + k];
+    const double q2 = A.qsums[0] + A.ion_q2, qs = A.qsums[1] + A.ion_qsum;
+    const double e_real = ep + A.ion_real + 0.5 * q2 * A.xi_r;
+    const double e_self = -A.self_coef * q2;
+    const double e_bg = -0.5 * A.bg_coef * qs * qs;
+    A.energies[w] = er + e_real + e_self + e_bg;
+    if (A.components) {
+        A.components[4 * w + 0] = er;
+        A.components[4 * w + 1] = e_real;
+        A.components[4 * w + 2] = e_self;
+        A.components[4 * w + 3] = e_bg;
+    }
+}
+
+template <typename T>
+__global__ void charge_sums_kernel(const T *q, int n, double *out)
+{
+    __shared__ double red[32];
+    double s2 = 0, s1 = 0;
+    for (int i = threadIdx.x; i < n; i += blockDim.x) { double v = (double)q[i]; s2 += v * v; s1 += v; }
+    s2 = block_sum(s2, red);
+    s1 = block_sum(s1, red);
+    if (threadIdx.x == 0) { out[0] = s2; out[1] = s1; }
+}
+
+/* ------------------------------------------------------------------------------------------ */
+/* [S7] single-particle move.  grid = n_moves, one CTA per move. */
+
+template <typename T> struct MoveArgs {
+    T *pos;            /* stored [W][DIM][npad] */
+    const T *q;        /* stored [n] */
+    T *rho;            /* stored [W][2][ngp_pad] */
+    int n, npad, n_walkers;
+    const short4 *gn; const T *w2; int ngp, ngp_pad;
+    int nmax[3]; int off[3], rowlen;
+    const T *img; int nimg;
+    const T *ion_pos; const T *ion_q; int n_ion;
+    const int *walker; const int *electron; const T *new_r; /* [n_moves], [n_moves], [n_moves][DIM] */
+    int commit;
+    double *delta_e;
+    CellT<T> cell;
+};
+
+constexpr int MOVE_THREADS = 256;
+
+template <typename T, int DIM>
+__global__ void __launch_bounds__(MOVE_THREADS) move_kernel(MoveArgs<T> A)
+{
+    typedef typename Num<T>::T2 T2;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    T2 *tab = reinterpret_cast<T2 *>(smem_raw); /* [2][rowlen]: old, new */
+    T *simg = reinterpret_cast<T *>(tab + 2 * A.rowlen);
+    __shared__ double red[32];
+    const int m = blockIdx.x, tid = threadIdx.x;
+    const int w = A.walker[m], k = A.electron[m];
+    if (w < 0 || w >= A.n_walkers || k < 0 || k >= A.n) {
+        if (tid == 0) A.delta_e[m] = __longlong_as_double(0x7ff8000000000000LL);
+        return;
+    }
+    T *pw = A.pos + (size_t)w * DIM * A.npad;
+    T r_old[3] = {0, 0, 0}, r_new[3] = {0, 0, 0};
+#pragma unroll
+    for (int x = 0; x < DIM; x++) { r_old[x] = pw[x * A.npad + k]; r_new[x] = A.new_r[(size_t)m * DIM + x]; }
+    const T qk = A.q[k];
+
+    /* [S7a] power tables of the two points */
+    if (tid < 2 * DIM) {
+        const int which = tid / DIM, d = tid - which * DIM;
+        const T *r = which ? r_new : r_old;
+        T s = 0;
+#pragma unroll
+        for (int x = 0; x < DIM; x++) s += r[x] * A.cell.binv[3 * d + x];
+        power_row<T>(s, T(1), A.nmax[d], tab + which * A.rowlen + A.off[d]);
+    }
+    for (int t = tid; t < 3 * A.nimg; t += MOVE_THREADS) simg[t] = A.img[t];
+    __syncthreads();
+
+    /* [S7b] Delta E_recip and the patch of rho(G) */
+    T *rr = A.rho + (size_t)w * 2 * A.ngp_pad;
+    double acc = 0;
+    for (int g = tid; g < A.ngp; g += MOVE_THREADS) {
+        const short4 nn = A.gn[g];
+        T2 ph[2];
+#pragma unroll
+        for (int which = 0; which < 2; which++) {
+            const T2 *row = tab + which * A.rowlen;
+            T2 e1 = row[A.off[0] + nn.x];
+            T2 e2 = row[A.off[1] + (nn.y < 0 ? -nn.y : nn.y)];
+            if (nn.y < 0) e2.y = -e2.y;
+            T2 e;
+            e.x = e1.x * e2.x - e1.y * e2.y;
+            e.y = e1.x * e2.y + e1.y * e2.x;
+            if (DIM == 3) {
+                T2 e3 = row[A.off[2] + (nn.z < 0 ? -nn.z : nn.z)];
+                if (nn.z < 0) e3.y = -e3.y;
+                T2 f;
+                f.x = e.x * e3.x - e.y * e3.y;
+                f.y = e.x * e3.y + e.y * e3.x;
+                e = f;
+            }
+            ph[which] = e;
+        }
+        const T dr = ph[1].x - ph[0].x, di = ph[1].y - ph[0].y;
+        const T re = rr[g], im = rr[A.ngp_pad + g];
+        acc += (double)(A.w2[g] * (2 * qk * (re * dr + im * di) + qk * qk * (dr * dr + di * di)));
+        if (A.commit) { rr[g] = re + qk * dr; rr[A.ngp_pad + g] = im + qk * di; }
+    }
+
+    /* [S7c] Delta E_real = q_k sum_{j != k} q_j [psi(r'-r_j) - psi(r-r_j)] */
+    double accr = 0;
+    for (int j = tid; j < A.n + A.n_ion; j += MOVE_THREADS) {
+        if (j == k) continue;
+        T rj[3] = {0, 0, 0};
+        T qj;
+        if (j < A.n) {
+#pragma unroll
+            for (int x = 0; x < DIM; x++) rj[x] = pw[x * A.npad + j];
+            qj = A.q[j];
+        } else {
+#pragma unroll
+            for (int x = 0; x < DIM; x++) rj[x] = A.ion_pos[3 * (j - A.n) + x];
+            qj = A.ion_q[j - A.n];
+        }
+        T dn[3], dold[3];
+#pragma unroll
+        for (int x = 0; x < 3; x++) { dn[x] = r_new[x] - rj[x]; dold[x] = r_old[x] - rj[x]; }
+        reduce_disp<T, DIM>(A.cell, dn);
+        reduce_disp<T, DIM>(A.cell, dold);
+        accr += (double)(qj * (psi_images<T, DIM>(A.cell, simg, A.nimg, dn) -
+                               psi_images<T, DIM>(A.cell, simg, A.nimg, dold)));
+    }
+    acc += (double)qk * accr;
+    acc = block_sum(acc, red); /* its barriers also order every read of r_old before the commit */
+    if (tid == 0) {
+        A.delta_e[m] = acc;
+        if (A.commit) {
+#pragma unroll
+            for (int x = 0; x < DIM; x++) pw[x * A.npad + k] = r_new[x];
+        }
+    }
+}
+
+/* ------------------------------------------------------------------------------------------ */
+/* FMA-pipe probe: 8 independent dependent chains per thread. */
+template <typename T>
+__global__ void __launch_bounds__(256) fma_probe_kernel(int iters, T a, T b, T *sink)
+{
+    T x0 = threadIdx.x, x1 = x0 + 1, x2 = x0 + 2, x3 = x0 + 3, x4 = x0 + 4, x5 = x0 + 5, x6 = x0 + 6, x7 = x0 + 7;
+    for (int i = 0; i < iters; i++) {
+#pragma unroll
+        for (int u = 0; u < 8; u++) {
+            x0 = x0 * a + b; x1 = x1 * a + b; x2 = x2 * a + b; x3 = x3 * a + b;
+            x4 = x4 * a + b; x5 = x5 * a + b; x6 = x6 * a + b; x7 = x7 * a + b;
+        }
+    }
+    T s = x0 + x1 + x2 + x3 + x4 + x5 + x6 + x7;
+    if (s == T(123456789)) sink[0] = s;
+}
+
+} // namespace ewald

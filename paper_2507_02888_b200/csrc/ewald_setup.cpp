@@ -1,0 +1,224 @@
+/* ewald_setup.cpp -- host-side table construction for the B200 Ewald library.
+ *
+ * Everything walker-independent in Eqs. 2-4 is evaluated here once, in
+ * long double, and handed to the device rounded to FP64 / FP32 (the Ewald lookup
+ * tables are "numerically sensitive and are always performed using DP"; "much of the
+ * data required can be moved to the GPU once, at the outset").
+ */
+#include <cmath>
+#include <cstring>
+
+#include "ewald_internal.h"
+
+namespace ewald {
+
+typedef long double real;
+static const real kPi = 3.141592653589793238462643383279502884L;
+
+static real dot3(const real *x, const real *y) { return x[0] * y[0] + x[1] * y[1] + x[2] * y[2]; }
+static real len3(const real *x) { return sqrtl(dot3(x, x)); }
+
+/* w(G): E_recip = sum over the full sphere of w(G) |rho(G)|^2.
+ * 3D: Eq. 3's (4pi/Omega) exp(-G^2/4gamma)/G^2 summed over ordered pairs -> 2pi/Omega.
+ * 2D (reading R2): (pi/A) erfc(G/2kappa)/G. */
+static real weight(int dim, real volume, real kappa, real g2)
+{
+    if (dim == 3) return 2 * kPi / volume * expl(-g2 / (4 * kappa * kappa)) / g2;
+    real g = sqrtl(g2);
+    return kPi / volume * erfcl(g / (2 * kappa)) / g;
+}
+
+ewald_status build_tables(int dim, const double *cell, double kappa_d, double g_cutoff,
+                          double r_cutoff, HostTables *t, std::string *err)
+{
+    if (dim != 2 && dim != 3) { *err = "dim must be 2 or 3"; return EWALD_EINVAL; }
+    if (!cell) { *err = "cell is null"; return EWALD_EINVAL; }
+    if (!(kappa_d > 0) || !std::isfinite(kappa_d)) { *err = "gamma (kappa) must be > 0"; return EWALD_ERANGE; }
+    if (!(g_cutoff > 0) || !std::isfinite(g_cutoff)) { *err = "g_cutoff must be > 0"; return EWALD_ERANGE; }
+    if (r_cutoff < 0 || !std::isfinite(r_cutoff)) { *err = "r_cutoff must be >= 0"; return EWALD_ERANGE; }
+    for (int i = 0; i < 9; i++)
+        if (!std::isfinite(cell[i])) { *err = "cell has a non-finite entry"; return EWALD_EINVAL; }
+
+    real a[3][3] = {{0, 0, 0}, {0, 0, 0}, {0, 0, 1}};
+    for (int i = 0; i < dim; i++)
+        for (int j = 0; j < dim; j++) a[i][j] = cell[3 * i + j];
+
+    /* reciprocal rows b_k with a_i . b_k = 2pi delta_ik, via cross products */
+    real c[3][3];
+    for (int k = 0; k < 3; k++) {
+        const real *u = a[(k + 1) % 3], *v = a[(k + 2) % 3];
+        c[k][0] = u[1] * v[2] - u[2] * v[1];
+        c[k][1] = u[2] * v[0] - u[0] * v[2];
+        c[k][2] = u[0] * v[1] - u[1] * v[0];
+    }
+    real det = dot3(a[0], c[0]);
+    real scale = len3(a[0]) * len3(a[1]) * len3(a[2]);
+    if (!(fabsl(det) > 1e-14L * scale) || !std::isfinite((double)det)) {
+        *err = "cell is singular";
+        return EWALD_ESINGULAR;
+    }
+    real b[3][3];
+    for (int k = 0; k < 3; k++)
+        for (int x = 0; x < 3; x++) b[k][x] = 2 * kPi * c[k][x] / det;
+
+    const real kappa = kappa_d;
+    t->dim = dim;
+    t->kappa = kappa_d;
+    t->g_cutoff = g_cutoff;
+    t->volume = (double)fabsl(det);
+    if (r_cutoff == 0) r_cutoff = (double)(sqrtl(-logl(1e-17L)) / kappa);
+    t->r_cutoff = r_cutoff;
+    bool ortho = true;
+    for (int i = 0; i < 3; i++)
+        for (int j = 0; j < 3; j++) {
+            t->a[3 * i + j] = (double)a[i][j];
+            t->binv[3 * i + j] = (double)(b[i][j] / (2 * kPi));
+            if (i != j && a[i][j] != 0) ortho = false;
+        }
+    t->orthogonal = ortho;
+
+    /* ---- half set G+ (first non-zero integer component positive), lexicographic ---- */
+    const real g2max = (real)g_cutoff * g_cutoff * (1 + 1e-12L); /* reading R6 */
+    int lim[3];
+    for (int k = 0; k < 3; k++) {
+        /* n_k = G . a_k / 2pi  =>  |n_k| <= |G| |a_k| / 2pi */
+        lim[k] = k < dim ? (int)floorl(sqrtl(g2max) * len3(a[k]) / (2 * kPi) + 1e-9L) : 0;
+        if (lim[k] > 1023) { *err = "G index range exceeds 1023"; return EWALD_ERANGE; }
+    }
+    t->g_n.clear();
+    t->g_w2.clear();
+    t->n_max[0] = t->n_max[1] = t->n_max[2] = 0;
+    for (int n1 = 0; n1 <= lim[0]; n1++)
+        for (int n2 = -lim[1]; n2 <= lim[1]; n2++)
+            for (int n3 = -lim[2]; n3 <= lim[2]; n3++) {
+                bool plus = n1 > 0 || (n1 == 0 && (n2 > 0 || (n2 == 0 && n3 > 0)));
+                if (!plus) continue;
+                real g[3];
+                for (int x = 0; x < 3; x++) g[x] = n1 * b[0][x] + n2 * b[1][x] + n3 * b[2][x];
+                real g2 = dot3(g, g);
+                if (g2 > g2max) continue;
+                t->g_n.push_back(n1); t->g_n.push_back(n2); t->g_n.push_back(n3);
+                t->g_w2.push_back((double)(2 * weight(dim, fabsl(det), kappa, g2)));
+                if (n1 > t->n_max[0]) t->n_max[0] = n1;
+                if (abs(n2) > t->n_max[1]) t->n_max[1] = abs(n2);
+                if (abs(n3) > t->n_max[2]) t->n_max[2] = abs(n3);
+            }
+    if (t->g_w2.empty()) { *err = "g_cutoff admits no reciprocal vector"; return EWALD_ERANGE; }
+
+    /* ---- lattice images that can come within r_cutoff of a reduced displacement ----
+     * A displacement reduced to fractional coordinates |s_k| <= 1/2 lies in the parallelepiped P.
+     * Image R = m.a is needed iff dist(R, P) < r_cutoff.  Lower bounds on that distance:
+     *   planes: (|m_k| - 1/2) h_k with h_k = 2pi/|b_k| (spacing of the a-planes normal to b_k);
+     *   orthogonal cells: root-sum-square of the plane bounds;  any cell: |R| - reach.          */
+    const real rc = r_cutoff;
+    real reach = 0, h[3];
+    for (int k = 0; k < dim; k++) reach += len3(a[k]) / 2;
+    for (int k = 0; k < 3; k++) h[k] = 2 * kPi / len3(b[k]);
+    int mlim[3];
+    for (int k = 0; k < 3; k++) mlim[k] = k < dim ? (int)floorl(rc / h[k] + 0.5L + 1e-9L) : 0;
+    t->img.clear();
+    t->img_m.clear();
+    real xi = 0;
+    for (int m1 = -mlim[0]; m1 <= mlim[0]; m1++)
+        for (int m2 = -mlim[1]; m2 <= mlim[1]; m2++)
+            for (int m3 = -mlim[2]; m3 <= mlim[2]; m3++) {
+                int m[3] = {m1, m2, m3};
+                real R[3];
+                for (int x = 0; x < 3; x++) R[x] = m1 * a[0][x] + m2 * a[1][x] + m3 * a[2][x];
+                real rl = len3(R);
+                if ((m1 || m2 || m3) && rl < rc) xi += erfcl(kappa * rl) / rl; /* Eq. 4 real sum */
+                real lb_max = 0, lb_ss = 0;
+                for (int k = 0; k < dim; k++) {
+                    real d = (fabsl((real)m[k]) - 0.5L) * h[k];
+                    if (d < 0) d = 0;
+                    if (d > lb_max) lb_max = d;
+                    lb_ss += d * d;
+                }
+                real lb = ortho ? sqrtl(lb_ss) : lb_max;
+                if (rl - reach > lb) lb = rl - reach;
+                if (lb >= rc * (1 + 1e-12L)) continue;
+                for (int x = 0; x < 3; x++) { t->img.push_back((double)R[x]); t->img_m.push_back(m[x]); }
+            }
+    t->xi_r = (double)xi;
+    t->self_coef = (double)(kappa / sqrtl(kPi));
+    real bgc = dim == 3 ? kPi / (fabsl(det) * kappa * kappa) : 2 * sqrtl(kPi) / (fabsl(det) * kappa);
+    t->bg_coef = (double)bgc;
+    real wsum = 0; /* sum over the full sphere of 2 w(G) = the reciprocal sum of Eq. 4 */
+    for (size_t k = 0; k < t->g_w2.size(); k++) wsum += 2 * (real)t->g_w2[k];
+    t->v_m = (double)(wsum + xi - 2 * kappa / sqrtl(kPi) - bgc);
+
+    t->n_ion = 0;
+    t->ion_pos.clear(); t->ion_q.clear(); t->ion_rho.clear();
+    t->ion_q2 = t->ion_qsum = t->ion_real = 0;
+    return EWALD_OK;
+}
+
+ewald_status build_fixed_charges(HostTables *t, int n_ion, const double *pos, const double *q,
+                                 std::string *err)
+{
+    if (n_ion < 0 || (n_ion > 0 && (!pos || !q))) { *err = "bad fixed-charge arguments"; return EWALD_EINVAL; }
+    const int dim = t->dim;
+    const size_t ngp = t->g_w2.size();
+    t->n_ion = n_ion;
+    t->ion_pos.assign((size_t)3 * n_ion, 0.0);
+    t->ion_q.assign(q, q + n_ion);
+    t->ion_rho.assign(2 * ngp, 0.0);
+    for (int i = 0; i < n_ion; i++)
+        for (int x = 0; x < dim; x++) {
+            if (!std::isfinite(pos[(size_t)i * dim + x])) { *err = "non-finite ion position"; return EWALD_EINVAL; }
+            t->ion_pos[3 * i + x] = pos[(size_t)i * dim + x];
+        }
+    real q2 = 0, qs = 0;
+    for (int i = 0; i < n_ion; i++) { q2 += (real)q[i] * q[i]; qs += q[i]; }
+    t->ion_q2 = (double)q2;
+    t->ion_qsum = (double)qs;
+
+    /* rho_ion(G) = sum_I q_I exp(2 pi i n.s_I) with s = fractional coordinates */
+    std::vector<real> s((size_t)3 * n_ion);
+    for (int i = 0; i < n_ion; i++)
+        for (int k = 0; k < 3; k++) {
+            real v = 0;
+            for (int x = 0; x < 3; x++) v += (real)t->ion_pos[3 * i + x] * (real)t->binv[3 * k + x];
+            s[3 * i + k] = v - nearbyintl(v);
+        }
+    for (size_t g = 0; g < ngp; g++) {
+        real re = 0, im = 0;
+        for (int i = 0; i < n_ion; i++) {
+            real ph = 0;
+            for (int k = 0; k < 3; k++) ph += t->g_n[3 * g + k] * s[3 * i + k];
+            ph -= nearbyintl(ph);
+            re += q[i] * cosl(2 * kPi * ph);
+            im += q[i] * sinl(2 * kPi * ph);
+        }
+        t->ion_rho[2 * g] = (double)re;
+        t->ion_rho[2 * g + 1] = (double)im;
+    }
+
+    /* sum_{I<J} q_I q_J psi(r_I - r_J): the real-space part of Eq. 3 between fixed charges */
+    const real rc2 = (real)t->r_cutoff * t->r_cutoff, kappa = t->kappa;
+    const size_t nimg = t->img.size() / 3;
+    real e = 0;
+    for (int i = 0; i < n_ion; i++)
+        for (int j = i + 1; j < n_ion; j++) {
+            real d[3], f[3];
+            for (int x = 0; x < 3; x++) d[x] = (real)t->ion_pos[3 * i + x] - (real)t->ion_pos[3 * j + x];
+            for (int k = 0; k < 3; k++) {
+                f[k] = 0;
+                for (int x = 0; x < 3; x++) f[k] += d[x] * (real)t->binv[3 * k + x];
+                f[k] = k < dim ? nearbyintl(f[k]) : 0;
+            }
+            for (int x = 0; x < 3; x++)
+                d[x] -= f[0] * t->a[x] + f[1] * t->a[3 + x] + f[2] * t->a[6 + x];
+            real psi = 0;
+            for (size_t m = 0; m < nimg; m++) {
+                real x = d[0] - t->img[3 * m], y = d[1] - t->img[3 * m + 1], z = d[2] - t->img[3 * m + 2];
+                real r2 = x * x + y * y + z * z;
+                if (r2 < rc2) { real r = sqrtl(r2); psi += erfcl(kappa * r) / r; }
+            }
+            e += (real)q[i] * q[j] * psi;
+        }
+    t->ion_real = (double)e;
+    return EWALD_OK;
+}
+
+} // namespace ewald

@@ -1,0 +1,99 @@
+"""CPU-side checks of the boundary: the C-ABI library builds, loads and exports every symbol that
+include/ewald.h declares; the host-only setup tables reproduce the closed forms of Eq. 4
+(PAPER.md:120); argument validation.  No compute call is made (there is no GPU here)."""
+import ctypes
+import math
+import os
+import re
+
+import numpy as np
+import pytest
+
+from paper_2507_02888_b200 import ewald as E
+from paper_2507_02888_b200 import workloads
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def _declared_symbols():
+    text = open(os.path.join(ROOT, "include", "ewald.h")).read()
+    text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
+    return sorted(set(re.findall(r"\b(ewald_[a-z0-9_]+)\s*\(", text)))
+
+
+def test_header_symbols_all_exported():
+    lib = ctypes.CDLL(E.load_library()._name)
+    declared = _declared_symbols()
+    assert len(declared) >= 20
+    for name in declared:
+        assert hasattr(lib, name), "library does not export %s" % name
+    assert sorted(E.SYMBOLS) == declared, "binding's symbol list differs from the header"
+
+
+def test_binding_has_same_names():
+    for name in _declared_symbols():
+        if name in ("ewald_last_error", "ewald_destroy"):
+            continue
+        assert hasattr(E, name), "python binding lacks %s" % name
+
+
+def test_version_and_padding():
+    assert "sm_100a" in E.ewald_version()
+    assert [E.ewald_padded_n(n) for n in (0, 1, 4, 5, 250, 1000)] == [0, 4, 4, 8, 252, 1000]
+
+
+def test_setup_summary_counts_match_config_table():
+    # SURVEY.md 8(d) / DESIGN.md: full-sphere G counts of the five configs (reading R5)
+    want = {1: (924, [6, 6, 6]), 2: (2006, [7, 7, 7]), 3: (1516, [22, 22, 0]), 4: (3070, [9, 9, 9]),
+            5: (3958, [9, 9, 9])}
+    for idx, (ng, nmax) in want.items():
+        w = workloads.config(idx)
+        s = E.ewald_setup_summary(w.dim, w.cell, w.kappa, w.g_cutoff, w.r_cutoff)
+        assert s["num_g"] == ng and s["n_max"] == nmax
+        assert 1 <= s["num_images"] <= 125
+
+
+def test_setup_madelung_constant_closed_forms(golden):
+    # v_M L of a cubic / square cell is a pure number: -2.837297... (3D), 4 zeta(1/2) beta(1/2) (2D)
+    for idx in (1, 2, 4, 5):
+        w = workloads.config(idx)
+        s = E.ewald_setup_summary(w.dim, w.cell, w.kappa, w.g_cutoff, w.r_cutoff)
+        assert abs(s["v_m"] * w.L - golden["vm_L_sc_3d"]) < 2e-13
+    w = workloads.config(3)
+    s = E.ewald_setup_summary(w.dim, w.cell, w.kappa, w.g_cutoff, w.r_cutoff)
+    assert abs(s["v_m"] * w.L - golden["vm_L_square_2d"]) < 2e-13
+
+
+def test_setup_v_m_independent_of_kappa_noncubic():
+    cell = np.array([[5.0, 0.3, 0.1], [0.4, 6.0, -0.2], [0.2, 0.5, 7.0]])
+    vals = []
+    for kappa in (0.5, 0.65, 0.8):
+        x = math.sqrt(-math.log(1e-17))
+        s = E.ewald_setup_summary(3, cell, kappa, 2 * kappa * x, x / kappa)
+        vals.append(s["v_m"])
+    assert max(vals) - min(vals) < 1e-13 * abs(vals[0])
+
+
+def test_setup_argument_errors():
+    cell = np.eye(3) * 4.0
+    for args, status in (((4, cell, 1.0, 3.0), 1), ((3, cell, -1.0, 3.0), 3), ((3, cell, 1.0, 0.0), 3),
+                         ((3, np.zeros((3, 3)), 1.0, 3.0), 2), ((3, cell, 1.0, 1e-3), 3)):
+        with pytest.raises(E.EwaldError) as ei:
+            E.ewald_setup_summary(*args)
+        assert ei.value.status == status
+
+
+def test_setup_without_gpu_fails_loudly():
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("a GPU is present")
+    with pytest.raises(E.EwaldError) as ei:
+        E.ewald_setup(3, np.eye(3) * 4.0, 1.0, 3.0)
+    assert ei.value.status == 5  # EWALD_ECUDA: no fallback path
+
+
+def test_to_soa_layout():
+    pos = np.arange(2 * 5 * 3, dtype=np.float64).reshape(2, 5, 3)
+    soa = E.to_soa(pos)
+    assert soa.shape == (2, 3, 8)
+    assert np.array_equal(soa[1, 2, :5], pos[1, :, 2]) and np.all(soa[:, :, 5:] == 0)

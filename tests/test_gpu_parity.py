@@ -1,0 +1,328 @@
+"""GPU parity: the CUDA path (through the C ABI) against the CPU oracle, element by element, on the same
+seeded inputs (paper_2507_02888_b200.workloads).  Tolerances are BASELINE.json's: 1e-11 relative
+per walker (FP64), 2e-5 (FP32); Delta E per reading R12: tol * max(|dE|, rms dE of the step).
+"""
+import math
+
+import numpy as np
+import pytest
+
+from oracle import ewald_ref as ref
+from paper_2507_02888_b200 import ewald as E
+from paper_2507_02888_b200 import workloads
+
+pytestmark = pytest.mark.gpu
+
+TOL64, TOL32 = 1e-11, 2e-5
+
+
+@pytest.fixture(scope="module")
+def torch_cuda():
+    import torch
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    return torch
+
+
+def _ctx(w, **kw):
+    ctx = E.ewald_setup(w.dim, w.cell, w.kappa, w.g_cutoff, w.r_cutoff, **kw)
+    if w.ion_pos is not None:
+        E.ewald_set_fixed_charges(ctx, w.ion_pos, w.ion_q)
+    return ctx
+
+
+def _gpu_energy(torch, ctx, pos, q, dtype, components=True):
+    npdt = np.float64 if dtype == "f64" else np.float32
+    W, n, _ = pos.shape
+    d_pos = torch.from_numpy(E.to_soa(pos, npdt)).cuda()
+    d_q = torch.from_numpy(np.asarray(q, dtype=npdt)).cuda()
+    d_e = torch.full((W,), float("nan"), dtype=torch.float64, device="cuda")
+    d_c = torch.full((W, 4), float("nan"), dtype=torch.float64, device="cuda") if components else None
+    E.ewald_energy_batch(ctx, n, d_pos, d_q, d_e, d_c)
+    torch.cuda.synchronize()
+    return d_e.cpu().numpy(), (d_c.cpu().numpy() if components else None)
+
+
+def _oracle_energy(w, pos):
+    return ref.energy_batch(w.dim, w.cell, w.kappa, w.g_cutoff, w.r_cutoff, pos, w.charges,
+                            w.ion_pos, w.ion_q)
+
+
+def _assert_energy(e, c, e_ref, c_ref, tol):
+    assert np.all(np.isfinite(e))
+    rel = np.abs(e - e_ref) / np.abs(e_ref)
+    assert rel.max() <= tol, "max relative energy error %.3e > %.1e" % (rel.max(), tol)
+    if c is not None:
+        scale = np.maximum(np.abs(c_ref), np.abs(e_ref)[:, None])
+        assert (np.abs(c - c_ref) / scale).max() <= tol
+        assert np.allclose(c.sum(axis=1), e, rtol=1e-13, atol=0)
+
+
+# walkers per config for the element-by-element comparison (oracle: seconds on 8 cores)
+N_WALKERS = {1: 8, 2: 12, 3: 12, 4: 6}
+
+
+@pytest.mark.parametrize("idx", [1, 2, 3, 4])
+def test_energy_fp64_matches_oracle(torch_cuda, idx):
+    w = workloads.config(idx)
+    pos = w.positions(N_WALKERS[idx])
+    e_ref, c_ref = _oracle_energy(w, pos)
+    ctx = _ctx(w)
+    e, c = _gpu_energy(torch_cuda, ctx, pos, w.charges, "f64")
+    _assert_energy(e, c, e_ref, c_ref, TOL64)
+    assert E.ewald_num_g(ctx) == ref.num_g(w.dim, w.cell, w.g_cutoff)
+
+
+@pytest.mark.parametrize("idx", [2, 3])
+def test_energy_fp32_matches_oracle(torch_cuda, idx):
+    w = workloads.config(idx)
+    pos = w.positions(N_WALKERS[idx])
+    e_ref, c_ref = _oracle_energy(w, pos)  # oracle on the unrounded FP64 inputs (reading R16)
+    ctx = _ctx(w)
+    e, c = _gpu_energy(torch_cuda, ctx, pos, w.charges, "f32")
+    _assert_energy(e, None, e_ref, None, TOL32)
+    scale = np.maximum(np.abs(c_ref), np.abs(e_ref)[:, None])
+    assert (np.abs(c - c_ref) / scale).max() <= TOL32
+
+
+def test_fp32_also_passes_on_configs_1_and_4(torch_cuda):
+    for idx in (1, 4):
+        w = workloads.config(idx)
+        pos = w.positions(4)
+        e_ref, _ = _oracle_energy(w, pos)
+        e, _ = _gpu_energy(torch_cuda, _ctx(w), pos, w.charges, "f32", components=False)
+        assert (np.abs(e - e_ref) / np.abs(e_ref)).max() <= TOL32
+
+
+def test_g_list_and_rho_match_oracle(torch_cuda):
+    torch = torch_cuda
+    for idx, tol in ((2, 1e-12), (3, 1e-12), (4, 1e-12)):
+        w = workloads.config(idx)
+        ctx = _ctx(w)
+        g = E.ewald_get_g(ctx)
+        assert np.array_equal(g, ref.gplus(w.dim, w.cell, w.g_cutoff))
+        pos = w.positions(3)
+        d_pos = torch.from_numpy(E.to_soa(pos)).cuda()
+        d_q = torch.from_numpy(w.charges).cuda()
+        E.ewald_load_walkers(ctx, w.n, d_pos, d_q)
+        for k in (0, 2):
+            pts, q = pos[k], w.charges
+            if w.ion_pos is not None:
+                pts, q = np.concatenate([pts, w.ion_pos]), np.concatenate([q, w.ion_q])
+            rho_ref = ref.rho(w.dim, w.cell, w.g_cutoff, pts, q)
+            rho = E.ewald_get_rho(ctx, k)
+            assert np.abs(rho - rho_ref).max() <= tol * np.abs(q).sum()
+            assert np.allclose(E.ewald_get_positions(ctx, k, w.n), pos[k], rtol=0, atol=0)
+
+
+def _random_cell(rng, dim, scale=6.0):
+    a = np.eye(dim) * scale + rng.uniform(-0.15, 0.15, (dim, dim)) * scale
+    return a
+
+
+@pytest.mark.parametrize("dim", [2, 3])
+def test_small_general_cells_ragged_sizes(torch_cuda, dim):
+    """Non-orthogonal cells, mixed charges (charged and neutral), N = 1, 2, 3, 5, 7, 33 (pad tails,
+    fewer particles than a tile), auto r_cutoff."""
+    rng = np.random.default_rng(7 + dim)
+    for n in (1, 2, 3, 5, 7, 33):
+        cell = _random_cell(rng, dim)
+        kappa = 0.9
+        gc, rc = ref.auto_cutoffs(dim, cell, kappa, 1e-17)
+        q = rng.choice([-1.0, 1.0, 2.0, -0.5], size=n)
+        frac = rng.random((3, n, dim)) * 1.6 - 0.3  # some positions outside the cell (reading R9)
+        pos = frac @ cell
+        e_ref, c_ref = ref.energy_batch(dim, cell, kappa, gc, rc, pos, q)
+        ctx = E.ewald_setup(dim, cell, kappa, gc)  # r_cutoff = 0: automatic
+        assert abs(E.ewald_r_cutoff(ctx) - rc) < 1e-12
+        e, c = _gpu_energy(torch_cuda, ctx, pos, q, "f64")
+        # tiny neutral cells can have |E| << terms: compare against the largest component
+        scale = np.abs(c_ref).max(axis=1)
+        assert (np.abs(e - e_ref) / scale).max() <= TOL64
+        assert (np.abs(c - c_ref) / scale[:, None]).max() <= TOL64
+
+
+def test_fixed_charges_equal_mobile_charges(torch_cuda):
+    """Ions passed as fixed charges give the same energy as the same ions passed as mobile particles."""
+    rng = np.random.default_rng(11)
+    cell = _random_cell(rng, 3)
+    kappa = 0.8
+    gc, rc = ref.auto_cutoffs(3, cell, kappa, 1e-17)
+    n, ni = 6, 3
+    pos = rng.random((4, n, 3)) @ cell
+    ion = rng.random((ni, 3)) @ cell
+    q, qi = -np.ones(n), np.array([2.0, 3.0, 1.0])
+    ctx = E.ewald_setup(3, cell, kappa, gc, rc)
+    E.ewald_set_fixed_charges(ctx, ion, qi)
+    e1, c1 = _gpu_energy(torch_cuda, ctx, pos, q, "f64")
+    ctx2 = E.ewald_setup(3, cell, kappa, gc, rc)
+    allpos = np.concatenate([pos, np.broadcast_to(ion, (4, ni, 3))], axis=1)
+    e2, c2 = _gpu_energy(torch_cuda, ctx2, allpos, np.concatenate([q, qi]), "f64")
+    e_ref, c_ref = ref.energy_batch(3, cell, kappa, gc, rc, pos, q, ion, qi)
+    scale = np.abs(c_ref).max(axis=1)
+    assert (np.abs(e1 - e_ref) / scale).max() <= TOL64 and (np.abs(e2 - e_ref) / scale).max() <= TOL64
+    _, _, e_fixed = E.ewald_get_constants(ctx)
+    e_ion_ref, _ = ref.energy_batch(3, cell, kappa, gc, rc, ion[None], qi)
+    assert abs(e_fixed - e_ion_ref[0]) <= 1e-12 * abs(e_ion_ref[0])
+
+
+def test_empty_batch_and_host_entry_point(torch_cuda):
+    torch = torch_cuda
+    w = workloads.config(1)
+    ctx = _ctx(w)
+    pos = w.positions(5)
+    d_q = torch.from_numpy(w.charges).cuda()
+    d_e = torch.zeros(0, dtype=torch.float64, device="cuda")
+    E.ewald_energy_batch(ctx, w.n, torch.zeros((0, 3, E.ewald_padded_n(w.n)), dtype=torch.float64, device="cuda"),
+                         d_q, d_e)
+    e, c = _gpu_energy(torch, ctx, pos, w.charges, "f64")
+    eh, ch = np.zeros(5), np.zeros((5, 4))
+    E.ewald_energy_batch_host(ctx, w.n, E.to_soa(pos), w.charges.copy(), eh, ch)
+    assert np.array_equal(e, eh) and np.array_equal(c, ch)  # same kernels, same order: bit-identical
+
+
+def _move_inputs(w, n_walkers, n_steps):
+    pos0 = w.positions(n_walkers)
+    electron, disp = w.moves(n_walkers, n_steps)
+    cur = pos0.copy()
+    new_r = np.zeros((n_steps, n_walkers, w.dim))
+    for s in range(n_steps):  # absolute targets: current position of that electron + Gaussian step
+        idx = electron[s]
+        new_r[s] = cur[np.arange(n_walkers), idx] + disp[s]
+        cur[np.arange(n_walkers), idx] = new_r[s]
+    return pos0, electron, new_r, cur
+
+
+def _run_moves(torch, ctx, w, pos0, electron, new_r, dtype):
+    npdt = np.float64 if dtype == "f64" else np.float32
+    tdt = torch.float64 if dtype == "f64" else torch.float32
+    S, W = electron.shape
+    E.ewald_load_walkers(ctx, w.n, torch.from_numpy(E.to_soa(pos0, npdt)).cuda(),
+                         torch.from_numpy(w.charges.astype(npdt)).cuda())
+    d_w = torch.arange(W, dtype=torch.int32, device="cuda")
+    de = np.zeros((S, W))
+    for s in range(S):
+        d_el = torch.from_numpy(electron[s]).cuda()
+        d_r = torch.from_numpy(new_r[s].astype(npdt)).cuda().to(tdt).contiguous()
+        d_de = torch.zeros(W, dtype=torch.float64, device="cuda")
+        E.ewald_move_delta_batch(ctx, d_w, d_el, d_r, 1, d_de)
+        de[s] = d_de.cpu().numpy()
+    return de
+
+
+def _assert_delta(de, de_ref, tol):
+    rms = np.sqrt((de_ref ** 2).mean(axis=1, keepdims=True))
+    err = np.abs(de - de_ref) / np.maximum(np.abs(de_ref), rms)
+    assert err.max() <= tol, "max Delta-E error %.3e > %.1e" % (err.max(), tol)
+
+
+@pytest.mark.parametrize("dtype,tol", [("f64", TOL64), ("f32", TOL32)])
+def test_move_chain_config5_matches_oracle(torch_cuda, dtype, tol):
+    w = workloads.config(5)
+    W, S = 6, 12
+    pos0, electron, new_r, final = _move_inputs(w, W, S)
+    de_ref, pos_ref, rho_ref = ref.move_chain(w.dim, w.cell, w.kappa, w.g_cutoff, w.r_cutoff, pos0,
+                                              w.charges, electron, new_r, want_rho=True)
+    ctx = _ctx(w)
+    de = _run_moves(torch_cuda, ctx, w, pos0, electron, new_r, dtype)
+    _assert_delta(de, de_ref, tol)
+    # the stored state after the chain equals a fresh evaluation of the final configuration
+    rho = E.ewald_get_rho(ctx, 3)
+    assert np.abs(rho - rho_ref[3]).max() <= (1e-12 if dtype == "f64" else 3e-6) * w.n
+    got = E.ewald_get_positions(ctx, 3, w.n)
+    assert np.abs(got - final[3]).max() <= (0 if dtype == "f64" else 2e-6)
+    if dtype == "f64":
+        e0, _ = _gpu_energy(torch_cuda, ctx, pos0, w.charges, "f64", components=False)
+        e1, _ = _gpu_energy(torch_cuda, ctx, final, w.charges, "f64", components=False)
+        assert np.abs(e0 + de.sum(axis=0) - e1).max() <= 1e-11 * np.abs(e1).max()
+
+
+def test_moves_with_ions_2d_and_uncommitted(torch_cuda):
+    torch = torch_cuda
+    rng = np.random.default_rng(5)
+    for dim in (2, 3):
+        cell = _random_cell(rng, dim, 7.0)
+        kappa = 0.75
+        gc, rc = ref.auto_cutoffs(dim, cell, kappa, 1e-17)
+        n, ni, W, S = 9, 2, 3, 5
+        q = rng.choice([-1.0, 1.0], size=n)
+        pos0 = rng.random((W, n, dim)) @ cell
+        ion, qi = rng.random((ni, dim)) @ cell, np.array([2.0, -1.0])
+        electron = rng.integers(0, n, (S, W)).astype(np.int32)
+        new_r = rng.random((S, W, dim)) @ cell
+        de_ref, _, rho_ref = ref.move_chain(dim, cell, kappa, gc, rc, pos0, q, electron, new_r, ion, qi,
+                                            want_rho=True)
+        ctx = E.ewald_setup(dim, cell, kappa, gc, rc)
+        E.ewald_set_fixed_charges(ctx, ion, qi)
+        E.ewald_load_walkers(ctx, n, torch.from_numpy(E.to_soa(pos0)).cuda(), torch.from_numpy(q).cuda())
+        d_w = torch.arange(W, dtype=torch.int32, device="cuda")
+        for s in range(S):
+            d_el, d_r = torch.from_numpy(electron[s]).cuda(), torch.from_numpy(new_r[s]).cuda()
+            trial = torch.zeros(W, dtype=torch.float64, device="cuda")
+            E.ewald_move_delta_batch(ctx, d_w, d_el, d_r, 0, trial)   # rejected proposal: no change
+            d_de = torch.zeros(W, dtype=torch.float64, device="cuda")
+            E.ewald_move_delta_batch(ctx, d_w, d_el, d_r, 1, d_de)
+            assert torch.equal(trial, d_de)
+            scale = np.abs(de_ref).max()
+            assert np.abs(d_de.cpu().numpy() - de_ref[s]).max() <= 1e-11 * scale
+        for k in range(W):
+            assert np.abs(E.ewald_get_rho(ctx, k) - rho_ref[k]).max() <= 1e-12 * (n + 3)
+        # scalar form: move there and back again sums to zero and restores rho
+        before = E.ewald_get_rho(ctx, 1)
+        old = E.ewald_get_positions(ctx, 1, n)[4]
+        d1 = E.ewald_move_delta(ctx, 1, 4, new_r[0, 0], commit=True)
+        d2 = E.ewald_move_delta(ctx, 1, 4, old, commit=True)
+        assert abs(d1 + d2) <= 1e-12 * max(abs(d1), 1.0)
+        assert np.abs(E.ewald_get_rho(ctx, 1) - before).max() <= 1e-13 * (n + 3)
+
+
+def test_state_errors(torch_cuda):
+    torch = torch_cuda
+    w = workloads.config(1)
+    ctx = _ctx(w)
+    with pytest.raises(E.EwaldError) as ei:
+        E.ewald_move_delta(ctx, 0, 0, [0.0, 0.0, 0.0])
+    assert ei.value.status == 4
+    E.ewald_load_walkers(ctx, w.n, torch.from_numpy(E.to_soa(w.positions(2))).cuda(),
+                         torch.from_numpy(w.charges).cuda())
+    for wk, el in ((2, 0), (0, w.n), (-1, 0)):
+        with pytest.raises(E.EwaldError) as ei:
+            E.ewald_move_delta(ctx, wk, el, [0.0, 0.0, 0.0])
+        assert ei.value.status == 4
+    # batch form: out-of-range entries give NaN and leave the state alone
+    before = E.ewald_get_rho(ctx, 1)
+    d_de = torch.zeros(2, dtype=torch.float64, device="cuda")
+    E.ewald_move_delta_batch(ctx, torch.tensor([0, 1], dtype=torch.int32, device="cuda"),
+                             torch.tensor([3, 9999], dtype=torch.int32, device="cuda"),
+                             torch.zeros((2, 3), dtype=torch.float64, device="cuda"), 1, d_de)
+    out = d_de.cpu().numpy()
+    assert np.isfinite(out[0]) and np.isnan(out[1])
+    assert np.array_equal(E.ewald_get_rho(ctx, 1), before)
+
+
+def test_full_size_config2_sampled_walkers(torch_cuda):
+    """BASELINE configs[1] at its full size (1024 walkers), in the launch configuration bench.py
+    times; the oracle checks a sample of walkers one by one."""
+    w = workloads.config(2)
+    pos = w.positions()
+    ctx = _ctx(w)
+    sample = np.array([0, 1, 511, 777, 1023])
+    e_ref, _ = _oracle_energy(w, pos[sample])
+    for dtype, tol in (("f64", TOL64), ("f32", TOL32)):
+        e, _ = _gpu_energy(torch_cuda, ctx, pos, w.charges, dtype, components=False)
+        assert np.all(np.isfinite(e))
+        assert (np.abs(e[sample] - e_ref) / np.abs(e_ref)).max() <= tol
+        # property that holds at any size: identical walkers give identical energies
+        e2, _ = _gpu_energy(torch_cuda, ctx, pos[::-1].copy(), w.charges, dtype, components=False)
+        assert np.array_equal(e2[::-1], e)
+
+
+def test_translation_and_permutation_invariance_on_gpu(torch_cuda):
+    w = workloads.config(2)
+    pos = w.positions(4)
+    ctx = _ctx(w)
+    e, _ = _gpu_energy(torch_cuda, ctx, pos, w.charges, "f64", components=False)
+    shift = np.array([0.37, -2.11, 5.3]) * w.L
+    e_t, _ = _gpu_energy(torch_cuda, ctx, pos + shift, w.charges, "f64", components=False)
+    perm = np.random.default_rng(3).permutation(w.n)
+    e_p, _ = _gpu_energy(torch_cuda, ctx, pos[:, perm], w.charges, "f64", components=False)
+    assert (np.abs(e_t - e) / np.abs(e)).max() <= 1e-11 and (np.abs(e_p - e) / np.abs(e)).max() <= 1e-12
