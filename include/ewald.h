@@ -81,6 +81,11 @@ ewald_status ewald_setup_summary(int dim, const double cell[9], double gamma, do
                                  double r_cutoff, int *num_g, int *num_images, int n_max[3],
                                  double *xi_r, double *v_m);
 
+/* Host-only evaluation of the setup's piecewise-polynomial table for erfc (the table the real-space
+ * kernels read; 16 bins on [0, z_max], degree 11 for FP64 kernels, 6 for FP32): value = P_bin(z).
+ * For tests of the table builder; 0 <= z <= z_max.                                                 */
+ewald_status ewald_erfc_table_eval(double z_max, int degree, int n, const double *z, double *value);
+
 /* Change the stream later calls are issued on (cudaStream_t; NULL = default stream). */
 ewald_status ewald_set_stream(ewald_ctx *ctx, void *stream);
 

@@ -42,6 +42,7 @@ struct ewald_ctx {
     double *d_ion_rho = nullptr; float *d_ion_rhof = nullptr;
     double *d_ion_pos = nullptr; float *d_ion_posf = nullptr;
     double *d_ion_q = nullptr; float *d_ion_qf = nullptr;
+    double *d_erfc = nullptr; float *d_erfcf = nullptr;   /* erfc piecewise polynomials */
 
     /* scratch */
     DevBuf partial_recip, partial_real, qsums;
@@ -125,11 +126,22 @@ static std::vector<float> to_f32(const std::vector<double> &v)
     return f;
 }
 
-template <typename T> static void fill_cell(const HostTables &t, CellT<T> *c)
+/* Real-space geometry in kappa-scaled lengths (ewald_realspace.cuh). */
+template <typename T> static void fill_geom(const HostTables &t, RealGeom<T> *g)
 {
-    for (int i = 0; i < 9; i++) { c->a[i] = (T)t.a[i]; c->binv[i] = (T)t.binv[i]; }
-    c->kappa = (T)t.kappa;
-    c->rcut2 = (T)(t.r_cutoff * t.r_cutoff);
+    for (int i = 0; i < 9; i++) { g->a[i] = (T)(t.a[i] * t.kappa); g->binv[i] = (T)(t.binv[i] / t.kappa); }
+    for (int k = 0; k < 3; k++) { g->L[k] = (T)(t.a[4 * k] * t.kappa); g->invL[k] = (T)(1.0 / (t.a[4 * k] * t.kappa)); }
+    g->rc2 = (T)(t.r_cutoff * t.r_cutoff * t.kappa * t.kappa);
+    g->inv_h = (T)(ERFC_BINS / t.z_max);
+    g->kappa = (T)t.kappa;
+    g->m_shift = t.m_shift;
+}
+
+static std::vector<double> scaled(const std::vector<double> &v, double f)
+{
+    std::vector<double> o(v);
+    for (double &x : o) x *= f;
+    return o;
 }
 
 extern "C" int ewald_padded_n(int n) { return n <= 0 ? 0 : (n + 3) & ~3; }
@@ -165,8 +177,10 @@ extern "C" ewald_status ewald_setup(ewald_ctx **out, int dim, const double *cell
     st = upload(c, &c->d_gn, gn);
     if (st == EWALD_OK) st = upload(c, &c->d_w2, t.g_w2);
     if (st == EWALD_OK) st = upload(c, &c->d_w2f, to_f32(t.g_w2));
-    if (st == EWALD_OK) st = upload(c, &c->d_img, t.img);
-    if (st == EWALD_OK) st = upload(c, &c->d_imgf, to_f32(t.img));
+    if (st == EWALD_OK) st = upload(c, &c->d_img, scaled(t.img, t.kappa));
+    if (st == EWALD_OK) st = upload(c, &c->d_imgf, to_f32(scaled(t.img, t.kappa)));
+    if (st == EWALD_OK) st = upload(c, &c->d_erfc, t.erfc_tab64);
+    if (st == EWALD_OK) st = upload(c, &c->d_erfcf, to_f32(t.erfc_tab32));
     if (st == EWALD_OK) st = ensure(c, &c->qsums, 2 * sizeof(double));
     if (st != EWALD_OK) { ewald_destroy(c); return st; }
     *out = c;
@@ -189,6 +203,23 @@ extern "C" ewald_status ewald_setup_summary(int dim, const double *cell, double 
     return EWALD_OK;
 }
 
+extern "C" ewald_status ewald_erfc_table_eval(double z_max, int degree, int n, const double *z, double *value)
+{
+    if (!(z_max > 0) || degree < 1 || degree > 24 || n < 0 || (n > 0 && (!z || !value))) return EWALD_EINVAL;
+    std::vector<double> tab;
+    build_erfc_table(z_max, ERFC_BINS, degree, &tab);
+    const double inv_h = ERFC_BINS / z_max;
+    for (int i = 0; i < n; i++) {
+        int b = (int)((float)z[i] * (float)inv_h);
+        b = b < 0 ? 0 : (b > ERFC_BINS - 1 ? ERFC_BINS - 1 : b);
+        const double u = fma(z[i], 2 * inv_h, tab[(size_t)(degree + 1) * ERFC_BINS + b]);
+        double p = tab[(size_t)degree * ERFC_BINS + b];
+        for (int k = degree - 1; k >= 0; k--) p = fma(p, u, tab[(size_t)k * ERFC_BINS + b]);
+        value[i] = p;
+    }
+    return EWALD_OK;
+}
+
 extern "C" void ewald_destroy(ewald_ctx *c)
 {
     if (!c) return;
@@ -196,7 +227,7 @@ extern "C" void ewald_destroy(ewald_ctx *c)
     cudaStreamSynchronize(c->stream);
     cudaFree(c->d_gn); cudaFree(c->d_w2); cudaFree(c->d_w2f); cudaFree(c->d_img); cudaFree(c->d_imgf);
     cudaFree(c->d_ion_rho); cudaFree(c->d_ion_rhof); cudaFree(c->d_ion_pos); cudaFree(c->d_ion_posf);
-    cudaFree(c->d_ion_q); cudaFree(c->d_ion_qf);
+    cudaFree(c->d_ion_q); cudaFree(c->d_ion_qf); cudaFree(c->d_erfc); cudaFree(c->d_erfcf);
     DevBuf *bufs[] = {&c->partial_recip, &c->partial_real, &c->qsums, &c->stage_pos, &c->stage_q,
                       &c->stage_e, &c->stage_comp, &c->mv_walker, &c->mv_electron, &c->mv_newr,
                       &c->mv_de, &c->st_pos, &c->st_q, &c->st_rho};
@@ -239,6 +270,7 @@ template <> struct Tabs<double> {
     static const double *ion_rho(const ewald_ctx *c) { return c->d_ion_rho; }
     static const double *ion_pos(const ewald_ctx *c) { return c->d_ion_pos; }
     static const double *ion_q(const ewald_ctx *c) { return c->d_ion_q; }
+    static const double *erfc(const ewald_ctx *c) { return c->d_erfc; }
 };
 template <> struct Tabs<float> {
     static const float *w2(const ewald_ctx *c) { return c->d_w2f; }
@@ -246,6 +278,7 @@ template <> struct Tabs<float> {
     static const float *ion_rho(const ewald_ctx *c) { return c->d_ion_rhof; }
     static const float *ion_pos(const ewald_ctx *c) { return c->d_ion_posf; }
     static const float *ion_q(const ewald_ctx *c) { return c->d_ion_qf; }
+    static const float *erfc(const ewald_ctx *c) { return c->d_erfcf; }
 };
 
 template <typename K> static ewald_status allow_smem(ewald_ctx *c, K kernel, size_t bytes)
@@ -310,23 +343,35 @@ static ewald_status launch_real(ewald_ctx *c, int W, int n, const T *pos, const 
     A.pos = pos; A.q = q; A.n = n; A.npad = ewald_padded_n(n);
     A.img = Tabs<T>::img(c); A.nimg = c->nimg;
     A.ion_pos = Tabs<T>::ion_pos(c); A.ion_q = Tabs<T>::ion_q(c); A.n_ion = c->t.n_ion;
+    A.erfc_tab = Tabs<T>::erfc(c);
     A.partial = (double *)c->partial_real.p;
     A.n_tiles = (int)n_tiles;
-    fill_cell(c->t, &A.cell);
-    const size_t smem = ((size_t)(c->t.dim + 1) * n + 3 * (size_t)c->nimg) * sizeof(T);
+    fill_geom(c->t, &A.g);
+    const bool ortho = c->t.orthogonal && c->t.m_shift <= 2;
+    if (ortho) A.nimg = 0; /* the orthorhombic path does not read the image list */
+    const size_t smem = RealSmem<T>::bytes(REAL_WARPS, A.nimg, A.n_ion, (size_t)(c->t.dim + 1) * n);
     const long long grid = (long long)W * n_tiles;
     if (grid > 0x7fffffffLL) return fail(c, EWALD_ERANGE, "grid too large");
+#define EWALD_LAUNCH_REAL(DIM, ORTHO, M)                                                          \
+    do {                                                                                          \
+        st = allow_smem(c, real_kernel<T, DIM, ORTHO, M>, smem);                                  \
+        if (st != EWALD_OK) return st;                                                            \
+        ProfScope ps(c, 1);                                                                       \
+        real_kernel<T, DIM, ORTHO, M><<<(unsigned)grid, REAL_THREADS, smem, c->stream>>>(A);      \
+    } while (0)
+    const int m = c->t.m_shift;
     if (c->t.dim == 3) {
-        st = allow_smem(c, real_kernel<T, 3>, smem);
-        if (st != EWALD_OK) return st;
-        ProfScope ps(c, 1);
-        real_kernel<T, 3><<<(unsigned)grid, REAL_THREADS, smem, c->stream>>>(A);
+        if (!ortho) EWALD_LAUNCH_REAL(3, false, 0);
+        else if (m == 0) EWALD_LAUNCH_REAL(3, true, 0);
+        else if (m == 1) EWALD_LAUNCH_REAL(3, true, 1);
+        else EWALD_LAUNCH_REAL(3, true, 2);
     } else {
-        st = allow_smem(c, real_kernel<T, 2>, smem);
-        if (st != EWALD_OK) return st;
-        ProfScope ps(c, 1);
-        real_kernel<T, 2><<<(unsigned)grid, REAL_THREADS, smem, c->stream>>>(A);
+        if (!ortho) EWALD_LAUNCH_REAL(2, false, 0);
+        else if (m == 0) EWALD_LAUNCH_REAL(2, true, 0);
+        else if (m == 1) EWALD_LAUNCH_REAL(2, true, 1);
+        else EWALD_LAUNCH_REAL(2, true, 2);
     }
+#undef EWALD_LAUNCH_REAL
     CU_TRY(c, cudaGetLastError());
     *n_tiles_out = (int)n_tiles;
     return EWALD_OK;
@@ -453,19 +498,33 @@ static ewald_status move_batch_t(ewald_ctx *c, int n_moves, const int *walker, c
     A.rowlen = c->rowlen;
     A.img = Tabs<T>::img(c); A.nimg = c->nimg;
     A.ion_pos = Tabs<T>::ion_pos(c); A.ion_q = Tabs<T>::ion_q(c); A.n_ion = c->t.n_ion;
+    A.erfc_tab = Tabs<T>::erfc(c);
     A.walker = walker; A.electron = electron; A.new_r = new_r; A.commit = commit; A.delta_e = delta_e;
-    fill_cell(c->t, &A.cell);
-    const size_t smem = 2 * (size_t)c->rowlen * sizeof(T2) + 3 * (size_t)c->nimg * sizeof(T);
+    for (int i = 0; i < 9; i++) A.binv[i] = (T)c->t.binv[i];
+    fill_geom(c->t, &A.g);
+    const bool ortho = c->t.orthogonal && c->t.m_shift <= 2;
+    if (ortho) A.nimg = 0;
+    const size_t smem = RealSmem<T>::bytes(MOVE_WARPS, A.nimg, A.n_ion, 4 * (size_t)c->rowlen);
     ewald_status st;
+#define EWALD_LAUNCH_MOVE(DIM, ORTHO, M)                                                          \
+    do {                                                                                          \
+        if ((st = allow_smem(c, move_kernel<T, DIM, ORTHO, M>, smem)) != EWALD_OK) return st;     \
+        ProfScope ps(c, 3);                                                                       \
+        move_kernel<T, DIM, ORTHO, M><<<n_moves, MOVE_THREADS, smem, c->stream>>>(A);             \
+    } while (0)
+    const int m = c->t.m_shift;
     if (c->t.dim == 3) {
-        if ((st = allow_smem(c, move_kernel<T, 3>, smem)) != EWALD_OK) return st;
-        ProfScope ps(c, 3);
-        move_kernel<T, 3><<<n_moves, MOVE_THREADS, smem, c->stream>>>(A);
+        if (!ortho) EWALD_LAUNCH_MOVE(3, false, 0);
+        else if (m == 0) EWALD_LAUNCH_MOVE(3, true, 0);
+        else if (m == 1) EWALD_LAUNCH_MOVE(3, true, 1);
+        else EWALD_LAUNCH_MOVE(3, true, 2);
     } else {
-        if ((st = allow_smem(c, move_kernel<T, 2>, smem)) != EWALD_OK) return st;
-        ProfScope ps(c, 3);
-        move_kernel<T, 2><<<n_moves, MOVE_THREADS, smem, c->stream>>>(A);
+        if (!ortho) EWALD_LAUNCH_MOVE(2, false, 0);
+        else if (m == 0) EWALD_LAUNCH_MOVE(2, true, 0);
+        else if (m == 1) EWALD_LAUNCH_MOVE(2, true, 1);
+        else EWALD_LAUNCH_MOVE(2, true, 2);
     }
+#undef EWALD_LAUNCH_MOVE
     CU_TRY(c, cudaGetLastError());
     return EWALD_OK;
 }

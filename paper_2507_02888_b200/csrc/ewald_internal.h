@@ -30,6 +30,11 @@ struct HostTables {
     double self_coef = 0;  /* E_self = -self_coef * sum q^2,  self_coef = kappa/sqrt(pi)          */
     double bg_coef = 0;    /* E_bg = -bg_coef/2 * Q^2 ; pi/(Omega kappa^2) (3D), 2 sqrt(pi)/(A kappa) (2D) */
     double v_m = 0;        /* Eq. 4 */
+    /* real-space evaluation tables (ewald_realspace.cuh): erfc on 16 bins of z = kappa r in [0, z_max],
+     * rows c_0..c_deg then -(2b+1); FP64 table of degree 11 and FP32 table of degree 6 */
+    double z_max = 0;
+    int m_shift = 0;              /* orthorhombic cells: images -m..m per axis reach r_cutoff      */
+    std::vector<double> erfc_tab64, erfc_tab32;
     /* fixed charges */
     int n_ion = 0;
     std::vector<double> ion_pos; /* [n_ion][3] */
@@ -41,6 +46,7 @@ struct HostTables {
 /* Returns EWALD_OK or an error status with a message. */
 ewald_status build_tables(int dim, const double *cell, double kappa, double g_cutoff,
                           double r_cutoff, HostTables *out, std::string *err);
+void build_erfc_table(double z_max, int n_bins, int degree, std::vector<double> *tab);
 ewald_status build_fixed_charges(HostTables *t, int n_ion, const double *pos, const double *q,
                                  std::string *err);
 

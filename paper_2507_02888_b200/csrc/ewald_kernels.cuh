@@ -13,76 +13,10 @@
  * combining loop) is kept as three kernels; everything inside them is new.
  */
 #pragma once
-#include <cuda_runtime.h>
-#include <stdint.h>
+#include "ewald_kernels_common.cuh"
+#include "ewald_realspace.cuh"
 
 namespace ewald {
-
-template <typename T> struct Num;
-template <> struct Num<double> {
-    typedef double2 T2;
-    static __device__ __forceinline__ void sincospi_(double x, double *s, double *c) { sincospi(x, s, c); }
-    static __device__ __forceinline__ double rint_(double x) { return rint(x); }
-    static __device__ __forceinline__ double erfc_(double x) { return erfc(x); }
-    static __device__ __forceinline__ double rsqrt_(double x) { return rsqrt(x); }
-};
-template <> struct Num<float> {
-    typedef float2 T2;
-    static __device__ __forceinline__ void sincospi_(float x, float *s, float *c) { sincospif(x, s, c); }
-    static __device__ __forceinline__ float rint_(float x) { return rintf(x); }
-    static __device__ __forceinline__ float erfc_(float x) { return erfcf(x); }
-    static __device__ __forceinline__ float rsqrt_(float x) { return rsqrtf(x); }
-};
-
-/* Cell geometry in the kernel's precision. */
-template <typename T> struct CellT {
-    T a[9];    /* lattice rows */
-    T binv[9]; /* s_k = r . binv[k] */
-    T kappa;
-    T rcut2;
-};
-
-__device__ __forceinline__ double warp_sum(double v)
-{
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
-    return v;
-}
-
-/* Sum over the block in FP64; result valid in thread 0.  `red` holds >= 32 doubles. */
-__device__ __forceinline__ double block_sum(double v, double *red)
-{
-    v = warp_sum(v);
-    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
-    __syncthreads();
-    if (lane == 0) red[wid] = v;
-    __syncthreads();
-    if (wid == 0) {
-        const int nw = (blockDim.x + 31) >> 5;
-        v = lane < nw ? red[lane] : 0.0;
-        v = warp_sum(v);
-    }
-    return v;
-}
-
-/* Power table of one point for one direction: tab[n] = scale * exp(2 pi i s)^n, n = 0..nmax. */
-template <typename T>
-__device__ __forceinline__ void power_row(T s, T scale, int nmax, typename Num<T>::T2 *tab)
-{
-    typedef typename Num<T>::T2 T2;
-    s -= Num<T>::rint_(s); /* exact: the phase is periodic in s */
-    T sn, cs;
-    Num<T>::sincospi_(2 * s, &sn, &cs);
-    T2 e; e.x = scale; e.y = 0;
-    tab[0] = e;
-    for (int n = 1; n <= nmax; n++) {
-        T2 f;
-        f.x = e.x * cs - e.y * sn;
-        f.y = e.x * sn + e.y * cs;
-        e = f;
-        tab[n] = e;
-    }
-}
 
 /* ------------------------------------------------------------------------------------------ */
 /* [S1-S4] rho(G) and E_recip.  grid = n_walkers * n_slabs; each thread owns GPT members of G+. */
@@ -189,74 +123,78 @@ __global__ void __launch_bounds__(RECIP_THREADS) recip_kernel(RecipArgs<T> A)
 }
 
 /* ------------------------------------------------------------------------------------------ */
-/* [S5] real-space pair sum.  grid = n_walkers * n_tiles. */
+/* [S5] real-space pair sum.  grid = n_walkers * n_tiles; machinery in ewald_realspace.cuh. */
 
 template <typename T> struct RealArgs {
     const T *pos; const T *q;
     int n, npad;
-    const T *img; int nimg;          /* [nimg][3] */
-    const T *ion_pos; const T *ion_q; int n_ion; /* [n_ion][3] */
-    double *partial;                 /* [W][n_tiles] */
+    const T *img; int nimg;                       /* [nimg][3], kappa-scaled (general cells)   */
+    const T *ion_pos; const T *ion_q; int n_ion;  /* [n_ion][3], [n_ion]                        */
+    const T *erfc_tab;                            /* [ERFC_ROWS][ERFC_BINS]                     */
+    double *partial;                              /* [W][n_tiles] */
     int n_tiles;
-    CellT<T> cell;
+    RealGeom<T> g;
 };
 
 constexpr int REAL_THREADS = 256;
+constexpr int REAL_WARPS = REAL_THREADS / 32;
 
-/* minimum-image style reduction to fractional coordinates in [-1/2,1/2] (reading R10) */
-template <typename T, int DIM>
-__device__ __forceinline__ void reduce_disp(const CellT<T> &c, T *d)
-{
-    T f[3];
-#pragma unroll
-    for (int k = 0; k < DIM; k++) {
-        T s = 0;
-#pragma unroll
-        for (int x = 0; x < DIM; x++) s += d[x] * c.binv[3 * k + x];
-        f[k] = Num<T>::rint_(s);
+/* Shared-memory carve-up common to the real-space and move kernels. */
+template <typename T> struct RealSmem {
+    typedef typename Num<T>::T2 T2;
+    T2 *queue;  /* [n_warps][QUEUE_CAP] */
+    T *tab;     /* [ERFC_ROWS][ERFC_BINS] */
+    T *img;     /* [nimg][3] */
+    T *ion;     /* [n_ion][4] = x,y,z,q */
+    T *rest;
+    __device__ __forceinline__ RealSmem(unsigned char *raw, int n_warps, int nimg, int n_ion)
+    {
+        queue = reinterpret_cast<T2 *>(raw);
+        tab = reinterpret_cast<T *>(queue + n_warps * QUEUE_CAP);
+        img = tab + ErfcRows<T>::value * ERFC_BINS;
+        ion = img + 3 * nimg;
+        rest = tab + table_elems(nimg, n_ion);
     }
-#pragma unroll
-    for (int x = 0; x < DIM; x++) {
-        T v = d[x];
-#pragma unroll
-        for (int k = 0; k < DIM; k++) v -= f[k] * c.a[3 * k + x];
-        d[x] = v;
+    /* elements before `rest`, rounded so that `rest` stays 16-byte aligned */
+    static __host__ __device__ size_t table_elems(int nimg, int n_ion)
+    {
+        return ((size_t)ErfcRows<T>::value * ERFC_BINS + 3 * (size_t)nimg + 4 * (size_t)n_ion + 3) & ~(size_t)3;
     }
-}
-
-/* psi(d) = sum_R erfc(kappa|d-R|)/|d-R| over images within the cut-off; d already reduced */
-template <typename T, int DIM>
-__device__ __forceinline__ T psi_images(const CellT<T> &c, const T *img, int nimg, const T *d)
-{
-    T s = 0;
-    for (int m = 0; m < nimg; m++) {
-        T r2 = 0;
-#pragma unroll
-        for (int x = 0; x < DIM; x++) { T v = d[x] - img[3 * m + x]; r2 += v * v; }
-        if (r2 < c.rcut2) {
-            T ri = Num<T>::rsqrt_(r2);
-            s += Num<T>::erfc_(c.kappa * (r2 * ri)) * ri;
+    static size_t bytes(int n_warps, int nimg, int n_ion, size_t rest_elems)
+    {
+        return (size_t)n_warps * QUEUE_CAP * sizeof(T2) + (table_elems(nimg, n_ion) + rest_elems) * sizeof(T);
+    }
+    __device__ __forceinline__ void fill(const T *erfc_tab, const T *gimg, int nimg, const T *ion_pos,
+                                         const T *ion_q, int n_ion, int tid, int nthreads)
+    {
+        for (int t = tid; t < ErfcRows<T>::value * ERFC_BINS; t += nthreads) tab[t] = erfc_tab[t];
+        for (int t = tid; t < 3 * nimg; t += nthreads) img[t] = gimg[t];
+        for (int t = tid; t < n_ion; t += nthreads) {
+            ion[4 * t + 0] = ion_pos[3 * t + 0];
+            ion[4 * t + 1] = ion_pos[3 * t + 1];
+            ion[4 * t + 2] = ion_pos[3 * t + 2];
+            ion[4 * t + 3] = ion_q[t];
         }
     }
-    return s;
-}
+};
 
-template <typename T, int DIM>
+template <typename T, int DIM, bool ORTHO, int M>
 __global__ void __launch_bounds__(REAL_THREADS) real_kernel(RealArgs<T> A)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    T *sp = reinterpret_cast<T *>(smem_raw);        /* [DIM][n] positions, then [n] charges */
-    T *sq = sp + DIM * A.n;
-    T *simg = sq + A.n;                              /* [nimg][3] */
+    RealSmem<T> S(smem_raw, REAL_WARPS, A.nimg, A.n_ion);
+    T *sp = S.rest;             /* [DIM][n] positions (unscaled: differences are taken first) */
+    T *sq = sp + DIM * A.n;     /* [n] charges */
     __shared__ double red[32];
     const int w = blockIdx.x / A.n_tiles, tile = blockIdx.x - w * A.n_tiles, tid = threadIdx.x;
+    const int lane = tid & 31, warp = tid >> 5;
     const T *pw = A.pos + (size_t)w * DIM * A.npad;
     for (int t = tid; t < A.n; t += REAL_THREADS) {
 #pragma unroll
         for (int x = 0; x < DIM; x++) sp[x * A.n + t] = pw[x * A.npad + t];
         sq[t] = A.q[t];
     }
-    for (int t = tid; t < 3 * A.nimg; t += REAL_THREADS) simg[t] = A.img[t];
+    S.fill(A.erfc_tab, A.img, A.nimg, A.ion_pos, A.ion_q, A.n_ion, tid, REAL_THREADS);
     __syncthreads();
 
     const int n = A.n;
@@ -266,30 +204,36 @@ __global__ void __launch_bounds__(REAL_THREADS) real_kernel(RealArgs<T> A)
     const long long per = (total + A.n_tiles - 1) / A.n_tiles;
     const long long lo = per * tile, hi = min(total, lo + per);
 
+    WarpQueue<T> wq;
+    wq.buf = S.queue + warp * QUEUE_CAP; wq.cnt = 0; wq.lane = lane;
     double acc = 0;
-    for (long long p = lo + tid; p < hi; p += REAL_THREADS) {
+    for (long long base = lo + warp * 32; base < hi; base += REAL_THREADS) {
+        const long long p = base + lane;
+        const bool valid = p < hi;
         T d[3] = {0, 0, 0};
-        T qq;
-        if (p < n_mm) {
-            int i, j;
-            if (p < (long long)n * H) { i = (int)(p % n); j = i + (int)(p / n) + 1; }
-            else { i = (int)(p - (long long)n * H); j = i + n / 2; }
-            if (j >= n) j -= n;
+        T qq = 0;
+        if (valid) {
+            if (p < n_mm) {
+                int i, j;
+                if (p < (long long)n * H) { i = (int)(p % n); j = i + (int)(p / n) + 1; }
+                else { i = (int)(p - (long long)n * H); j = i + n / 2; }
+                if (j >= n) j -= n;
 #pragma unroll
-            for (int x = 0; x < DIM; x++) d[x] = sp[x * n + i] - sp[x * n + j];
-            qq = sq[i] * sq[j];
-        } else {
-            const long long e = p - n_mm;
-            const int i = (int)(e % n), I = (int)(e / n);
+                for (int x = 0; x < DIM; x++) d[x] = (sp[x * n + i] - sp[x * n + j]) * A.g.kappa;
+                qq = sq[i] * sq[j];
+            } else {
+                const long long e = p - n_mm;
+                const int i = (int)(e % n), I = (int)(e / n);
 #pragma unroll
-            for (int x = 0; x < DIM; x++) d[x] = sp[x * n + i] - A.ion_pos[3 * I + x];
-            qq = sq[i] * A.ion_q[I];
+                for (int x = 0; x < DIM; x++) d[x] = (sp[x * n + i] - S.ion[4 * I + x]) * A.g.kappa;
+                qq = sq[i] * S.ion[4 * I + 3];
+            }
         }
-        reduce_disp<T, DIM>(A.cell, d);
-        acc += (double)(qq * psi_images<T, DIM>(A.cell, simg, A.nimg, d));
+        acc += (double)scan_pair<T, DIM, ORTHO, M>(A.g, d, qq, valid, wq, S.tab, S.img, A.nimg);
     }
+    acc += (double)wq.finish(S.tab, A.g.inv_h);
     acc = block_sum(acc, red);
-    if (tid == 0) A.partial[(size_t)w * A.n_tiles + tile] = acc;
+    if (tid == 0) A.partial[(size_t)w * A.n_tiles + tile] = acc * (double)A.g.kappa;
 }
 
 /* ------------------------------------------------------------------------------------------ */
@@ -345,23 +289,27 @@ template <typename T> struct MoveArgs {
     int n, npad, n_walkers;
     const short4 *gn; const T *w2; int ngp, ngp_pad;
     int nmax[3]; int off[3], rowlen;
-    const T *img; int nimg;
+    const T *img; int nimg;                       /* kappa-scaled image list (general cells) */
     const T *ion_pos; const T *ion_q; int n_ion;
+    const T *erfc_tab;
     const int *walker; const int *electron; const T *new_r; /* [n_moves], [n_moves], [n_moves][DIM] */
     int commit;
     double *delta_e;
-    CellT<T> cell;
+    T binv[9];                                    /* unscaled: s_k = r . binv[k] */
+    RealGeom<T> g;
 };
 
 constexpr int MOVE_THREADS = 256;
 
-template <typename T, int DIM>
+constexpr int MOVE_WARPS = MOVE_THREADS / 32;
+
+template <typename T, int DIM, bool ORTHO, int M>
 __global__ void __launch_bounds__(MOVE_THREADS) move_kernel(MoveArgs<T> A)
 {
     typedef typename Num<T>::T2 T2;
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    T2 *tab = reinterpret_cast<T2 *>(smem_raw); /* [2][rowlen]: old, new */
-    T *simg = reinterpret_cast<T *>(tab + 2 * A.rowlen);
+    RealSmem<T> S(smem_raw, MOVE_WARPS, A.nimg, A.n_ion);
+    T2 *tab = reinterpret_cast<T2 *>(S.rest); /* [2][rowlen]: old, new */
     __shared__ double red[32];
     const int m = blockIdx.x, tid = threadIdx.x;
     const int w = A.walker[m], k = A.electron[m];
@@ -381,10 +329,10 @@ __global__ void __launch_bounds__(MOVE_THREADS) move_kernel(MoveArgs<T> A)
         const T *r = which ? r_new : r_old;
         T s = 0;
 #pragma unroll
-        for (int x = 0; x < DIM; x++) s += r[x] * A.cell.binv[3 * d + x];
+        for (int x = 0; x < DIM; x++) s += r[x] * A.binv[3 * d + x];
         power_row<T>(s, T(1), A.nmax[d], tab + which * A.rowlen + A.off[d]);
     }
-    for (int t = tid; t < 3 * A.nimg; t += MOVE_THREADS) simg[t] = A.img[t];
+    S.fill(A.erfc_tab, A.img, A.nimg, A.ion_pos, A.ion_q, A.n_ion, tid, MOVE_THREADS);
     __syncthreads();
 
     /* [S7b] Delta E_recip and the patch of rho(G) */
@@ -418,28 +366,41 @@ __global__ void __launch_bounds__(MOVE_THREADS) move_kernel(MoveArgs<T> A)
         if (A.commit) { rr[g] = re + qk * dr; rr[A.ngp_pad + g] = im + qk * di; }
     }
 
-    /* [S7c] Delta E_real = q_k sum_{j != k} q_j [psi(r'-r_j) - psi(r-r_j)] */
+    /* [S7c] Delta E_real = q_k sum_{j != k} q_j [psi(r'-r_j) - psi(r-r_j)]: the new-position terms are
+     * queued with +q_j, the old-position terms with -q_j */
     double accr = 0;
-    for (int j = tid; j < A.n + A.n_ion; j += MOVE_THREADS) {
-        if (j == k) continue;
-        T rj[3] = {0, 0, 0};
-        T qj;
-        if (j < A.n) {
+    {
+        const int lane = tid & 31, warp = tid >> 5;
+        WarpQueue<T> wq;
+        wq.buf = S.queue + warp * QUEUE_CAP; wq.cnt = 0; wq.lane = lane;
+        const int ntot = A.n + A.n_ion;
+        for (int base = warp * 32; base < ntot; base += MOVE_THREADS) {
+            const int j = base + lane;
+            const bool valid = j < ntot && j != k;
+            T rj[3] = {0, 0, 0};
+            T qj = 0;
+            if (valid) {
+                if (j < A.n) {
 #pragma unroll
-            for (int x = 0; x < DIM; x++) rj[x] = pw[x * A.npad + j];
-            qj = A.q[j];
-        } else {
+                    for (int x = 0; x < DIM; x++) rj[x] = pw[x * A.npad + j];
+                    qj = A.q[j];
+                } else {
 #pragma unroll
-            for (int x = 0; x < DIM; x++) rj[x] = A.ion_pos[3 * (j - A.n) + x];
-            qj = A.ion_q[j - A.n];
+                    for (int x = 0; x < DIM; x++) rj[x] = S.ion[4 * (j - A.n) + x];
+                    qj = S.ion[4 * (j - A.n) + 3];
+                }
+            }
+            T dn[3] = {0, 0, 0}, dold[3] = {0, 0, 0};
+#pragma unroll
+            for (int x = 0; x < DIM; x++) {
+                dn[x] = (r_new[x] - rj[x]) * A.g.kappa;
+                dold[x] = (r_old[x] - rj[x]) * A.g.kappa;
+            }
+            accr += (double)scan_pair<T, DIM, ORTHO, M>(A.g, dn, qj, valid, wq, S.tab, S.img, A.nimg);
+            accr += (double)scan_pair<T, DIM, ORTHO, M>(A.g, dold, -qj, valid, wq, S.tab, S.img, A.nimg);
         }
-        T dn[3], dold[3];
-#pragma unroll
-        for (int x = 0; x < 3; x++) { dn[x] = r_new[x] - rj[x]; dold[x] = r_old[x] - rj[x]; }
-        reduce_disp<T, DIM>(A.cell, dn);
-        reduce_disp<T, DIM>(A.cell, dold);
-        accr += (double)(qj * (psi_images<T, DIM>(A.cell, simg, A.nimg, dn) -
-                               psi_images<T, DIM>(A.cell, simg, A.nimg, dold)));
+        accr += (double)wq.finish(S.tab, A.g.inv_h);
+        accr *= (double)A.g.kappa;
     }
     acc += (double)qk * accr;
     acc = block_sum(acc, red); /* its barriers also order every read of r_old before the commit */

@@ -28,6 +28,41 @@ static real weight(int dim, real volume, real kappa, real g2)
     return kPi / volume * erfcl(g / (2 * kappa)) / g;
 }
 
+/* Piecewise polynomial for erfc(z) on n_bins equal bins of [0, z_max]: on bin b, with
+ * u = 2 z / h - (2b+1) in [-1,1], erfc(z) ~ sum_k c_k u^k.  Interpolation at Chebyshev nodes of a
+ * slightly widened interval (the kernel picks the bin from an FP32 product), Chebyshev series
+ * converted to monomials, all in long double.  Layout [row][bin]: rows c_0..c_degree, then -(2b+1). */
+void build_erfc_table(double z_max, int n_bins, int degree, std::vector<double> *tab)
+{
+    const int n = degree + 1;
+    const real h = (real)z_max / n_bins, widen = 1 + 1e-4L;
+    tab->assign((size_t)(degree + 2) * n_bins, 0.0);
+    std::vector<real> fv(n), cheb(n), mono(n), t0(n), t1(n), t2(n);
+    for (int b = 0; b < n_bins; b++) {
+        const real centre = (b + 0.5L) * h, half = 0.5L * h * widen;
+        for (int i = 0; i < n; i++) fv[i] = erfcl(centre + half * cosl(kPi * (2 * i + 1) / (2 * n)));
+        for (int k = 0; k < n; k++) {
+            real s = 0;
+            for (int i = 0; i < n; i++) s += fv[i] * cosl(k * kPi * (2 * i + 1) / (2 * n));
+            cheb[k] = (k == 0 ? 1 : 2) * s / n;
+        }
+        /* sum_k cheb[k] T_k(v) -> monomials in v via T_{k+1} = 2 v T_k - T_{k-1} */
+        for (int i = 0; i < n; i++) { mono[i] = 0; t0[i] = 0; t1[i] = 0; }
+        t0[0] = 1;                 /* T_0 */
+        if (n > 1) t1[1] = 1;      /* T_1 */
+        for (int i = 0; i < n; i++) mono[i] += cheb[0] * t0[i];
+        if (n > 1) for (int i = 0; i < n; i++) mono[i] += cheb[1] * t1[i];
+        for (int k = 2; k < n; k++) {
+            for (int i = 0; i < n; i++) t2[i] = (i > 0 ? 2 * t1[i - 1] : 0) - t0[i];
+            for (int i = 0; i < n; i++) mono[i] += cheb[k] * t2[i];
+            t0 = t1; t1 = t2;
+        }
+        real scale = 1; /* v = u / widen */
+        for (int k = 0; k < n; k++) { (*tab)[(size_t)k * n_bins + b] = (double)(mono[k] * scale); scale /= widen; }
+        (*tab)[(size_t)(degree + 1) * n_bins + b] = -(double)(2 * b + 1);
+    }
+}
+
 ewald_status build_tables(int dim, const double *cell, double kappa_d, double g_cutoff,
                           double r_cutoff, HostTables *t, std::string *err)
 {
@@ -67,7 +102,12 @@ ewald_status build_tables(int dim, const double *cell, double kappa_d, double g_
     t->g_cutoff = g_cutoff;
     t->volume = (double)fabsl(det);
     if (r_cutoff == 0) r_cutoff = (double)(sqrtl(-logl(1e-17L)) / kappa);
+    /* erfc(6.5) = 4e-20: beyond kappa r = 6.5 no term can matter at FP64; keeps the erfc table's range fixed */
+    if (r_cutoff * kappa_d > 6.5) r_cutoff = 6.5 / kappa_d;
     t->r_cutoff = r_cutoff;
+    t->z_max = r_cutoff * kappa_d * (1 + 4e-6);
+    build_erfc_table(t->z_max, 16, 11, &t->erfc_tab64);
+    build_erfc_table(t->z_max, 16, 6, &t->erfc_tab32);
     bool ortho = true;
     for (int i = 0; i < 3; i++)
         for (int j = 0; j < 3; j++) {
@@ -76,6 +116,12 @@ ewald_status build_tables(int dim, const double *cell, double kappa_d, double g_
             if (i != j && a[i][j] != 0) ortho = false;
         }
     t->orthogonal = ortho;
+    t->m_shift = 0;
+    for (int k = 0; k < dim; k++) {
+        /* image m of axis k is needed iff (|m| - 1/2) L_k < r_c */
+        int m = (int)floorl((real)r_cutoff / len3(a[k]) + 0.5L - 1e-12L);
+        if (m > t->m_shift) t->m_shift = m;
+    }
 
     /* ---- half set G+ (first non-zero integer component positive), lexicographic ---- */
     const real g2max = (real)g_cutoff * g_cutoff * (1 + 1e-12L); /* reading R6 */

@@ -18,7 +18,8 @@ _STATUS = {0: "EWALD_OK", 1: "EWALD_EINVAL", 2: "EWALD_ESINGULAR", 3: "EWALD_ERA
            4: "EWALD_ESTATE", 5: "EWALD_ECUDA", 6: "EWALD_ENOMEM"}
 
 # every symbol include/ewald.h declares (checked by tests/test_abi.py against the header text)
-SYMBOLS = ["ewald_padded_n", "ewald_setup", "ewald_setup_summary", "ewald_destroy", "ewald_set_stream",
+SYMBOLS = ["ewald_padded_n", "ewald_setup", "ewald_setup_summary", "ewald_erfc_table_eval",
+           "ewald_destroy", "ewald_set_stream",
            "ewald_set_fixed_charges", "ewald_energy_batch", "ewald_energy_batch_host",
            "ewald_load_walkers", "ewald_move_delta_batch", "ewald_move_delta_batch_host",
            "ewald_move_delta", "ewald_num_g", "ewald_num_images", "ewald_r_cutoff", "ewald_get_g",
@@ -57,6 +58,7 @@ def load_library():
         "ewald_padded_n": (i, [i]),
         "ewald_setup": (i, [ctypes.POINTER(vp), i, dp, d, d, ctypes.POINTER(_Opts)]),
         "ewald_setup_summary": (i, [i, dp, d, d, d, ip, ip, ip, dp, dp]),
+        "ewald_erfc_table_eval": (i, [d, i, i, dp, dp]),
         "ewald_destroy": (None, [vp]),
         "ewald_set_stream": (i, [vp, vp]),
         "ewald_set_fixed_charges": (i, [vp, i, dp, dp]),
@@ -184,6 +186,16 @@ def ewald_setup_summary(dim, cell, gamma, g_cutoff, r_cutoff=0.0):
     if st != 0:
         raise EwaldError(st, "ewald_setup_summary failed")
     return dict(num_g=ng.value, num_images=ni.value, n_max=list(nm), xi_r=xi.value, v_m=vm.value)
+
+
+def ewald_erfc_table_eval(z_max, degree, z):
+    """Host-only: the setup's piecewise polynomial for erfc evaluated at z (array)."""
+    z = np.ascontiguousarray(z, dtype=np.float64)
+    out = np.zeros_like(z)
+    st = load_library().ewald_erfc_table_eval(float(z_max), int(degree), z.size, _dp(z), _dp(out))
+    if st != 0:
+        raise EwaldError(st, "ewald_erfc_table_eval failed")
+    return out
 
 
 def ewald_destroy(ctx):
