@@ -81,6 +81,15 @@ ewald_status ewald_setup_summary(int dim, const double cell[9], double gamma, do
                                  double r_cutoff, int *num_g, int *num_images, int n_max[3],
                                  double *xi_r, double *v_m);
 
+/* Host-only summary of the work plan of the octant-form reciprocal kernel (orthorhombic cells; else
+ * EWALD_ESTATE): items per walker, n1 pairs per block, warps of a CTA of n_walkers_per_cta walkers,
+ * the sum of all octant weights w(G_n) 2^nz (must equal the full-sphere sum of w(G): the plan covers
+ * every G exactly once) and the FMA + product operations the kernel executes per particle and walker
+ * (to compare with the algorithmic N_G + 1).  Any output pointer may be null. */
+ewald_status ewald_oct_plan_summary(int dim, const double cell[9], double gamma, double g_cutoff,
+                                    int n_walkers_per_cta, int *n_items, int *npb, int *n_warps,
+                                    double *weight_sum, double *fma_per_particle);
+
 /* Host-only evaluation of the setup's piecewise-polynomial table for erfc (the table the real-space
  * kernels read; 16 bins on [0, z_max], degree 11 for FP64 kernels, 6 for FP32): value = P_bin(z).
  * For tests of the table builder; 0 <= z <= z_max.                                                 */
@@ -88,6 +97,12 @@ ewald_status ewald_erfc_table_eval(double z_max, int degree, int n, const double
 
 /* Change the stream later calls are issued on (cudaStream_t; NULL = default stream). */
 ewald_status ewald_set_stream(ewald_ctx *ctx, void *stream);
+
+/* Which reciprocal-space kernel ewald_energy_batch uses (both compute the same E_recip; for tests
+ * and measurements): 0 = automatic (octant real-product form on orthorhombic cells, complex
+ * half-set form otherwise), 1 = complex half-set form, 2 = octant form (EWALD_ESTATE at the next
+ * energy call if the cell is not orthorhombic). */
+ewald_status ewald_set_recip_variant(ewald_ctx *ctx, int variant);
 
 /* Fixed charges (ions) that belong to every walker and never move (config 4; reading R13).  They
  * enter rho(G), the real-space sum, E_self and E_bg exactly like mobile particles (Eq. 2 over all

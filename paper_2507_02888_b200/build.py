@@ -11,10 +11,11 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 ROOT = os.path.dirname(HERE)
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libewald_b200.so")
-SOURCES = ["ewald_api.cu", "ewald_setup.cpp"]
+SOURCES = ["ewald_api.cu", "ewald_setup.cpp", "ewald_octplan.cpp"]
 HEADERS = [os.path.join(ROOT, "include", "ewald.h"), os.path.join(CSRC, "ewald_internal.h"),
            os.path.join(CSRC, "ewald_kernels.cuh"),
-           os.path.join(CSRC, "ewald_kernels_common.cuh"), os.path.join(CSRC, "ewald_realspace.cuh")]
+           os.path.join(CSRC, "ewald_kernels_common.cuh"), os.path.join(CSRC, "ewald_realspace.cuh"),
+           os.path.join(CSRC, "ewald_recip_oct.cuh")]
 
 NVCC_FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
               "-Xcompiler", "-fPIC", "-shared", "-cudart", "static"]

@@ -11,6 +11,8 @@
 #include "ewald.h"
 #include "ewald_internal.h"
 #include "ewald_kernels.cuh"
+#include "ewald_recip_oct.cuh"
+#include <map>
 
 using namespace ewald;
 
@@ -24,8 +26,21 @@ struct ProfRec {
     cudaEvent_t a, b;
 };
 
+/* Device copy of one OctLaunch and the launch shape chosen for it. */
+struct OctDev {
+    OctLaunch L;
+    int4 *d_lane = nullptr;
+    int *d_variant = nullptr;
+    int pc = 0, wstride = 0;
+    size_t smem = 0;
+};
+
 struct ewald_ctx {
     bool prof = false;
+    int recip_variant = 0;                 /* 0 auto, 1 complex half-set kernel, 2 octant kernel */
+    double *d_oct_wt = nullptr, *d_oct_tion = nullptr;
+    std::map<long long, OctDev> oct_dev;   /* key: wc | prec << 16 */
+    std::map<long long, int> oct_choice;   /* key: W | prec << 40 | n << 41 ... -> wc */
     std::vector<ProfRec> recs;
     long long launches = 0; /* kernels launched since setup */
     HostTables t;
@@ -182,6 +197,11 @@ extern "C" ewald_status ewald_setup(ewald_ctx **out, int dim, const double *cell
     if (st == EWALD_OK) st = upload(c, &c->d_erfc, t.erfc_tab64);
     if (st == EWALD_OK) st = upload(c, &c->d_erfcf, to_f32(t.erfc_tab32));
     if (st == EWALD_OK) st = ensure(c, &c->qsums, 2 * sizeof(double));
+    if (st == EWALD_OK && t.oct.valid) {
+        std::vector<double> wt(t.oct.wt);
+        wt.resize(wt.size() + (size_t)(t.oct.npb + 1) * 2, 0.0); /* the zero-weight dummy item */
+        st = upload(c, &c->d_oct_wt, wt);
+    }
     if (st != EWALD_OK) { ewald_destroy(c); return st; }
     *out = c;
     return EWALD_OK;
@@ -200,6 +220,33 @@ extern "C" ewald_status ewald_setup_summary(int dim, const double *cell, double 
     if (n_max) for (int k = 0; k < 3; k++) n_max[k] = t.n_max[k];
     if (xi_r) *xi_r = t.xi_r;
     if (v_m) *v_m = t.v_m;
+    return EWALD_OK;
+}
+
+extern "C" ewald_status ewald_oct_plan_summary(int dim, const double *cell, double gamma, double g_cutoff,
+                                               int n_walkers_per_cta, int *n_items, int *npb, int *n_warps,
+                                               double *weight_sum, double *fma_per_particle)
+{
+    HostTables t;
+    std::string err;
+    ewald_status st = build_tables(dim, cell, gamma, g_cutoff, 0.0, &t, &err);
+    if (st != EWALD_OK) return st;
+    if (!t.oct.valid) return EWALD_ESTATE;
+    if (n_walkers_per_cta < 1) return EWALD_EINVAL;
+    const OctPlan &P = t.oct;
+    long double ws = 0;
+    for (int it = 0; it < P.n_items; it++)
+        for (int j = 0; j <= P.npb; j++) {
+            ws += P.wt[((size_t)it * (P.npb + 1) + j) * 2];
+            if (dim == 2) ws += P.wt[((size_t)it * (P.npb + 1) + j) * 2 + 1];
+        }
+    OctLaunch L;
+    make_oct_launch(P, n_walkers_per_cta, &L);
+    if (n_items) *n_items = P.n_items;
+    if (npb) *npb = P.npb;
+    if (n_warps) *n_warps = L.n_warps;
+    if (weight_sum) *weight_sum = (double)ws;
+    if (fma_per_particle) *fma_per_particle = L.cost / n_walkers_per_cta;
     return EWALD_OK;
 }
 
@@ -228,11 +275,20 @@ extern "C" void ewald_destroy(ewald_ctx *c)
     cudaFree(c->d_gn); cudaFree(c->d_w2); cudaFree(c->d_w2f); cudaFree(c->d_img); cudaFree(c->d_imgf);
     cudaFree(c->d_ion_rho); cudaFree(c->d_ion_rhof); cudaFree(c->d_ion_pos); cudaFree(c->d_ion_posf);
     cudaFree(c->d_ion_q); cudaFree(c->d_ion_qf); cudaFree(c->d_erfc); cudaFree(c->d_erfcf);
+    cudaFree(c->d_oct_wt); cudaFree(c->d_oct_tion);
+    for (auto &kv : c->oct_dev) { cudaFree(kv.second.d_lane); cudaFree(kv.second.d_variant); }
     DevBuf *bufs[] = {&c->partial_recip, &c->partial_real, &c->qsums, &c->stage_pos, &c->stage_q,
                       &c->stage_e, &c->stage_comp, &c->mv_walker, &c->mv_electron, &c->mv_newr,
                       &c->mv_de, &c->st_pos, &c->st_q, &c->st_rho};
     for (DevBuf *b : bufs) release(b);
     delete c;
+}
+
+extern "C" ewald_status ewald_set_recip_variant(ewald_ctx *c, int variant)
+{
+    if (!c || variant < 0 || variant > 2) return EWALD_EINVAL;
+    c->recip_variant = variant;
+    return EWALD_OK;
 }
 
 extern "C" ewald_status ewald_set_stream(ewald_ctx *c, void *stream)
@@ -257,6 +313,11 @@ extern "C" ewald_status ewald_set_fixed_charges(ewald_ctx *c, int n_ion, const d
     if (st == EWALD_OK) st = upload(c, &c->d_ion_posf, to_f32(t.ion_pos));
     if (st == EWALD_OK) st = upload(c, &c->d_ion_q, t.ion_q);
     if (st == EWALD_OK) st = upload(c, &c->d_ion_qf, to_f32(t.ion_q));
+    if (st == EWALD_OK) {
+        std::vector<double> ti(t.oct.tion);
+        if (!ti.empty()) ti.resize(ti.size() + (size_t)(1 + 2 * t.oct.npb) * 4, 0.0);
+        st = upload(c, &c->d_oct_tion, ti);
+    }
     c->loaded = false; /* a stored rho(G) would no longer match */
     return st;
 }
@@ -328,6 +389,147 @@ static ewald_status launch_recip(ewald_ctx *c, int W, int n, const T *pos, const
     return EWALD_OK;
 }
 
+/* ---- octant-form reciprocal kernel: launch shape and launch -------------------------------- */
+
+template <typename T, int DIM, int NPB>
+static ewald_status oct_launch_inst(ewald_ctx *c, const OctArgs<T> &A, int grid, int threads, size_t smem,
+                                    int *ctas_per_sm /* nullable: query only */)
+{
+    ewald_status st = allow_smem(c, recip_oct_kernel<T, DIM, NPB>, smem);
+    if (st != EWALD_OK) return st;
+    if (ctas_per_sm) {
+        CU_TRY(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(ctas_per_sm, recip_oct_kernel<T, DIM, NPB>,
+                                                                threads, smem));
+        return EWALD_OK;
+    }
+    ProfScope ps(c, 0);
+    recip_oct_kernel<T, DIM, NPB><<<grid, threads, smem, c->stream>>>(A);
+    return EWALD_OK;
+}
+
+template <typename T>
+static ewald_status oct_launch_any(ewald_ctx *c, const OctArgs<T> &A, int grid, int threads, size_t smem,
+                                   int *ctas_per_sm)
+{
+    const int dim = c->t.dim, npb = c->t.oct.npb;
+#define EWALD_OCT_INST(D, N) if (dim == D && npb == N) return oct_launch_inst<T, D, N>(c, A, grid, threads, smem, ctas_per_sm);
+    EWALD_OCT_INST(3, 4) EWALD_OCT_INST(3, 5) EWALD_OCT_INST(3, 6) EWALD_OCT_INST(3, 7)
+    EWALD_OCT_INST(2, 4) EWALD_OCT_INST(2, 5) EWALD_OCT_INST(2, 6) EWALD_OCT_INST(2, 7)
+#undef EWALD_OCT_INST
+    return fail(c, EWALD_ERANGE, "no octant kernel for this block length");
+}
+
+template <typename T> static int oct_max_threads(int npb)
+{
+    return sizeof(T) == 8 ? (npb >= 6 ? 256 : 384) : (npb >= 6 ? 384 : 512);
+}
+
+/* Shared-memory shape of a CTA of wc walkers: particles per chunk, slab stride, bytes. */
+static bool oct_shape(const OctPlan &P, int wc, int n_warps, int n, size_t es2, int *pc, int *wstride, size_t *smem)
+{
+    const int threads = 32 * n_warps;
+    int p = (OCT_MAX_TASKS * threads) / (wc * P.dim);
+    if (p > 32) p = 32;
+    if (p > n) p = n;
+    for (; p >= 1; p--) {
+        const int ws = p * P.rowlen + 1; /* +1 pair: staggers the walkers' slabs over the banks */
+        const size_t b = ((size_t)wc * ws + P.npb + 1) * es2 + (size_t)threads * sizeof(double);
+        if (b <= 200 * 1024) { *pc = p; *wstride = ws; *smem = b; return true; }
+    }
+    return false;
+}
+
+template <typename T>
+static ewald_status get_oct_dev(ewald_ctx *c, int wc, OctDev **out)
+{
+    const long long key = wc;
+    auto it = c->oct_dev.find(key);
+    if (it == c->oct_dev.end()) {
+        OctDev d;
+        make_oct_launch(c->t.oct, wc, &d.L);
+        CU_TRY(c, cudaMalloc((void **)&d.d_lane, d.L.lane.size() * sizeof(int)));
+        CU_TRY(c, cudaMemcpy(d.d_lane, d.L.lane.data(), d.L.lane.size() * sizeof(int), cudaMemcpyHostToDevice));
+        CU_TRY(c, cudaMalloc((void **)&d.d_variant, d.L.variant.size() * sizeof(int)));
+        CU_TRY(c, cudaMemcpy(d.d_variant, d.L.variant.data(), d.L.variant.size() * sizeof(int), cudaMemcpyHostToDevice));
+        it = c->oct_dev.emplace(key, d).first;
+    }
+    *out = &it->second;
+    return EWALD_OK;
+}
+
+template <typename T>
+static void oct_fill_args(ewald_ctx *c, OctArgs<T> *A, int W, int n, const T *pos, const T *q,
+                          const OctDev &d, int pc, int wstride, double *e_recip)
+{
+    const OctPlan &P = c->t.oct;
+    A->pos = pos; A->q = q; A->n = n; A->npad = ewald_padded_n(n); A->n_walkers = W;
+    A->wc = d.L.wc; A->pc = pc; A->rowlen = P.rowlen; A->wstride = wstride;
+    for (int k = 0; k < 3; k++) { A->off[k] = P.off[k]; A->nmax[k] = c->t.n_max[k]; }
+    A->lane = d.d_lane; A->variant = d.d_variant;
+    A->wt = c->d_oct_wt; A->tion = c->t.n_ion ? c->d_oct_tion : nullptr;
+    A->e_recip = e_recip;
+    for (int i = 0; i < 9; i++) A->binv[i] = (T)c->t.binv[i];
+}
+
+/* Picks the walkers-per-CTA that minimises (waves x work per wave) on this device. */
+template <typename T>
+static ewald_status oct_choose(ewald_ctx *c, int W, int n, int *wc_out)
+{
+    const long long key = (long long)W | ((long long)n << 24) | ((long long)(sizeof(T) == 4) << 60);
+    auto it = c->oct_choice.find(key);
+    if (it != c->oct_choice.end()) { *wc_out = it->second; return EWALD_OK; }
+    const OctPlan &P = c->t.oct;
+    cudaDeviceProp prop;
+    CU_TRY(c, cudaGetDeviceProperties(&prop, c->device));
+    const int sms = prop.multiProcessorCount, max_warps = oct_max_threads<T>(P.npb) / 32;
+    double best = 1e300;
+    int best_wc = 0;
+    for (int wc = 1; wc <= 16 && wc <= W; wc++) {
+        if ((long long)wc * P.n_items > 32LL * max_warps) break;
+        OctDev *d;
+        ewald_status st = get_oct_dev<T>(c, wc, &d);
+        if (st != EWALD_OK) return st;
+        int pc, ws; size_t smem;
+        if (!oct_shape(P, wc, d->L.n_warps, n, 2 * sizeof(T), &pc, &ws, &smem)) continue;
+        OctArgs<T> A;
+        int per_sm = 0;
+        st = oct_launch_any<T>(c, A, 0, 32 * d->L.n_warps, smem, &per_sm);
+        if (st != EWALD_OK) return st;
+        if (per_sm < 1) continue;
+        const long long ctas = (W + wc - 1) / wc;
+        const long long waves = (ctas + (long long)sms * per_sm - 1) / ((long long)sms * per_sm);
+        /* work of one CTA per particle: FMA phase + table rows (~90 operations per (walker, axis)) */
+        const double cta_work = d->L.cost + 90.0 * P.dim * wc;
+        const double t = (double)waves * per_sm * cta_work;
+        if (t < best * (1 - 1e-9)) { best = t; best_wc = wc; }
+    }
+    if (!best_wc) return fail(c, EWALD_ERANGE, "octant kernel: no launch shape fits");
+    c->oct_choice[key] = best_wc;
+    *wc_out = best_wc;
+    return EWALD_OK;
+}
+
+template <typename T>
+static ewald_status launch_recip_oct(ewald_ctx *c, int W, int n, const T *pos, const T *q, int *n_slabs_out)
+{
+    ewald_status st = ensure(c, &c->partial_recip, (size_t)W * sizeof(double));
+    if (st != EWALD_OK) return st;
+    int wc = 0;
+    if ((st = oct_choose<T>(c, W, n, &wc)) != EWALD_OK) return st;
+    OctDev *d;
+    if ((st = get_oct_dev<T>(c, wc, &d)) != EWALD_OK) return st;
+    int pc, ws; size_t smem;
+    if (!oct_shape(c->t.oct, wc, d->L.n_warps, n, 2 * sizeof(T), &pc, &ws, &smem))
+        return fail(c, EWALD_ERANGE, "octant kernel: shared memory");
+    OctArgs<T> A;
+    oct_fill_args<T>(c, &A, W, n, pos, q, *d, pc, ws, (double *)c->partial_recip.p);
+    st = oct_launch_any<T>(c, A, (W + wc - 1) / wc, 32 * d->L.n_warps, smem, nullptr);
+    if (st != EWALD_OK) return st;
+    CU_TRY(c, cudaGetLastError());
+    *n_slabs_out = 1;
+    return EWALD_OK;
+}
+
 template <typename T>
 static ewald_status launch_real(ewald_ctx *c, int W, int n, const T *pos, const T *q, int *n_tiles_out)
 {
@@ -387,7 +589,10 @@ static ewald_status energy_batch_t(ewald_ctx *c, int W, int n, const T *pos, con
         charge_sums_kernel<T><<<1, 256, 0, c->stream>>>(q, n, (double *)c->qsums.p);
     }
     CU_TRY(c, cudaGetLastError());
-    ewald_status st = launch_recip<T>(c, W, n, pos, q, nullptr, &n_slabs);
+    const bool oct = c->recip_variant != 1 && c->t.oct.valid;
+    if (c->recip_variant == 2 && !oct) return fail(c, EWALD_ESTATE, "octant kernel needs an orthorhombic cell");
+    ewald_status st = oct ? launch_recip_oct<T>(c, W, n, pos, q, &n_slabs)
+                          : launch_recip<T>(c, W, n, pos, q, nullptr, &n_slabs);
     if (st != EWALD_OK) return st;
     st = launch_real<T>(c, W, n, pos, q, &n_tiles);
     if (st != EWALD_OK) return st;

@@ -10,6 +10,28 @@
 
 namespace ewald {
 
+/* Host plan of the octant-form reciprocal kernel (ewald_recip_oct.cuh; orthorhombic cells only).
+ * An item is a column (n2, n3) -- in 2D a pair of n2 values -- with a block of <= npb consecutive
+ * n1 >= 1 (block 0 also carries n1 = 0).  Offsets are in (cos,sin)-pair units within a table row. */
+struct OctPlan {
+    bool valid = false;
+    int dim = 3, npb = 0;
+    int rowlen = 0, off[3] = {0, 0, 0};
+    int n_items = 0;
+    std::vector<int> offA, offB, offX, np, c0; /* [n_items] */
+    std::vector<int> col;                      /* [n_items][3] = n2 (2D: n2a), n3 (2D: n2b or -1), first n1 of the block - 1 */
+    std::vector<double> wt;                    /* [n_items][1 + npb][2] */
+    std::vector<double> tion;                  /* [n_items][1 + 2 npb][4]; empty without fixed charges */
+};
+
+/* Lane assignment of one CTA of `wc` walkers: items of all its walkers sorted by block length. */
+struct OctLaunch {
+    int wc = 0, n_warps = 0;
+    double cost = 0;            /* executed FMA + product operations per particle, whole CTA */
+    std::vector<int> lane;      /* [32 n_warps][4] = local walker, item, offA | offB << 16, offX */
+    std::vector<int> variant;   /* [n_warps] np | c0 << 8 */
+};
+
 /* Everything ewald_setup computes on the host, in long double, before rounding (PAPER.md:359:
  * "lookup tables for Ewald interactions ... always performed using DP arithmetic"). */
 struct HostTables {
@@ -41,7 +63,14 @@ struct HostTables {
     std::vector<double> ion_q;
     std::vector<double> ion_rho; /* [ngp][2], sum_I q_I exp(iG.r_I)                              */
     double ion_q2 = 0, ion_qsum = 0, ion_real = 0; /* sum q^2, sum q, sum_{I<J} q_I q_J psi(r_IJ) */
+    OctPlan oct;
 };
+
+struct HostTables;
+void build_oct_plan(HostTables *t);
+void fill_oct_ion(HostTables *t);
+void make_oct_launch(const OctPlan &p, int wc, OctLaunch *out);
+
 
 /* Returns EWALD_OK or an error status with a message. */
 ewald_status build_tables(int dim, const double *cell, double kappa, double g_cutoff,

@@ -1,0 +1,211 @@
+/* ewald_recip_oct.cuh -- [S1-S4] reciprocal-space energy in the octant (real-product) form.
+ *
+ * For an orthorhombic cell G.r = 2 pi sum_k n_k s_k (s = fractional coordinates) and Eq. 8
+ * factorises exp(iG.r) into per-axis powers.  Taking real and imaginary parts per axis,
+ * the eight real sums over particles
+ *     T_abc(n) = sum_i q_i t^a(2 pi n1 s_i1) t^b(2 pi n2 s_i2) t^c(2 pi n3 s_i3),  t in {cos, sin}, n_k >= 0
+ * give rho(+-n1, +-n2, +-n3) for all sign choices, and summing |rho|^2 over the sign choices leaves
+ *     E_recip = sum_{n >= 0, n != 0} w(G_n) 2^{nz(n)} sum_abc T_abc(n)^2
+ * (nz = number of non-zero n_k; every cross term cancels).  One real FMA per (particle, G of the
+ * full sphere): the algorithmic count 2 N N_G flops per walker, half of the complex half-set form.
+ *
+ * Work decomposition (host plan, ewald_octplan.cpp):
+ *   row    per (walker, particle): the "powers ... computed and buffered" of PAPER.md:157, in shared
+ *          memory as (cos, sin) pairs: X1[n=1..], X2[n=0..], X3[n=0..] (the last axis carries q_i)
+ *   item   a column (n2, n3) and a block of <= NPB consecutive n1 (plus n1 = 0 in the first block);
+ *          in 2D a pair of n2 values
+ *   lane   owns one (walker, item) for the whole kernel: 4 products p = X2 (x) X3 (unique per lane)
+ *          times the X1 pairs of the block (one broadcast LDS.128 per pair) -> 4 x (1 + 2 NP) register
+ *          accumulators, 4 (1 + 2 NP) FMA per 2 + NP shared-memory loads
+ *   warp   32 lanes of equal block length: the items of all walkers of the CTA are sorted by length, so
+ *          the spherical cut-off costs no divergent lanes
+ */
+#pragma once
+#include "ewald_kernels_common.cuh"
+
+namespace ewald {
+
+template <typename T> struct OctArgs {
+    const T *pos;       /* [W][DIM][npad] */
+    const T *q;         /* [n] */
+    int n, npad, n_walkers;
+    int wc;             /* walkers per CTA */
+    int pc;             /* particles per chunk */
+    int rowlen;         /* (cos,sin) pairs per (walker, particle) row */
+    int wstride;        /* pairs per walker slab (pc * rowlen + bank stagger) */
+    int off[3];         /* pair offset of X1 (n = 1..), X2 (n = 0..), X3 (n = 0..) within a row */
+    int nmax[3];
+    const int4 *lane;   /* [blockDim.x] {local walker, item, offA | offB << 16, offX} */
+    const int *variant; /* [n_warps] NP | C0 << 8 */
+    const double *wt;   /* [n_items][1 + NPB][2]: w(G) 2^nz per entry for products (0,1) and (2,3) */
+    const double *tion; /* [n_items][1 + 2 NPB][4] fixed-charge sums, or null */
+    double *e_recip;    /* [W] */
+    T binv[9];
+};
+
+/* Threads per CTA the register file allows: 4 (1 + 2 NPB) accumulators per lane (doubles take two
+ * registers each): FP64 NPB = 7 needs ~254 registers -> 256 threads; NPB <= 5 fits 168 -> 384. */
+template <typename T, int NPB> struct OctCfg {
+    static constexpr int MAX_THREADS = sizeof(T) == 8 ? (NPB >= 6 ? 256 : 384) : (NPB >= 6 ? 384 : 512);
+};
+constexpr int OCT_MAX_TASKS = 3; /* table rows built per thread per chunk */
+
+/* One chunk of particles for one lane: acc[k][e] += p_k * X1_e. */
+template <typename T, int NPB, int NP, bool C0, int MODE>
+__device__ __forceinline__ void oct_fma(T (&acc)[4][1 + 2 * NPB], const typename Num<T>::T2 *rA,
+                                        const typename Num<T>::T2 *rB, const typename Num<T>::T2 *rX,
+                                        int cnt, int rowlen)
+{
+    typedef typename Num<T>::T2 T2;
+#pragma unroll 2
+    for (int p = 0; p < cnt; p++) {
+        const T2 a = *rA, b = *rB;
+        T pr[4];
+        if (MODE == 0) { pr[0] = a.x * b.x; pr[1] = a.x * b.y; pr[2] = a.y * b.x; pr[3] = a.y * b.y; }
+        else { pr[0] = a.x; pr[1] = a.y; pr[2] = b.x; pr[3] = b.y; }
+        if (C0) {
+#pragma unroll
+            for (int k = 0; k < 4; k++) acc[k][0] += pr[k];
+        }
+#pragma unroll
+        for (int j = 0; j < NP; j++) {
+            const T2 cs = rX[j];
+#pragma unroll
+            for (int k = 0; k < 4; k++) {
+                acc[k][1 + 2 * j] = fma(pr[k], cs.x, acc[k][1 + 2 * j]);
+                acc[k][2 + 2 * j] = fma(pr[k], cs.y, acc[k][2 + 2 * j]);
+            }
+        }
+        rA += rowlen; rB += rowlen; rX += rowlen;
+    }
+}
+
+template <typename T, int NPB, int MODE, int NP>
+__device__ __forceinline__ void oct_dispatch_c0(T (&acc)[4][1 + 2 * NPB], bool c0,
+                                                const typename Num<T>::T2 *rA, const typename Num<T>::T2 *rB,
+                                                const typename Num<T>::T2 *rX, int cnt, int rowlen)
+{
+    if (c0) oct_fma<T, NPB, NP, true, MODE>(acc, rA, rB, rX, cnt, rowlen);
+    else oct_fma<T, NPB, NP, false, MODE>(acc, rA, rB, rX, cnt, rowlen);
+}
+
+template <typename T, int DIM, int NPB>
+__global__ void __launch_bounds__(OctCfg<T, NPB>::MAX_THREADS) recip_oct_kernel(OctArgs<T> A)
+{
+    typedef typename Num<T>::T2 T2;
+    constexpr int MODE = DIM == 3 ? 0 : 1;
+    constexpr int NE = 1 + 2 * NPB;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    T2 *tab = reinterpret_cast<T2 *>(smem_raw);                                   /* [wc][wstride] + slack */
+    double *part = reinterpret_cast<double *>(tab + (size_t)A.wc * A.wstride + NPB + 1); /* [blockDim.x] */
+
+    const int tid = threadIdx.x, nthreads = blockDim.x, warp = tid >> 5;
+    const int w0 = blockIdx.x * A.wc;
+    const int4 L = A.lane[tid];
+    const int var = A.variant[warp];
+    const int np = var & 255;
+    const bool c0 = (var >> 8) != 0;
+    const T2 *lane_base = tab + (size_t)L.x * A.wstride;
+    const T2 *baseA = lane_base + (L.z & 0xffff), *baseB = lane_base + (L.z >> 16), *baseX = lane_base + L.w;
+
+    T acc[4][NE];
+#pragma unroll
+    for (int k = 0; k < 4; k++)
+#pragma unroll
+        for (int e = 0; e < NE; e++) acc[k][e] = 0;
+
+    /* build tasks of this thread: t = tid + u * nthreads -> (axis k, local walker wl, particle p) */
+    const int per_axis = A.wc * A.pc, n_tasks = per_axis * DIM;
+    T xin[OCT_MAX_TASKS][DIM];
+
+    auto fetch = [&](int base_p) {
+#pragma unroll
+        for (int u = 0; u < OCT_MAX_TASKS; u++) {
+            const int t = tid + u * nthreads;
+            const int rem = t % per_axis, wl = rem / A.pc, p = rem - wl * A.pc;
+            const bool ok = t < n_tasks && base_p + p < A.n && w0 + wl < A.n_walkers;
+            const T *pw = A.pos + (size_t)(ok ? w0 + wl : 0) * DIM * A.npad + (ok ? base_p + p : 0);
+#pragma unroll
+            for (int x = 0; x < DIM; x++) xin[u][x] = pw[x * A.npad];
+        }
+    };
+
+    fetch(0);
+    for (int base_p = 0; base_p < A.n; base_p += A.pc) {
+        const int cnt = min(A.pc, A.n - base_p);
+        __syncthreads(); /* the previous chunk has been consumed */
+        /* [S1,S2] phase seeds and power rows */
+#pragma unroll
+        for (int u = 0; u < OCT_MAX_TASKS; u++) {
+            const int t = tid + u * nthreads;
+            if (t >= n_tasks) continue;
+            const int k = t / per_axis, rem = t - k * per_axis, wl = rem / A.pc, p = rem - wl * A.pc;
+            if (p >= cnt || w0 + wl >= A.n_walkers) continue;
+            T s = 0;
+#pragma unroll
+            for (int x = 0; x < DIM; x++) s += xin[u][x] * A.binv[3 * k + x];
+            s -= Num<T>::rint_(s);
+            T sn, cs;
+            Num<T>::sincospi_(2 * s, &sn, &cs);
+            const T scale = k == DIM - 1 ? A.q[base_p + p] : T(1);
+            T2 *row = tab + (size_t)wl * A.wstride + (size_t)p * A.rowlen + A.off[k];
+            T2 e; e.x = scale; e.y = 0;
+            if (k > 0) row[0] = e; else row -= 1; /* axis 1 stores n = 1.. only */
+            for (int n = 1; n <= A.nmax[k]; n++) {
+                T2 f;
+                f.x = e.x * cs - e.y * sn;
+                f.y = e.x * sn + e.y * cs;
+                e = f;
+                row[n] = e;
+            }
+        }
+        __syncthreads();
+        if (base_p + A.pc < A.n) fetch(base_p + A.pc); /* next chunk's positions fly during the FMA phase */
+        /* [S3] */
+        switch (np) {
+#define EWALD_OCT_CASE(NP)                                                                              \
+    case NP:                                                                                            \
+        if (NP <= NPB) oct_dispatch_c0<T, NPB, MODE, (NP <= NPB ? NP : 0)>(acc, c0, baseA, baseB, baseX, cnt, A.rowlen); \
+        break;
+            EWALD_OCT_CASE(0) EWALD_OCT_CASE(1) EWALD_OCT_CASE(2) EWALD_OCT_CASE(3)
+            EWALD_OCT_CASE(4) EWALD_OCT_CASE(5) EWALD_OCT_CASE(6) EWALD_OCT_CASE(7)
+#undef EWALD_OCT_CASE
+        default: break;
+        }
+    }
+
+    /* [S4] E_recip = sum w 2^nz T^2, in FP64; entries of weight zero are padding (never read as values) */
+    double e = 0;
+    {
+        const double *wt = A.wt + (size_t)L.y * (NPB + 1) * 2;
+        const double *ti = A.tion ? A.tion + (size_t)L.y * NE * 4 : nullptr;
+#pragma unroll
+        for (int j = 0; j <= NPB; j++) {
+            const double wlo = wt[2 * j], whi = wt[2 * j + 1];
+#pragma unroll
+            for (int k = 0; k < 4; k++) {
+                const double wk = k < 2 ? wlo : whi;
+                if (j == 0) {
+                    double v = (double)acc[k][0];
+                    if (ti) v += ti[k];
+                    e += wk != 0 ? wk * v * v : 0.0;
+                } else {
+                    double vc = (double)acc[k][2 * j - 1], vs = (double)acc[k][2 * j];
+                    if (ti) { vc += ti[(2 * j - 1) * 4 + k]; vs += ti[(2 * j) * 4 + k]; }
+                    e += wk != 0 ? wk * (vc * vc + vs * vs) : 0.0;
+                }
+            }
+        }
+    }
+    __syncthreads();
+    part[tid] = e;
+    __syncthreads();
+    if (tid < A.wc && w0 + tid < A.n_walkers) {
+        double s = 0; /* fixed order: deterministic */
+        for (int t = 0; t < nthreads; t++)
+            if (A.lane[t].x == tid) s += part[t];
+        A.e_recip[w0 + tid] = s;
+    }
+}
+
+} // namespace ewald

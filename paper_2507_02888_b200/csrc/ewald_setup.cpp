@@ -196,6 +196,7 @@ ewald_status build_tables(int dim, const double *cell, double kappa_d, double g_
     t->n_ion = 0;
     t->ion_pos.clear(); t->ion_q.clear(); t->ion_rho.clear();
     t->ion_q2 = t->ion_qsum = t->ion_real = 0;
+    build_oct_plan(t);
     return EWALD_OK;
 }
 
@@ -264,6 +265,7 @@ ewald_status build_fixed_charges(HostTables *t, int n_ion, const double *pos, co
             e += (real)q[i] * q[j] * psi;
         }
     t->ion_real = (double)e;
+    fill_oct_ion(t);
     return EWALD_OK;
 }
 

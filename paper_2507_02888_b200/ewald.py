@@ -18,8 +18,9 @@ _STATUS = {0: "EWALD_OK", 1: "EWALD_EINVAL", 2: "EWALD_ESINGULAR", 3: "EWALD_ERA
            4: "EWALD_ESTATE", 5: "EWALD_ECUDA", 6: "EWALD_ENOMEM"}
 
 # every symbol include/ewald.h declares (checked by tests/test_abi.py against the header text)
-SYMBOLS = ["ewald_padded_n", "ewald_setup", "ewald_setup_summary", "ewald_erfc_table_eval",
-           "ewald_destroy", "ewald_set_stream",
+SYMBOLS = ["ewald_padded_n", "ewald_setup", "ewald_setup_summary", "ewald_oct_plan_summary",
+           "ewald_erfc_table_eval",
+           "ewald_destroy", "ewald_set_stream", "ewald_set_recip_variant",
            "ewald_set_fixed_charges", "ewald_energy_batch", "ewald_energy_batch_host",
            "ewald_load_walkers", "ewald_move_delta_batch", "ewald_move_delta_batch_host",
            "ewald_move_delta", "ewald_num_g", "ewald_num_images", "ewald_r_cutoff", "ewald_get_g",
@@ -59,8 +60,10 @@ def load_library():
         "ewald_setup": (i, [ctypes.POINTER(vp), i, dp, d, d, ctypes.POINTER(_Opts)]),
         "ewald_setup_summary": (i, [i, dp, d, d, d, ip, ip, ip, dp, dp]),
         "ewald_erfc_table_eval": (i, [d, i, i, dp, dp]),
+        "ewald_oct_plan_summary": (i, [i, dp, d, d, i, ip, ip, ip, dp, dp]),
         "ewald_destroy": (None, [vp]),
         "ewald_set_stream": (i, [vp, vp]),
+        "ewald_set_recip_variant": (i, [vp, i]),
         "ewald_set_fixed_charges": (i, [vp, i, dp, dp]),
         "ewald_energy_batch": (i, [vp, i, i, i, vp, vp, vp, vp]),
         "ewald_energy_batch_host": (i, [vp, i, i, i, vp, vp, vp, vp]),
@@ -188,6 +191,20 @@ def ewald_setup_summary(dim, cell, gamma, g_cutoff, r_cutoff=0.0):
     return dict(num_g=ng.value, num_images=ni.value, n_max=list(nm), xi_r=xi.value, v_m=vm.value)
 
 
+def ewald_oct_plan_summary(dim, cell, gamma, g_cutoff, n_walkers_per_cta=1):
+    """Host-only: work plan of the octant-form reciprocal kernel (orthorhombic cells)."""
+    c = _cell9(cell, dim)
+    ni, nb, nw = ctypes.c_int(), ctypes.c_int(), ctypes.c_int()
+    ws, fm = ctypes.c_double(), ctypes.c_double()
+    st = load_library().ewald_oct_plan_summary(dim, _dp(c), float(gamma), float(g_cutoff),
+                                               int(n_walkers_per_cta), ctypes.byref(ni), ctypes.byref(nb),
+                                               ctypes.byref(nw), ctypes.byref(ws), ctypes.byref(fm))
+    if st != 0:
+        raise EwaldError(st, "ewald_oct_plan_summary failed")
+    return dict(n_items=ni.value, npb=nb.value, n_warps=nw.value, weight_sum=ws.value,
+                fma_per_particle=fm.value)
+
+
 def ewald_erfc_table_eval(z_max, degree, z):
     """Host-only: the setup's piecewise polynomial for erfc evaluated at z (array)."""
     z = np.ascontiguousarray(z, dtype=np.float64)
@@ -200,6 +217,11 @@ def ewald_erfc_table_eval(z_max, degree, z):
 
 def ewald_destroy(ctx):
     ctx.close()
+
+
+def ewald_set_recip_variant(ctx, variant):
+    """0 automatic, 1 complex half-set reciprocal kernel, 2 octant-form kernel."""
+    _check(ctx, load_library().ewald_set_recip_variant(ctx.handle, int(variant)))
 
 
 def ewald_set_stream(ctx, stream):

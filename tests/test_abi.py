@@ -112,3 +112,47 @@ def test_erfc_table_matches_erfc():
         got32 = E.ewald_erfc_table_eval(z_max, 6, z)
         assert np.abs(got64 - want).max() < 2.5e-15
         assert np.abs(got32 - want).max() < 2e-8
+
+
+def _full_sphere_weight_sum(dim, L, kappa, n2_max):
+    """sum over 0 < n^2 <= n2_max of w(G), G = 2 pi n / L, with w of DESIGN.md section 2 (cubic / square)."""
+    nm = math.isqrt(n2_max)
+    rng = range(-nm, nm + 1)
+    tot = 0.0
+    for n1 in rng:
+        for n2 in rng:
+            for n3 in (rng if dim == 3 else (0,)):
+                m = n1 * n1 + n2 * n2 + n3 * n3
+                if m == 0 or m > n2_max:
+                    continue
+                g = 2 * math.pi / L * math.sqrt(m)
+                if dim == 3:
+                    tot += 2 * math.pi / L ** 3 * math.exp(-g * g / (4 * kappa * kappa)) / (g * g)
+                else:
+                    tot += math.pi / L ** 2 * math.erfc(g / (2 * kappa)) / g
+    return tot
+
+
+def test_octant_plan_covers_every_g_once():
+    # sum over the octant of w(G_n) 2^nz must equal the full-sphere sum of w(G) (DESIGN.md section 5.1)
+    for idx in range(1, 6):
+        w = workloads.config(idx)
+        ng = E.ewald_setup_summary(w.dim, w.cell, w.kappa, w.g_cutoff, w.r_cutoff)["num_g"]
+        for wc in (1, 3, 7):
+            o = E.ewald_oct_plan_summary(w.dim, w.cell, w.kappa, w.g_cutoff, wc)
+            want = _full_sphere_weight_sum(w.dim, w.L, w.kappa, w.n2_max)
+            assert abs(o["weight_sum"] - want) <= 1e-13 * want
+            assert 4 <= o["npb"] <= 7 and o["n_warps"] == -(-wc * o["n_items"] // 32)
+            # executed FMA + products per particle can never be below the algorithmic N_G + 1
+            assert o["fma_per_particle"] >= ng + 1
+        assert (ng + 1) / o["fma_per_particle"] > 0.6   # wc = 7: the cut-off wastes < 40 % of the lanes
+
+
+def test_octant_plan_orthorhombic_only():
+    cell = np.array([[4.0, 0, 0], [0, 5.0, 0], [0, 0, 6.5]])
+    o = E.ewald_oct_plan_summary(3, cell, 0.9, 5.0, 2)
+    assert o["n_items"] > 0
+    tri = np.array([[4.0, 0, 0], [1.0, 5.0, 0], [0, 0, 6.5]])
+    with pytest.raises(E.EwaldError) as ei:
+        E.ewald_oct_plan_summary(3, tri, 0.9, 5.0, 2)
+    assert ei.value.status == 4

@@ -83,6 +83,55 @@ def test_energy_fp64_matches_oracle(torch_cuda, idx):
     assert E.ewald_num_g(ctx) == ref.num_g(w.dim, w.cell, w.g_cutoff)
 
 
+@pytest.mark.parametrize("idx", [1, 2, 3, 4])
+def test_both_reciprocal_kernels_match_oracle(torch_cuda, idx):
+    """Octant real-product form (variant 2) and complex half-set form (variant 1), FP64 and FP32, on
+    walker counts that leave the last CTA of the octant kernel partly empty."""
+    w = workloads.config(idx)
+    nw = {1: 8, 2: 9, 3: 11, 4: 5}[idx]
+    pos = w.positions(nw)
+    e_ref, c_ref = _oracle_energy(w, pos)
+    e32_ref, c32_ref = _oracle_energy(w, _r32(pos))
+    ctx = _ctx(w)
+    for variant in (1, 2):
+        E.ewald_set_recip_variant(ctx, variant)
+        e, c = _gpu_energy(torch_cuda, ctx, pos, w.charges, "f64")
+        _assert_energy(e, c, e_ref, c_ref, TOL64)
+        assert (np.abs(c[:, 0] - c_ref[:, 0]) / np.abs(c_ref[:, 0])).max() <= 1e-12  # E_recip itself
+        e, c = _gpu_energy(torch_cuda, ctx, _r32(pos), w.charges, "f32")
+        assert (np.abs(e - e32_ref) / np.abs(e32_ref)).max() <= TOL32
+        assert (np.abs(c[:, 0] - c32_ref[:, 0]) / np.abs(c32_ref[:, 0])).max() <= TOL32
+    with pytest.raises(E.EwaldError):
+        E.ewald_set_recip_variant(ctx, 3)
+
+
+def test_octant_kernel_orthorhombic_cells_and_single_walker(torch_cuda):
+    rng = np.random.default_rng(77)
+    for dim in (2, 3):
+        cell = np.diag([5.0, 6.5, 4.2][:dim])
+        kappa = 1.1
+        gc, rc = ref.auto_cutoffs(dim, cell, kappa, 1e-17)
+        for n, nw in ((1, 1), (3, 2), (37, 17)):
+            pos = rng.random((nw, n, dim)) @ cell
+            q = rng.choice([-1.0, 2.0], size=n)
+            e_ref, c_ref = ref.energy_batch(dim, cell, kappa, gc, rc, pos, q)
+            ctx = E.ewald_setup(dim, cell, kappa, gc, rc)
+            E.ewald_set_recip_variant(ctx, 2)
+            e, c = _gpu_energy(torch_cuda, ctx, pos, q, "f64")
+            assert (np.abs(c[:, 0] - c_ref[:, 0]) / np.abs(c_ref[:, 0])).max() <= 1e-12
+            _assert_energy(e, c, e_ref, c_ref, TOL64)
+
+
+def test_octant_kernel_refuses_general_cells(torch_cuda):
+    cell = np.array([[5.0, 0, 0], [1.5, 4.0, 0], [0.3, 0.2, 6.0]])
+    ctx = E.ewald_setup(3, cell, 1.0, 6.0)
+    E.ewald_set_recip_variant(ctx, 2)
+    pos = np.random.default_rng(1).random((2, 5, 3)) @ cell
+    with pytest.raises(E.EwaldError) as ei:
+        _gpu_energy(torch_cuda, ctx, pos, -np.ones(5), "f64")
+    assert ei.value.status == 4
+
+
 @pytest.mark.parametrize("idx", [2, 3])
 def test_energy_fp32_matches_oracle(torch_cuda, idx):
     w = workloads.config(idx)
