@@ -241,7 +241,7 @@ extern "C" ewald_status ewald_oct_plan_summary(int dim, const double *cell, doub
             if (dim == 2) ws += P.wt[((size_t)it * (P.npb + 1) + j) * 2 + 1];
         }
     OctLaunch L;
-    make_oct_launch(P, n_walkers_per_cta, &L);
+    make_oct_launch(P, n_walkers_per_cta, 1 << 20, &L);
     if (n_items) *n_items = P.n_items;
     if (npb) *npb = P.npb;
     if (n_warps) *n_warps = L.n_warps;
@@ -442,11 +442,12 @@ static bool oct_shape(const OctPlan &P, int wc, int n_warps, int n, size_t es2, 
 template <typename T>
 static ewald_status get_oct_dev(ewald_ctx *c, int wc, OctDev **out)
 {
-    const long long key = wc;
+    const int max_warps = oct_max_threads<T>(c->t.oct.npb) / 32;
+    const long long key = wc | ((long long)max_warps << 16);
     auto it = c->oct_dev.find(key);
     if (it == c->oct_dev.end()) {
         OctDev d;
-        make_oct_launch(c->t.oct, wc, &d.L);
+        make_oct_launch(c->t.oct, wc, max_warps, &d.L);
         CU_TRY(c, cudaMalloc((void **)&d.d_lane, d.L.lane.size() * sizeof(int)));
         CU_TRY(c, cudaMemcpy(d.d_lane, d.L.lane.data(), d.L.lane.size() * sizeof(int), cudaMemcpyHostToDevice));
         CU_TRY(c, cudaMalloc((void **)&d.d_variant, d.L.variant.size() * sizeof(int)));
@@ -463,7 +464,7 @@ static void oct_fill_args(ewald_ctx *c, OctArgs<T> *A, int W, int n, const T *po
 {
     const OctPlan &P = c->t.oct;
     A->pos = pos; A->q = q; A->n = n; A->npad = ewald_padded_n(n); A->n_walkers = W;
-    A->wc = d.L.wc; A->pc = pc; A->rowlen = P.rowlen; A->wstride = wstride;
+    A->wc = d.L.wc; A->n_slabs = d.L.n_slabs; A->pc = pc; A->rowlen = P.rowlen; A->wstride = wstride;
     for (int k = 0; k < 3; k++) { A->off[k] = P.off[k]; A->nmax[k] = c->t.n_max[k]; }
     A->lane = d.d_lane; A->variant = d.d_variant;
     A->wt = c->d_oct_wt; A->tion = c->t.n_ion ? c->d_oct_tion : nullptr;
@@ -481,11 +482,10 @@ static ewald_status oct_choose(ewald_ctx *c, int W, int n, int *wc_out)
     const OctPlan &P = c->t.oct;
     cudaDeviceProp prop;
     CU_TRY(c, cudaGetDeviceProperties(&prop, c->device));
-    const int sms = prop.multiProcessorCount, max_warps = oct_max_threads<T>(P.npb) / 32;
+    const int sms = prop.multiProcessorCount;
     double best = 1e300;
     int best_wc = 0;
     for (int wc = 1; wc <= 16 && wc <= W; wc++) {
-        if ((long long)wc * P.n_items > 32LL * max_warps) break;
         OctDev *d;
         ewald_status st = get_oct_dev<T>(c, wc, &d);
         if (st != EWALD_OK) return st;
@@ -496,10 +496,11 @@ static ewald_status oct_choose(ewald_ctx *c, int W, int n, int *wc_out)
         st = oct_launch_any<T>(c, A, 0, 32 * d->L.n_warps, smem, &per_sm);
         if (st != EWALD_OK) return st;
         if (per_sm < 1) continue;
-        const long long ctas = (W + wc - 1) / wc;
+        const long long ctas = (long long)((W + wc - 1) / wc) * d->L.n_slabs;
         const long long waves = (ctas + (long long)sms * per_sm - 1) / ((long long)sms * per_sm);
         /* work of one CTA per particle: FMA phase + table rows (~90 operations per (walker, axis)) */
-        const double cta_work = d->L.cost + 90.0 * P.dim * wc;
+        const double cta_work = d->L.cost / d->L.n_slabs + 90.0 * P.dim * wc;
+        if (d->L.n_slabs > 1 && wc > 1) break; /* several slabs: one walker per group is enough */
         const double t = (double)waves * per_sm * cta_work;
         if (t < best * (1 - 1e-9)) { best = t; best_wc = wc; }
     }
@@ -512,21 +513,23 @@ static ewald_status oct_choose(ewald_ctx *c, int W, int n, int *wc_out)
 template <typename T>
 static ewald_status launch_recip_oct(ewald_ctx *c, int W, int n, const T *pos, const T *q, int *n_slabs_out)
 {
-    ewald_status st = ensure(c, &c->partial_recip, (size_t)W * sizeof(double));
-    if (st != EWALD_OK) return st;
     int wc = 0;
-    if ((st = oct_choose<T>(c, W, n, &wc)) != EWALD_OK) return st;
+    ewald_status st = oct_choose<T>(c, W, n, &wc);
+    if (st != EWALD_OK) return st;
     OctDev *d;
     if ((st = get_oct_dev<T>(c, wc, &d)) != EWALD_OK) return st;
+    if ((st = ensure(c, &c->partial_recip, (size_t)W * d->L.n_slabs * sizeof(double))) != EWALD_OK) return st;
     int pc, ws; size_t smem;
     if (!oct_shape(c->t.oct, wc, d->L.n_warps, n, 2 * sizeof(T), &pc, &ws, &smem))
         return fail(c, EWALD_ERANGE, "octant kernel: shared memory");
     OctArgs<T> A;
     oct_fill_args<T>(c, &A, W, n, pos, q, *d, pc, ws, (double *)c->partial_recip.p);
-    st = oct_launch_any<T>(c, A, (W + wc - 1) / wc, 32 * d->L.n_warps, smem, nullptr);
+    const long long grid = (long long)((W + wc - 1) / wc) * d->L.n_slabs;
+    if (grid > 0x7fffffffLL) return fail(c, EWALD_ERANGE, "grid too large");
+    st = oct_launch_any<T>(c, A, (int)grid, 32 * d->L.n_warps, smem, nullptr);
     if (st != EWALD_OK) return st;
     CU_TRY(c, cudaGetLastError());
-    *n_slabs_out = 1;
+    *n_slabs_out = d->L.n_slabs;
     return EWALD_OK;
 }
 

@@ -26,10 +26,10 @@ struct OctPlan {
 
 /* Lane assignment of one CTA of `wc` walkers: items of all its walkers sorted by block length. */
 struct OctLaunch {
-    int wc = 0, n_warps = 0;
+    int wc = 0, n_warps = 0, n_slabs = 1; /* warps per CTA; CTAs per walker group */
     double cost = 0;            /* executed FMA + product operations per particle, whole CTA */
-    std::vector<int> lane;      /* [32 n_warps][4] = local walker, item, offA | offB << 16, offX */
-    std::vector<int> variant;   /* [n_warps] np | c0 << 8 */
+    std::vector<int> lane;      /* [n_slabs][32 n_warps][4] = local walker, item, offA | offB << 16, offX */
+    std::vector<int> variant;   /* [n_slabs][n_warps] np | c0 << 8 */
 };
 
 /* Everything ewald_setup computes on the host, in long double, before rounding (PAPER.md:359:
@@ -69,7 +69,7 @@ struct HostTables {
 struct HostTables;
 void build_oct_plan(HostTables *t);
 void fill_oct_ion(HostTables *t);
-void make_oct_launch(const OctPlan &p, int wc, OctLaunch *out);
+void make_oct_launch(const OctPlan &p, int wc, int max_warps, OctLaunch *out);
 
 
 /* Returns EWALD_OK or an error status with a message. */

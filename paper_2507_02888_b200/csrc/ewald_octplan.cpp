@@ -139,7 +139,7 @@ void fill_oct_ion(HostTables *t)
     }
 }
 
-void make_oct_launch(const OctPlan &P, int wc, OctLaunch *L)
+void make_oct_launch(const OctPlan &P, int wc, int max_warps, OctLaunch *L)
 {
     struct Key { int len, wl, item; };
     std::vector<Key> v;
@@ -151,9 +151,14 @@ void make_oct_launch(const OctPlan &P, int wc, OctLaunch *L)
         if (x.wl != y.wl) return x.wl < y.wl;
         return x.item < y.item;
     });
-    const int n_warps = (int)((v.size() + 31) / 32);
+    /* the sorted list is cut into n_slabs CTAs of n_warps warps each (one CTA when it fits) */
+    const int total_warps = (int)((v.size() + 31) / 32);
+    const int n_slabs = (total_warps + max_warps - 1) / max_warps;
+    const int per_cta = (total_warps + n_slabs - 1) / n_slabs;
+    const int n_warps = per_cta * n_slabs; /* padded: trailing warps hold dummy items only */
     L->wc = wc;
-    L->n_warps = n_warps;
+    L->n_warps = per_cta;
+    L->n_slabs = n_slabs;
     L->lane.assign((size_t)n_warps * 32 * 4, 0);
     L->variant.assign(n_warps, 0);
     L->cost = 0;
@@ -177,7 +182,7 @@ void make_oct_launch(const OctPlan &P, int wc, OctLaunch *L)
             }
         }
         L->variant[wp] = np | (c0 << 8);
-        L->cost += 32.0 * (4.0 * (2 * np + c0) + (P.dim == 3 ? 4.0 : 0.0));
+        if ((size_t)wp * 32 < v.size()) L->cost += 32.0 * (4.0 * (2 * np + c0) + (P.dim == 3 ? 4.0 : 0.0));
     }
 }
 

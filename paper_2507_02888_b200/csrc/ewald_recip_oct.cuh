@@ -30,16 +30,17 @@ template <typename T> struct OctArgs {
     const T *q;         /* [n] */
     int n, npad, n_walkers;
     int wc;             /* walkers per CTA */
+    int n_slabs;        /* CTAs per walker group: the sorted item list is cut into slabs */
     int pc;             /* particles per chunk */
     int rowlen;         /* (cos,sin) pairs per (walker, particle) row */
     int wstride;        /* pairs per walker slab (pc * rowlen + bank stagger) */
     int off[3];         /* pair offset of X1 (n = 1..), X2 (n = 0..), X3 (n = 0..) within a row */
     int nmax[3];
-    const int4 *lane;   /* [blockDim.x] {local walker, item, offA | offB << 16, offX} */
-    const int *variant; /* [n_warps] NP | C0 << 8 */
+    const int4 *lane;   /* [n_slabs][blockDim.x] {local walker, item, offA | offB << 16, offX} */
+    const int *variant; /* [n_slabs][n_warps] NP | C0 << 8 */
     const double *wt;   /* [n_items][1 + NPB][2]: w(G) 2^nz per entry for products (0,1) and (2,3) */
     const double *tion; /* [n_items][1 + 2 NPB][4] fixed-charge sums, or null */
-    double *e_recip;    /* [W] */
+    double *e_recip;    /* [W][n_slabs] */
     T binv[9];
 };
 
@@ -100,9 +101,11 @@ __global__ void __launch_bounds__(OctCfg<T, NPB>::MAX_THREADS) recip_oct_kernel(
     double *part = reinterpret_cast<double *>(tab + (size_t)A.wc * A.wstride + NPB + 1); /* [blockDim.x] */
 
     const int tid = threadIdx.x, nthreads = blockDim.x, warp = tid >> 5;
-    const int w0 = blockIdx.x * A.wc;
-    const int4 L = A.lane[tid];
-    const int var = A.variant[warp];
+    const int group = blockIdx.x / A.n_slabs, slab = blockIdx.x - group * A.n_slabs;
+    const int w0 = group * A.wc;
+    const int4 *lanes = A.lane + (size_t)slab * nthreads;
+    const int4 L = lanes[tid];
+    const int var = A.variant[slab * (nthreads >> 5) + warp];
     const int np = var & 255;
     const bool c0 = (var >> 8) != 0;
     const T2 *lane_base = tab + (size_t)L.x * A.wstride;
@@ -203,8 +206,8 @@ __global__ void __launch_bounds__(OctCfg<T, NPB>::MAX_THREADS) recip_oct_kernel(
     if (tid < A.wc && w0 + tid < A.n_walkers) {
         double s = 0; /* fixed order: deterministic */
         for (int t = 0; t < nthreads; t++)
-            if (A.lane[t].x == tid) s += part[t];
-        A.e_recip[w0 + tid] = s;
+            if (lanes[t].x == tid) s += part[t];
+        A.e_recip[(size_t)(w0 + tid) * A.n_slabs + slab] = s;
     }
 }
 
