@@ -90,10 +90,13 @@ ewald_status ewald_oct_plan_summary(int dim, const double cell[9], double gamma,
                                     int n_walkers_per_cta, int *n_items, int *npb, int *n_warps,
                                     double *weight_sum, double *fma_per_particle);
 
-/* Host-only evaluation of the setup's piecewise-polynomial table for erfc (the table the real-space
- * kernels read; 16 bins on [0, z_max], degree 11 for FP64 kernels, 6 for FP32): value = P_bin(z).
- * For tests of the table builder; 0 <= z <= z_max.                                                 */
-ewald_status ewald_erfc_table_eval(double z_max, int degree, int n, const double *z, double *value);
+/* Host-only evaluation of the pair-function table the real-space kernels read,
+ *     F(t) = erfc(sqrt t)/sqrt t,  t = kappa^2 |r_ij - R|^2   (a term of the real-lattice sum of Eq. 3,
+ * PAPER.md:117, is kappa q_i q_j F(t)): a piecewise polynomial in t on bins cut from the binary format of
+ * t (FP64 kernels: 128 bins per octave, quintic; FP32 kernels: 32 bins per octave, cubic), built in long
+ * double at setup to cover 2^-6 <= t < t_max; outside that range the direct formula is
+ * returned, as in the kernels.  t, value: HOST [n].  For tests of the table builder.               */
+ewald_status ewald_pair_table_eval(ewald_prec prec, double t_max, int n, const double *t, double *value);
 
 /* Change the stream later calls are issued on (cudaStream_t; NULL = default stream). */
 ewald_status ewald_set_stream(ewald_ctx *ctx, void *stream);

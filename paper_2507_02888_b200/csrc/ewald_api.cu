@@ -57,7 +57,8 @@ struct ewald_ctx {
     double *d_ion_rho = nullptr; float *d_ion_rhof = nullptr;
     double *d_ion_pos = nullptr; float *d_ion_posf = nullptr;
     double *d_ion_q = nullptr; float *d_ion_qf = nullptr;
-    double *d_erfc = nullptr; float *d_erfcf = nullptr;   /* erfc piecewise polynomials */
+    double *d_pair = nullptr; float *d_pairf = nullptr;   /* pair-function table F(t) */
+    int sm_count = 148; size_t smem_optin = 227 * 1024;
 
     /* scratch */
     DevBuf partial_recip, partial_real, qsums;
@@ -67,7 +68,7 @@ struct ewald_ctx {
     /* stored walker population */
     int st_walkers = 0, st_n = 0, st_npad = 0;
     ewald_prec st_prec = EWALD_F64;
-    DevBuf st_pos, st_q, st_rho;
+    DevBuf st_pos, st_q, st_rho, st_qinfo;
     bool loaded = false;
 };
 
@@ -141,15 +142,22 @@ static std::vector<float> to_f32(const std::vector<double> &v)
     return f;
 }
 
+static int host_key(double t) { uint64_t b; std::memcpy(&b, &t, 8); return (int)(b >> 32); }
+static int host_key(float t) { int b; std::memcpy(&b, &t, 4); return b; }
+template <typename T> static const PairTable &pair_of(const HostTables &t);
+template <> const PairTable &pair_of<double>(const HostTables &t) { return t.pair64; }
+template <> const PairTable &pair_of<float>(const HostTables &t) { return t.pair32; }
+
 /* Real-space geometry in kappa-scaled lengths (ewald_realspace.cuh). */
 template <typename T> static void fill_geom(const HostTables &t, RealGeom<T> *g)
 {
     for (int i = 0; i < 9; i++) { g->a[i] = (T)(t.a[i] * t.kappa); g->binv[i] = (T)(t.binv[i] / t.kappa); }
     for (int k = 0; k < 3; k++) { g->L[k] = (T)(t.a[4 * k] * t.kappa); g->invL[k] = (T)(1.0 / (t.a[4 * k] * t.kappa)); }
-    g->rc2 = (T)(t.r_cutoff * t.r_cutoff * t.kappa * t.kappa);
-    g->inv_h = (T)(ERFC_BINS / t.z_max);
     g->kappa = (T)t.kappa;
     g->m_shift = t.m_shift;
+    g->key_rc = host_key((T)(t.r_cutoff * t.r_cutoff * t.kappa * t.kappa));
+    g->key_min = host_key((T)pair_of<T>(t).t_min);
+    g->bias = (PairFmt<T>::EBIAS + pair_of<T>(t).e_min) << PairFmt<T>::K;
 }
 
 static std::vector<double> scaled(const std::vector<double> &v, double f)
@@ -194,9 +202,16 @@ extern "C" ewald_status ewald_setup(ewald_ctx **out, int dim, const double *cell
     if (st == EWALD_OK) st = upload(c, &c->d_w2f, to_f32(t.g_w2));
     if (st == EWALD_OK) st = upload(c, &c->d_img, scaled(t.img, t.kappa));
     if (st == EWALD_OK) st = upload(c, &c->d_imgf, to_f32(scaled(t.img, t.kappa)));
-    if (st == EWALD_OK) st = upload(c, &c->d_erfc, t.erfc_tab64);
-    if (st == EWALD_OK) st = upload(c, &c->d_erfcf, to_f32(t.erfc_tab32));
-    if (st == EWALD_OK) st = ensure(c, &c->qsums, 2 * sizeof(double));
+    if (st == EWALD_OK) st = upload(c, &c->d_pair, t.pair64.coef);
+    if (st == EWALD_OK) st = upload(c, &c->d_pairf, to_f32(t.pair32.coef));
+    if (st == EWALD_OK) st = ensure(c, &c->qsums, 4 * sizeof(double));
+    if (st == EWALD_OK) st = ensure(c, &c->st_qinfo, 4 * sizeof(double));
+    {
+        int v = 0;
+        if (cudaDeviceGetAttribute(&v, cudaDevAttrMultiProcessorCount, c->device) == cudaSuccess && v > 0) c->sm_count = v;
+        if (cudaDeviceGetAttribute(&v, cudaDevAttrMaxSharedMemoryPerBlockOptin, c->device) == cudaSuccess && v > 0)
+            c->smem_optin = (size_t)v;
+    }
     if (st == EWALD_OK && t.oct.valid) {
         std::vector<double> wt(t.oct.wt);
         wt.resize(wt.size() + (size_t)(t.oct.npb + 1) * 2, 0.0); /* the zero-weight dummy item */
@@ -250,20 +265,14 @@ extern "C" ewald_status ewald_oct_plan_summary(int dim, const double *cell, doub
     return EWALD_OK;
 }
 
-extern "C" ewald_status ewald_erfc_table_eval(double z_max, int degree, int n, const double *z, double *value)
+extern "C" ewald_status ewald_pair_table_eval(ewald_prec prec, double t_max, int n, const double *t, double *value)
 {
-    if (!(z_max > 0) || degree < 1 || degree > 24 || n < 0 || (n > 0 && (!z || !value))) return EWALD_EINVAL;
-    std::vector<double> tab;
-    build_erfc_table(z_max, ERFC_BINS, degree, &tab);
-    const double inv_h = ERFC_BINS / z_max;
-    for (int i = 0; i < n; i++) {
-        int b = (int)((float)z[i] * (float)inv_h);
-        b = b < 0 ? 0 : (b > ERFC_BINS - 1 ? ERFC_BINS - 1 : b);
-        const double u = fma(z[i], 2 * inv_h, tab[(size_t)(degree + 1) * ERFC_BINS + b]);
-        double p = tab[(size_t)degree * ERFC_BINS + b];
-        for (int k = degree - 1; k >= 0; k--) p = fma(p, u, tab[(size_t)k * ERFC_BINS + b]);
-        value[i] = p;
-    }
+    if (!(t_max > 0) || n < 0 || (n > 0 && (!t || !value))) return EWALD_EINVAL;
+    if (prec != EWALD_F64 && prec != EWALD_F32) return EWALD_EINVAL;
+    PairTable p;
+    if (prec == EWALD_F64) build_pair_table(PAIR_K64, PAIR_DEG64, PAIR_EMIN, t_max, &p);
+    else build_pair_table(PAIR_K32, PAIR_DEG32, PAIR_EMIN, t_max, &p);
+    for (int i = 0; i < n; i++) value[i] = eval_pair_table(p, t[i]);
     return EWALD_OK;
 }
 
@@ -274,7 +283,7 @@ extern "C" void ewald_destroy(ewald_ctx *c)
     cudaStreamSynchronize(c->stream);
     cudaFree(c->d_gn); cudaFree(c->d_w2); cudaFree(c->d_w2f); cudaFree(c->d_img); cudaFree(c->d_imgf);
     cudaFree(c->d_ion_rho); cudaFree(c->d_ion_rhof); cudaFree(c->d_ion_pos); cudaFree(c->d_ion_posf);
-    cudaFree(c->d_ion_q); cudaFree(c->d_ion_qf); cudaFree(c->d_erfc); cudaFree(c->d_erfcf);
+    cudaFree(c->d_ion_q); cudaFree(c->d_ion_qf); cudaFree(c->d_pair); cudaFree(c->d_pairf);
     cudaFree(c->d_oct_wt); cudaFree(c->d_oct_tion);
     for (auto &kv : c->oct_dev) { cudaFree(kv.second.d_lane); cudaFree(kv.second.d_variant); }
     DevBuf *bufs[] = {&c->partial_recip, &c->partial_real, &c->qsums, &c->stage_pos, &c->stage_q,
@@ -331,7 +340,7 @@ template <> struct Tabs<double> {
     static const double *ion_rho(const ewald_ctx *c) { return c->d_ion_rho; }
     static const double *ion_pos(const ewald_ctx *c) { return c->d_ion_pos; }
     static const double *ion_q(const ewald_ctx *c) { return c->d_ion_q; }
-    static const double *erfc(const ewald_ctx *c) { return c->d_erfc; }
+    static const double *pair(const ewald_ctx *c) { return c->d_pair; }
 };
 template <> struct Tabs<float> {
     static const float *w2(const ewald_ctx *c) { return c->d_w2f; }
@@ -339,7 +348,7 @@ template <> struct Tabs<float> {
     static const float *ion_rho(const ewald_ctx *c) { return c->d_ion_rhof; }
     static const float *ion_pos(const ewald_ctx *c) { return c->d_ion_posf; }
     static const float *ion_q(const ewald_ctx *c) { return c->d_ion_qf; }
-    static const float *erfc(const ewald_ctx *c) { return c->d_erfcf; }
+    static const float *pair(const ewald_ctx *c) { return c->d_pairf; }
 };
 
 template <typename K> static ewald_status allow_smem(ewald_ctx *c, K kernel, size_t bytes)
@@ -533,28 +542,78 @@ static ewald_status launch_recip_oct(ewald_ctx *c, int W, int n, const T *pos, c
     return EWALD_OK;
 }
 
+/* The orthorhombic image scan needs boxes that reach the cut-off within +-2 images and that are wide enough
+ * for only the un-shifted image to fall below the pair table (kappa L_k / 2 > sqrt(t_min)). */
+static bool real_ortho(const ewald_ctx *c)
+{
+    if (!c->t.orthogonal || c->t.m_shift > 2) return false;
+    for (int k = 0; k < c->t.dim; k++)
+        if (c->t.a[4 * k] * c->t.kappa < 0.5) return false;
+    return true;
+}
+
+/* CTA size and per-lane stack capacities (bare-t items / (t, qq) items share the same bytes) that fit the
+ * shared memory left after `fixed` bytes of tables.  min_cap = ScanShape::MIN_CAP of the kernel variant. */
+template <typename T>
+static bool real_shape(const ewald_ctx *c, size_t fixed, int min_cap, int max_threads, int *threads, int *cap_u,
+                       int *cap_g, size_t *smem)
+{
+    const size_t budget = c->smem_optin > 2048 ? c->smem_optin - 2048 : 0; /* static arrays of the kernels */
+    for (int th = max_threads; th >= 32; th /= 2) {
+        if (fixed >= budget) return false;
+        const size_t per_cap = (size_t)(th / 32) * 32 * sizeof(T);
+        long long cu = (long long)((budget - fixed) / per_cap);
+        const long long want = 2 * min_cap > 64 ? 2 * min_cap : 64;
+        if (cu > want) cu = want;
+        cu &= ~1LL;
+        if (cu >= 2 * min_cap) {
+            *threads = th; *cap_u = (int)cu; *cap_g = (int)(cu / 2);
+            *smem = fixed + (size_t)cu * per_cap;
+            return true;
+        }
+    }
+    return false;
+}
+
+template <int DIM, bool ORTHO, int M> static int scan_min_cap() { return ScanShape<DIM, ORTHO, M>::MIN_CAP; }
+static int real_min_cap(const ewald_ctx *c, bool ortho)
+{
+    const int m = c->t.m_shift;
+    if (c->t.dim == 3) return !ortho ? scan_min_cap<3, false, 0>() : m == 0 ? scan_min_cap<3, true, 0>()
+                            : m == 1 ? scan_min_cap<3, true, 1>() : scan_min_cap<3, true, 2>();
+    return !ortho ? scan_min_cap<2, false, 0>() : m == 0 ? scan_min_cap<2, true, 0>()
+         : m == 1 ? scan_min_cap<2, true, 1>() : scan_min_cap<2, true, 2>();
+}
+
 template <typename T>
 static ewald_status launch_real(ewald_ctx *c, int W, int n, const T *pos, const T *q, int *n_tiles_out)
 {
-    const long long H = (n - 1) / 2;
-    const long long total = (long long)n * H + ((n & 1) ? 0 : n / 2) + (long long)n * c->t.n_ion;
-    long long n_tiles = (4LL * 148 * 2 + W - 1) / W;
-    const long long max_tiles = (total + REAL_THREADS - 1) / REAL_THREADS;
-    if (n_tiles > max_tiles) n_tiles = max_tiles;
-    if (n_tiles < 1) n_tiles = 1;
-    ewald_status st = ensure(c, &c->partial_real, (size_t)W * n_tiles * sizeof(double));
-    if (st != EWALD_OK) return st;
     RealArgs<T> A;
     A.pos = pos; A.q = q; A.n = n; A.npad = ewald_padded_n(n);
     A.img = Tabs<T>::img(c); A.nimg = c->nimg;
     A.ion_pos = Tabs<T>::ion_pos(c); A.ion_q = Tabs<T>::ion_q(c); A.n_ion = c->t.n_ion;
-    A.erfc_tab = Tabs<T>::erfc(c);
+    const PairTable &pt = pair_of<T>(c->t);
+    A.pair_tab = Tabs<T>::pair(c); A.n_bins = pt.n_bins; A.t_safe = (T)pt.t_min;
+    A.qinfo = (const double *)c->qsums.p;
+    A.ion_uniform = c->t.ion_uniform ? 1 : 0;
+    fill_geom(c->t, &A.g);
+    const bool ortho = real_ortho(c);
+    if (ortho) A.nimg = 0; /* the orthorhombic path does not read the image list */
+    const size_t fixed = RealSmem<T>::fixed_bytes(A.n_bins, A.nimg, A.n_ion, (size_t)(c->t.dim + 1) * n);
+    int threads = 0; size_t smem = 0;
+    if (!real_shape<T>(c, fixed, real_min_cap(c, ortho), REAL_MAX_THREADS, &threads, &A.cap_u, &A.cap_g, &smem))
+        return fail(c, EWALD_ERANGE, "real-space kernel: problem too large for shared memory");
+
+    const long long H = (n - 1) / 2;
+    const long long total = (long long)n * H + ((n & 1) ? 0 : n / 2) + (long long)n * c->t.n_ion;
+    long long n_tiles = (4LL * c->sm_count + W - 1) / W;
+    const long long max_tiles = (total + threads - 1) / threads;
+    if (n_tiles > max_tiles) n_tiles = max_tiles;
+    if (n_tiles < 1) n_tiles = 1;
+    ewald_status st = ensure(c, &c->partial_real, (size_t)W * n_tiles * sizeof(double));
+    if (st != EWALD_OK) return st;
     A.partial = (double *)c->partial_real.p;
     A.n_tiles = (int)n_tiles;
-    fill_geom(c->t, &A.g);
-    const bool ortho = c->t.orthogonal && c->t.m_shift <= 2;
-    if (ortho) A.nimg = 0; /* the orthorhombic path does not read the image list */
-    const size_t smem = RealSmem<T>::bytes(REAL_WARPS, A.nimg, A.n_ion, (size_t)(c->t.dim + 1) * n);
     const long long grid = (long long)W * n_tiles;
     if (grid > 0x7fffffffLL) return fail(c, EWALD_ERANGE, "grid too large");
 #define EWALD_LAUNCH_REAL(DIM, ORTHO, M)                                                          \
@@ -562,7 +621,7 @@ static ewald_status launch_real(ewald_ctx *c, int W, int n, const T *pos, const 
         st = allow_smem(c, real_kernel<T, DIM, ORTHO, M>, smem);                                  \
         if (st != EWALD_OK) return st;                                                            \
         ProfScope ps(c, 1);                                                                       \
-        real_kernel<T, DIM, ORTHO, M><<<(unsigned)grid, REAL_THREADS, smem, c->stream>>>(A);      \
+        real_kernel<T, DIM, ORTHO, M><<<(unsigned)grid, threads, smem, c->stream>>>(A);           \
     } while (0)
     const int m = c->t.m_shift;
     if (c->t.dim == 3) {
@@ -688,6 +747,12 @@ extern "C" ewald_status ewald_load_walkers(ewald_ctx *c, int W, int n, ewald_pre
         st = launch_recip<float>(c, W, n, (const float *)c->st_pos.p, (const float *)c->st_q.p,
                                  (float *)c->st_rho.p, &n_slabs);
     if (st != EWALD_OK) return st;
+    {
+        ProfScope ps(c, 2);
+        if (prec == EWALD_F64) charge_sums_kernel<double><<<1, 256, 0, c->stream>>>((const double *)c->st_q.p, n, (double *)c->st_qinfo.p);
+        else charge_sums_kernel<float><<<1, 256, 0, c->stream>>>((const float *)c->st_q.p, n, (double *)c->st_qinfo.p);
+    }
+    CU_TRY(c, cudaGetLastError());
     c->st_walkers = W; c->st_n = n; c->st_npad = npad; c->st_prec = prec;
     c->loaded = true;
     return EWALD_OK;
@@ -706,19 +771,32 @@ static ewald_status move_batch_t(ewald_ctx *c, int n_moves, const int *walker, c
     A.rowlen = c->rowlen;
     A.img = Tabs<T>::img(c); A.nimg = c->nimg;
     A.ion_pos = Tabs<T>::ion_pos(c); A.ion_q = Tabs<T>::ion_q(c); A.n_ion = c->t.n_ion;
-    A.erfc_tab = Tabs<T>::erfc(c);
+    const PairTable &pt = pair_of<T>(c->t);
+    A.pair_tab = Tabs<T>::pair(c); A.n_bins = pt.n_bins; A.t_safe = (T)pt.t_min;
+    A.qinfo = (const double *)c->st_qinfo.p;
+    A.ion_uniform = c->t.ion_uniform ? 1 : 0;
+    A.n_moves = n_moves;
     A.walker = walker; A.electron = electron; A.new_r = new_r; A.commit = commit; A.delta_e = delta_e;
     for (int i = 0; i < 9; i++) A.binv[i] = (T)c->t.binv[i];
     fill_geom(c->t, &A.g);
-    const bool ortho = c->t.orthogonal && c->t.m_shift <= 2;
+    const bool ortho = real_ortho(c);
     if (ortho) A.nimg = 0;
-    const size_t smem = RealSmem<T>::bytes(MOVE_WARPS, A.nimg, A.n_ion, 4 * (size_t)c->rowlen);
+    const size_t fixed = RealSmem<T>::fixed_bytes(A.n_bins, A.nimg, A.n_ion, 4 * (size_t)c->rowlen);
+    int threads = 0; size_t smem = 0;
+    if (!real_shape<T>(c, fixed, real_min_cap(c, ortho), MOVE_THREADS, &threads, &A.cap_u, &A.cap_g, &smem) ||
+        threads != MOVE_THREADS)
+        return fail(c, EWALD_ERANGE, "move kernel: tables too large for shared memory");
+    /* persistent CTAs: the tables are staged once per CTA */
+    int per_sm = (int)(c->smem_optin / (smem + 1024));
+    if (per_sm < 1) per_sm = 1;
+    if (per_sm > 2048 / MOVE_THREADS) per_sm = 2048 / MOVE_THREADS;
+    const int grid = n_moves < c->sm_count * per_sm ? n_moves : c->sm_count * per_sm;
     ewald_status st;
 #define EWALD_LAUNCH_MOVE(DIM, ORTHO, M)                                                          \
     do {                                                                                          \
         if ((st = allow_smem(c, move_kernel<T, DIM, ORTHO, M>, smem)) != EWALD_OK) return st;     \
         ProfScope ps(c, 3);                                                                       \
-        move_kernel<T, DIM, ORTHO, M><<<n_moves, MOVE_THREADS, smem, c->stream>>>(A);             \
+        move_kernel<T, DIM, ORTHO, M><<<grid, MOVE_THREADS, smem, c->stream>>>(A);             \
     } while (0)
     const int m = c->t.m_shift;
     if (c->t.dim == 3) {

@@ -32,6 +32,17 @@ struct OctLaunch {
     std::vector<int> variant;   /* [n_slabs][n_warps] np | c0 << 8 */
 };
 
+/* Pair-function table F(t) = erfc(sqrt t)/sqrt t on bins cut from the bits of t (ewald_setup.cpp). */
+struct PairTable {
+    int kbits = 0, degree = 0, e_min = 0; /* 2^kbits bins per binary octave, from 2^e_min upwards   */
+    int n_bins = 0;
+    double t_min = 0, t_max = 0;          /* the table covers [t_min, t_max)                         */
+    std::vector<double> coef;             /* [n_bins][degree + 1], variable u = t - bin centre       */
+};
+constexpr int PAIR_K64 = 7, PAIR_DEG64 = 5;  /* FP64: 128 bins per octave, quintic: rel. error < 1e-16 */
+constexpr int PAIR_K32 = 5, PAIR_DEG32 = 3;  /* FP32:  32 bins per octave, cubic:   rel. error < 3e-9  */
+constexpr int PAIR_EMIN = -6;                /* t < 2^-6 (kappa r < 1/8) takes the direct formula      */
+
 /* Everything ewald_setup computes on the host, in long double, before rounding (PAPER.md:359:
  * "lookup tables for Ewald interactions ... always performed using DP arithmetic"). */
 struct HostTables {
@@ -57,11 +68,13 @@ struct HostTables {
     double z_max = 0;
     int m_shift = 0;              /* orthorhombic cells: images -m..m per axis reach r_cutoff      */
     std::vector<double> erfc_tab64, erfc_tab32;
+    PairTable pair64, pair32;
     /* fixed charges */
     int n_ion = 0;
     std::vector<double> ion_pos; /* [n_ion][3] */
     std::vector<double> ion_q;
     std::vector<double> ion_rho; /* [ngp][2], sum_I q_I exp(iG.r_I)                              */
+    bool ion_uniform = true;     /* no fixed charges, or all of them equal */
     double ion_q2 = 0, ion_qsum = 0, ion_real = 0; /* sum q^2, sum q, sum_{I<J} q_I q_J psi(r_IJ) */
     OctPlan oct;
 };
@@ -76,6 +89,8 @@ void make_oct_launch(const OctPlan &p, int wc, int max_warps, OctLaunch *out);
 ewald_status build_tables(int dim, const double *cell, double kappa, double g_cutoff,
                           double r_cutoff, HostTables *out, std::string *err);
 void build_erfc_table(double z_max, int n_bins, int degree, std::vector<double> *tab);
+void build_pair_table(int kbits, int degree, int e_min, double t_max, PairTable *out);
+double eval_pair_table(const PairTable &p, double t);
 ewald_status build_fixed_charges(HostTables *t, int n_ion, const double *pos, const double *q,
                                  std::string *err);
 

@@ -130,44 +130,50 @@ template <typename T> struct RealArgs {
     int n, npad;
     const T *img; int nimg;                       /* [nimg][3], kappa-scaled (general cells)   */
     const T *ion_pos; const T *ion_q; int n_ion;  /* [n_ion][3], [n_ion]                        */
-    const T *erfc_tab;                            /* [ERFC_ROWS][ERFC_BINS]                     */
+    const T *pair_tab; int n_bins;                /* [n_bins][PairFmt<T>::NC]                   */
+    T t_safe;                                     /* some t inside the table                    */
+    const double *qinfo;                          /* device [4]: sum q^2, sum q, all-equal flag, q_0 */
+    int ion_uniform;                              /* no fixed charges, or all of them equal     */
+    int cap_u, cap_g;                             /* stack capacity per lane: t items / (t, qq) items */
     double *partial;                              /* [W][n_tiles] */
     int n_tiles;
     RealGeom<T> g;
 };
 
-constexpr int REAL_THREADS = 256;
-constexpr int REAL_WARPS = REAL_THREADS / 32;
+constexpr int REAL_MAX_THREADS = 256;
 
 /* Shared-memory carve-up common to the real-space and move kernels. */
 template <typename T> struct RealSmem {
-    typedef typename Num<T>::T2 T2;
-    T2 *queue;  /* [n_warps][QUEUE_CAP] */
-    T *tab;     /* [ERFC_ROWS][ERFC_BINS] */
+    T *tab;     /* [n_bins][NC] */
     T *img;     /* [nimg][3] */
     T *ion;     /* [n_ion][4] = x,y,z,q */
-    T *rest;
-    __device__ __forceinline__ RealSmem(unsigned char *raw, int n_warps, int nimg, int n_ion)
+    T *rest;    /* caller's arrays (rest_elems), then the stacks */
+    unsigned char *stacks;
+    static __host__ __device__ size_t up4(size_t e) { return (e + 3) & ~(size_t)3; }
+    static __host__ __device__ size_t table_elems(int n_bins, int nimg, int n_ion)
     {
-        queue = reinterpret_cast<T2 *>(raw);
-        tab = reinterpret_cast<T *>(queue + n_warps * QUEUE_CAP);
-        img = tab + ErfcRows<T>::value * ERFC_BINS;
-        ion = img + 3 * nimg;
-        rest = tab + table_elems(nimg, n_ion);
+        return up4((size_t)n_bins * PairFmt<T>::NC) + up4(3 * (size_t)nimg) + up4(4 * (size_t)n_ion);
     }
-    /* elements before `rest`, rounded so that `rest` stays 16-byte aligned */
-    static __host__ __device__ size_t table_elems(int nimg, int n_ion)
+    __device__ __forceinline__ RealSmem(unsigned char *raw, int n_bins, int nimg, int n_ion, size_t rest_elems)
     {
-        return ((size_t)ErfcRows<T>::value * ERFC_BINS + 3 * (size_t)nimg + 4 * (size_t)n_ion + 3) & ~(size_t)3;
+        tab = reinterpret_cast<T *>(raw);
+        img = tab + up4((size_t)n_bins * PairFmt<T>::NC);
+        ion = img + up4(3 * (size_t)nimg);
+        rest = ion + up4(4 * (size_t)n_ion);
+        stacks = reinterpret_cast<unsigned char *>(rest + up4(rest_elems));
     }
-    static size_t bytes(int n_warps, int nimg, int n_ion, size_t rest_elems)
+    /* bytes before the stacks */
+    static size_t fixed_bytes(int n_bins, int nimg, int n_ion, size_t rest_elems)
     {
-        return (size_t)n_warps * QUEUE_CAP * sizeof(T2) + (table_elems(nimg, n_ion) + rest_elems) * sizeof(T);
+        return (table_elems(n_bins, nimg, n_ion) + up4(rest_elems)) * sizeof(T);
     }
-    __device__ __forceinline__ void fill(const T *erfc_tab, const T *gimg, int nimg, const T *ion_pos,
+    __device__ __forceinline__ void fill(const T *pair_tab, int n_bins, const T *gimg, int nimg, const T *ion_pos,
                                          const T *ion_q, int n_ion, int tid, int nthreads)
     {
-        for (int t = tid; t < ErfcRows<T>::value * ERFC_BINS; t += nthreads) tab[t] = erfc_tab[t];
+        const int n4 = n_bins * PairFmt<T>::NC * (int)sizeof(T) / 16;   /* NC * sizeof(T) is a multiple of 16 */
+        const int4 *src = reinterpret_cast<const int4 *>(pair_tab);
+        int4 *dst = reinterpret_cast<int4 *>(tab);
+        for (int t = tid; t < n4; t += nthreads) dst[t] = src[t];
         for (int t = tid; t < 3 * nimg; t += nthreads) img[t] = gimg[t];
         for (int t = tid; t < n_ion; t += nthreads) {
             ion[4 * t + 0] = ion_pos[3 * t + 0];
@@ -178,60 +184,104 @@ template <typename T> struct RealSmem {
     }
 };
 
+/* Pairs (i, j = i + k + 1 mod n), rows k = 0..H-1 (H = (n-1)/2) and, for even n, half of row H, dealt
+ * round-robin to `team` threads; the cursor advances without divisions. */
+struct PairWalk {
+    int i, k, di, dk, n;
+    __device__ __forceinline__ void init(int gid, int team, int n_)
+    {
+        n = n_; k = gid / n; i = gid - k * n; dk = team / n; di = team - dk * n;
+    }
+    __device__ __forceinline__ void next()
+    {
+        i += di; k += dk;
+        if (i >= n) { i -= n; k++; }
+    }
+};
+
+template <typename T, int DIM, bool ORTHO, int M, bool UQ>
+__device__ __forceinline__ double real_body(const RealArgs<T> &A, RealSmem<T> &S, const T *sp, const T *sq,
+                                            int tile, T q0, T qion0)
+{
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, n = A.n;
+    const int cap = UQ ? A.cap_u : A.cap_g;
+    LaneStack<T, UQ> st;
+    st.init(S.stacks + (size_t)warp * cap * 32 * sizeof(PairItem<T, UQ>), lane, cap, S.tab, A.g.bias, A.t_safe);
+    __syncwarp();
+    const int team = A.n_tiles * blockDim.x, gid = tile * blockDim.x + tid;
+    double total = 0, direct = 0;
+
+    /* mobile-mobile pairs */
+    {
+        const int H = (n - 1) / 2;
+        const bool even = (n & 1) == 0;
+        PairWalk pw; pw.init(gid, team, n);
+        for (;;) {
+            const bool valid = pw.k < H || (even && pw.k == H && pw.i < n / 2);
+            if (!__any_sync(0xffffffffu, valid)) break;
+            T d[3] = {0, 0, 0};
+            T w = UQ ? q0 * q0 : T(0);
+            if (valid) {
+                const int i = pw.i;
+                int j = i + pw.k + 1;
+                if (j >= n) j -= n;
+#pragma unroll
+                for (int x = 0; x < DIM; x++) d[x] = (sp[x * n + i] - sp[x * n + j]) * A.g.kappa;
+                if (!UQ) w = sq[i] * sq[j];
+            }
+            scan_pair<T, DIM, ORTHO, M, UQ>(A.g, d, w, valid, st, direct, S.img, A.nimg);
+            pw.next();
+        }
+        st.finish();
+        total += UQ ? st.sum * (double)(q0 * q0) : st.sum;
+        st.sum = 0;
+    }
+    /* mobile particles against the fixed charges */
+    if (A.n_ion > 0) {
+        PairWalk pw; pw.init(gid, team, n);
+        for (;;) {
+            const bool valid = pw.k < A.n_ion;
+            if (!__any_sync(0xffffffffu, valid)) break;
+            T d[3] = {0, 0, 0};
+            T w = UQ ? q0 * qion0 : T(0);
+            if (valid) {
+                const int i = pw.i, I = pw.k;
+#pragma unroll
+                for (int x = 0; x < DIM; x++) d[x] = (sp[x * n + i] - S.ion[4 * I + x]) * A.g.kappa;
+                if (!UQ) w = sq[i] * S.ion[4 * I + 3];
+            }
+            scan_pair<T, DIM, ORTHO, M, UQ>(A.g, d, w, valid, st, direct, S.img, A.nimg);
+            pw.next();
+        }
+        st.finish();
+        total += UQ ? st.sum * (double)(q0 * qion0) : st.sum;
+    }
+    return total + direct;
+}
+
 template <typename T, int DIM, bool ORTHO, int M>
-__global__ void __launch_bounds__(REAL_THREADS) real_kernel(RealArgs<T> A)
+__global__ void __launch_bounds__(REAL_MAX_THREADS) real_kernel(RealArgs<T> A)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    RealSmem<T> S(smem_raw, REAL_WARPS, A.nimg, A.n_ion);
+    RealSmem<T> S(smem_raw, A.n_bins, A.nimg, A.n_ion, (size_t)(DIM + 1) * A.n);
     T *sp = S.rest;             /* [DIM][n] positions (unscaled: differences are taken first) */
     T *sq = sp + DIM * A.n;     /* [n] charges */
     __shared__ double red[32];
     const int w = blockIdx.x / A.n_tiles, tile = blockIdx.x - w * A.n_tiles, tid = threadIdx.x;
-    const int lane = tid & 31, warp = tid >> 5;
     const T *pw = A.pos + (size_t)w * DIM * A.npad;
-    for (int t = tid; t < A.n; t += REAL_THREADS) {
+    for (int t = tid; t < A.n; t += blockDim.x) {
 #pragma unroll
         for (int x = 0; x < DIM; x++) sp[x * A.n + t] = pw[x * A.npad + t];
         sq[t] = A.q[t];
     }
-    S.fill(A.erfc_tab, A.img, A.nimg, A.ion_pos, A.ion_q, A.n_ion, tid, REAL_THREADS);
+    S.fill(A.pair_tab, A.n_bins, A.img, A.nimg, A.ion_pos, A.ion_q, A.n_ion, tid, blockDim.x);
     __syncthreads();
 
-    const int n = A.n;
-    const int H = (n - 1) / 2;
-    const long long n_mm = (long long)n * H + ((n & 1) ? 0 : n / 2);
-    const long long total = n_mm + (long long)n * A.n_ion;
-    const long long per = (total + A.n_tiles - 1) / A.n_tiles;
-    const long long lo = per * tile, hi = min(total, lo + per);
-
-    WarpQueue<T> wq;
-    wq.buf = S.queue + warp * QUEUE_CAP; wq.cnt = 0; wq.lane = lane;
-    double acc = 0;
-    for (long long base = lo + warp * 32; base < hi; base += REAL_THREADS) {
-        const long long p = base + lane;
-        const bool valid = p < hi;
-        T d[3] = {0, 0, 0};
-        T qq = 0;
-        if (valid) {
-            if (p < n_mm) {
-                int i, j;
-                if (p < (long long)n * H) { i = (int)(p % n); j = i + (int)(p / n) + 1; }
-                else { i = (int)(p - (long long)n * H); j = i + n / 2; }
-                if (j >= n) j -= n;
-#pragma unroll
-                for (int x = 0; x < DIM; x++) d[x] = (sp[x * n + i] - sp[x * n + j]) * A.g.kappa;
-                qq = sq[i] * sq[j];
-            } else {
-                const long long e = p - n_mm;
-                const int i = (int)(e % n), I = (int)(e / n);
-#pragma unroll
-                for (int x = 0; x < DIM; x++) d[x] = (sp[x * n + i] - S.ion[4 * I + x]) * A.g.kappa;
-                qq = sq[i] * S.ion[4 * I + 3];
-            }
-        }
-        acc += (double)scan_pair<T, DIM, ORTHO, M>(A.g, d, qq, valid, wq, S.tab, S.img, A.nimg);
-    }
-    acc += (double)wq.finish(S.tab, A.g.inv_h);
+    const bool uq = A.qinfo[2] != 0.0 && A.ion_uniform;
+    const T q0 = (T)A.qinfo[3], qion0 = A.n_ion > 0 ? S.ion[3] : T(0);
+    double acc;
+    if (uq) acc = real_body<T, DIM, ORTHO, M, true>(A, S, sp, sq, tile, q0, qion0);
+    else acc = real_body<T, DIM, ORTHO, M, false>(A, S, sp, sq, tile, q0, qion0);
     acc = block_sum(acc, red);
     if (tid == 0) A.partial[(size_t)w * A.n_tiles + tile] = acc * (double)A.g.kappa;
 }
@@ -272,26 +322,35 @@ template <typename T>
 __global__ void charge_sums_kernel(const T *q, int n, double *out)
 {
     __shared__ double red[32];
-    double s2 = 0, s1 = 0;
-    for (int i = threadIdx.x; i < n; i += blockDim.x) { double v = (double)q[i]; s2 += v * v; s1 += v; }
+    double s2 = 0, s1 = 0, diff = 0;
+    const T q0 = q[0];
+    for (int i = threadIdx.x; i < n; i += blockDim.x) {
+        double v = (double)q[i]; s2 += v * v; s1 += v;
+        if (q[i] != q0) diff += 1;
+    }
     s2 = block_sum(s2, red);
     s1 = block_sum(s1, red);
-    if (threadIdx.x == 0) { out[0] = s2; out[1] = s1; }
+    diff = block_sum(diff, red);
+    /* out[2]: all charges equal (the real-space kernel then keeps t alone on its stacks); out[3] = q_0 */
+    if (threadIdx.x == 0) { out[0] = s2; out[1] = s1; out[2] = diff == 0 ? 1.0 : 0.0; out[3] = (double)q0; }
 }
 
 /* ------------------------------------------------------------------------------------------ */
-/* [S7] single-particle move.  grid = n_moves, one CTA per move. */
+/* [S7] single-particle move.  Persistent CTAs: the tables are staged once, then each CTA takes moves
+ * blockIdx.x, blockIdx.x + gridDim.x, ... */
 
 template <typename T> struct MoveArgs {
     T *pos;            /* stored [W][DIM][npad] */
     const T *q;        /* stored [n] */
     T *rho;            /* stored [W][2][ngp_pad] */
-    int n, npad, n_walkers;
+    int n, npad, n_walkers, n_moves;
     const short4 *gn; const T *w2; int ngp, ngp_pad;
     int nmax[3]; int off[3], rowlen;
     const T *img; int nimg;                       /* kappa-scaled image list (general cells) */
     const T *ion_pos; const T *ion_q; int n_ion;
-    const T *erfc_tab;
+    const T *pair_tab; int n_bins; T t_safe;
+    const double *qinfo; int ion_uniform;         /* as in RealArgs, for the stored charges  */
+    int cap_u, cap_g;
     const int *walker; const int *electron; const T *new_r; /* [n_moves], [n_moves], [n_moves][DIM] */
     int commit;
     double *delta_e;
@@ -301,93 +360,34 @@ template <typename T> struct MoveArgs {
 
 constexpr int MOVE_THREADS = 256;
 
-constexpr int MOVE_WARPS = MOVE_THREADS / 32;
-
-template <typename T, int DIM, bool ORTHO, int M>
-__global__ void __launch_bounds__(MOVE_THREADS) move_kernel(MoveArgs<T> A)
+/* [S7c] sum over the partners j != k of w_j [F-sum(r_new - r_j) - F-sum(r_old - r_j)], w_j = q_j (or 1
+ * with the common charge applied by the caller when UQ). */
+template <typename T, int DIM, bool ORTHO, int M, bool UQ>
+__device__ __forceinline__ double move_real(const MoveArgs<T> &A, RealSmem<T> &S, const T *pw, int k,
+                                            const T *r_old, const T *r_new, T q0, T qion0)
 {
-    typedef typename Num<T>::T2 T2;
-    extern __shared__ __align__(16) unsigned char smem_raw[];
-    RealSmem<T> S(smem_raw, MOVE_WARPS, A.nimg, A.n_ion);
-    T2 *tab = reinterpret_cast<T2 *>(S.rest); /* [2][rowlen]: old, new */
-    __shared__ double red[32];
-    const int m = blockIdx.x, tid = threadIdx.x;
-    const int w = A.walker[m], k = A.electron[m];
-    if (w < 0 || w >= A.n_walkers || k < 0 || k >= A.n) {
-        if (tid == 0) A.delta_e[m] = __longlong_as_double(0x7ff8000000000000LL);
-        return;
-    }
-    T *pw = A.pos + (size_t)w * DIM * A.npad;
-    T r_old[3] = {0, 0, 0}, r_new[3] = {0, 0, 0};
-#pragma unroll
-    for (int x = 0; x < DIM; x++) { r_old[x] = pw[x * A.npad + k]; r_new[x] = A.new_r[(size_t)m * DIM + x]; }
-    const T qk = A.q[k];
-
-    /* [S7a] power tables of the two points */
-    if (tid < 2 * DIM) {
-        const int which = tid / DIM, d = tid - which * DIM;
-        const T *r = which ? r_new : r_old;
-        T s = 0;
-#pragma unroll
-        for (int x = 0; x < DIM; x++) s += r[x] * A.binv[3 * d + x];
-        power_row<T>(s, T(1), A.nmax[d], tab + which * A.rowlen + A.off[d]);
-    }
-    S.fill(A.erfc_tab, A.img, A.nimg, A.ion_pos, A.ion_q, A.n_ion, tid, MOVE_THREADS);
-    __syncthreads();
-
-    /* [S7b] Delta E_recip and the patch of rho(G) */
-    T *rr = A.rho + (size_t)w * 2 * A.ngp_pad;
-    double acc = 0;
-    for (int g = tid; g < A.ngp; g += MOVE_THREADS) {
-        const short4 nn = A.gn[g];
-        T2 ph[2];
-#pragma unroll
-        for (int which = 0; which < 2; which++) {
-            const T2 *row = tab + which * A.rowlen;
-            T2 e1 = row[A.off[0] + nn.x];
-            T2 e2 = row[A.off[1] + (nn.y < 0 ? -nn.y : nn.y)];
-            if (nn.y < 0) e2.y = -e2.y;
-            T2 e;
-            e.x = e1.x * e2.x - e1.y * e2.y;
-            e.y = e1.x * e2.y + e1.y * e2.x;
-            if (DIM == 3) {
-                T2 e3 = row[A.off[2] + (nn.z < 0 ? -nn.z : nn.z)];
-                if (nn.z < 0) e3.y = -e3.y;
-                T2 f;
-                f.x = e.x * e3.x - e.y * e3.y;
-                f.y = e.x * e3.y + e.y * e3.x;
-                e = f;
-            }
-            ph[which] = e;
-        }
-        const T dr = ph[1].x - ph[0].x, di = ph[1].y - ph[0].y;
-        const T re = rr[g], im = rr[A.ngp_pad + g];
-        acc += (double)(A.w2[g] * (2 * qk * (re * dr + im * di) + qk * qk * (dr * dr + di * di)));
-        if (A.commit) { rr[g] = re + qk * dr; rr[A.ngp_pad + g] = im + qk * di; }
-    }
-
-    /* [S7c] Delta E_real = q_k sum_{j != k} q_j [psi(r'-r_j) - psi(r-r_j)]: the new-position terms are
-     * queued with +q_j, the old-position terms with -q_j */
-    double accr = 0;
-    {
-        const int lane = tid & 31, warp = tid >> 5;
-        WarpQueue<T> wq;
-        wq.buf = S.queue + warp * QUEUE_CAP; wq.cnt = 0; wq.lane = lane;
-        const int ntot = A.n + A.n_ion;
-        for (int base = warp * 32; base < ntot; base += MOVE_THREADS) {
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int cap = UQ ? A.cap_u : A.cap_g;
+    LaneStack<T, UQ, true> st;
+    st.init(S.stacks + (size_t)warp * cap * 32 * sizeof(PairItem<T, UQ>), lane, cap, S.tab, A.g.bias, A.t_safe);
+    __syncwarp();
+    double total = 0, direct = 0;
+    for (int seg = 0; seg < 2; seg++) {
+        const int cnt = seg == 0 ? A.n : A.n_ion;
+        for (int base = warp * 32; base < cnt; base += MOVE_THREADS) {
             const int j = base + lane;
-            const bool valid = j < ntot && j != k;
+            const bool valid = j < cnt && (seg == 1 || j != k);
             T rj[3] = {0, 0, 0};
-            T qj = 0;
+            T w = UQ ? T(1) : T(0);
             if (valid) {
-                if (j < A.n) {
+                if (seg == 0) {
 #pragma unroll
                     for (int x = 0; x < DIM; x++) rj[x] = pw[x * A.npad + j];
-                    qj = A.q[j];
+                    if (!UQ) w = A.q[j];
                 } else {
 #pragma unroll
-                    for (int x = 0; x < DIM; x++) rj[x] = S.ion[4 * (j - A.n) + x];
-                    qj = S.ion[4 * (j - A.n) + 3];
+                    for (int x = 0; x < DIM; x++) rj[x] = S.ion[4 * j + x];
+                    if (!UQ) w = S.ion[4 * j + 3];
                 }
             }
             T dn[3] = {0, 0, 0}, dold[3] = {0, 0, 0};
@@ -396,20 +396,99 @@ __global__ void __launch_bounds__(MOVE_THREADS) move_kernel(MoveArgs<T> A)
                 dn[x] = (r_new[x] - rj[x]) * A.g.kappa;
                 dold[x] = (r_old[x] - rj[x]) * A.g.kappa;
             }
-            accr += (double)scan_pair<T, DIM, ORTHO, M>(A.g, dn, qj, valid, wq, S.tab, S.img, A.nimg);
-            accr += (double)scan_pair<T, DIM, ORTHO, M>(A.g, dold, -qj, valid, wq, S.tab, S.img, A.nimg);
+            scan_pair<T, DIM, ORTHO, M, UQ, true, false>(A.g, dn, w, valid, st, direct, S.img, A.nimg);
+            scan_pair<T, DIM, ORTHO, M, UQ, true, true>(A.g, dold, UQ ? w : -w, valid, st, direct, S.img, A.nimg);
         }
-        accr += (double)wq.finish(S.tab, A.g.inv_h);
-        accr *= (double)A.g.kappa;
+        st.finish();
+        const double wseg = UQ ? (double)(seg == 0 ? q0 : qion0) : 1.0;
+        total += (st.sum + direct) * wseg;
+        st.sum = 0; direct = 0;
     }
-    acc += (double)qk * accr;
-    acc = block_sum(acc, red); /* its barriers also order every read of r_old before the commit */
-    if (tid == 0) {
-        A.delta_e[m] = acc;
-        if (A.commit) {
-#pragma unroll
-            for (int x = 0; x < DIM; x++) pw[x * A.npad + k] = r_new[x];
+    return total;
+}
+
+template <typename T, int DIM, bool ORTHO, int M>
+__global__ void __launch_bounds__(MOVE_THREADS) move_kernel(MoveArgs<T> A)
+{
+    typedef typename Num<T>::T2 T2;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    RealSmem<T> S(smem_raw, A.n_bins, A.nimg, A.n_ion, 4 * (size_t)A.rowlen);
+    T2 *tab = reinterpret_cast<T2 *>(S.rest); /* [2][rowlen]: old, new */
+    __shared__ double red[32];
+    const int tid = threadIdx.x;
+    S.fill(A.pair_tab, A.n_bins, A.img, A.nimg, A.ion_pos, A.ion_q, A.n_ion, tid, MOVE_THREADS);
+    __syncthreads();
+    const bool uq = A.qinfo[2] != 0.0 && A.ion_uniform;
+    const T q0 = (T)A.qinfo[3], qion0 = A.n_ion > 0 ? S.ion[3] : T(0);
+
+    for (int m = blockIdx.x; m < A.n_moves; m += gridDim.x) {
+        const int w = A.walker[m], k = A.electron[m];
+        if (w < 0 || w >= A.n_walkers || k < 0 || k >= A.n) { /* block-uniform */
+            if (tid == 0) A.delta_e[m] = __longlong_as_double(0x7ff8000000000000LL);
+            continue;
         }
+        T *pw = A.pos + (size_t)w * DIM * A.npad;
+        T r_old[3] = {0, 0, 0}, r_new[3] = {0, 0, 0};
+#pragma unroll
+        for (int x = 0; x < DIM; x++) { r_old[x] = pw[x * A.npad + k]; r_new[x] = A.new_r[(size_t)m * DIM + x]; }
+        const T qk = A.q[k];
+
+        /* [S7a] power tables of the two points */
+        if (tid < 2 * DIM) {
+            const int which = tid / DIM, d = tid - which * DIM;
+            const T *r = which ? r_new : r_old;
+            T s = 0;
+#pragma unroll
+            for (int x = 0; x < DIM; x++) s += r[x] * A.binv[3 * d + x];
+            power_row<T>(s, T(1), A.nmax[d], tab + which * A.rowlen + A.off[d]);
+        }
+        __syncthreads();
+
+        /* [S7b] Delta E_recip and the patch of rho(G) */
+        T *rr = A.rho + (size_t)w * 2 * A.ngp_pad;
+        double acc = 0;
+        for (int g = tid; g < A.ngp; g += MOVE_THREADS) {
+            const short4 nn = A.gn[g];
+            T2 ph[2];
+#pragma unroll
+            for (int which = 0; which < 2; which++) {
+                const T2 *row = tab + which * A.rowlen;
+                T2 e1 = row[A.off[0] + nn.x];
+                T2 e2 = row[A.off[1] + (nn.y < 0 ? -nn.y : nn.y)];
+                if (nn.y < 0) e2.y = -e2.y;
+                T2 e;
+                e.x = e1.x * e2.x - e1.y * e2.y;
+                e.y = e1.x * e2.y + e1.y * e2.x;
+                if (DIM == 3) {
+                    T2 e3 = row[A.off[2] + (nn.z < 0 ? -nn.z : nn.z)];
+                    if (nn.z < 0) e3.y = -e3.y;
+                    T2 f;
+                    f.x = e.x * e3.x - e.y * e3.y;
+                    f.y = e.x * e3.y + e.y * e3.x;
+                    e = f;
+                }
+                ph[which] = e;
+            }
+            const T dr = ph[1].x - ph[0].x, di = ph[1].y - ph[0].y;
+            const T re = rr[g], im = rr[A.ngp_pad + g];
+            acc += (double)(A.w2[g] * (2 * qk * (re * dr + im * di) + qk * qk * (dr * dr + di * di)));
+            if (A.commit) { rr[g] = re + qk * dr; rr[A.ngp_pad + g] = im + qk * di; }
+        }
+
+        /* [S7c] Delta E_real = q_k sum_{j != k} q_j [psi(r'-r_j) - psi(r-r_j)] */
+        double accr;
+        if (uq) accr = move_real<T, DIM, ORTHO, M, true>(A, S, pw, k, r_old, r_new, q0, qion0);
+        else accr = move_real<T, DIM, ORTHO, M, false>(A, S, pw, k, r_old, r_new, q0, qion0);
+        acc += (double)qk * accr * (double)A.g.kappa;
+        acc = block_sum(acc, red); /* its barriers also order every read of r_old before the commit */
+        if (tid == 0) {
+            A.delta_e[m] = acc;
+            if (A.commit) {
+#pragma unroll
+                for (int x = 0; x < DIM; x++) pw[x * A.npad + k] = r_new[x];
+            }
+        }
+        __syncthreads(); /* the power tables and red[] are reused by the next move */
     }
 }
 

@@ -1,30 +1,31 @@
 /* ewald_realspace.cuh -- the real-lattice sum of Eq. 3,
  *     psi(d) = sum_R erfc(kappa |d - R|) / |d - R|,
- * organised for the B200's FP64 pipe (64 lanes/SM): everything works in kappa-scaled lengths
- * (t = kappa^2 r^2), so a term is kappa * qq * erfc(sqrt t)/sqrt t.
+ * organised for the B200's FP64 pipe (64 lanes/SM) and its 128 B/clk of shared-memory bandwidth.
+ * Everything works in kappa-scaled squared lengths t = kappa^2 |d - R|^2, and a term is
+ *     kappa q_i q_j F(t),   F(t) = erfc(sqrt t)/sqrt t,
+ * with F read from a piecewise polynomial IN t (no square root, no exponential on the device):
+ * bins are cut from the floating-point bits of t (2^K per binary octave), the local variable is
+ * u = t - (bin centre), the coefficients were fitted in long double at setup ("lookup tables ...
+ * always DP"; ewald_setup.cpp build_pair_table) and sit in shared memory as
+ * [bin][degree+1] (FP64: quintic, 3 LDS.128 per term; FP32: cubic, 1 LDS.128).
  *
  * Two phases per warp:
- *   A  cull: per pair, the displacement is reduced to the cell and the candidate images are
- *      scanned; the squared distances that pass t < kappa^2 r_c^2 are pushed (ballot-compacted)
- *      into a per-warp shared-memory queue.  Orthorhombic cells build t from per-axis squares
- *      (1 add per candidate); general cells scan the image list.
- *   B  evaluate: 32 queued items at a time, one per lane, no divergence:
- *      y = t^-1/2 (MUFU seed + one cubic Newton step), z = t y, erfc(z) by a piecewise polynomial
- *      (16 bins in z, degree ERFC_DEG, coefficients built in long double at setup -- the "lookup
- *      tables ... always DP" of PAPER.md:359 -- laid out [coef][bin] so a warp's loads hit one
- *      128-byte row without bank conflicts), term = qq y erfc(z).
+ *   A  cull: each lane owns one pair, reduces its displacement to the cell, scans the candidate
+ *      images and pushes the t that pass t < kappa^2 r_c^2 on its PRIVATE stack in shared memory
+ *      (layout [slot][lane]: one predicated store and one predicated add per candidate, no votes);
+ *   B  evaluate: whenever every lane holds >= R items the warp pops R per lane and evaluates them with
+ *      all 32 lanes busy; a stack that would overflow forces a masked round; the tail is masked.
+ * With all charge products equal (the electron gas; electrons against one ion species) the stack holds
+ * t alone and the product is applied to the lane's sum; otherwise items are (t, q_i q_j).
  */
 #pragma once
 #include "ewald_kernels_common.cuh"
 
 namespace ewald {
 
-constexpr int ERFC_BINS = 16;
-template <typename T> struct ErfcDeg;
-template <> struct ErfcDeg<double> { static constexpr int value = 11; };
-template <> struct ErfcDeg<float> { static constexpr int value = 6; };
-/* table rows: coefficients c_0..c_DEG of erfc on the bin in u in [-1,1], then the row -(2b+1) */
-template <typename T> struct ErfcRows { static constexpr int value = ErfcDeg<T>::value + 2; };
+template <typename T> struct PairFmt;
+template <> struct PairFmt<double> { static constexpr int K = 7, DEG = 5, NC = 6, SHIFT = 20 - 7, EBIAS = 1023; };
+template <> struct PairFmt<float> { static constexpr int K = 5, DEG = 3, NC = 4, SHIFT = 23 - 5, EBIAS = 127; };
 
 /* Geometry in kappa-scaled units. */
 template <typename T> struct RealGeom {
@@ -32,125 +33,190 @@ template <typename T> struct RealGeom {
     T binv[9];   /* fractional rows / kappa: s_k = d . binv[k]    */
     T L[3];      /* orthorhombic box lengths * kappa              */
     T invL[3];
-    T rc2;       /* kappa^2 r_c^2                                  */
-    T inv_h;     /* ERFC_BINS / z_max                              */
     T kappa;
+    int key_rc;  /* order key of kappa^2 r_c^2                    */
+    int key_min; /* order key of the table's lower end t_min      */
+    int bias;    /* bin index = (key >> SHIFT) - bias             */
     int m_shift; /* images -m_shift..m_shift scanned per axis (orthorhombic path) */
 };
 
-template <typename T> __device__ __forceinline__ T inv_sqrt(T t);
-template <> __device__ __forceinline__ float inv_sqrt<float>(float t) { return rsqrtf(t); }
-template <> __device__ __forceinline__ double inv_sqrt<double>(double t)
+/* Positive floating-point numbers order like their leading bits.  FP64 uses the high word: ties within
+ * 2^-20 are accepted (the cut-off is converged: a term at r_c is below 1e-16 of the sum, reading R19),
+ * which keeps every comparison off the FP64 pipe. */
+__device__ __forceinline__ int order_key(double t) { return __double2hiint(t); }
+__device__ __forceinline__ int order_key(float t) { return __float_as_int(t); }
+
+/* Centre of the bin of t: the low mantissa bits replaced by 100..0. */
+__device__ __forceinline__ double bin_centre(double, int key)
 {
-    /* FP32 MUFU seed (rel. error ~2^-22), then one third-order step:
-     * y <- y (1 + e/2 + 3 e^2/8), e = 1 - t y^2; remaining error ~ (5/16) e^3 < 1e-19 */
-    double y = (double)rsqrtf((float)t);
-    double e = fma(-(t * y), y, 1.0);
-    double p = fma(e, 0.375, 0.5);
-    return fma(y * e, p, y);
+    constexpr int S = PairFmt<double>::SHIFT;
+    return __hiloint2double((key & ~((1 << S) - 1)) | (1 << (S - 1)), 0);
+}
+__device__ __forceinline__ float bin_centre(float, int key)
+{
+    constexpr int S = PairFmt<float>::SHIFT;
+    return __int_as_float((key & ~((1 << S) - 1)) | (1 << (S - 1)));
 }
 
-/* qq * erfc(sqrt t)/sqrt t for one queued item; tab = shared [DEG+1][ERFC_BINS]. */
-template <typename T>
-__device__ __forceinline__ T eval_item(T t, T qq, const T *tab, T inv_h)
+/* F(t) from the shared-memory table; requires t_min <= t < t_max. */
+__device__ __forceinline__ double pair_f(double t, const double *tab, int bias)
 {
-    constexpr int DEG = ErfcDeg<T>::value;
-    const T y = inv_sqrt<T>(t);
-    const T z = t * y;
-    int b = (int)((float)z * (float)inv_h);
-    b = b > ERFC_BINS - 1 ? ERFC_BINS - 1 : b;
-    const T u = fma(z, 2 * inv_h, tab[(DEG + 1) * ERFC_BINS + b]); /* bin [b h, (b+1) h] -> [-1, 1] */
-    T p = tab[DEG * ERFC_BINS + b];
+    const int key = order_key(t);
+    const double u = t - bin_centre(t, key);
+    const double2 *c = reinterpret_cast<const double2 *>(tab) + 3 * ((key >> PairFmt<double>::SHIFT) - bias);
+    const double2 c01 = c[0], c23 = c[1], c45 = c[2];
+    double p = fma(c45.y, u, c45.x);
+    p = fma(p, u, c23.y);
+    p = fma(p, u, c23.x);
+    p = fma(p, u, c01.y);
+    return fma(p, u, c01.x);
+}
+__device__ __forceinline__ float pair_f(float t, const float *tab, int bias)
+{
+    const int key = order_key(t);
+    const float u = t - bin_centre(t, key);
+    const float4 c = reinterpret_cast<const float4 *>(tab)[(key >> PairFmt<float>::SHIFT) - bias];
+    float p = fmaf(c.w, u, c.z);
+    p = fmaf(p, u, c.y);
+    return fmaf(p, u, c.x);
+}
+
+/* The direct formula, for the rare t below the table (kappa r < 1/8) and for coincident particles
+ * (t = 0 gives inf, reading R11). */
+__device__ __forceinline__ double pair_f_direct(double t) { const double z = sqrt(t); return erfc(z) / z; }
+__device__ __forceinline__ float pair_f_direct(float t) { const float z = sqrtf(t); return erfcf(z) / z; }
+
+/* +-1 with the sign of t; |t| */
+__device__ __forceinline__ double sign_unit(double t)
+{
+    return __hiloint2double((__double2hiint(t) & 0x80000000) | 0x3ff00000, 0);
+}
+__device__ __forceinline__ float sign_unit(float t) { return __int_as_float((__float_as_int(t) & 0x80000000) | 0x3f800000); }
+__device__ __forceinline__ double abs_of(double t) { return fabs(t); }
+__device__ __forceinline__ float abs_of(float t) { return fabsf(t); }
+
+/* Item of a lane's stack: t alone when all charge products are equal (UQ), else (t, q_i q_j). */
+template <typename T, bool UQ> struct PairItem;
+template <typename T> struct PairItem<T, true> {
+    T t;
+    __device__ __forceinline__ static PairItem make(T t, T) { PairItem i; i.t = t; return i; }
+    __device__ __forceinline__ T weight() const { return T(1); }
+};
+template <typename T> struct __align__(2 * sizeof(T)) PairItem<T, false> {
+    T t, w;
+    __device__ __forceinline__ static PairItem make(T t, T w) { PairItem i; i.t = t; i.w = w; return i; }
+    __device__ __forceinline__ T weight() const { return w; }
+};
+
+constexpr int PAIR_R = 4; /* items per lane per evaluation round (independent FMA chains) */
+
+/* Per-lane stack in shared memory, layout [slot][lane] per warp; all control flow that touches it is
+ * warp-uniform, the contents are lane-private. */
+template <typename T, bool UQ, bool SIGNED = false> struct LaneStack {
+    typedef PairItem<T, UQ> Item;
+    Item *base;  /* this lane's slot 0 */
+    int top;     /* 32 * number of items */
+    int cap32;   /* 32 * capacity */
+    const T *tab;
+    int bias;
+    double sum;  /* lane's running sum of weight * F(t) */
+
+    /* t_safe: any t inside the table; slot 0 always holds a valid item so that masked rounds can read it */
+    __device__ __forceinline__ void init(void *warp_mem, int lane, int cap, const T *table, int b, T t_safe)
+    {
+        base = reinterpret_cast<Item *>(warp_mem) + lane;
+        top = 0; cap32 = 32 * cap; tab = table; bias = b; sum = 0;
+        base[0] = Item::make(t_safe, T(0));
+    }
+    __device__ __forceinline__ void push(bool ok, T t, T w)
+    {
+        if (ok) { base[top] = Item::make(t, w); top += 32; }
+    }
+    /* one round: pop up to R items per lane and add their terms (MASKED: lanes may hold fewer) */
+    template <bool MASKED> __device__ __forceinline__ void round()
+    {
+        T part = 0;
 #pragma unroll
-    for (int k = DEG - 1; k >= 0; k--) p = fma(p, u, tab[k * ERFC_BINS + b]);
-    return (qq * y) * p;
-}
-
-template <typename T> __device__ __forceinline__ bool below(T t, T lim);
-template <> __device__ __forceinline__ bool below<float>(float t, float lim) { return t < lim; }
-/* positive doubles order like their high words; ties within 2^-20 are accepted (the cut-off is
- * converged: a term at r_c is below 1e-16 of the sum, reading R19) -- keeps the test off the FP64 pipe */
-template <> __device__ __forceinline__ bool below<double>(double t, double lim)
-{
-    return __double2hiint(t) <= __double2hiint(lim);
-}
-
-/* Per-warp queue of (t, qq) items in shared memory. */
-template <typename T> struct WarpQueue {
-    typedef typename Num<T>::T2 T2;
-    T2 *buf;
-    int cnt; /* warp-uniform */
-    int lane;
-    __device__ __forceinline__ void push(bool ok, T t, T qq)
-    {
-        const unsigned m = __ballot_sync(0xffffffffu, ok);
-        if (ok) {
-            T2 it; it.x = t; it.y = qq;
-            buf[cnt + __popc(m & ((1u << lane) - 1u))] = it;
+        for (int r = 0; r < PAIR_R; r++) {
+            const int s = top - 32 * (r + 1);
+            const bool have = !MASKED || s >= 0;
+            const Item it = base[have ? s : 0];
+            /* SIGNED stacks of bare t carry the sign of the term in the sign bit of t */
+            const T wt = UQ ? (SIGNED ? sign_unit(it.t) : T(1)) : it.weight();
+            const T f = pair_f(UQ && SIGNED ? abs_of(it.t) : it.t, tab, bias);
+            if (MASKED) part += have ? f * wt : T(0);
+            else part = UQ && !SIGNED ? part + f : fma(f, wt, part);
         }
-        cnt += __popc(m);
+        top = MASKED ? max(top - 32 * PAIR_R, 0) : top - 32 * PAIR_R;
+        sum += (double)part;
     }
-    /* evaluate full groups of 32 */
-    __device__ __forceinline__ T drain(const T *tab, T inv_h)
+    /* Called by the whole warp after each group of at most `limit` pushes per lane. */
+    __device__ __forceinline__ void service(int limit)
     {
-        T acc = 0;
-        __syncwarp();
-        while (cnt >= 32) {
-            cnt -= 32;
-            const T2 it = buf[cnt + lane];
-            acc += eval_item<T>(it.x, it.y, tab, inv_h);
-        }
-        __syncwarp();
-        return acc;
+        int mn = __reduce_min_sync(0xffffffffu, top);
+        while (mn >= 32 * PAIR_R) { round<false>(); mn -= 32 * PAIR_R; }
+        int mx = __reduce_max_sync(0xffffffffu, top);
+        while (mx > cap32 - 32 * limit) { round<true>(); mx -= 32 * PAIR_R; }
     }
-    /* evaluate what is left (< 32 items) */
-    __device__ __forceinline__ T finish(const T *tab, T inv_h)
+    __device__ __forceinline__ void finish()
     {
-        T acc = drain(tab, inv_h);
-        T2 it; it.x = 1; it.y = 0;
-        if (lane < cnt) it = buf[lane];
-        acc += eval_item<T>(it.x, it.y, tab, inv_h);
-        cnt = 0;
-        __syncwarp();
-        return acc;
+        int mx = __reduce_max_sync(0xffffffffu, top);
+        while (mx > 0) { round<true>(); mx -= 32 * PAIR_R; }
     }
 };
 
-constexpr int QUEUE_CAP_ORTHO = 5 * 32 + 32;  /* one x-row of candidates (<= 5) + carry-over */
-constexpr int QUEUE_IMG_STEP = 4;             /* general cells: drain every 4 images          */
-constexpr int QUEUE_CAP = 192;
+/* Images scanned between two services of the stack on the image-list path. */
+constexpr int IMG_STEP = 8;
 
-/* Phase A for one pair per lane.  d = r_i - r_j (kappa-scaled, not yet reduced).  Returns the sum of
- * the terms evaluated while draining. */
-template <typename T, int DIM, bool ORTHO, int M>
-__device__ __forceinline__ T scan_pair(const RealGeom<T> &g, T *d, T qq, bool valid, WarpQueue<T> &q,
-                                       const T *tab, const T *simg, int nimg)
+/* Pushes per lane between two services of the stack, and the stack capacity that allows them. */
+template <int DIM, bool ORTHO, int M> struct ScanShape {
+    static constexpr int ROW = 2 * M + 1;
+    static constexpr int ALL = DIM == 3 ? ROW * ROW * ROW : ROW * ROW;
+    static constexpr bool WHOLE = ALL <= 27;               /* service once per pair, else once per x-row */
+    static constexpr int LIMIT = ORTHO ? (WHOLE ? ALL : ROW) : IMG_STEP;
+    static constexpr int MIN_CAP = LIMIT + PAIR_R;
+};
+
+/* Phase A for one pair per lane.  d = kappa (r_i - r_j), not yet reduced; w = q_i q_j.  Terms below the
+ * table (t < t_min) are evaluated directly into `direct` (weighted by w); the rest go to the stack. */
+template <typename T, int DIM, bool ORTHO, int M, bool UQ, bool SIGNED = false, bool NEG = false>
+__device__ __forceinline__ void scan_pair(const RealGeom<T> &g, T *d, T w, bool valid,
+                                          LaneStack<T, UQ, SIGNED> &st, double &direct, const T *simg, int nimg)
 {
-    T acc = 0;
+    /* NEG (move kernel, old position): the term enters with a minus sign -- in w for (t, w) items (the
+     * caller passes -w), in the sign bit of t for bare-t items */
+    constexpr bool FLIP = NEG && UQ && SIGNED;
+    typedef ScanShape<DIM, ORTHO, M> Shape;
     if (ORTHO) {
+        constexpr int ROW = Shape::ROW;
+        T sq[DIM][ROW];
 #pragma unroll
-        for (int k = 0; k < DIM; k++) d[k] = fma(-Num<T>::rint_(d[k] * g.invL[k]), g.L[k], d[k]);
-        T sx[2 * M + 1];
+        for (int k = 0; k < DIM; k++) {
+            d[k] = fma(-Num<T>::rint_(d[k] * g.invL[k]), g.L[k], d[k]);
 #pragma unroll
-        for (int m = 0; m <= 2 * M; m++) { T x = fma((T)(M - m), g.L[0], d[0]); sx[m] = x * x; }
-        const int mz_hi = DIM == 3 ? M : 0;
-        T zz = DIM == 3 ? fma((T)M, g.L[2], d[2]) : T(0);
-        for (int mz = -mz_hi; mz <= mz_hi; mz++) {
-            const T sz = zz * zz;
-            zz -= g.L[2];
-            T yy = fma((T)M, g.L[1], d[1]);
-            for (int my = -M; my <= M; my++) {
-                const T syz = fma(yy, yy, sz);
-                yy -= g.L[1];
-                if (!__any_sync(0xffffffffu, valid && below<T>(syz, g.rc2))) continue;
+            for (int m = 0; m < ROW; m++) { const T x = fma((T)(M - m), g.L[k], d[k]); sq[k][m] = x * x; }
+        }
+        /* only the un-shifted candidate can fall below the table: |d_k - m L_k| >= L_k/2 otherwise */
+        T t0 = sq[0][M] + sq[1][M];
+        if (DIM == 3) t0 += sq[2][M];
+        const bool tiny = valid && order_key(t0) < g.key_min;
+        if (tiny) direct += (double)((FLIP ? -w : w) * pair_f_direct(t0));
+        const bool central_ok = valid && !tiny;
 #pragma unroll
-                for (int m = 0; m <= 2 * M; m++) {
-                    const T t = sx[m] + syz;
-                    q.push(valid && below<T>(t, g.rc2), t, qq);
+        for (int mz = 0; mz < (DIM == 3 ? ROW : 1); mz++) {
+#pragma unroll
+            for (int my = 0; my < ROW; my++) {
+                const T syz = DIM == 3 ? sq[1][my] + sq[2][mz] : sq[1][my];
+#pragma unroll
+                for (int mx = 0; mx < ROW; mx++) {
+                    const T t = sq[0][mx] + syz;
+                    const bool centre = mx == M && my == M && (DIM == 2 || mz == M);
+                    st.push((centre ? central_ok : valid) && order_key(t) <= g.key_rc, FLIP ? -t : t, w);
                 }
-                acc += q.drain(tab, g.inv_h);
+                if (!Shape::WHOLE) st.service(Shape::LIMIT);
             }
         }
+        if (Shape::WHOLE) st.service(Shape::LIMIT);
     } else {
         T f[3];
 #pragma unroll
@@ -165,21 +231,23 @@ __device__ __forceinline__ T scan_pair(const RealGeom<T> &g, T *d, T qq, bool va
 #pragma unroll
             for (int k = 0; k < DIM; k++) d[x] = fma(-f[k], g.a[3 * k + x], d[x]);
         }
-        for (int m0 = 0; m0 < nimg; m0 += QUEUE_IMG_STEP) {
+        for (int m0 = 0; m0 < nimg; m0 += IMG_STEP) {
 #pragma unroll
-            for (int u = 0; u < QUEUE_IMG_STEP; u++) {
+            for (int u = 0; u < IMG_STEP; u++) {
                 const int m = m0 + u;
-                const bool in = m < nimg;
-                const int mm = in ? m : 0;
+                const bool in = valid && m < nimg;
+                const int mm = m < nimg ? m : 0;
                 T t = 0;
 #pragma unroll
                 for (int x = 0; x < DIM; x++) { const T v = d[x] - simg[3 * mm + x]; t = fma(v, v, t); }
-                q.push(valid && in && below<T>(t, g.rc2), t, qq);
+                const int key = order_key(t);
+                const bool tiny = in && key < g.key_min;
+                if (tiny) direct += (double)((FLIP ? -w : w) * pair_f_direct(t));
+                st.push(in && !tiny && key <= g.key_rc, FLIP ? -t : t, w);
             }
-            acc += q.drain(tab, g.inv_h);
+            st.service(Shape::LIMIT);
         }
     }
-    return acc;
 }
 
 } // namespace ewald

@@ -6,6 +6,7 @@
  * data required can be moved to the GPU once, at the outset").
  */
 #include <cmath>
+#include <cstdint>
 #include <cstring>
 
 #include "ewald_internal.h"
@@ -63,6 +64,74 @@ void build_erfc_table(double z_max, int n_bins, int degree, std::vector<double> 
     }
 }
 
+/* Pair-function table of the real-space kernels (ewald_realspace.cuh):
+ *     F(t) = erfc(sqrt t)/sqrt t,  t = kappa^2 r^2,
+ * so that a term of the real-lattice sum of Eq. 3 is kappa q_i q_j F(t) -- no square
+ * root on the device.  Bins are cut from the floating-point format of t itself: bin number
+ * (e - e_min) 2^K + (top K mantissa bits), e the binary exponent; the same bins serve FP64 (index from
+ * the high word) and FP32.  On a bin [t_lo, t_lo + D), D = 2^(e-K), F is replaced by the polynomial
+ * through the Chebyshev nodes, expressed in the centred variable u = t - (t_lo + D/2) (t_lo + D/2 is
+ * t with its low mantissa bits replaced by 100..0: one logic operation).  Long double throughout
+ * ("lookup tables ... always performed using DP arithmetic").  Layout [bin][degree+1]. */
+void build_pair_table(int kbits, int degree, int e_min, double t_max, PairTable *out)
+{
+    out->kbits = kbits; out->degree = degree; out->e_min = e_min;
+    out->t_min = std::ldexp(1.0, e_min);
+    const int n = degree + 1, per = 1 << kbits;
+    int e_top; std::frexp(t_max, &e_top); e_top -= 1;          /* t_max in [2^e_top, 2^(e_top+1)) */
+    if (e_top < e_min) e_top = e_min;
+    const real frac = (real)t_max / ldexpl(1.0L, e_top) - 1;   /* in [0,1) */
+    int last = (int)floorl(frac * per);
+    if (last > per - 1) last = per - 1;
+    out->n_bins = (e_top - e_min) * per + last + 1;
+    out->t_max = (double)(ldexpl(1.0L, e_top) * (1 + (real)(last + 1) / per));
+    out->coef.assign((size_t)out->n_bins * n, 0.0);
+    std::vector<real> fv(n), cheb(n), mono(n), t0(n), t1(n), t2(n);
+    for (int b = 0; b < out->n_bins; b++) {
+        const int e = e_min + b / per, m = b % per;
+        const real width = ldexpl(1.0L, e - kbits), half = width / 2;
+        const real mid = ldexpl(1.0L, e) + m * width + half;
+        for (int i = 0; i < n; i++) {
+            const real t = mid + half * cosl(kPi * (2 * i + 1) / (2 * n)), z = sqrtl(t);
+            fv[i] = erfcl(z) / z;
+        }
+        for (int k = 0; k < n; k++) {
+            real s = 0;
+            for (int i = 0; i < n; i++) s += fv[i] * cosl(k * kPi * (2 * i + 1) / (2 * n));
+            cheb[k] = (k == 0 ? 1 : 2) * s / n;
+        }
+        for (int i = 0; i < n; i++) { mono[i] = 0; t0[i] = 0; t1[i] = 0; }
+        t0[0] = 1;
+        if (n > 1) t1[1] = 1;
+        for (int i = 0; i < n; i++) mono[i] += cheb[0] * t0[i];
+        if (n > 1) for (int i = 0; i < n; i++) mono[i] += cheb[1] * t1[i];
+        for (int k = 2; k < n; k++) {
+            for (int i = 0; i < n; i++) t2[i] = (i > 0 ? 2 * t1[i - 1] : 0) - t0[i];
+            for (int i = 0; i < n; i++) mono[i] += cheb[k] * t2[i];
+            t0 = t1; t1 = t2;
+        }
+        real scale = 1; /* v = u / half */
+        for (int k = 0; k < n; k++) { out->coef[(size_t)b * n + k] = (double)(mono[k] * scale); scale /= half; }
+    }
+}
+
+/* Host evaluation of the table exactly as the kernels index it (FP64 format). */
+double eval_pair_table(const PairTable &p, double t)
+{
+    uint64_t bits; std::memcpy(&bits, &t, 8);
+    const int hi = (int)(bits >> 32), sh = 20 - p.kbits;
+    int idx = (hi >> sh) - ((1023 + p.e_min) << p.kbits);
+    if (idx < 0 || idx >= p.n_bins) { const long double z = sqrtl((long double)t); return (double)(erfcl(z) / z); }
+    const uint64_t mid_hi = ((uint64_t)(uint32_t)hi & ~((1ull << sh) - 1)) | (1ull << (sh - 1));
+    const uint64_t mb = mid_hi << 32;
+    double mid; std::memcpy(&mid, &mb, 8);
+    const double u = t - mid;
+    const double *c = &p.coef[(size_t)idx * (p.degree + 1)];
+    double v = c[p.degree];
+    for (int k = p.degree - 1; k >= 0; k--) v = std::fma(v, u, c[k]);
+    return v;
+}
+
 ewald_status build_tables(int dim, const double *cell, double kappa_d, double g_cutoff,
                           double r_cutoff, HostTables *t, std::string *err)
 {
@@ -108,6 +177,10 @@ ewald_status build_tables(int dim, const double *cell, double kappa_d, double g_
     t->z_max = r_cutoff * kappa_d * (1 + 4e-6);
     build_erfc_table(t->z_max, 16, 11, &t->erfc_tab64);
     build_erfc_table(t->z_max, 16, 6, &t->erfc_tab32);
+    /* the cull compares high words / FP32 values: cover a little beyond kappa^2 r_c^2 */
+    const double t_top = r_cutoff * r_cutoff * kappa_d * kappa_d * (1 + 1e-5);
+    build_pair_table(PAIR_K64, PAIR_DEG64, PAIR_EMIN, t_top, &t->pair64);
+    build_pair_table(PAIR_K32, PAIR_DEG32, PAIR_EMIN, t_top, &t->pair32);
     bool ortho = true;
     for (int i = 0; i < 3; i++)
         for (int j = 0; j < 3; j++) {
@@ -196,6 +269,7 @@ ewald_status build_tables(int dim, const double *cell, double kappa_d, double g_
     t->n_ion = 0;
     t->ion_pos.clear(); t->ion_q.clear(); t->ion_rho.clear();
     t->ion_q2 = t->ion_qsum = t->ion_real = 0;
+    t->ion_uniform = true;
     build_oct_plan(t);
     return EWALD_OK;
 }
@@ -219,6 +293,9 @@ ewald_status build_fixed_charges(HostTables *t, int n_ion, const double *pos, co
     for (int i = 0; i < n_ion; i++) { q2 += (real)q[i] * q[i]; qs += q[i]; }
     t->ion_q2 = (double)q2;
     t->ion_qsum = (double)qs;
+    t->ion_uniform = true; /* one ion species: the real-space kernels keep bare t on their stacks */
+    for (int i = 1; i < n_ion; i++)
+        if (q[i] != q[0]) t->ion_uniform = false;
 
     /* rho_ion(G) = sum_I q_I exp(2 pi i n.s_I) with s = fractional coordinates */
     std::vector<real> s((size_t)3 * n_ion);

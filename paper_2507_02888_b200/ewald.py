@@ -19,7 +19,7 @@ _STATUS = {0: "EWALD_OK", 1: "EWALD_EINVAL", 2: "EWALD_ESINGULAR", 3: "EWALD_ERA
 
 # every symbol include/ewald.h declares (checked by tests/test_abi.py against the header text)
 SYMBOLS = ["ewald_padded_n", "ewald_setup", "ewald_setup_summary", "ewald_oct_plan_summary",
-           "ewald_erfc_table_eval",
+           "ewald_pair_table_eval",
            "ewald_destroy", "ewald_set_stream", "ewald_set_recip_variant",
            "ewald_set_fixed_charges", "ewald_energy_batch", "ewald_energy_batch_host",
            "ewald_load_walkers", "ewald_move_delta_batch", "ewald_move_delta_batch_host",
@@ -59,7 +59,7 @@ def load_library():
         "ewald_padded_n": (i, [i]),
         "ewald_setup": (i, [ctypes.POINTER(vp), i, dp, d, d, ctypes.POINTER(_Opts)]),
         "ewald_setup_summary": (i, [i, dp, d, d, d, ip, ip, ip, dp, dp]),
-        "ewald_erfc_table_eval": (i, [d, i, i, dp, dp]),
+        "ewald_pair_table_eval": (i, [i, d, i, dp, dp]),
         "ewald_oct_plan_summary": (i, [i, dp, d, d, i, ip, ip, ip, dp, dp]),
         "ewald_destroy": (None, [vp]),
         "ewald_set_stream": (i, [vp, vp]),
@@ -205,13 +205,13 @@ def ewald_oct_plan_summary(dim, cell, gamma, g_cutoff, n_walkers_per_cta=1):
                 fma_per_particle=fm.value)
 
 
-def ewald_erfc_table_eval(z_max, degree, z):
-    """Host-only: the setup's piecewise polynomial for erfc evaluated at z (array)."""
-    z = np.ascontiguousarray(z, dtype=np.float64)
-    out = np.zeros_like(z)
-    st = load_library().ewald_erfc_table_eval(float(z_max), int(degree), z.size, _dp(z), _dp(out))
+def ewald_pair_table_eval(prec, t_max, t):
+    """Host-only: the setup's piecewise polynomial for F(t) = erfc(sqrt t)/sqrt t evaluated at t (array)."""
+    t = np.ascontiguousarray(t, dtype=np.float64)
+    out = np.zeros_like(t)
+    st = load_library().ewald_pair_table_eval(int(prec), float(t_max), t.size, _dp(t), _dp(out))
     if st != 0:
-        raise EwaldError(st, "ewald_erfc_table_eval failed")
+        raise EwaldError(st, "ewald_pair_table_eval failed")
     return out
 
 

@@ -99,19 +99,28 @@ def test_to_soa_layout():
     assert np.array_equal(soa[1, 2, :5], pos[1, :, 2]) and np.all(soa[:, :, 5:] == 0)
 
 
-def test_erfc_table_matches_erfc():
-    """The real-space kernels' erfc table (built in long double at setup) against
-    mpmath's erfc: absolute error, which is what enters the energy sum."""
+def test_pair_table_matches_erfc():
+    """The real-space kernels' table of F(t) = erfc(sqrt t)/sqrt t (built in long double at setup,
+    PAPER.md:359) against mpmath.  Bound: |error| <= eps_rel F(t) + eps_abs, so a real-space sum of n
+    terms is off by at most eps_rel * sum + n * eps_abs (FP64: 1e-15 and 3e-17 -- the bins widen with t,
+    where F ~ exp(-t) is tiny).  Samples include both ends of every bin (bits of t next to the bin
+    boundaries) and values below the table, where the direct formula answers."""
     import mpmath as mp
     mp.mp.dps = 30
     rng = np.random.default_rng(0)
-    for z_max in (5.72, 6.16, 6.5):
-        z = np.concatenate([rng.random(1500) * z_max, np.linspace(0, z_max, 161)])  # includes bin edges
-        want = np.array([float(mp.erfc(mp.mpf(float(v)))) for v in z])
-        got64 = E.ewald_erfc_table_eval(z_max, 11, z)
-        got32 = E.ewald_erfc_table_eval(z_max, 6, z)
-        assert np.abs(got64 - want).max() < 2.5e-15
-        assert np.abs(got32 - want).max() < 2e-8
+    for t_max in (5.72 ** 2, 6.16 ** 2, 42.25):
+        edges = []
+        for e in range(-6, 6):
+            for m in range(0, 128, 5):
+                lo = 2.0 ** e * (1 + m / 128)
+                edges += [lo, np.nextafter(lo, 0), np.nextafter(lo, 100)]
+        t = np.concatenate([np.exp(rng.uniform(np.log(2.0 ** -9), np.log(t_max), 1500)), np.array(edges)])
+        t = t[(t > 0) & (t < t_max)]
+        want = np.array([float(mp.erfc(mp.sqrt(mp.mpf(float(v)))) / mp.sqrt(mp.mpf(float(v)))) for v in t])
+        got64 = E.ewald_pair_table_eval(E.EWALD_F64, t_max, t)
+        got32 = E.ewald_pair_table_eval(E.EWALD_F32, t_max, t)
+        assert (np.abs(got64 - want) <= 1e-15 * want + 3e-17).all()
+        assert (np.abs(got32 - want) <= 6e-8 * want + 1e-9).all()
 
 
 def _full_sphere_weight_sum(dim, L, kappa, n2_max):
