@@ -107,6 +107,13 @@ ewald_status ewald_set_stream(ewald_ctx *ctx, void *stream);
  * energy call if the cell is not orthorhombic). */
 ewald_status ewald_set_recip_variant(ewald_ctx *ctx, int variant);
 
+/* How the FP64 real-space kernels treat the far shell of the real-lattice sum of Eq. 3:
+ * 0 = default: terms with kappa^2 |r_ij - R|^2 >= 16 (each below erfc(4)/4 = 3.9e-9 in units of
+ *     kappa q_i q_j) are evaluated in FP32 arithmetic from a fixed-point copy of t; this changes the sum
+ *     by less than 1e-7 of the far shell's own total, i.e. < 1e-14 of E_real;
+ * 1 = every term in FP64.  FP32 contexts ignore the setting.  For tests and measurements. */
+ewald_status ewald_set_real_variant(ewald_ctx *ctx, int variant);
+
 /* Fixed charges (ions) that belong to every walker and never move (config 4; reading R13).  They
  * enter rho(G), the real-space sum, E_self and E_bg exactly like mobile particles (Eq. 2 over all
  * charges); their mutual terms are evaluated once here.  n_ion = 0 removes them.

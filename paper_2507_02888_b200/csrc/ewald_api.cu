@@ -58,6 +58,8 @@ struct ewald_ctx {
     double *d_ion_pos = nullptr; float *d_ion_posf = nullptr;
     double *d_ion_q = nullptr; float *d_ion_qf = nullptr;
     double *d_pair = nullptr; float *d_pairf = nullptr;   /* pair-function table F(t) */
+    float *d_far = nullptr;                               /* far-shell cubics (FP64 kernels) */
+    int real_variant = 0;                                 /* 0: far shell t >= 16 in FP32; 1: every term in FP64 */
     int sm_count = 148; size_t smem_optin = 227 * 1024;
 
     /* scratch */
@@ -204,6 +206,7 @@ extern "C" ewald_status ewald_setup(ewald_ctx **out, int dim, const double *cell
     if (st == EWALD_OK) st = upload(c, &c->d_imgf, to_f32(scaled(t.img, t.kappa)));
     if (st == EWALD_OK) st = upload(c, &c->d_pair, t.pair64.coef);
     if (st == EWALD_OK) st = upload(c, &c->d_pairf, to_f32(t.pair32.coef));
+    if (st == EWALD_OK) st = upload(c, &c->d_far, t.far_tab);
     if (st == EWALD_OK) st = ensure(c, &c->qsums, 4 * sizeof(double));
     if (st == EWALD_OK) st = ensure(c, &c->st_qinfo, 4 * sizeof(double));
     {
@@ -283,7 +286,7 @@ extern "C" void ewald_destroy(ewald_ctx *c)
     cudaStreamSynchronize(c->stream);
     cudaFree(c->d_gn); cudaFree(c->d_w2); cudaFree(c->d_w2f); cudaFree(c->d_img); cudaFree(c->d_imgf);
     cudaFree(c->d_ion_rho); cudaFree(c->d_ion_rhof); cudaFree(c->d_ion_pos); cudaFree(c->d_ion_posf);
-    cudaFree(c->d_ion_q); cudaFree(c->d_ion_qf); cudaFree(c->d_pair); cudaFree(c->d_pairf);
+    cudaFree(c->d_ion_q); cudaFree(c->d_ion_qf); cudaFree(c->d_pair); cudaFree(c->d_pairf); cudaFree(c->d_far);
     cudaFree(c->d_oct_wt); cudaFree(c->d_oct_tion);
     for (auto &kv : c->oct_dev) { cudaFree(kv.second.d_lane); cudaFree(kv.second.d_variant); }
     DevBuf *bufs[] = {&c->partial_recip, &c->partial_real, &c->qsums, &c->stage_pos, &c->stage_q,
@@ -297,6 +300,13 @@ extern "C" ewald_status ewald_set_recip_variant(ewald_ctx *c, int variant)
 {
     if (!c || variant < 0 || variant > 2) return EWALD_EINVAL;
     c->recip_variant = variant;
+    return EWALD_OK;
+}
+
+extern "C" ewald_status ewald_set_real_variant(ewald_ctx *c, int variant)
+{
+    if (!c || variant < 0 || variant > 1) return EWALD_EINVAL;
+    c->real_variant = variant;
     return EWALD_OK;
 }
 
@@ -552,22 +562,51 @@ static bool real_ortho(const ewald_ctx *c)
     return true;
 }
 
-/* CTA size and per-lane stack capacities (bare-t items / (t, qq) items share the same bytes) that fit the
- * shared memory left after `fixed` bytes of tables.  min_cap = ScanShape::MIN_CAP of the kernel variant. */
+/* Fills the table part of PairTabs and returns the bytes of shared memory the tables take. */
+template <typename T> static void fill_pair_tabs(const ewald_ctx *c, const double *qinfo, PairTabs<T> *P);
+template <> void fill_pair_tabs<float>(const ewald_ctx *c, const double *qinfo, PairTabs<float> *P)
+{
+    const PairTable &pt = c->t.pair32;
+    P->pair_tab = c->d_pairf; P->n_bins = pt.n_bins; P->t_safe = (float)pt.t_min;
+    P->far_tab = nullptr; P->n_far = 0; P->key_far = 0x7fffffff;
+    P->qinfo = qinfo; P->ion_uniform = c->t.ion_uniform ? 1 : 0;
+    P->capf_u = P->capf_g = 0;
+}
+template <> void fill_pair_tabs<double>(const ewald_ctx *c, const double *qinfo, PairTabs<double> *P)
+{
+    const PairTable &pt = c->t.pair64;
+    const bool far = c->real_variant == 0 && c->t.n_far > 0;
+    P->pair_tab = c->d_pair; P->t_safe = pt.t_min;
+    /* with the far shell on, the quintic table is needed below t = FAR_T0 only (FAR_T0 = 2^4) */
+    const int near_bins = (4 - pt.e_min) << pt.kbits;
+    P->n_bins = far && near_bins < pt.n_bins ? near_bins : pt.n_bins;
+    P->far_tab = far ? c->d_far : nullptr; P->n_far = far ? c->t.n_far : 0;
+    P->key_far = far ? host_key((double)FAR_T0) : 0x7fffffff;
+    P->qinfo = qinfo; P->ion_uniform = c->t.ion_uniform ? 1 : 0;
+    P->capf_u = P->capf_g = 0;
+}
+
+/* CTA size and per-lane stack capacities that fit the shared memory left after `fixed` bytes of tables.
+ * The two item kinds of a stack (bare t / (t, qq)) share the same bytes, so the (t, qq) capacity is half.
+ * min_cap = ScanShape::MIN_CAP of the kernel variant. */
 template <typename T>
-static bool real_shape(const ewald_ctx *c, size_t fixed, int min_cap, int max_threads, int *threads, int *cap_u,
-                       int *cap_g, size_t *smem)
+static bool real_shape(const ewald_ctx *c, size_t fixed, int min_cap_u, int min_cap_g, int max_threads,
+                       PairTabs<T> *P, int *threads, size_t *smem)
 {
     const size_t budget = c->smem_optin > 2048 ? c->smem_optin - 2048 : 0; /* static arrays of the kernels */
+    const bool far = P->n_far > 0;
     for (int th = max_threads; th >= 32; th /= 2) {
         if (fixed >= budget) return false;
-        const size_t per_cap = (size_t)(th / 32) * 32 * sizeof(T);
+        /* bytes per unit of capacity: near item + (far item: 4 bytes), per lane, per warp */
+        const size_t per_cap = (size_t)(th / 32) * 32 * (sizeof(T) + (far ? 4 : 0));
         long long cu = (long long)((budget - fixed) / per_cap);
-        const long long want = 2 * min_cap > 64 ? 2 * min_cap : 64;
+        const long long want = 64;
         if (cu > want) cu = want;
         cu &= ~1LL;
-        if (cu >= 2 * min_cap) {
-            *threads = th; *cap_u = (int)cu; *cap_g = (int)(cu / 2);
+        if (cu >= min_cap_u + 8 && cu >= 2 * min_cap_g) {
+            *threads = th;
+            P->cap_u = (int)cu; P->cap_g = (int)(cu / 2);
+            P->capf_u = far ? (int)cu : 0; P->capf_g = far ? (int)(cu / 2) : 0;
             *smem = fixed + (size_t)cu * per_cap;
             return true;
         }
@@ -575,14 +614,17 @@ static bool real_shape(const ewald_ctx *c, size_t fixed, int min_cap, int max_th
     return false;
 }
 
-template <int DIM, bool ORTHO, int M> static int scan_min_cap() { return ScanShape<DIM, ORTHO, M>::MIN_CAP; }
-static int real_min_cap(const ewald_ctx *c, bool ortho)
+template <int DIM, bool ORTHO, int M> static int scan_min_cap(bool uq)
+{
+    return uq ? ScanShape<DIM, ORTHO, M, true>::MIN_CAP : ScanShape<DIM, ORTHO, M, false>::MIN_CAP;
+}
+static int real_min_cap(const ewald_ctx *c, bool ortho, bool uq)
 {
     const int m = c->t.m_shift;
-    if (c->t.dim == 3) return !ortho ? scan_min_cap<3, false, 0>() : m == 0 ? scan_min_cap<3, true, 0>()
-                            : m == 1 ? scan_min_cap<3, true, 1>() : scan_min_cap<3, true, 2>();
-    return !ortho ? scan_min_cap<2, false, 0>() : m == 0 ? scan_min_cap<2, true, 0>()
-         : m == 1 ? scan_min_cap<2, true, 1>() : scan_min_cap<2, true, 2>();
+    if (c->t.dim == 3) return !ortho ? scan_min_cap<3, false, 0>(uq) : m == 0 ? scan_min_cap<3, true, 0>(uq)
+                            : m == 1 ? scan_min_cap<3, true, 1>(uq) : scan_min_cap<3, true, 2>(uq);
+    return !ortho ? scan_min_cap<2, false, 0>(uq) : m == 0 ? scan_min_cap<2, true, 0>(uq)
+         : m == 1 ? scan_min_cap<2, true, 1>(uq) : scan_min_cap<2, true, 2>(uq);
 }
 
 template <typename T>
@@ -592,16 +634,14 @@ static ewald_status launch_real(ewald_ctx *c, int W, int n, const T *pos, const 
     A.pos = pos; A.q = q; A.n = n; A.npad = ewald_padded_n(n);
     A.img = Tabs<T>::img(c); A.nimg = c->nimg;
     A.ion_pos = Tabs<T>::ion_pos(c); A.ion_q = Tabs<T>::ion_q(c); A.n_ion = c->t.n_ion;
-    const PairTable &pt = pair_of<T>(c->t);
-    A.pair_tab = Tabs<T>::pair(c); A.n_bins = pt.n_bins; A.t_safe = (T)pt.t_min;
-    A.qinfo = (const double *)c->qsums.p;
-    A.ion_uniform = c->t.ion_uniform ? 1 : 0;
+    fill_pair_tabs<T>(c, (const double *)c->qsums.p, &A.P);
     fill_geom(c->t, &A.g);
     const bool ortho = real_ortho(c);
     if (ortho) A.nimg = 0; /* the orthorhombic path does not read the image list */
-    const size_t fixed = RealSmem<T>::fixed_bytes(A.n_bins, A.nimg, A.n_ion, (size_t)(c->t.dim + 1) * n);
+    const size_t fixed = RealSmem<T>::fixed_bytes(A.P.n_bins, A.P.n_far, A.nimg, A.n_ion, (size_t)(c->t.dim + 1) * n);
     int threads = 0; size_t smem = 0;
-    if (!real_shape<T>(c, fixed, real_min_cap(c, ortho), REAL_MAX_THREADS, &threads, &A.cap_u, &A.cap_g, &smem))
+    if (!real_shape<T>(c, fixed, real_min_cap(c, ortho, true), real_min_cap(c, ortho, false), REAL_MAX_THREADS, &A.P,
+                       &threads, &smem))
         return fail(c, EWALD_ERANGE, "real-space kernel: problem too large for shared memory");
 
     const long long H = (n - 1) / 2;
@@ -771,19 +811,17 @@ static ewald_status move_batch_t(ewald_ctx *c, int n_moves, const int *walker, c
     A.rowlen = c->rowlen;
     A.img = Tabs<T>::img(c); A.nimg = c->nimg;
     A.ion_pos = Tabs<T>::ion_pos(c); A.ion_q = Tabs<T>::ion_q(c); A.n_ion = c->t.n_ion;
-    const PairTable &pt = pair_of<T>(c->t);
-    A.pair_tab = Tabs<T>::pair(c); A.n_bins = pt.n_bins; A.t_safe = (T)pt.t_min;
-    A.qinfo = (const double *)c->st_qinfo.p;
-    A.ion_uniform = c->t.ion_uniform ? 1 : 0;
+    fill_pair_tabs<T>(c, (const double *)c->st_qinfo.p, &A.P);
     A.n_moves = n_moves;
     A.walker = walker; A.electron = electron; A.new_r = new_r; A.commit = commit; A.delta_e = delta_e;
     for (int i = 0; i < 9; i++) A.binv[i] = (T)c->t.binv[i];
     fill_geom(c->t, &A.g);
     const bool ortho = real_ortho(c);
     if (ortho) A.nimg = 0;
-    const size_t fixed = RealSmem<T>::fixed_bytes(A.n_bins, A.nimg, A.n_ion, 4 * (size_t)c->rowlen);
+    const size_t fixed = RealSmem<T>::fixed_bytes(A.P.n_bins, A.P.n_far, A.nimg, A.n_ion, 4 * (size_t)c->rowlen);
     int threads = 0; size_t smem = 0;
-    if (!real_shape<T>(c, fixed, real_min_cap(c, ortho), MOVE_THREADS, &threads, &A.cap_u, &A.cap_g, &smem) ||
+    if (!real_shape<T>(c, fixed, real_min_cap(c, ortho, true), real_min_cap(c, ortho, false), MOVE_THREADS, &A.P, &threads,
+                       &smem) ||
         threads != MOVE_THREADS)
         return fail(c, EWALD_ERANGE, "move kernel: tables too large for shared memory");
     /* persistent CTAs: the tables are staged once per CTA */

@@ -41,6 +41,7 @@ struct PairTable {
 };
 constexpr int PAIR_K64 = 7, PAIR_DEG64 = 5;  /* FP64: 128 bins per octave, quintic: rel. error < 1e-16 */
 constexpr int PAIR_K32 = 5, PAIR_DEG32 = 3;  /* FP32:  32 bins per octave, cubic:   rel. error < 3e-9  */
+constexpr int FAR_T0 = 16, FAR_KB = 3, FAR_REP = 8; /* far shell of the FP64 kernels (FarFmt)       */
 constexpr int PAIR_EMIN = -6;                /* t < 2^-6 (kappa r < 1/8) takes the direct formula      */
 
 /* Everything ewald_setup computes on the host, in long double, before rounding (PAPER.md:359:
@@ -69,6 +70,8 @@ struct HostTables {
     int m_shift = 0;              /* orthorhombic cells: images -m..m per axis reach r_cutoff      */
     std::vector<double> erfc_tab64, erfc_tab32;
     PairTable pair64, pair32;
+    std::vector<float> far_tab;   /* [n_far][FAR_REP][4] */
+    int n_far = 0;
     /* fixed charges */
     int n_ion = 0;
     std::vector<double> ion_pos; /* [n_ion][3] */
@@ -91,6 +94,7 @@ ewald_status build_tables(int dim, const double *cell, double kappa, double g_cu
 void build_erfc_table(double z_max, int n_bins, int degree, std::vector<double> *tab);
 void build_pair_table(int kbits, int degree, int e_min, double t_max, PairTable *out);
 double eval_pair_table(const PairTable &p, double t);
+void build_far_table(int t0, int kb, int rep, double t_max, std::vector<float> *tab, int *n_far);
 ewald_status build_fixed_charges(HostTables *t, int n_ion, const double *pos, const double *q,
                                  std::string *err);
 

@@ -125,16 +125,24 @@ __global__ void __launch_bounds__(RECIP_THREADS) recip_kernel(RecipArgs<T> A)
 /* ------------------------------------------------------------------------------------------ */
 /* [S5] real-space pair sum.  grid = n_walkers * n_tiles; machinery in ewald_realspace.cuh. */
 
+/* Tables and stack shapes of the real-space machinery, common to the energy and move kernels. */
+template <typename T> struct PairTabs {
+    const T *pair_tab; int n_bins;   /* [n_bins][PairFmt<T>::NC]                                        */
+    T t_safe;                        /* some t inside the table                                         */
+    const float *far_tab; int n_far; /* FP64 kernels: [n_far][FarFmt::REP][4] far-shell cubics; 0 = none */
+    int key_far;                     /* order key of the far shell's start, INT_MAX = none              */
+    const double *qinfo;             /* device [4]: sum q^2, sum q, all-equal flag, q_0                  */
+    int ion_uniform;                 /* no fixed charges, or all of them equal                          */
+    int cap_u, cap_g;                /* near-stack capacity per lane: bare t items / (t, qq) items      */
+    int capf_u, capf_g;              /* far-stack capacity per lane                                     */
+};
+
 template <typename T> struct RealArgs {
     const T *pos; const T *q;
     int n, npad;
     const T *img; int nimg;                       /* [nimg][3], kappa-scaled (general cells)   */
     const T *ion_pos; const T *ion_q; int n_ion;  /* [n_ion][3], [n_ion]                        */
-    const T *pair_tab; int n_bins;                /* [n_bins][PairFmt<T>::NC]                   */
-    T t_safe;                                     /* some t inside the table                    */
-    const double *qinfo;                          /* device [4]: sum q^2, sum q, all-equal flag, q_0 */
-    int ion_uniform;                              /* no fixed charges, or all of them equal     */
-    int cap_u, cap_g;                             /* stack capacity per lane: t items / (t, qq) items */
+    PairTabs<T> P;
     double *partial;                              /* [W][n_tiles] */
     int n_tiles;
     RealGeom<T> g;
@@ -145,35 +153,48 @@ constexpr int REAL_MAX_THREADS = 256;
 /* Shared-memory carve-up common to the real-space and move kernels. */
 template <typename T> struct RealSmem {
     T *tab;     /* [n_bins][NC] */
+    float *far; /* [n_far][REP][4] */
     T *img;     /* [nimg][3] */
     T *ion;     /* [n_ion][4] = x,y,z,q */
     T *rest;    /* caller's arrays (rest_elems), then the stacks */
     unsigned char *stacks;
     static __host__ __device__ size_t up4(size_t e) { return (e + 3) & ~(size_t)3; }
-    static __host__ __device__ size_t table_elems(int n_bins, int nimg, int n_ion)
-    {
-        return up4((size_t)n_bins * PairFmt<T>::NC) + up4(3 * (size_t)nimg) + up4(4 * (size_t)n_ion);
-    }
-    __device__ __forceinline__ RealSmem(unsigned char *raw, int n_bins, int nimg, int n_ion, size_t rest_elems)
+    static __host__ __device__ size_t far_bytes(int n_far) { return (size_t)n_far * FarFmt::REP * 16; }
+    __device__ __forceinline__ RealSmem(unsigned char *raw, const PairTabs<T> &P, int nimg, int n_ion, size_t rest_elems)
     {
         tab = reinterpret_cast<T *>(raw);
-        img = tab + up4((size_t)n_bins * PairFmt<T>::NC);
+        far = reinterpret_cast<float *>(tab + up4((size_t)P.n_bins * PairFmt<T>::NC));
+        img = reinterpret_cast<T *>(reinterpret_cast<unsigned char *>(far) + far_bytes(P.n_far));
         ion = img + up4(3 * (size_t)nimg);
         rest = ion + up4(4 * (size_t)n_ion);
         stacks = reinterpret_cast<unsigned char *>(rest + up4(rest_elems));
     }
     /* bytes before the stacks */
-    static size_t fixed_bytes(int n_bins, int nimg, int n_ion, size_t rest_elems)
+    static size_t fixed_bytes(int n_bins, int n_far, int nimg, int n_ion, size_t rest_elems)
     {
-        return (table_elems(n_bins, nimg, n_ion) + up4(rest_elems)) * sizeof(T);
+        return (up4((size_t)n_bins * PairFmt<T>::NC) + up4(3 * (size_t)nimg) + up4(4 * (size_t)n_ion) +
+                up4(rest_elems)) * sizeof(T) + far_bytes(n_far);
     }
-    __device__ __forceinline__ void fill(const T *pair_tab, int n_bins, const T *gimg, int nimg, const T *ion_pos,
+    /* bytes of one warp's stacks (the two item kinds of a stack share the same bytes) */
+    static __host__ __device__ size_t warp_stack_bytes(const PairTabs<T> &P)
+    {
+        return (size_t)P.cap_u * 32 * sizeof(T) + (size_t)P.capf_u * 32 * 4;
+    }
+    __device__ __forceinline__ void fill(const PairTabs<T> &P, const T *gimg, int nimg, const T *ion_pos,
                                          const T *ion_q, int n_ion, int tid, int nthreads)
     {
-        const int n4 = n_bins * PairFmt<T>::NC * (int)sizeof(T) / 16;   /* NC * sizeof(T) is a multiple of 16 */
-        const int4 *src = reinterpret_cast<const int4 *>(pair_tab);
-        int4 *dst = reinterpret_cast<int4 *>(tab);
-        for (int t = tid; t < n4; t += nthreads) dst[t] = src[t];
+        {   /* NC * sizeof(T) is a multiple of 16 */
+            const int n4 = P.n_bins * PairFmt<T>::NC * (int)sizeof(T) / 16;
+            const int4 *src = reinterpret_cast<const int4 *>(P.pair_tab);
+            int4 *dst = reinterpret_cast<int4 *>(tab);
+            for (int t = tid; t < n4; t += nthreads) dst[t] = src[t];
+        }
+        {
+            const int n4 = P.n_far * FarFmt::REP;
+            const int4 *src = reinterpret_cast<const int4 *>(P.far_tab);
+            int4 *dst = reinterpret_cast<int4 *>(far);
+            for (int t = tid; t < n4; t += nthreads) dst[t] = src[t];
+        }
         for (int t = tid; t < 3 * nimg; t += nthreads) img[t] = gimg[t];
         for (int t = tid; t < n_ion; t += nthreads) {
             ion[4 * t + 0] = ion_pos[3 * t + 0];
@@ -183,6 +204,25 @@ template <typename T> struct RealSmem {
         }
     }
 };
+
+/* Points one lane's stacks at its warp's region of shared memory. */
+template <bool UQ, bool SIGNED>
+__device__ __forceinline__ void init_stacks(PairStacks<float, UQ, SIGNED> &st, RealSmem<float> &S,
+                                            const PairTabs<float> &P, int bias, int warp, int lane)
+{
+    unsigned char *mem = S.stacks + (size_t)warp * RealSmem<float>::warp_stack_bytes(P);
+    st.nr.init(mem, lane, UQ ? P.cap_u : P.cap_g, S.tab, bias, P.t_safe);
+}
+template <bool UQ, bool SIGNED>
+__device__ __forceinline__ void init_stacks(PairStacks<double, UQ, SIGNED> &st, RealSmem<double> &S,
+                                            const PairTabs<double> &P, int bias, int warp, int lane)
+{
+    unsigned char *mem = S.stacks + (size_t)warp * RealSmem<double>::warp_stack_bytes(P);
+    st.nr.init(mem, lane, UQ ? P.cap_u : P.cap_g, S.tab, bias, P.t_safe);
+    st.key_far = P.key_far;
+    if (st.has_far()) st.fr.init(mem + (size_t)P.cap_u * 32 * sizeof(double), lane, UQ ? P.capf_u : P.capf_g, S.far);
+    else { st.fr.base_a = st.fr.top_a = 0; st.fr.cap_b = 0; st.fr.sum = 0; }
+}
 
 /* Pairs (i, j = i + k + 1 mod n), rows k = 0..H-1 (H = (n-1)/2) and, for even n, half of row H, dealt
  * round-robin to `team` threads; the cursor advances without divisions. */
@@ -204,9 +244,8 @@ __device__ __forceinline__ double real_body(const RealArgs<T> &A, RealSmem<T> &S
                                             int tile, T q0, T qion0)
 {
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, n = A.n;
-    const int cap = UQ ? A.cap_u : A.cap_g;
-    LaneStack<T, UQ> st;
-    st.init(S.stacks + (size_t)warp * cap * 32 * sizeof(PairItem<T, UQ>), lane, cap, S.tab, A.g.bias, A.t_safe);
+    PairStacks<T, UQ, false> st;
+    init_stacks(st, S, A.P, A.g.bias, warp, lane);
     __syncwarp();
     const int team = A.n_tiles * blockDim.x, gid = tile * blockDim.x + tid;
     double total = 0, direct = 0;
@@ -233,8 +272,7 @@ __device__ __forceinline__ double real_body(const RealArgs<T> &A, RealSmem<T> &S
             pw.next();
         }
         st.finish();
-        total += UQ ? st.sum * (double)(q0 * q0) : st.sum;
-        st.sum = 0;
+        total += st.take() * (UQ ? (double)(q0 * q0) : 1.0);
     }
     /* mobile particles against the fixed charges */
     if (A.n_ion > 0) {
@@ -254,7 +292,7 @@ __device__ __forceinline__ double real_body(const RealArgs<T> &A, RealSmem<T> &S
             pw.next();
         }
         st.finish();
-        total += UQ ? st.sum * (double)(q0 * qion0) : st.sum;
+        total += st.take() * (UQ ? (double)(q0 * qion0) : 1.0);
     }
     return total + direct;
 }
@@ -263,7 +301,7 @@ template <typename T, int DIM, bool ORTHO, int M>
 __global__ void __launch_bounds__(REAL_MAX_THREADS) real_kernel(RealArgs<T> A)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    RealSmem<T> S(smem_raw, A.n_bins, A.nimg, A.n_ion, (size_t)(DIM + 1) * A.n);
+    RealSmem<T> S(smem_raw, A.P, A.nimg, A.n_ion, (size_t)(DIM + 1) * A.n);
     T *sp = S.rest;             /* [DIM][n] positions (unscaled: differences are taken first) */
     T *sq = sp + DIM * A.n;     /* [n] charges */
     __shared__ double red[32];
@@ -274,11 +312,11 @@ __global__ void __launch_bounds__(REAL_MAX_THREADS) real_kernel(RealArgs<T> A)
         for (int x = 0; x < DIM; x++) sp[x * A.n + t] = pw[x * A.npad + t];
         sq[t] = A.q[t];
     }
-    S.fill(A.pair_tab, A.n_bins, A.img, A.nimg, A.ion_pos, A.ion_q, A.n_ion, tid, blockDim.x);
+    S.fill(A.P, A.img, A.nimg, A.ion_pos, A.ion_q, A.n_ion, tid, blockDim.x);
     __syncthreads();
 
-    const bool uq = A.qinfo[2] != 0.0 && A.ion_uniform;
-    const T q0 = (T)A.qinfo[3], qion0 = A.n_ion > 0 ? S.ion[3] : T(0);
+    const bool uq = A.P.qinfo[2] != 0.0 && A.P.ion_uniform;
+    const T q0 = (T)A.P.qinfo[3], qion0 = A.n_ion > 0 ? S.ion[3] : T(0);
     double acc;
     if (uq) acc = real_body<T, DIM, ORTHO, M, true>(A, S, sp, sq, tile, q0, qion0);
     else acc = real_body<T, DIM, ORTHO, M, false>(A, S, sp, sq, tile, q0, qion0);
@@ -348,9 +386,7 @@ template <typename T> struct MoveArgs {
     int nmax[3]; int off[3], rowlen;
     const T *img; int nimg;                       /* kappa-scaled image list (general cells) */
     const T *ion_pos; const T *ion_q; int n_ion;
-    const T *pair_tab; int n_bins; T t_safe;
-    const double *qinfo; int ion_uniform;         /* as in RealArgs, for the stored charges  */
-    int cap_u, cap_g;
+    PairTabs<T> P;                                /* qinfo: of the stored charges            */
     const int *walker; const int *electron; const T *new_r; /* [n_moves], [n_moves], [n_moves][DIM] */
     int commit;
     double *delta_e;
@@ -367,9 +403,8 @@ __device__ __forceinline__ double move_real(const MoveArgs<T> &A, RealSmem<T> &S
                                             const T *r_old, const T *r_new, T q0, T qion0)
 {
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const int cap = UQ ? A.cap_u : A.cap_g;
-    LaneStack<T, UQ, true> st;
-    st.init(S.stacks + (size_t)warp * cap * 32 * sizeof(PairItem<T, UQ>), lane, cap, S.tab, A.g.bias, A.t_safe);
+    PairStacks<T, UQ, true> st;
+    init_stacks(st, S, A.P, A.g.bias, warp, lane);
     __syncwarp();
     double total = 0, direct = 0;
     for (int seg = 0; seg < 2; seg++) {
@@ -401,8 +436,8 @@ __device__ __forceinline__ double move_real(const MoveArgs<T> &A, RealSmem<T> &S
         }
         st.finish();
         const double wseg = UQ ? (double)(seg == 0 ? q0 : qion0) : 1.0;
-        total += (st.sum + direct) * wseg;
-        st.sum = 0; direct = 0;
+        total += (st.take() + direct) * wseg;
+        direct = 0;
     }
     return total;
 }
@@ -412,14 +447,14 @@ __global__ void __launch_bounds__(MOVE_THREADS) move_kernel(MoveArgs<T> A)
 {
     typedef typename Num<T>::T2 T2;
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    RealSmem<T> S(smem_raw, A.n_bins, A.nimg, A.n_ion, 4 * (size_t)A.rowlen);
+    RealSmem<T> S(smem_raw, A.P, A.nimg, A.n_ion, 4 * (size_t)A.rowlen);
     T2 *tab = reinterpret_cast<T2 *>(S.rest); /* [2][rowlen]: old, new */
     __shared__ double red[32];
     const int tid = threadIdx.x;
-    S.fill(A.pair_tab, A.n_bins, A.img, A.nimg, A.ion_pos, A.ion_q, A.n_ion, tid, MOVE_THREADS);
+    S.fill(A.P, A.img, A.nimg, A.ion_pos, A.ion_q, A.n_ion, tid, MOVE_THREADS);
     __syncthreads();
-    const bool uq = A.qinfo[2] != 0.0 && A.ion_uniform;
-    const T q0 = (T)A.qinfo[3], qion0 = A.n_ion > 0 ? S.ion[3] : T(0);
+    const bool uq = A.P.qinfo[2] != 0.0 && A.P.ion_uniform;
+    const T q0 = (T)A.P.qinfo[3], qion0 = A.n_ion > 0 ? S.ion[3] : T(0);
 
     for (int m = blockIdx.x; m < A.n_moves; m += gridDim.x) {
         const int w = A.walker[m], k = A.electron[m];

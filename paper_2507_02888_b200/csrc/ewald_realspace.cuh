@@ -95,84 +95,185 @@ __device__ __forceinline__ float sign_unit(float t) { return __int_as_float((__f
 __device__ __forceinline__ double abs_of(double t) { return fabs(t); }
 __device__ __forceinline__ float abs_of(float t) { return fabsf(t); }
 
-/* Item of a lane's stack: t alone when all charge products are equal (UQ), else (t, q_i q_j). */
-template <typename T, bool UQ> struct PairItem;
-template <typename T> struct PairItem<T, true> {
-    T t;
-    __device__ __forceinline__ static PairItem make(T t, T) { PairItem i; i.t = t; return i; }
-    __device__ __forceinline__ T weight() const { return T(1); }
+/* Shared-memory accesses by 32-bit window address: the stacks keep byte addresses, so a push is one store
+ * and one add, and a pop is a load at a constant (negative) offset. */
+__device__ __forceinline__ unsigned smem_addr(const void *p) { return (unsigned)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void st_s(unsigned a, double v) { asm volatile("st.shared.f64 [%0], %1;" ::"r"(a), "d"(v) : "memory"); }
+__device__ __forceinline__ void st_s(unsigned a, double v, double w) { asm volatile("st.shared.v2.f64 [%0], {%1, %2};" ::"r"(a), "d"(v), "d"(w) : "memory"); }
+__device__ __forceinline__ void st_s(unsigned a, float v) { asm volatile("st.shared.f32 [%0], %1;" ::"r"(a), "f"(v) : "memory"); }
+__device__ __forceinline__ void st_s(unsigned a, float v, float w) { asm volatile("st.shared.v2.f32 [%0], {%1, %2};" ::"r"(a), "f"(v), "f"(w) : "memory"); }
+__device__ __forceinline__ void st_s(unsigned a, unsigned v) { asm volatile("st.shared.b32 [%0], %1;" ::"r"(a), "r"(v) : "memory"); }
+__device__ __forceinline__ void st_s(unsigned a, unsigned v, float w) { asm volatile("st.shared.v2.b32 [%0], {%1, %2};" ::"r"(a), "r"(v), "r"(__float_as_uint(w)) : "memory"); }
+__device__ __forceinline__ void ld_s(unsigned a, double &v) { asm volatile("ld.shared.f64 %0, [%1];" : "=d"(v) : "r"(a) : "memory"); }
+__device__ __forceinline__ void ld_s(unsigned a, double &v, double &w) { asm volatile("ld.shared.v2.f64 {%0, %1}, [%2];" : "=d"(v), "=d"(w) : "r"(a) : "memory"); }
+__device__ __forceinline__ void ld_s(unsigned a, float &v) { asm volatile("ld.shared.f32 %0, [%1];" : "=f"(v) : "r"(a) : "memory"); }
+__device__ __forceinline__ void ld_s(unsigned a, float &v, float &w) { asm volatile("ld.shared.v2.f32 {%0, %1}, [%2];" : "=f"(v), "=f"(w) : "r"(a) : "memory"); }
+__device__ __forceinline__ void ld_s(unsigned a, unsigned &v) { asm volatile("ld.shared.b32 %0, [%1];" : "=r"(v) : "r"(a) : "memory"); }
+__device__ __forceinline__ void ld_s(unsigned a, unsigned &v, float &w)
+{
+    unsigned wb;
+    asm volatile("ld.shared.v2.b32 {%0, %1}, [%2];" : "=r"(v), "=r"(wb) : "r"(a) : "memory");
+    w = __uint_as_float(wb);
+}
+
+/* Item of a lane's stack: t alone when all charge products are equal (UQ), else (t, q_i q_j).
+ * K = the stored key type (T for the near stack, 32-bit fixed point for the far stack), W = weight type. */
+template <typename K, typename W, bool UQ> struct StackItem;
+template <typename K, typename W> struct StackItem<K, W, true> {
+    static constexpr int BYTES = sizeof(K);
+    __device__ __forceinline__ static void store(unsigned a, K t, W) { st_s(a, t); }
+    __device__ __forceinline__ static void load(unsigned a, K &t, W &w) { ld_s(a, t); w = W(1); }
 };
-template <typename T> struct __align__(2 * sizeof(T)) PairItem<T, false> {
-    T t, w;
-    __device__ __forceinline__ static PairItem make(T t, T w) { PairItem i; i.t = t; i.w = w; return i; }
-    __device__ __forceinline__ T weight() const { return w; }
+template <typename K, typename W> struct StackItem<K, W, false> {
+    static constexpr int BYTES = sizeof(K) + sizeof(W);
+    __device__ __forceinline__ static void store(unsigned a, K t, W w) { st_s(a, t, w); }
+    __device__ __forceinline__ static void load(unsigned a, K &t, W &w) { ld_s(a, t, w); }
 };
 
 constexpr int PAIR_R = 4; /* items per lane per evaluation round (independent FMA chains) */
 
-/* Per-lane stack in shared memory, layout [slot][lane] per warp; all control flow that touches it is
- * warp-uniform, the contents are lane-private. */
-template <typename T, bool UQ, bool SIGNED = false> struct LaneStack {
-    typedef PairItem<T, UQ> Item;
-    Item *base;  /* this lane's slot 0 */
-    int top;     /* 32 * number of items */
-    int cap32;   /* 32 * capacity */
-    const T *tab;
-    int bias;
-    double sum;  /* lane's running sum of weight * F(t) */
+/* Per-lane stack in shared memory, layout [slot][lane] per warp, kept as byte addresses; all control flow
+ * that touches it is warp-uniform, the contents are lane-private.  Derived classes supply term(). */
+template <typename K, typename W, bool UQ, typename Derived> struct StackBase {
+    typedef StackItem<K, W, UQ> Item;
+    static constexpr int SLOT = 32 * Item::BYTES;  /* bytes between two slots of a lane */
+    unsigned base_a;  /* this lane's slot 0 */
+    unsigned top_a;   /* this lane's first free slot */
+    int cap_b;        /* capacity in bytes of address range (cap * SLOT) */
+    double sum;       /* lane's running sum of weight * F(t) */
 
-    /* t_safe: any t inside the table; slot 0 always holds a valid item so that masked rounds can read it */
-    __device__ __forceinline__ void init(void *warp_mem, int lane, int cap, const T *table, int b, T t_safe)
+    __device__ __forceinline__ void init_base(void *warp_mem, int lane, int cap, K safe)
     {
-        base = reinterpret_cast<Item *>(warp_mem) + lane;
-        top = 0; cap32 = 32 * cap; tab = table; bias = b; sum = 0;
-        base[0] = Item::make(t_safe, T(0));
+        base_a = smem_addr(warp_mem) + lane * Item::BYTES;
+        top_a = base_a; cap_b = cap * SLOT; sum = 0;
+        Item::store(base_a, safe, W(0)); /* slot 0 always holds a valid item: masked rounds may read it */
     }
-    __device__ __forceinline__ void push(bool ok, T t, T w)
+    __device__ __forceinline__ void push(bool ok, K t, W w)
     {
-        if (ok) { base[top] = Item::make(t, w); top += 32; }
+        if (ok) { Item::store(top_a, t, w); top_a += SLOT; }
     }
     /* one round: pop up to R items per lane and add their terms (MASKED: lanes may hold fewer) */
     template <bool MASKED> __device__ __forceinline__ void round()
     {
-        T part = 0;
+        typename Derived::Acc part = 0;
 #pragma unroll
         for (int r = 0; r < PAIR_R; r++) {
-            const int s = top - 32 * (r + 1);
-            const bool have = !MASKED || s >= 0;
-            const Item it = base[have ? s : 0];
-            /* SIGNED stacks of bare t carry the sign of the term in the sign bit of t */
-            const T wt = UQ ? (SIGNED ? sign_unit(it.t) : T(1)) : it.weight();
-            const T f = pair_f(UQ && SIGNED ? abs_of(it.t) : it.t, tab, bias);
-            if (MASKED) part += have ? f * wt : T(0);
-            else part = UQ && !SIGNED ? part + f : fma(f, wt, part);
+            const unsigned a = top_a - SLOT * (r + 1);
+            const bool have = !MASKED || (int)(a - base_a) >= 0;
+            K t; W w;
+            Item::load(have ? a : base_a, t, w);
+            const typename Derived::Acc f = static_cast<Derived *>(this)->term(t, w);
+            part += MASKED ? (have ? f : typename Derived::Acc(0)) : f;
         }
-        top = MASKED ? max(top - 32 * PAIR_R, 0) : top - 32 * PAIR_R;
+        top_a = MASKED ? base_a + max((int)(top_a - base_a) - SLOT * PAIR_R, 0) : top_a - SLOT * PAIR_R;
         sum += (double)part;
     }
     /* Called by the whole warp after each group of at most `limit` pushes per lane. */
     __device__ __forceinline__ void service(int limit)
     {
-        int mn = __reduce_min_sync(0xffffffffu, top);
-        while (mn >= 32 * PAIR_R) { round<false>(); mn -= 32 * PAIR_R; }
-        int mx = __reduce_max_sync(0xffffffffu, top);
-        while (mx > cap32 - 32 * limit) { round<true>(); mx -= 32 * PAIR_R; }
+        int mn = __reduce_min_sync(0xffffffffu, (int)(top_a - base_a));
+        while (mn >= SLOT * PAIR_R) { round<false>(); mn -= SLOT * PAIR_R; }
+        int mx = __reduce_max_sync(0xffffffffu, (int)(top_a - base_a));
+        while (mx > cap_b - SLOT * limit) { round<true>(); mx -= SLOT * PAIR_R; }
     }
     __device__ __forceinline__ void finish()
     {
-        int mx = __reduce_max_sync(0xffffffffu, top);
-        while (mx > 0) { round<true>(); mx -= 32 * PAIR_R; }
+        int mx = __reduce_max_sync(0xffffffffu, (int)(top_a - base_a));
+        while (mx > 0) { round<true>(); mx -= SLOT * PAIR_R; }
     }
+};
+
+/* Near stack: t in the kernel's precision, F from the quintic (FP32: cubic) table. */
+template <typename T, bool UQ, bool SIGNED = false>
+struct LaneStack : StackBase<T, T, UQ, LaneStack<T, UQ, SIGNED>> {
+    typedef T Acc;
+    const T *tab;
+    int bias;
+    __device__ __forceinline__ void init(void *warp_mem, int lane, int cap, const T *table, int b, T t_safe)
+    {
+        tab = table; bias = b;
+        this->init_base(warp_mem, lane, cap, t_safe);
+    }
+    __device__ __forceinline__ T term(T t, T w) const
+    {
+        /* SIGNED stacks of bare t carry the sign of the term in the sign bit of t */
+        if (UQ && SIGNED) return pair_f(abs_of(t), tab, bias) * sign_unit(t);
+        return UQ ? pair_f(t, tab, bias) : pair_f(t, tab, bias) * w;
+    }
+};
+
+/* ---- the far shell (FP64 kernels only) ------------------------------------------------------------
+ * Terms with t >= 16 are below F(16) = 3.9e-9 each, and their total is < 4e-5 of a sum of order N^2/2:
+ * FP32 arithmetic on them (relative error ~1e-7) changes the sum by < 4e-12 in the worst, fully
+ * coherent case and ~3e-14 for random rounding (DESIGN.md section 5.2 derives both).  They are kept as
+ * 32-bit fixed point x = round(t 2^25) (one FP64 add with 2^27 puts it in the low word; resolution
+ * 3e-8 in t, so F keeps 3e-8 relative), evaluated by an FP32 cubic on bins of width 1/8 in t whose index
+ * and local variable are bit fields of x, from a table replicated 8 times so that the 8 lanes of a
+ * quarter-warp read 8 different 16-byte columns: LDS.128 without bank conflicts. */
+struct FarFmt {
+    static constexpr int S = 25;            /* x = t 2^S, t < 64; bit 31 = sign of the term       */
+    static constexpr int KB = 3;            /* 2^KB bins per unit of t                             */
+    static constexpr int MB = S - KB;       /* bits of x inside a bin                              */
+    static constexpr int REP = 8;           /* table copies                                        */
+    static constexpr int T0 = 16;           /* the far shell starts at t = T0                      */
+};
+__device__ __forceinline__ unsigned far_fixed(double t) { return (unsigned)__double2loint(t + 134217728.0 /* 2^27 */); }
+
+template <bool UQ, bool SIGNED> struct FarStack : StackBase<unsigned, float, UQ, FarStack<UQ, SIGNED>> {
+    typedef float Acc;
+    const float4 *tab; /* [bin][REP] cubic in u = (fraction of the bin) - 1/2; this lane's copy pre-selected */
+    __device__ __forceinline__ void init(void *warp_mem, int lane, int cap, const float *table)
+    {
+        tab = reinterpret_cast<const float4 *>(table) + (lane & (FarFmt::REP - 1));
+        this->init_base(warp_mem, lane, cap, (unsigned)FarFmt::T0 << FarFmt::S);
+    }
+    __device__ __forceinline__ float term(unsigned x, float w) const
+    {
+        const int idx = (int)((x & 0x7fffffffu) >> FarFmt::MB) - (FarFmt::T0 << FarFmt::KB);
+        /* the MB bits inside the bin become the mantissa of a float in [1, 2) */
+        const float u = __uint_as_float(((x << (23 - FarFmt::MB)) & 0x7fffffu) | 0x3f800000u) - 1.5f;
+        const float4 c = tab[idx * FarFmt::REP];
+        float f = fmaf(fmaf(fmaf(c.w, u, c.z), u, c.y), u, c.x);
+        if (UQ && SIGNED) f = __uint_as_float(__float_as_uint(f) ^ (x & 0x80000000u));
+        return UQ ? f : f * w;
+    }
+};
+
+/* The stacks of one lane: near (t in the kernel's precision) and, for FP64 kernels, far. */
+template <typename T, bool UQ, bool SIGNED> struct PairStacks;
+template <bool UQ, bool SIGNED> struct PairStacks<float, UQ, SIGNED> {
+    LaneStack<float, UQ, SIGNED> nr;
+    template <bool FLIP> __device__ __forceinline__ void push(bool ok, float t, int, float w) { nr.push(ok, FLIP ? -t : t, w); }
+    __device__ __forceinline__ void service(int limit) { nr.service(limit); }
+    __device__ __forceinline__ void finish() { nr.finish(); }
+    __device__ __forceinline__ double take() { const double v = nr.sum; nr.sum = 0; return v; }
+};
+template <bool UQ, bool SIGNED> struct PairStacks<double, UQ, SIGNED> {
+    LaneStack<double, UQ, SIGNED> nr;
+    FarStack<UQ, SIGNED> fr;
+    int key_far; /* order key of T0, or INT_MAX when the far shell is switched off */
+    template <bool FLIP> __device__ __forceinline__ void push(bool ok, double t, int key, double w)
+    {
+        const bool far = key >= key_far;
+        nr.push(ok && !far, FLIP ? -t : t, w);
+        fr.push(ok && far, far_fixed(t) | (FLIP ? 0x80000000u : 0u), (float)w);
+    }
+    /* key_far is uniform over the grid: the far stack is either used by every lane or by none */
+    __device__ __forceinline__ bool has_far() const { return key_far != 0x7fffffff; }
+    __device__ __forceinline__ void service(int limit) { nr.service(limit); if (has_far()) fr.service(limit); }
+    __device__ __forceinline__ void finish() { nr.finish(); if (has_far()) fr.finish(); }
+    __device__ __forceinline__ double take() { const double v = nr.sum + fr.sum; nr.sum = 0; fr.sum = 0; return v; }
 };
 
 /* Images scanned between two services of the stack on the image-list path. */
 constexpr int IMG_STEP = 8;
 
 /* Pushes per lane between two services of the stack, and the stack capacity that allows them. */
-template <int DIM, bool ORTHO, int M> struct ScanShape {
+template <int DIM, bool ORTHO, int M, bool UQ> struct ScanShape {
     static constexpr int ROW = 2 * M + 1;
     static constexpr int ALL = DIM == 3 ? ROW * ROW * ROW : ROW * ROW;
-    static constexpr bool WHOLE = ALL <= 27;               /* service once per pair, else once per x-row */
+    /* service once per pair, else once per x-row ((t, qq) items take twice the bytes: half the capacity) */
+    static constexpr bool WHOLE = UQ && ALL <= 27;
     static constexpr int LIMIT = ORTHO ? (WHOLE ? ALL : ROW) : IMG_STEP;
     static constexpr int MIN_CAP = LIMIT + PAIR_R;
 };
@@ -181,12 +282,12 @@ template <int DIM, bool ORTHO, int M> struct ScanShape {
  * table (t < t_min) are evaluated directly into `direct` (weighted by w); the rest go to the stack. */
 template <typename T, int DIM, bool ORTHO, int M, bool UQ, bool SIGNED = false, bool NEG = false>
 __device__ __forceinline__ void scan_pair(const RealGeom<T> &g, T *d, T w, bool valid,
-                                          LaneStack<T, UQ, SIGNED> &st, double &direct, const T *simg, int nimg)
+                                          PairStacks<T, UQ, SIGNED> &st, double &direct, const T *simg, int nimg)
 {
     /* NEG (move kernel, old position): the term enters with a minus sign -- in w for (t, w) items (the
      * caller passes -w), in the sign bit of t for bare-t items */
     constexpr bool FLIP = NEG && UQ && SIGNED;
-    typedef ScanShape<DIM, ORTHO, M> Shape;
+    typedef ScanShape<DIM, ORTHO, M, UQ> Shape;
     if (ORTHO) {
         constexpr int ROW = Shape::ROW;
         T sq[DIM][ROW];
@@ -202,21 +303,43 @@ __device__ __forceinline__ void scan_pair(const RealGeom<T> &g, T *d, T w, bool 
         const bool tiny = valid && order_key(t0) < g.key_min;
         if (tiny) direct += (double)((FLIP ? -w : w) * pair_f_direct(t0));
         const bool central_ok = valid && !tiny;
+        if (Shape::WHOLE) {
 #pragma unroll
-        for (int mz = 0; mz < (DIM == 3 ? ROW : 1); mz++) {
+            for (int mz = 0; mz < (DIM == 3 ? ROW : 1); mz++) {
 #pragma unroll
-            for (int my = 0; my < ROW; my++) {
-                const T syz = DIM == 3 ? sq[1][my] + sq[2][mz] : sq[1][my];
+                for (int my = 0; my < ROW; my++) {
+                    const T syz = DIM == 3 ? sq[1][my] + sq[2][mz] : sq[1][my];
 #pragma unroll
-                for (int mx = 0; mx < ROW; mx++) {
-                    const T t = sq[0][mx] + syz;
-                    const bool centre = mx == M && my == M && (DIM == 2 || mz == M);
-                    st.push((centre ? central_ok : valid) && order_key(t) <= g.key_rc, FLIP ? -t : t, w);
+                    for (int mx = 0; mx < ROW; mx++) {
+                        const T t = sq[0][mx] + syz;
+                        const bool centre = mx == M && my == M && (DIM == 2 || mz == M);
+                        const int key = order_key(t);
+                        st.template push<FLIP>((centre ? central_ok : valid) && key <= g.key_rc, t, key, w);
+                    }
                 }
-                if (!Shape::WHOLE) st.service(Shape::LIMIT);
+            }
+            st.service(Shape::LIMIT);
+        } else {
+            /* rolled loops over the y and z images (the stacks are serviced after every x-row) */
+#pragma unroll 1
+            for (int mz = 0; mz < (DIM == 3 ? ROW : 1); mz++) {
+                T sz = 0;
+                if (DIM == 3) { const T z = fma((T)(M - mz), g.L[2], d[2]); sz = z * z; }
+#pragma unroll 1
+                for (int my = 0; my < ROW; my++) {
+                    const T y = fma((T)(M - my), g.L[1], d[1]);
+                    const T syz = fma(y, y, sz);
+                    const bool crow = my == M && (DIM == 2 || mz == M);
+#pragma unroll
+                    for (int mx = 0; mx < ROW; mx++) {
+                        const T t = sq[0][mx] + syz;
+                        const int key = order_key(t);
+                        st.template push<FLIP>((mx == M && crow ? central_ok : valid) && key <= g.key_rc, t, key, w);
+                    }
+                    st.service(Shape::LIMIT);
+                }
             }
         }
-        if (Shape::WHOLE) st.service(Shape::LIMIT);
     } else {
         T f[3];
 #pragma unroll
@@ -243,7 +366,7 @@ __device__ __forceinline__ void scan_pair(const RealGeom<T> &g, T *d, T w, bool 
                 const int key = order_key(t);
                 const bool tiny = in && key < g.key_min;
                 if (tiny) direct += (double)((FLIP ? -w : w) * pair_f_direct(t));
-                st.push(in && !tiny && key <= g.key_rc, FLIP ? -t : t, w);
+                st.template push<FLIP>(in && !tiny && key <= g.key_rc, t, key, w);
             }
             st.service(Shape::LIMIT);
         }

@@ -115,6 +115,38 @@ void build_pair_table(int kbits, int degree, int e_min, double t_max, PairTable 
     }
 }
 
+/* Far-shell table of the FP64 kernels (ewald_realspace.cuh, FarStack): F(t) for t >= t0 on bins of width
+ * 2^-kb, cubic in u = (position inside the bin) - 1/2, FP32 coefficients, `rep` copies interleaved as
+ * [bin][copy][4] (each copy is one 16-byte column: conflict-free LDS.128). */
+void build_far_table(int t0, int kb, int rep, double t_max, std::vector<float> *tab, int *n_far)
+{
+    tab->clear();
+    *n_far = 0;
+    if (!(t_max > t0)) return;
+    const int nb = (int)floorl(((real)t_max - t0) * (1 << kb)) + 1;
+    const int n = 4;
+    tab->assign((size_t)nb * rep * 4, 0.0f);
+    for (int b = 0; b < nb; b++) {
+        const real width = ldexpl(1.0L, -kb), mid = t0 + (b + 0.5L) * width;
+        real fv[4], cheb[4];
+        for (int i = 0; i < n; i++) {
+            const real t = mid + 0.5L * width * cosl(kPi * (2 * i + 1) / (2 * n)), z = sqrtl(t);
+            fv[i] = erfcl(z) / z;
+        }
+        for (int k = 0; k < n; k++) {
+            real s = 0;
+            for (int i = 0; i < n; i++) s += fv[i] * cosl(k * kPi * (2 * i + 1) / (2 * n));
+            cheb[k] = (k == 0 ? 1 : 2) * s / n;
+        }
+        /* T0 = 1, T1 = v, T2 = 2v^2 - 1, T3 = 4v^3 - 3v; v = 2u */
+        const real m0 = cheb[0] - cheb[2], m1 = cheb[1] - 3 * cheb[3], m2 = 2 * cheb[2], m3 = 4 * cheb[3];
+        const float c[4] = {(float)m0, (float)(2 * m1), (float)(4 * m2), (float)(8 * m3)};
+        for (int r = 0; r < rep; r++)
+            for (int k = 0; k < 4; k++) (*tab)[((size_t)b * rep + r) * 4 + k] = c[k];
+    }
+    *n_far = nb;
+}
+
 /* Host evaluation of the table exactly as the kernels index it (FP64 format). */
 double eval_pair_table(const PairTable &p, double t)
 {
@@ -181,6 +213,7 @@ ewald_status build_tables(int dim, const double *cell, double kappa_d, double g_
     const double t_top = r_cutoff * r_cutoff * kappa_d * kappa_d * (1 + 1e-5);
     build_pair_table(PAIR_K64, PAIR_DEG64, PAIR_EMIN, t_top, &t->pair64);
     build_pair_table(PAIR_K32, PAIR_DEG32, PAIR_EMIN, t_top, &t->pair32);
+    build_far_table(FAR_T0, FAR_KB, FAR_REP, t_top, &t->far_tab, &t->n_far);
     bool ortho = true;
     for (int i = 0; i < 3; i++)
         for (int j = 0; j < 3; j++) {

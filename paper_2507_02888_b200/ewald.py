@@ -20,7 +20,7 @@ _STATUS = {0: "EWALD_OK", 1: "EWALD_EINVAL", 2: "EWALD_ESINGULAR", 3: "EWALD_ERA
 # every symbol include/ewald.h declares (checked by tests/test_abi.py against the header text)
 SYMBOLS = ["ewald_padded_n", "ewald_setup", "ewald_setup_summary", "ewald_oct_plan_summary",
            "ewald_pair_table_eval",
-           "ewald_destroy", "ewald_set_stream", "ewald_set_recip_variant",
+           "ewald_destroy", "ewald_set_stream", "ewald_set_recip_variant", "ewald_set_real_variant",
            "ewald_set_fixed_charges", "ewald_energy_batch", "ewald_energy_batch_host",
            "ewald_load_walkers", "ewald_move_delta_batch", "ewald_move_delta_batch_host",
            "ewald_move_delta", "ewald_num_g", "ewald_num_images", "ewald_r_cutoff", "ewald_get_g",
@@ -64,6 +64,7 @@ def load_library():
         "ewald_destroy": (None, [vp]),
         "ewald_set_stream": (i, [vp, vp]),
         "ewald_set_recip_variant": (i, [vp, i]),
+        "ewald_set_real_variant": (i, [vp, i]),
         "ewald_set_fixed_charges": (i, [vp, i, dp, dp]),
         "ewald_energy_batch": (i, [vp, i, i, i, vp, vp, vp, vp]),
         "ewald_energy_batch_host": (i, [vp, i, i, i, vp, vp, vp, vp]),
@@ -217,6 +218,11 @@ def ewald_pair_table_eval(prec, t_max, t):
 
 def ewald_destroy(ctx):
     ctx.close()
+
+
+def ewald_set_real_variant(ctx, variant):
+    """0 default (FP64 kernels evaluate the far shell t >= 16 in FP32), 1 every term in FP64."""
+    _check(ctx, load_library().ewald_set_real_variant(ctx.handle, int(variant)))
 
 
 def ewald_set_recip_variant(ctx, variant):

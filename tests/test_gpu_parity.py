@@ -83,6 +83,24 @@ def test_energy_fp64_matches_oracle(torch_cuda, idx):
     assert E.ewald_num_g(ctx) == ref.num_g(w.dim, w.cell, w.g_cutoff)
 
 
+@pytest.mark.parametrize("idx", [1, 2, 4])
+def test_both_real_space_variants_match_oracle(torch_cuda, idx):
+    """FP64 real-space kernel with the far shell (kappa^2 r^2 >= 16) in FP32 (default) and with every
+    term in FP64: both within the FP64 tolerance of the oracle, and within 1e-13 of E_real of each other
+    (the bound DESIGN.md section 5.2 derives for the far shell is 1e-14 of E_real)."""
+    w = workloads.config(idx)
+    pos = w.positions(N_WALKERS[idx])
+    e_ref, c_ref = _oracle_energy(w, pos)
+    ctx = _ctx(w)
+    got = {}
+    for variant in (0, 1):
+        E.ewald_set_real_variant(ctx, variant)
+        e, c = _gpu_energy(torch_cuda, ctx, pos, w.charges, "f64")
+        _assert_energy(e, c, e_ref, c_ref, TOL64)
+        got[variant] = c[:, 1]
+    assert (np.abs(got[0] - got[1]) / np.abs(c_ref[:, 1])).max() <= 1e-13
+
+
 @pytest.mark.parametrize("idx", [1, 2, 3, 4])
 def test_both_reciprocal_kernels_match_oracle(torch_cuda, idx):
     """Octant real-product form (variant 2) and complex half-set form (variant 1), FP64 and FP32, on
