@@ -600,10 +600,10 @@ static bool real_shape(const ewald_ctx *c, size_t fixed, int min_cap_u, int min_
         /* bytes per unit of capacity: near item + (far item: 4 bytes), per lane, per warp */
         const size_t per_cap = (size_t)(th / 32) * 32 * (sizeof(T) + (far ? 4 : 0));
         long long cu = (long long)((budget - fixed) / per_cap);
-        const long long want = 64;
+        const long long want = 2 * (min_cap_u > min_cap_g ? min_cap_u : min_cap_g) + 8;
         if (cu > want) cu = want;
         cu &= ~1LL;
-        if (cu >= min_cap_u + 8 && cu >= 2 * min_cap_g) {
+        if (cu >= min_cap_u + 4 && cu >= 2 * min_cap_g) {
             *threads = th;
             P->cap_u = (int)cu; P->cap_g = (int)(cu / 2);
             P->capf_u = far ? (int)cu : 0; P->capf_g = far ? (int)(cu / 2) : 0;

@@ -148,7 +148,7 @@ template <typename T> struct RealArgs {
     RealGeom<T> g;
 };
 
-constexpr int REAL_MAX_THREADS = 256;
+constexpr int REAL_MAX_THREADS = 512;
 
 /* Shared-memory carve-up common to the real-space and move kernels. */
 template <typename T> struct RealSmem {

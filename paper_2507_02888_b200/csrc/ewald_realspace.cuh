@@ -272,9 +272,12 @@ constexpr int IMG_STEP = 8;
 template <int DIM, bool ORTHO, int M, bool UQ> struct ScanShape {
     static constexpr int ROW = 2 * M + 1;
     static constexpr int ALL = DIM == 3 ? ROW * ROW * ROW : ROW * ROW;
-    /* service once per pair, else once per x-row ((t, qq) items take twice the bytes: half the capacity) */
-    static constexpr bool WHOLE = UQ && ALL <= 27;
-    static constexpr int LIMIT = ORTHO ? (WHOLE ? ALL : ROW) : IMG_STEP;
+    /* the stacks are serviced once per pair (few images), once per z-plane of 9 images (|m| <= 1 in 3D),
+     * else once per x-row: small LIMIT = small stacks = more warps per SM */
+    /* (t, qq) items take twice the bytes, i.e. half the capacity: always once per x-row */
+    static constexpr bool WHOLE = ALL <= (UQ ? 9 : 3);
+    static constexpr bool PLANE = UQ && !WHOLE && DIM == 3 && ROW == 3;
+    static constexpr int LIMIT = ORTHO ? (WHOLE ? ALL : PLANE ? ROW * ROW : ROW) : IMG_STEP;
     static constexpr int MIN_CAP = LIMIT + PAIR_R;
 };
 
@@ -303,7 +306,7 @@ __device__ __forceinline__ void scan_pair(const RealGeom<T> &g, T *d, T w, bool 
         const bool tiny = valid && order_key(t0) < g.key_min;
         if (tiny) direct += (double)((FLIP ? -w : w) * pair_f_direct(t0));
         const bool central_ok = valid && !tiny;
-        if (Shape::WHOLE) {
+        if (Shape::WHOLE || Shape::PLANE) {
 #pragma unroll
             for (int mz = 0; mz < (DIM == 3 ? ROW : 1); mz++) {
 #pragma unroll
@@ -317,8 +320,9 @@ __device__ __forceinline__ void scan_pair(const RealGeom<T> &g, T *d, T w, bool 
                         st.template push<FLIP>((centre ? central_ok : valid) && key <= g.key_rc, t, key, w);
                     }
                 }
+                if (Shape::PLANE) st.service(Shape::LIMIT);
             }
-            st.service(Shape::LIMIT);
+            if (Shape::WHOLE) st.service(Shape::LIMIT);
         } else {
             /* rolled loops over the y and z images (the stacks are serviced after every x-row) */
 #pragma unroll 1
