@@ -5,17 +5,16 @@ A "step" is one pass of the hot path over one batch: ewald_energy_batch on all w
 (BASELINE.json configs[1]: 3D HEG, N = 250, 1024 walkers, ~2000 G-vectors), i.e. S1-S6 of DESIGN.md.
 Prints ONE JSON line (rank 0).  `--impl reference` times the CPU oracle instead (rank 0 only).
 
-  python bench.py --gpus 1 --steps 20 --warmup 3
+  python bench.py --gpus 1 --steps 500 --warmup 3
   python -m torch.distributed.run --nnodes=1 --nproc-per-node N --master-addr 127.0.0.1 \
       --master-port P bench.py --gpus N --steps K --warmup W
 """
 import argparse
 import json
+import math
 import os
 import statistics
-import subprocess
 import sys
-import tempfile
 import time
 
 import numpy as np
@@ -34,10 +33,10 @@ SM_COUNT, FP64_LANES, FP32_LANES = 148, 64, 128   # B200: lanes per SM per clock
 def parse():
     p = argparse.ArgumentParser()
     p.add_argument("--gpus", type=int, default=1)
-    p.add_argument("--steps", type=int, default=20)
+    p.add_argument("--steps", type=int, default=500)
     p.add_argument("--warmup", type=int, default=3)
     p.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    p.add_argument("--config", type=int, default=2, help="BASELINE.json config index (1-based), 1..4")
+    p.add_argument("--config", type=int, default=2, help="BASELINE.json config index (1-based): 1..4 energies, 5 moves")
     p.add_argument("--prec", default="f64", choices=["f64", "f32"])
     p.add_argument("--no-extras", action="store_true", help="skip FP32 / move / cpu_baseline legs")
     return p.parse_args()
@@ -51,48 +50,57 @@ def measured_peaks():
 
 
 class ClockSampler:
-    """nvidia-smi clocks and throttle reasons DURING the timed region (B200_PROFILING.md)."""
-    Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,"
-         "clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
-         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+    """SM clock, power and throttle reasons sampled through NVML from a thread DURING the timed region
+    (the recipe's clocks line in B200_PROFILING.md; same counters as its nvidia-smi query)."""
 
-    def __init__(self, gpu_index):
-        self.f = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
+    def __init__(self, torch, cuda_index, period_s=0.01):
+        import threading
+        self.samples, self.reasons, self.power = [], set(), []
+        self.sm_max = None
+        self._stop = threading.Event()
+        self._thread = None
         try:
-            self.p = subprocess.Popen(["nvidia-smi", "-i", str(gpu_index), "--query-gpu=" + self.Q,
-                                       "--format=csv,noheader,nounits", "-lms", "100"],
-                                      stdout=self.f, stderr=subprocess.DEVNULL)
-        except Exception:
-            self.p = None
+            import pynvml
+            pynvml.nvmlInit()
+            p = torch.cuda.get_device_properties(cuda_index)
+            bus = "%08x:%02x:%02x.0" % (p.pci_domain_id, p.pci_bus_id, p.pci_device_id)
+            h = pynvml.nvmlDeviceGetHandleByPciBusId(bus.encode())
+            self.sm_max = float(pynvml.nvmlDeviceGetMaxClockInfo(h, pynvml.NVML_CLOCK_SM))
+            names = {"hw_slowdown": getattr(pynvml, "nvmlClocksEventReasonHwSlowdown", 0x8),
+                     "hw_thermal_slowdown": getattr(pynvml, "nvmlClocksEventReasonHwThermalSlowdown", 0x40),
+                     "sw_thermal_slowdown": getattr(pynvml, "nvmlClocksEventReasonSwThermalSlowdown", 0x20),
+                     "sw_power_cap": getattr(pynvml, "nvmlClocksEventReasonSwPowerCap", 0x4)}
+            get_reasons = getattr(pynvml, "nvmlDeviceGetCurrentClocksEventReasons", None) or \
+                pynvml.nvmlDeviceGetCurrentClocksThrottleReasons
+
+            def loop():
+                while not self._stop.is_set():
+                    try:
+                        self.samples.append(float(pynvml.nvmlDeviceGetClockInfo(h, pynvml.NVML_CLOCK_SM)))
+                        self.power.append(pynvml.nvmlDeviceGetPowerUsage(h) / 1000.0)
+                        r = get_reasons(h)
+                        for k, bit in names.items():
+                            if r & bit:
+                                self.reasons.add(k)
+                    except Exception:
+                        pass
+                    self._stop.wait(period_s)
+
+            self._thread = threading.Thread(target=loop, daemon=True)
+            self._thread.start()
+        except Exception as ex:  # no NVML: the line says so instead of inventing clocks
+            self.error = str(ex)
 
     def stop(self):
-        out = {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
-        if self.p is None:
+        out = {"sm_mhz": None, "sm_max_mhz": self.sm_max, "reasons": [], "samples": 0}
+        if self._thread is None:
+            out["error"] = getattr(self, "error", "NVML unavailable")
             return out
-        self.p.terminate()
-        try:
-            self.p.wait(timeout=5)
-        except Exception:
-            self.p.kill()
-        self.f.flush()
-        self.f.seek(0)
-        sm, smax, reasons, power = [], [], set(), []
-        for line in self.f:
-            c = [x.strip() for x in line.split(",")]
-            if len(c) < 9:
-                continue
-            try:
-                sm.append(float(c[1])); smax.append(float(c[2])); power.append(float(c[3]))
-            except ValueError:
-                continue
-            for name, v in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"),
-                               c[5:9]):
-                if v.lower().startswith("active"):
-                    reasons.add(name)
-        os.unlink(self.f.name)
-        if sm:
-            out.update(sm_mhz=statistics.median(sm), sm_max_mhz=max(smax), samples=len(sm),
-                       power_w_max=max(power), reasons=sorted(reasons))
+        self._stop.set()
+        self._thread.join(timeout=2)
+        if self.samples:
+            out.update(sm_mhz=statistics.median(self.samples), samples=len(self.samples),
+                       power_w_max=max(self.power) if self.power else None, reasons=sorted(self.reasons))
         return out
 
 
@@ -125,6 +133,78 @@ def run_reference(args, rank):
         "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
         "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0}))
+
+
+def count_pair_terms(w, pos):
+    """Pairs and pair-image terms (|r_ij - R| < r_c) per walker of an orthorhombic workload, counted with
+    numpy on a few walkers: the unit count of the real-space kernel's roofline."""
+    sides = np.diag(w.cell)[:w.dim]
+    m = int(math.floor(w.r_cutoff / sides.min() + 0.5 - 1e-12))
+    shifts = np.array(np.meshgrid(*[np.arange(-m, m + 1)] * w.dim, indexing="ij")).reshape(w.dim, -1).T * sides
+    terms = []
+    for p in pos:
+        others = [p] if w.ion_pos is None else [p, w.ion_pos]
+        cnt = 0
+        for k, o in enumerate(others):
+            d = p[:, None, :] - o[None, :, :]
+            d -= np.rint(d / sides) * sides
+            r2 = ((d[:, :, None, :] - shifts[None, None, :, :]) ** 2).sum(-1)
+            inside = r2 < w.r_cutoff ** 2
+            if k == 0:
+                iu = np.triu_indices(len(p), 1)
+                cnt += int(inside[iu].sum())
+            else:
+                cnt += int(inside.sum())
+        terms.append(cnt)
+    n_ion = 0 if w.ion_pos is None else len(w.ion_pos)
+    pairs = w.n * (w.n - 1) // 2 + w.n * n_ion
+    return pairs, float(np.mean(terms)), (2 * m + 1) ** w.dim, m
+
+
+def move_leg(torch, E, device, stream, prec, n_steps, flush, hbm_peak_gbs):
+    """BASELINE configs[4]: 3D HEG N = 1000, 4096 walkers with stored rho(G); each step moves one seeded-random
+    electron per walker by a Gaussian step (reading R14), always committed.  Returns moves/s (device-resident,
+    CUDA events around each batch of 4096 moves, L2 flushed in between) and the HBM roofline of the move kernel:
+    algorithmic bytes per move = read + write of rho(G+) (2 x N_G+ complex) + one read of the walker's
+    positions."""
+    w = workloads.config(5)
+    npdt, tdt = (np.float64, torch.float64) if prec == "f64" else (np.float32, torch.float32)
+    es = 8 if prec == "f64" else 4
+    W, S = w.n_walkers, min(n_steps, w.n_steps)
+    pos0 = w.positions(W)
+    electron, disp = w.moves(W, S)
+    cur = pos0.copy()
+    new_r = np.zeros((S, W, w.dim))
+    ar = np.arange(W)
+    for s_ in range(S):
+        new_r[s_] = cur[ar, electron[s_]] + disp[s_]
+        cur[ar, electron[s_]] = new_r[s_]
+    ctx = E.ewald_setup(w.dim, w.cell, w.kappa, w.g_cutoff, w.r_cutoff, device=device, stream=stream)
+    E.ewald_load_walkers(ctx, w.n, torch.from_numpy(E.to_soa(pos0, npdt)).cuda(),
+                         torch.from_numpy(w.charges.astype(npdt)).cuda())
+    d_w = torch.arange(W, dtype=torch.int32, device="cuda")
+    d_el = torch.from_numpy(electron).cuda()
+    d_r = torch.from_numpy(new_r.astype(npdt)).cuda()
+    d_de = torch.zeros((S, W), dtype=torch.float64, device="cuda")
+    warm = min(3, S // 2)
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(S)]
+    for s_ in range(S):
+        flush.zero_()
+        ev[s_][0].record()
+        E.ewald_move_delta_batch(ctx, d_w, d_el[s_], d_r[s_], 1, d_de[s_])
+        ev[s_][1].record()
+    torch.cuda.synchronize()
+    ms = [a.elapsed_time(b) for a, b in ev][warm:]
+    t = sum(ms) * 1e-3 / len(ms)
+    ngp = E.ewald_num_g(ctx) // 2
+    bytes_per_move = 2 * ngp * 2 * es + w.dim * w.n * es
+    gbs = bytes_per_move * W / t / 1e9
+    E.ewald_destroy(ctx)
+    return {"workload": "BASELINE configs[4]: %s" % w.name, "dtype": prec, "moves_per_s": W / t,
+            "ms_per_batch_of_%d_moves" % W: t * 1e3, "timed_batches": len(ms), "warmup_batches": warm,
+            "roofline": {"kernel": "move", "bound": "hbm", "unit": "GB/s", "achieved": gbs, "peak": hbm_peak_gbs,
+                         "frac": gbs / hbm_peak_gbs, "alg_bytes_per_move": bytes_per_move, "traffic": None},
+            "delta_e_finite": bool(torch.isfinite(d_de).all().item())}
 
 
 def workload_config(w, walkers_per_gpu, l2_note):
@@ -165,6 +245,20 @@ def main():
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
         return float(t.item())
 
+    if args.config == 5:   # the single-move metric alone (used for profiling; the default run reports it in extras)
+        flush = torch.empty(256 * 1024 * 1024, dtype=torch.uint8, device="cuda")
+        r = move_leg(torch, E, local, torch.cuda.current_stream().cuda_stream, args.prec, args.steps, flush,
+                     float(measured_peaks().get("hbm_gbs", 6542.1)))
+        if rank == 0:
+            print(json.dumps({"metric": "single_move_delta_e_per_s", "value": r["moves_per_s"] * world,
+                              "unit": "moves/s", "n_gpus": world, "steps": r["timed_batches"],
+                              "warmup": r["warmup_batches"], "ms_per_step": r["ms_per_batch_of_4096_moves"],
+                              "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": args.prec,
+                              "data": "synthetic", "config": {"workload": r["workload"]}, "roofline": r["roofline"]}))
+        if world > 1:
+            dist.destroy_process_group()
+        return
+
     w = workloads.config(args.config)
     W = w.n_walkers
     npdt, tdt = (np.float64, torch.float64) if args.prec == "f64" else (np.float32, torch.float32)
@@ -186,7 +280,7 @@ def main():
     for _ in range(max(args.warmup, 3)):
         step()
     barrier()
-    sampler = ClockSampler(local) if rank == 0 else None
+    sampler = ClockSampler(torch, local) if rank == 0 else None
     lc0 = E.ewald_launch_count(ctx)
     ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
     t_wall0 = time.perf_counter()
@@ -220,8 +314,9 @@ def main():
     assert np.array_equal(h_e.numpy(), d_e.cpu().numpy())
 
     # ---- per-kernel device times (CUDA events inside the library, on its launch stream) -----
+    n_prof = min(args.steps, 50)
     E.ewald_profile_enable(ctx, True)
-    for _ in range(args.steps):
+    for _ in range(n_prof):
         flush.zero_()
         step()
     prof = E.ewald_profile_read(ctx)
@@ -234,7 +329,7 @@ def main():
     kernels = {}
     for name, (ms, cnt) in prof.items():
         if cnt:
-            kernels[name] = {"ms_per_launch": ms / cnt, "launches_per_step": cnt / args.steps}
+            kernels[name] = {"ms_per_launch": ms / cnt, "launches_per_step": cnt / n_prof}
     step_ms = sum(k["ms_per_launch"] * k["launches_per_step"] for k in kernels.values())
     for k in kernels.values():
         k["share_of_step"] = k["ms_per_launch"] * k["launches_per_step"] / step_ms
@@ -243,16 +338,24 @@ def main():
     kernels["recip"].update(alg_flops_per_launch=recip_flops,
                             achieved_tflops=recip_flops / (kernels["recip"]["ms_per_launch"] * 1e-3) / 1e12,
                             frac_of_peak=recip_flops / (kernels["recip"]["ms_per_launch"] * 1e-3) / peak_flops)
+    # real-space kernel: algorithmic flops = per pair (displacement, reduction to the cell, image squares and sums)
+    # + 12 per pair-image term (u = t - centre, quintic Horner, accumulate), all counted as FP64
+    pairs, terms, n_cand, m_img = count_pair_terms(w, pos[:4])
+    row = 2 * m_img + 1
+    per_pair = 21 + 2 * w.dim * row + (row * row if w.dim == 3 else 0) + n_cand
+    real_flops = (per_pair * pairs + 12.0 * terms) * W
+    t_real = kernels["real"]["ms_per_launch"] * 1e-3
+    kernels["real"].update(pairs_per_walker=pairs, pair_image_terms_per_walker=terms,
+                           pair_image_terms_per_s=terms * W / t_real, alg_flops_per_launch=real_flops,
+                           achieved_tflops=real_flops / t_real / 1e12, frac_of_peak=real_flops / t_real / peak_flops)
     dominant = max(("recip", "real"), key=lambda k: kernels[k]["share_of_step"])
     roofline = {"kernel": dominant, "bound": "alu", "unit": "TFLOP/s", "peak": peak_flops / 1e12,
-                "peak_source": "derived: %d SMs x %d %s lanes x 2 x %.0f MHz (sm_max_mhz)" %
-                               (SM_COUNT, lanes, args.prec, sm_max_hz / 1e6),
-                "traffic": None}
-    if dominant == "recip":
-        roofline.update(achieved=kernels["recip"]["achieved_tflops"], frac=kernels["recip"]["frac_of_peak"])
-    else:
-        roofline.update(achieved=None, frac=None,
-                        note="real-space kernel: no algorithmic flop count defined yet for erfc(kappa r)/r")
+                "peak_source": "derived: %d SMs x %d %s lanes x 2 x %.0f MHz (sm_max_mhz); the FMA-chain probe "
+                               "in extras measures it" % (SM_COUNT, lanes, args.prec, sm_max_hz / 1e6),
+                "achieved": kernels[dominant]["achieved_tflops"], "frac": kernels[dominant]["frac_of_peak"],
+                "traffic": None,
+                "note": "algorithmic flops per DESIGN.md section 6; the real-space kernel is limited by "
+                        "shared-memory wavefronts (table gathers), see profiles/"}
 
     out = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
            "warmup": max(args.warmup, 3), "ms_per_step": ms_total / args.steps, "higher_is_better": True,
@@ -268,11 +371,35 @@ def main():
                                           "f32": E.ewald_probe_fma(ctx, E.EWALD_F32, 4096) / 1e12}
         except Exception as ex:  # the probe is informative only
             extras["fma_chain_tflops"] = str(ex)
+        # the other precision of the same workload (BASELINE configs[1] is quoted in FP64 and FP32)
+        other = "f32" if args.prec == "f64" else "f64"
+        o_np, o_t = (np.float32, torch.float32) if other == "f32" else (np.float64, torch.float64)
+        o_pos = torch.from_numpy(E.to_soa(pos, o_np)).cuda()
+        o_q = torch.from_numpy(w.charges.astype(o_np)).cuda()
+        o_e = torch.zeros(W, dtype=torch.float64, device="cuda")
+        for _ in range(3):
+            E.ewald_energy_batch(ctx, w.n, o_pos, o_q, o_e)
+        oev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(20)]
+        for a, b in oev:
+            flush.zero_()
+            a.record()
+            E.ewald_energy_batch(ctx, w.n, o_pos, o_q, o_e)
+            b.record()
+        torch.cuda.synchronize()
+        o_ms = sum(a.elapsed_time(b) for a, b in oev) / len(oev)
+        extras["energy_other_precision"] = {"dtype": other, "value": W / (o_ms * 1e-3), "unit": UNIT,
+                                            "ms_per_step": o_ms}
+        # single-move Delta-E/s (BASELINE.json's second metric), both precisions
+        hbm = float(peaks.get("hbm_gbs", 6542.1))
+        extras["single_move"] = [move_leg(torch, E, local, stream, p, 100, flush, hbm) for p in ("f64", "f32")]
         out["extras"] = extras
     if rank == 0 and world == 1 and not args.no_extras:
         from oracle import ewald_ref as ref
         cores = ref.max_threads()
-        nsamp = min(W, 96)
+        t0 = time.perf_counter()   # size the sample for about 12 s of oracle time
+        ref.energy_batch(w.dim, w.cell, w.kappa, w.g_cutoff, w.r_cutoff, pos[:cores], w.charges, w.ion_pos, w.ion_q)
+        dt0 = time.perf_counter() - t0
+        nsamp = int(max(cores, min(W, cores * round(12.0 / max(dt0, 1e-3)))))
         t0 = time.perf_counter()
         e_ref, _ = ref.energy_batch(w.dim, w.cell, w.kappa, w.g_cutoff, w.r_cutoff, pos[:nsamp], w.charges,
                                     w.ion_pos, w.ion_q)
@@ -282,6 +409,7 @@ def main():
                                          (nsamp, W, w.name, cores, dt)}
         got = d_e.cpu().numpy()[:nsamp]
         out["parity_max_rel_err_vs_oracle"] = float((np.abs(got - e_ref) / np.abs(e_ref)).max())
+        out["parity_sample_min_abs_energy"] = float(np.abs(e_ref).min())  # a walker with E ~ 0 inflates the line above
     if rank == 0:
         print(json.dumps(out))
     if world > 1:

@@ -818,23 +818,25 @@ static ewald_status move_batch_t(ewald_ctx *c, int n_moves, const int *walker, c
     fill_geom(c->t, &A.g);
     const bool ortho = real_ortho(c);
     if (ortho) A.nimg = 0;
-    const size_t fixed = RealSmem<T>::fixed_bytes(A.P.n_bins, A.P.n_far, A.nimg, A.n_ion, 4 * (size_t)c->rowlen);
+    /* one warp per move; the CTA size follows from the shared memory the stacks need */
     int threads = 0; size_t smem = 0;
-    if (!real_shape<T>(c, fixed, real_min_cap(c, ortho, true), real_min_cap(c, ortho, false), MOVE_THREADS, &A.P, &threads,
-                       &smem) ||
-        threads != MOVE_THREADS)
-        return fail(c, EWALD_ERANGE, "move kernel: tables too large for shared memory");
-    /* persistent CTAs: the tables are staged once per CTA */
-    int per_sm = (int)(c->smem_optin / (smem + 1024));
-    if (per_sm < 1) per_sm = 1;
-    if (per_sm > 2048 / MOVE_THREADS) per_sm = 2048 / MOVE_THREADS;
-    const int grid = n_moves < c->sm_count * per_sm ? n_moves : c->sm_count * per_sm;
+    bool fits = false;
+    for (int th = MOVE_MAX_THREADS; th >= 32 && !fits; th /= 2) {
+        const size_t fixed = RealSmem<T>::fixed_bytes(A.P.n_bins, A.P.n_far, A.nimg, A.n_ion,
+                                                      4 * (size_t)c->rowlen * (th / 32));
+        fits = real_shape<T>(c, fixed, real_min_cap(c, ortho, true), real_min_cap(c, ortho, false), th, &A.P, &threads,
+                             &smem) && threads == th;
+    }
+    if (!fits) return fail(c, EWALD_ERANGE, "move kernel: tables too large for shared memory");
+    const int warps = threads / 32;
+    int grid = (n_moves + warps - 1) / warps;
+    if (grid > c->sm_count) grid = c->sm_count; /* persistent CTAs: the tables are staged once per CTA */
     ewald_status st;
 #define EWALD_LAUNCH_MOVE(DIM, ORTHO, M)                                                          \
     do {                                                                                          \
         if ((st = allow_smem(c, move_kernel<T, DIM, ORTHO, M>, smem)) != EWALD_OK) return st;     \
         ProfScope ps(c, 3);                                                                       \
-        move_kernel<T, DIM, ORTHO, M><<<grid, MOVE_THREADS, smem, c->stream>>>(A);             \
+        move_kernel<T, DIM, ORTHO, M><<<grid, threads, smem, c->stream>>>(A);             \
     } while (0)
     const int m = c->t.m_shift;
     if (c->t.dim == 3) {

@@ -374,8 +374,9 @@ __global__ void charge_sums_kernel(const T *q, int n, double *out)
 }
 
 /* ------------------------------------------------------------------------------------------ */
-/* [S7] single-particle move.  Persistent CTAs: the tables are staged once, then each CTA takes moves
- * blockIdx.x, blockIdx.x + gridDim.x, ... */
+/* [S7] single-particle move.  One WARP per move, persistent CTAs: the tables are staged once per CTA, then
+ * warp v of CTA b takes moves (b * warps + v), + gridDim.x * warps, ...  A warp needs no block barrier, its
+ * lanes run long loops (N_G+/32 vectors, N/32 partners), and the other warps of the SM hide its latencies. */
 
 template <typename T> struct MoveArgs {
     T *pos;            /* stored [W][DIM][npad] */
@@ -396,20 +397,20 @@ template <typename T> struct MoveArgs {
 
 constexpr int MOVE_THREADS = 256;
 
-/* [S7c] sum over the partners j != k of w_j [F-sum(r_new - r_j) - F-sum(r_old - r_j)], w_j = q_j (or 1
- * with the common charge applied by the caller when UQ). */
+/* [S7c] one warp: sum over the partners j != k of w_j [F-sum(r_new - r_j) - F-sum(r_old - r_j)], w_j = q_j
+ * (or 1 with the common charge applied here when UQ). */
 template <typename T, int DIM, bool ORTHO, int M, bool UQ>
 __device__ __forceinline__ double move_real(const MoveArgs<T> &A, RealSmem<T> &S, const T *pw, int k,
                                             const T *r_old, const T *r_new, T q0, T qion0)
 {
-    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     PairStacks<T, UQ, true> st;
     init_stacks(st, S, A.P, A.g.bias, warp, lane);
     __syncwarp();
     double total = 0, direct = 0;
     for (int seg = 0; seg < 2; seg++) {
         const int cnt = seg == 0 ? A.n : A.n_ion;
-        for (int base = warp * 32; base < cnt; base += MOVE_THREADS) {
+        for (int base = 0; base < cnt; base += 32) {
             const int j = base + lane;
             const bool valid = j < cnt && (seg == 1 || j != k);
             T rj[3] = {0, 0, 0};
@@ -434,7 +435,7 @@ __device__ __forceinline__ double move_real(const MoveArgs<T> &A, RealSmem<T> &S
             scan_pair<T, DIM, ORTHO, M, UQ, true, false>(A.g, dn, w, valid, st, direct, S.img, A.nimg);
             scan_pair<T, DIM, ORTHO, M, UQ, true, true>(A.g, dold, UQ ? w : -w, valid, st, direct, S.img, A.nimg);
         }
-        st.finish();
+        if (cnt > 0) st.finish();
         const double wseg = UQ ? (double)(seg == 0 ? q0 : qion0) : 1.0;
         total += (st.take() + direct) * wseg;
         direct = 0;
@@ -442,24 +443,25 @@ __device__ __forceinline__ double move_real(const MoveArgs<T> &A, RealSmem<T> &S
     return total;
 }
 
+constexpr int MOVE_MAX_THREADS = 512;
+
 template <typename T, int DIM, bool ORTHO, int M>
-__global__ void __launch_bounds__(MOVE_THREADS) move_kernel(MoveArgs<T> A)
+__global__ void __launch_bounds__(MOVE_MAX_THREADS) move_kernel(MoveArgs<T> A)
 {
     typedef typename Num<T>::T2 T2;
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    RealSmem<T> S(smem_raw, A.P, A.nimg, A.n_ion, 4 * (size_t)A.rowlen);
-    T2 *tab = reinterpret_cast<T2 *>(S.rest); /* [2][rowlen]: old, new */
-    __shared__ double red[32];
-    const int tid = threadIdx.x;
-    S.fill(A.P, A.img, A.nimg, A.ion_pos, A.ion_q, A.n_ion, tid, MOVE_THREADS);
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, n_warps = blockDim.x >> 5;
+    RealSmem<T> S(smem_raw, A.P, A.nimg, A.n_ion, 4 * (size_t)A.rowlen * n_warps);
+    T2 *tab = reinterpret_cast<T2 *>(S.rest) + (size_t)warp * 2 * A.rowlen; /* this warp's [2][rowlen]: old, new */
+    S.fill(A.P, A.img, A.nimg, A.ion_pos, A.ion_q, A.n_ion, tid, blockDim.x);
     __syncthreads();
     const bool uq = A.P.qinfo[2] != 0.0 && A.P.ion_uniform;
     const T q0 = (T)A.P.qinfo[3], qion0 = A.n_ion > 0 ? S.ion[3] : T(0);
 
-    for (int m = blockIdx.x; m < A.n_moves; m += gridDim.x) {
+    for (int m = blockIdx.x * n_warps + warp; m < A.n_moves; m += gridDim.x * n_warps) {
         const int w = A.walker[m], k = A.electron[m];
-        if (w < 0 || w >= A.n_walkers || k < 0 || k >= A.n) { /* block-uniform */
-            if (tid == 0) A.delta_e[m] = __longlong_as_double(0x7ff8000000000000LL);
+        if (w < 0 || w >= A.n_walkers || k < 0 || k >= A.n) { /* warp-uniform */
+            if (lane == 0) A.delta_e[m] = __longlong_as_double(0x7ff8000000000000LL);
             continue;
         }
         T *pw = A.pos + (size_t)w * DIM * A.npad;
@@ -469,21 +471,23 @@ __global__ void __launch_bounds__(MOVE_THREADS) move_kernel(MoveArgs<T> A)
         const T qk = A.q[k];
 
         /* [S7a] power tables of the two points */
-        if (tid < 2 * DIM) {
-            const int which = tid / DIM, d = tid - which * DIM;
+        if (lane < 2 * DIM) {
+            const int which = lane / DIM, d = lane - which * DIM;
             const T *r = which ? r_new : r_old;
             T s = 0;
 #pragma unroll
             for (int x = 0; x < DIM; x++) s += r[x] * A.binv[3 * d + x];
             power_row<T>(s, T(1), A.nmax[d], tab + which * A.rowlen + A.off[d]);
         }
-        __syncthreads();
+        __syncwarp();
 
         /* [S7b] Delta E_recip and the patch of rho(G) */
         T *rr = A.rho + (size_t)w * 2 * A.ngp_pad;
         double acc = 0;
-        for (int g = tid; g < A.ngp; g += MOVE_THREADS) {
+#pragma unroll 2
+        for (int g = lane; g < A.ngp; g += 32) {
             const short4 nn = A.gn[g];
+            const T re = rr[g], im = rr[A.ngp_pad + g];
             T2 ph[2];
 #pragma unroll
             for (int which = 0; which < 2; which++) {
@@ -505,7 +509,6 @@ __global__ void __launch_bounds__(MOVE_THREADS) move_kernel(MoveArgs<T> A)
                 ph[which] = e;
             }
             const T dr = ph[1].x - ph[0].x, di = ph[1].y - ph[0].y;
-            const T re = rr[g], im = rr[A.ngp_pad + g];
             acc += (double)(A.w2[g] * (2 * qk * (re * dr + im * di) + qk * qk * (dr * dr + di * di)));
             if (A.commit) { rr[g] = re + qk * dr; rr[A.ngp_pad + g] = im + qk * di; }
         }
@@ -515,15 +518,15 @@ __global__ void __launch_bounds__(MOVE_THREADS) move_kernel(MoveArgs<T> A)
         if (uq) accr = move_real<T, DIM, ORTHO, M, true>(A, S, pw, k, r_old, r_new, q0, qion0);
         else accr = move_real<T, DIM, ORTHO, M, false>(A, S, pw, k, r_old, r_new, q0, qion0);
         acc += (double)qk * accr * (double)A.g.kappa;
-        acc = block_sum(acc, red); /* its barriers also order every read of r_old before the commit */
-        if (tid == 0) {
+        acc = warp_sum(acc); /* its shuffles also order every lane's read of r_old before the commit */
+        if (lane == 0) {
             A.delta_e[m] = acc;
             if (A.commit) {
 #pragma unroll
                 for (int x = 0; x < DIM; x++) pw[x * A.npad + k] = r_new[x];
             }
         }
-        __syncthreads(); /* the power tables and red[] are reused by the next move */
+        __syncwarp(); /* the power tables are reused by this warp's next move */
     }
 }
 
