@@ -23,7 +23,7 @@ ROOT = os.path.dirname(os.path.abspath(__file__))
 if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
 
-from paper_2507_02888_b200 import workloads  # noqa: E402
+from paper_2507_02888_b200 import shard, workloads  # noqa: E402
 
 METRIC = "ewald_walker_energies_per_s"
 UNIT = "walker-energies/s"
@@ -262,7 +262,8 @@ def main():
     w = workloads.config(args.config)
     W = w.n_walkers
     npdt, tdt = (np.float64, torch.float64) if args.prec == "f64" else (np.float32, torch.float32)
-    pos = w.positions(W * world)[rank * W:(rank + 1) * W]     # every rank its own walkers (weak scaling)
+    lo, hi = shard.walker_range(W * world, rank, world)       # every rank its own W walkers (weak scaling)
+    pos = w.positions(W * world)[lo:hi]
     stream = torch.cuda.current_stream().cuda_stream
     ctx = E.ewald_setup(w.dim, w.cell, w.kappa, w.g_cutoff, w.r_cutoff, device=local, stream=stream)
     if w.ion_pos is not None:
