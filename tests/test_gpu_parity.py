@@ -422,6 +422,41 @@ def test_full_size_config2_sampled_walkers(torch_cuda):
         assert np.array_equal(e2[::-1], e)
 
 
+@pytest.mark.parametrize("idx", [3, 4])
+def test_full_size_configs_3_and_4_sampled_walkers(torch_cuda, idx):
+    """BASELINE configs[2] and configs[3] at their full sizes (1024 / 4096 walkers), in the launch
+    configuration bench.py --config 3 / 4 times; the oracle checks a sample of walkers one by one."""
+    w = workloads.config(idx)
+    pos = w.positions()
+    ctx = _ctx(w)
+    sample = np.array([0, 1, w.n_walkers // 2 + 3, w.n_walkers - 1])
+    for dtype, tol in (("f64", TOL64), ("f32", TOL32)):
+        p = pos if dtype == "f64" else _r32(pos)
+        e_ref, _ = _oracle_energy(w, p[sample])
+        e, _ = _gpu_energy(torch_cuda, ctx, p, w.charges, dtype, components=False)
+        assert np.all(np.isfinite(e))
+        assert (np.abs(e[sample] - e_ref) / np.abs(e_ref)).max() <= tol
+
+
+def test_full_size_config5_moves_sampled_walkers(torch_cuda):
+    """BASELINE configs[4] at its full size: 4096 walkers with stored rho(G), batches of 4096 committed moves
+    (the launch configuration bench.py times), 6 steps; walkers are independent, so the oracle runs the
+    chains of a sample of walkers and compares their Delta E, final rho(G) and positions."""
+    w = workloads.config(5)
+    W, S = w.n_walkers, 6
+    pos0, electron, new_r, final = _move_inputs(w, W, S)
+    ctx = _ctx(w)
+    de = _run_moves(torch_cuda, ctx, w, pos0, electron, new_r, "f64")
+    assert np.all(np.isfinite(de))
+    sample = np.array([0, 2047, 4095])
+    de_ref, pos_ref, rho_ref = ref.move_chain(w.dim, w.cell, w.kappa, w.g_cutoff, w.r_cutoff, pos0[sample],
+                                              w.charges, electron[:, sample], new_r[:, sample], want_rho=True)
+    _assert_delta(de[:, sample], de_ref, TOL64)
+    for k, wk in enumerate(sample):
+        assert np.abs(E.ewald_get_rho(ctx, int(wk)) - rho_ref[k]).max() <= 1e-12 * w.n
+        assert np.abs(E.ewald_get_positions(ctx, int(wk), w.n) - final[wk]).max() == 0
+
+
 def test_translation_and_permutation_invariance_on_gpu(torch_cuda):
     w = workloads.config(2)
     pos = w.positions(4)
