@@ -444,15 +444,13 @@ template <typename T> static int oct_max_threads(int npb)
 }
 
 /* Shared-memory shape of a CTA of wc walkers: particles per chunk, slab stride, bytes. */
-static bool oct_shape(const OctPlan &P, int wc, int n_warps, int n, size_t es2, int *pc, int *wstride, size_t *smem)
+static bool oct_shape(const OctPlan &P, int wc, int /*n_warps*/, int n, size_t es2, int *pc, int *wstride, size_t *smem)
 {
-    const int threads = 32 * n_warps;
-    int p = (OCT_MAX_TASKS * threads) / (wc * P.dim);
-    if (p > 32) p = 32;
-    if (p > n) p = n;
+    int p = n < 32 ? n : 32;
     for (; p >= 1; p--) {
         const int ws = p * P.rowlen + 1; /* +1 pair: staggers the walkers' slabs over the banks */
-        const size_t b = ((size_t)wc * ws + P.npb + 1) * es2 + (size_t)threads * sizeof(double);
+        /* two table buffers (the next chunk is built while this one is multiplied), partial sums, walker tags */
+        const size_t b = 2 * ((size_t)wc * ws + P.npb + 1) * es2 + (size_t)wc * (P.n_items + 1) * sizeof(double);
         if (b <= 200 * 1024) { *pc = p; *wstride = ws; *smem = b; return true; }
     }
     return false;
@@ -483,7 +481,7 @@ static void oct_fill_args(ewald_ctx *c, OctArgs<T> *A, int W, int n, const T *po
 {
     const OctPlan &P = c->t.oct;
     A->pos = pos; A->q = q; A->n = n; A->npad = ewald_padded_n(n); A->n_walkers = W;
-    A->wc = d.L.wc; A->n_slabs = d.L.n_slabs; A->pc = pc; A->rowlen = P.rowlen; A->wstride = wstride;
+    A->wc = d.L.wc; A->n_slabs = d.L.n_slabs; A->rank_stride = d.L.rank_stride; A->pc = pc; A->rowlen = P.rowlen; A->wstride = wstride;
     for (int k = 0; k < 3; k++) { A->off[k] = P.off[k]; A->nmax[k] = c->t.n_max[k]; }
     A->lane = d.d_lane; A->variant = d.d_variant;
     A->wt = c->d_oct_wt; A->tion = c->t.n_ion ? c->d_oct_tion : nullptr;

@@ -27,8 +27,9 @@ struct OctPlan {
 /* Lane assignment of one CTA of `wc` walkers: items of all its walkers sorted by block length. */
 struct OctLaunch {
     int wc = 0, n_warps = 0, n_slabs = 1; /* warps per CTA; CTAs per walker group */
+    int rank_stride = 1;        /* most lanes any walker has in one CTA */
     double cost = 0;            /* executed FMA + product operations per particle, whole CTA */
-    std::vector<int> lane;      /* [n_slabs][32 n_warps][4] = local walker, item, offA | offB << 16, offX */
+    std::vector<int> lane;      /* [n_slabs][32 n_warps][4] = local walker | rank << 8, item, offA | offB << 16, offX */
     std::vector<int> variant;   /* [n_slabs][n_warps] np | c0 << 8 */
 };
 

@@ -163,20 +163,27 @@ void make_oct_launch(const OctPlan &P, int wc, int max_warps, OctLaunch *L)
     L->variant.assign(n_warps, 0);
     L->cost = 0;
     /* padding lanes repeat the list's last entry with item = a zero-weight dummy: item index n_items */
+    /* rank = position of a lane among the lanes of its walker inside its CTA: the kernel adds a walker's
+     * lane sums in rank order, so the result does not depend on where in the batch the walker sits */
+    std::vector<int> next_rank((size_t)wc, 0);
+    L->rank_stride = 1;
     for (int wp = 0; wp < n_warps; wp++) {
+        if (wp % per_cta == 0) std::fill(next_rank.begin(), next_rank.end(), 0);
         int np = 0, c0 = 0;
         for (int l = 0; l < 32; l++) {
             const size_t i = (size_t)wp * 32 + l;
             int *o = &L->lane[i * 4];
             if (i < v.size()) {
                 const Key &k = v[i];
-                o[0] = k.wl; o[1] = k.item;
+                const int rank = next_rank[k.wl]++;
+                if (rank + 1 > L->rank_stride) L->rank_stride = rank + 1;
+                o[0] = k.wl | (rank << 8); o[1] = k.item;
                 o[2] = P.offA[k.item] | (P.offB[k.item] << 16);
                 o[3] = P.offX[k.item];
                 np = std::max(np, P.np[k.item]);
                 c0 = std::max(c0, P.c0[k.item]);
             } else {
-                o[0] = 0; o[1] = P.n_items; /* dummy item: all weights zero */
+                o[0] = 0 | (0xffffff << 8); o[1] = P.n_items; /* dummy item: all weights zero, no rank */
                 o[2] = P.offA[0] | (P.offB[0] << 16);
                 o[3] = P.offX[0];
             }

@@ -32,11 +32,12 @@ template <typename T> struct OctArgs {
     int wc;             /* walkers per CTA */
     int n_slabs;        /* CTAs per walker group: the sorted item list is cut into slabs */
     int pc;             /* particles per chunk */
+    int rank_stride;    /* most lanes any walker has in one CTA */
     int rowlen;         /* (cos,sin) pairs per (walker, particle) row */
     int wstride;        /* pairs per walker slab (pc * rowlen + bank stagger) */
     int off[3];         /* pair offset of X1 (n = 1..), X2 (n = 0..), X3 (n = 0..) within a row */
     int nmax[3];
-    const int4 *lane;   /* [n_slabs][blockDim.x] {local walker, item, offA | offB << 16, offX} */
+    const int4 *lane;   /* [n_slabs][blockDim.x] {local walker | rank << 8, item, offA | offB << 16, offX} */
     const int *variant; /* [n_slabs][n_warps] NP | C0 << 8 */
     const double *wt;   /* [n_items][1 + NPB][2]: w(G) 2^nz per entry for products (0,1) and (2,3) */
     const double *tion; /* [n_items][1 + 2 NPB][4] fixed-charge sums, or null */
@@ -49,7 +50,6 @@ template <typename T> struct OctArgs {
 template <typename T, int NPB> struct OctCfg {
     static constexpr int MAX_THREADS = sizeof(T) == 8 ? (NPB >= 6 ? 256 : 384) : (NPB >= 6 ? 384 : 512);
 };
-constexpr int OCT_MAX_TASKS = 3; /* table rows built per thread per chunk */
 
 /* One chunk of particles for one lane: acc[k][e] += p_k * X1_e. */
 template <typename T, int NPB, int NP, bool C0, int MODE>
@@ -90,6 +90,45 @@ __device__ __forceinline__ void oct_dispatch_c0(T (&acc)[4][1 + 2 * NPB], bool c
     else oct_fma<T, NPB, NP, false, MODE>(acc, rA, rB, rX, cnt, rowlen);
 }
 
+/* [S1,S2] Phase seeds and power rows of one chunk of particles, for all walkers of the CTA.  Tasks (axis,
+ * local walker, particle) are handed out 32 at a time from a shared counter, so warps whose FMA lists are
+ * short build most of the next chunk's tables while the long ones still multiply. */
+template <typename T, int DIM>
+__device__ __forceinline__ void oct_build_rows(const OctArgs<T> &A, typename Num<T>::T2 *tab, int *counter, int w0,
+                                               int base_p, int cnt, int lane)
+{
+    typedef typename Num<T>::T2 T2;
+    const int per_walker = (cnt + 31) & ~31;          /* tasks of one (axis, walker), padded to whole warps */
+    const int n_tasks = DIM * A.wc * per_walker;
+    for (;;) {
+        int t0 = 0;
+        if (lane == 0) t0 = atomicAdd(counter, 32);
+        t0 = __shfl_sync(0xffffffffu, t0, 0);
+        if (t0 >= n_tasks) break;
+        const int grp = t0 / per_walker, p = t0 - grp * per_walker + lane; /* grp = axis * wc + walker */
+        const int k = grp / A.wc, wl = grp - k * A.wc;
+        if (p >= cnt || w0 + wl >= A.n_walkers) continue;
+        const T *pw = A.pos + (size_t)(w0 + wl) * DIM * A.npad + base_p + p;
+        T s = 0;
+#pragma unroll
+        for (int x = 0; x < DIM; x++) s += __ldg(pw + x * A.npad) * A.binv[3 * k + x];
+        s -= Num<T>::rint_(s);
+        T sn, cs;
+        Num<T>::sincospi_(2 * s, &sn, &cs);
+        const T scale = k == DIM - 1 ? __ldg(A.q + base_p + p) : T(1);
+        T2 *row = tab + (size_t)wl * A.wstride + (size_t)p * A.rowlen + A.off[k];
+        T2 e; e.x = scale; e.y = 0;
+        if (k > 0) row[0] = e; else row -= 1; /* axis 1 stores n = 1.. only */
+        for (int n = 1; n <= A.nmax[k]; n++) {
+            T2 f;
+            f.x = e.x * cs - e.y * sn;
+            f.y = e.x * sn + e.y * cs;
+            e = f;
+            row[n] = e;
+        }
+    }
+}
+
 template <typename T, int DIM, int NPB>
 __global__ void __launch_bounds__(OctCfg<T, NPB>::MAX_THREADS) recip_oct_kernel(OctArgs<T> A)
 {
@@ -97,19 +136,22 @@ __global__ void __launch_bounds__(OctCfg<T, NPB>::MAX_THREADS) recip_oct_kernel(
     constexpr int MODE = DIM == 3 ? 0 : 1;
     constexpr int NE = 1 + 2 * NPB;
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    T2 *tab = reinterpret_cast<T2 *>(smem_raw);                                   /* [wc][wstride] + slack */
-    double *part = reinterpret_cast<double *>(tab + (size_t)A.wc * A.wstride + NPB + 1); /* [blockDim.x] */
+    /* two table buffers [wc][wstride] (+ slack), then the per-thread partial sums and walker tags */
+    const size_t buf_pairs = (size_t)A.wc * A.wstride + NPB + 1;
+    T2 *tab0 = reinterpret_cast<T2 *>(smem_raw);
+    double *part = reinterpret_cast<double *>(tab0 + 2 * buf_pairs); /* [wc][rank_stride] lane sums by rank */
+    __shared__ int counter[2];
 
-    const int tid = threadIdx.x, nthreads = blockDim.x, warp = tid >> 5;
+    const int tid = threadIdx.x, nthreads = blockDim.x, warp = tid >> 5, lane = tid & 31;
     const int group = blockIdx.x / A.n_slabs, slab = blockIdx.x - group * A.n_slabs;
     const int w0 = group * A.wc;
-    const int4 *lanes = A.lane + (size_t)slab * nthreads;
-    const int4 L = lanes[tid];
+    int4 L = A.lane[(size_t)slab * nthreads + tid];
+    const int rank = (int)((unsigned)L.x >> 8);
+    L.x &= 255;
     const int var = A.variant[slab * (nthreads >> 5) + warp];
     const int np = var & 255;
     const bool c0 = (var >> 8) != 0;
-    const T2 *lane_base = tab + (size_t)L.x * A.wstride;
-    const T2 *baseA = lane_base + (L.z & 0xffff), *baseB = lane_base + (L.z >> 16), *baseX = lane_base + L.w;
+    if (tid < 2) counter[tid] = 0;
 
     T acc[4][NE];
 #pragma unroll
@@ -117,53 +159,16 @@ __global__ void __launch_bounds__(OctCfg<T, NPB>::MAX_THREADS) recip_oct_kernel(
 #pragma unroll
         for (int e = 0; e < NE; e++) acc[k][e] = 0;
 
-    /* build tasks of this thread: t = tid + u * nthreads -> (axis k, local walker wl, particle p) */
-    const int per_axis = A.wc * A.pc, n_tasks = per_axis * DIM;
-    T xin[OCT_MAX_TASKS][DIM];
-
-    auto fetch = [&](int base_p) {
-#pragma unroll
-        for (int u = 0; u < OCT_MAX_TASKS; u++) {
-            const int t = tid + u * nthreads;
-            const int rem = t % per_axis, wl = rem / A.pc, p = rem - wl * A.pc;
-            const bool ok = t < n_tasks && base_p + p < A.n && w0 + wl < A.n_walkers;
-            const T *pw = A.pos + (size_t)(ok ? w0 + wl : 0) * DIM * A.npad + (ok ? base_p + p : 0);
-#pragma unroll
-            for (int x = 0; x < DIM; x++) xin[u][x] = pw[x * A.npad];
-        }
-    };
-
-    fetch(0);
-    for (int base_p = 0; base_p < A.n; base_p += A.pc) {
+    __syncthreads();
+    oct_build_rows<T, DIM>(A, tab0, &counter[1], w0, 0, min(A.pc, A.n), lane);
+    __syncthreads();
+    int it = 0;
+    for (int base_p = 0; base_p < A.n; base_p += A.pc, it++) {
         const int cnt = min(A.pc, A.n - base_p);
-        __syncthreads(); /* the previous chunk has been consumed */
-        /* [S1,S2] phase seeds and power rows */
-#pragma unroll
-        for (int u = 0; u < OCT_MAX_TASKS; u++) {
-            const int t = tid + u * nthreads;
-            if (t >= n_tasks) continue;
-            const int k = t / per_axis, rem = t - k * per_axis, wl = rem / A.pc, p = rem - wl * A.pc;
-            if (p >= cnt || w0 + wl >= A.n_walkers) continue;
-            T s = 0;
-#pragma unroll
-            for (int x = 0; x < DIM; x++) s += xin[u][x] * A.binv[3 * k + x];
-            s -= Num<T>::rint_(s);
-            T sn, cs;
-            Num<T>::sincospi_(2 * s, &sn, &cs);
-            const T scale = k == DIM - 1 ? A.q[base_p + p] : T(1);
-            T2 *row = tab + (size_t)wl * A.wstride + (size_t)p * A.rowlen + A.off[k];
-            T2 e; e.x = scale; e.y = 0;
-            if (k > 0) row[0] = e; else row -= 1; /* axis 1 stores n = 1.. only */
-            for (int n = 1; n <= A.nmax[k]; n++) {
-                T2 f;
-                f.x = e.x * cs - e.y * sn;
-                f.y = e.x * sn + e.y * cs;
-                e = f;
-                row[n] = e;
-            }
-        }
-        __syncthreads();
-        if (base_p + A.pc < A.n) fetch(base_p + A.pc); /* next chunk's positions fly during the FMA phase */
+        const T2 *tab = tab0 + (size_t)(it & 1) * buf_pairs;
+        if (tid == 0) counter[(it + 1) & 1] = 0; /* last used before the barrier that ended the previous pass */
+        const T2 *lane_base = tab + (size_t)L.x * A.wstride;
+        const T2 *baseA = lane_base + (L.z & 0xffff), *baseB = lane_base + (L.z >> 16), *baseX = lane_base + L.w;
         /* [S3] */
         switch (np) {
 #define EWALD_OCT_CASE(NP)                                                                              \
@@ -175,6 +180,11 @@ __global__ void __launch_bounds__(OctCfg<T, NPB>::MAX_THREADS) recip_oct_kernel(
 #undef EWALD_OCT_CASE
         default: break;
         }
+        /* the next chunk's tables go to the other buffer (read last in the previous pass) */
+        if (base_p + A.pc < A.n)
+            oct_build_rows<T, DIM>(A, tab0 + (size_t)((it + 1) & 1) * buf_pairs, &counter[it & 1], w0, base_p + A.pc,
+                                   min(A.pc, A.n - base_p - A.pc), lane);
+        __syncthreads();
     }
 
     /* [S4] E_recip = sum w 2^nz T^2, in FP64; entries of weight zero are padding (never read as values) */
@@ -200,14 +210,17 @@ __global__ void __launch_bounds__(OctCfg<T, NPB>::MAX_THREADS) recip_oct_kernel(
             }
         }
     }
+    for (int t = tid; t < A.wc * A.rank_stride; t += nthreads) part[t] = 0;
     __syncthreads();
-    part[tid] = e;
+    if (rank != 0xffffff) part[L.x * A.rank_stride + rank] = e;
     __syncthreads();
-    if (tid < A.wc && w0 + tid < A.n_walkers) {
-        double s = 0; /* fixed order: deterministic */
-        for (int t = 0; t < nthreads; t++)
-            if (lanes[t].x == tid) s += part[t];
-        A.e_recip[(size_t)(w0 + tid) * A.n_slabs + slab] = s;
+    /* one warp per walker adds that walker's lane sums in rank order: deterministic, and independent of
+     * the walker's place in the batch */
+    for (int wl = warp; wl < A.wc; wl += nthreads >> 5) {
+        double sum = 0;
+        for (int t = lane; t < A.rank_stride; t += 32) sum += part[wl * A.rank_stride + t];
+        sum = warp_sum(sum);
+        if (lane == 0 && w0 + wl < A.n_walkers) A.e_recip[(size_t)(w0 + wl) * A.n_slabs + slab] = sum;
     }
 }
 
