@@ -157,6 +157,13 @@ template <typename T> static void fill_geom(const HostTables &t, RealGeom<T> *g)
     for (int k = 0; k < 3; k++) { g->L[k] = (T)(t.a[4 * k] * t.kappa); g->invL[k] = (T)(1.0 / (t.a[4 * k] * t.kappa)); }
     g->kappa = (T)t.kappa;
     g->m_shift = t.m_shift;
+    g->multi_far = 0;
+    {
+        const double rc2 = t.r_cutoff * t.r_cutoff * (1 + 1e-5);
+        for (int j = 0; j < 3; j++)
+            for (int k = j + 1; k < 3; k++)
+                if (t.a[4 * j] * t.a[4 * j] + t.a[4 * k] * t.a[4 * k] < rc2) g->multi_far = 1;
+    }
     g->key_rc = host_key((T)(t.r_cutoff * t.r_cutoff * t.kappa * t.kappa));
     g->key_min = host_key((T)pair_of<T>(t).t_min);
     g->bias = (PairFmt<T>::EBIAS + pair_of<T>(t).e_min) << PairFmt<T>::K;

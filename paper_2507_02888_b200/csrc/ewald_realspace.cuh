@@ -38,6 +38,7 @@ template <typename T> struct RealGeom {
     int key_min; /* order key of the table's lower end t_min      */
     int bias;    /* bin index = (key >> SHIFT) - bias             */
     int m_shift; /* images -m_shift..m_shift scanned per axis (orthorhombic path) */
+    int multi_far; /* 3D, m_shift = 1: some L_j^2 + L_k^2 < kappa^2 r_c^2, i.e. two far images can be in range */
 };
 
 /* Positive floating-point numbers order like their leading bits.  FP64 uses the high word: ties within
@@ -272,8 +273,8 @@ constexpr int IMG_STEP = 8;
 template <int DIM, bool ORTHO, int M, bool UQ> struct ScanShape {
     static constexpr int ROW = 2 * M + 1;
     static constexpr int ALL = DIM == 3 ? ROW * ROW * ROW : ROW * ROW;
-    /* the stacks are serviced once per pair (few images), once per z-plane of 9 images (|m| <= 1 in 3D),
-     * else once per x-row: small LIMIT = small stacks = more warps per SM */
+    /* the stacks are serviced once per pair (few images), after every group of <= 9 candidates (|m| <= 1 in
+     * 3D, see scan_pair), else once per x-row: small LIMIT = small stacks = more warps per SM */
     /* (t, qq) items take twice the bytes, i.e. half the capacity: always once per x-row */
     static constexpr bool WHOLE = ALL <= (UQ ? 9 : 3);
     static constexpr bool PLANE = UQ && !WHOLE && DIM == 3 && ROW == 3;
@@ -291,7 +292,43 @@ __device__ __forceinline__ void scan_pair(const RealGeom<T> &g, T *d, T w, bool 
      * caller passes -w), in the sign bit of t for bare-t items */
     constexpr bool FLIP = NEG && UQ && SIGNED;
     typedef ScanShape<DIM, ORTHO, M, UQ> Shape;
-    if (ORTHO) {
+    if (ORTHO && Shape::PLANE) {
+        /* |m| <= 1 in 3D, bare-t items.  Only squared distances matter, so the three images of an axis are
+         * taken as {un-shifted, near, far} = {d^2, (L-|d|)^2, (L+|d|)^2}: the 8 core candidates (no far
+         * image), the 12 with one far image, and -- only if two box lengths fit inside the cut-off
+         * (g.multi_far, uniform over the grid) -- the 7 with two or three. */
+        T a[3][3];
+#pragma unroll
+        for (int k = 0; k < 3; k++) {
+            d[k] = fma(-Num<T>::rint_(d[k] * g.invL[k]), g.L[k], d[k]);
+            const T ad = abs_of(d[k]), x1 = g.L[k] - ad, x2 = g.L[k] + ad;
+            a[k][0] = d[k] * d[k]; a[k][1] = x1 * x1; a[k][2] = x2 * x2;
+        }
+        const T t0 = a[0][0] + (a[1][0] + a[2][0]);
+        const bool tiny = valid && order_key(t0) < g.key_min;
+        if (tiny) direct += (double)((FLIP ? -w : w) * pair_f_direct(t0));
+        const bool central_ok = valid && !tiny;
+        auto cand = [&](int i, int j, int k, bool ok) {
+            const T t = a[0][i] + (a[1][j] + a[2][k]);
+            const int key = order_key(t);
+            st.template push<FLIP>(ok && key <= g.key_rc, t, key, w);
+        };
+#pragma unroll
+        for (int c = 0; c < 8; c++) cand(c & 1, (c >> 1) & 1, c >> 2, c == 0 ? central_ok : valid);
+        st.service(Shape::LIMIT);
+#pragma unroll
+        for (int c = 0; c < 4; c++) { cand(2, c & 1, c >> 1, valid); cand(c & 1, 2, c >> 1, valid); }
+        st.service(Shape::LIMIT);
+#pragma unroll
+        for (int c = 0; c < 4; c++) cand(c & 1, c >> 1, 2, valid);
+        if (g.multi_far) {
+            st.service(Shape::LIMIT);
+#pragma unroll
+            for (int c = 0; c < 2; c++) { cand(2, 2, c, valid); cand(2, c, 2, valid); cand(c, 2, 2, valid); }
+            cand(2, 2, 2, valid);
+        }
+        st.service(Shape::LIMIT);
+    } else if (ORTHO) {
         constexpr int ROW = Shape::ROW;
         T sq[DIM][ROW];
 #pragma unroll
@@ -306,7 +343,7 @@ __device__ __forceinline__ void scan_pair(const RealGeom<T> &g, T *d, T w, bool 
         const bool tiny = valid && order_key(t0) < g.key_min;
         if (tiny) direct += (double)((FLIP ? -w : w) * pair_f_direct(t0));
         const bool central_ok = valid && !tiny;
-        if (Shape::WHOLE || Shape::PLANE) {
+        if (Shape::WHOLE) {
 #pragma unroll
             for (int mz = 0; mz < (DIM == 3 ? ROW : 1); mz++) {
 #pragma unroll
@@ -320,9 +357,8 @@ __device__ __forceinline__ void scan_pair(const RealGeom<T> &g, T *d, T w, bool 
                         st.template push<FLIP>((centre ? central_ok : valid) && key <= g.key_rc, t, key, w);
                     }
                 }
-                if (Shape::PLANE) st.service(Shape::LIMIT);
             }
-            if (Shape::WHOLE) st.service(Shape::LIMIT);
+            st.service(Shape::LIMIT);
         } else {
             /* rolled loops over the y and z images (the stacks are serviced after every x-row) */
 #pragma unroll 1

@@ -243,6 +243,37 @@ def test_orthorhombic_noncubic_cells_all_image_ranges(torch_cuda, dim):
         assert (np.abs(c32 - c_ref32) / np.abs(c_ref32).max(axis=1)[:, None]).max() <= TOL32, (kappa, rc)
 
 
+def test_uniform_charges_cutoff_reaching_two_far_images(torch_cuda):
+    """Equal charges (bare-t stacks, candidate images enumerated as core / one far image / two or more far
+    images) in cubic and orthorhombic cells whose cut-off r_c = 1.46 L_min exceeds sqrt(2) L_min: the branch
+    with two and three far images per pair is needed and taken.  Energies and a committed move."""
+    rng = np.random.default_rng(99)
+    for sides in (np.array([5.0, 5.0, 5.0]), np.array([5.0, 5.2, 7.5])):
+        cell = np.diag(sides)
+        rc = 1.46 * sides.min()
+        kappa = 6.1 / rc
+        gc, _ = ref.auto_cutoffs(3, cell, kappa, 1e-17)
+        n = 13
+        q = -np.ones(n)
+        pos = rng.random((4, n, 3)) * sides
+        e_ref, c_ref = ref.energy_batch(3, cell, kappa, gc, rc, pos, q)
+        ctx = E.ewald_setup(3, cell, kappa, gc, rc)
+        e, c = _gpu_energy(torch_cuda, ctx, pos, q, "f64")
+        scale = np.abs(c_ref).max(axis=1)
+        assert (np.abs(c - c_ref) / scale[:, None]).max() <= TOL64
+        electron = rng.integers(0, n, (2, 4)).astype(np.int32)
+        new_r = rng.random((2, 4, 3)) * sides
+        de_ref, _, _ = ref.move_chain(3, cell, kappa, gc, rc, pos, q, electron, new_r)
+        E.ewald_load_walkers(ctx, n, torch_cuda.from_numpy(E.to_soa(pos)).cuda(), torch_cuda.from_numpy(q).cuda())
+        d_w = torch_cuda.arange(4, dtype=torch_cuda.int32, device="cuda")
+        for s_ in range(2):
+            d_de = torch_cuda.zeros(4, dtype=torch_cuda.float64, device="cuda")
+            E.ewald_move_delta_batch(ctx, d_w, torch_cuda.from_numpy(electron[s_]).cuda(),
+                                     torch_cuda.from_numpy(new_r[s_]).cuda(), 1, d_de)
+            de = d_de.cpu().numpy()
+            assert (np.abs(de - de_ref[s_]) / np.maximum(np.abs(de_ref[s_]), scale)).max() <= TOL64
+
+
 def test_fixed_charges_equal_mobile_charges(torch_cuda):
     """Ions passed as fixed charges give the same energy as the same ions passed as mobile particles."""
     rng = np.random.default_rng(11)
