@@ -212,7 +212,15 @@ extern "C" ewald_status ewald_setup(ewald_ctx **out, int dim, const double *cell
     if (st == EWALD_OK) st = upload(c, &c->d_img, scaled(t.img, t.kappa));
     if (st == EWALD_OK) st = upload(c, &c->d_imgf, to_f32(scaled(t.img, t.kappa)));
     if (st == EWALD_OK) st = upload(c, &c->d_pair, t.pair64.coef);
-    if (st == EWALD_OK) st = upload(c, &c->d_pairf, to_f32(t.pair32.coef));
+    {   /* FP32 table: PairFmt<float>::REP interleaved copies */
+        const std::vector<float> one = to_f32(t.pair32.coef);
+        constexpr int R = PairFmt<float>::REP, NCF = PairFmt<float>::NC;
+        std::vector<float> rep(one.size() * R);
+        for (size_t b = 0; b < one.size() / NCF; b++)
+            for (int r = 0; r < R; r++)
+                for (int k = 0; k < NCF; k++) rep[(b * R + r) * NCF + k] = one[b * NCF + k];
+        if (st == EWALD_OK) st = upload(c, &c->d_pairf, rep);
+    }
     if (st == EWALD_OK) st = upload(c, &c->d_far, t.far_tab);
     if (st == EWALD_OK) st = ensure(c, &c->qsums, 4 * sizeof(double));
     if (st == EWALD_OK) st = ensure(c, &c->st_qinfo, 4 * sizeof(double));
@@ -596,24 +604,31 @@ template <> void fill_pair_tabs<double>(const ewald_ctx *c, const double *qinfo,
  * min_cap = ScanShape::MIN_CAP of the kernel variant. */
 template <typename T>
 static bool real_shape(const ewald_ctx *c, size_t fixed, int min_cap_u, int min_cap_g, int max_threads,
-                       PairTabs<T> *P, int *threads, size_t *smem)
+                       PairTabs<T> *P, int *threads, size_t *smem, bool allow_two = true)
 {
-    const size_t budget = c->smem_optin > 2048 ? c->smem_optin - 2048 : 0; /* static arrays of the kernels */
+    const size_t full = c->smem_optin > 2048 ? c->smem_optin - 2048 : 0; /* static arrays of the kernels */
+    /* first choice: two CTAs of max_threads per SM (228 KB per SM, 1 KB reserved per CTA), if the tables are
+     * small enough for that (the FP32 kernels); then one CTA, with fewer threads if need be */
+    const size_t half = (228 * 1024 - 2 * 1024) / 2 - 2048;
     const bool far = P->n_far > 0;
-    for (int th = max_threads; th >= 32; th /= 2) {
-        if (fixed >= budget) return false;
-        /* bytes per unit of capacity: near item + (far item: 4 bytes), per lane, per warp */
-        const size_t per_cap = (size_t)(th / 32) * 32 * (sizeof(T) + (far ? 4 : 0));
-        long long cu = (long long)((budget - fixed) / per_cap);
-        const long long want = 2 * (min_cap_u > min_cap_g ? min_cap_u : min_cap_g) + 8;
-        if (cu > want) cu = want;
-        cu &= ~1LL;
-        if (cu >= min_cap_u + 4 && cu >= 2 * min_cap_g) {
-            *threads = th;
-            P->cap_u = (int)cu; P->cap_g = (int)(cu / 2);
-            P->capf_u = far ? (int)cu : 0; P->capf_g = far ? (int)(cu / 2) : 0;
-            *smem = fixed + (size_t)cu * per_cap;
-            return true;
+    for (int pass = allow_two && 2 * max_threads <= 2048 ? 0 : 1; pass < 2; pass++) {
+        const size_t budget = pass == 0 ? (half < full ? half : full) : full;
+        for (int th = max_threads; th >= 32; th /= 2) {
+            if (fixed >= budget) break;
+            /* bytes per unit of capacity: near item + (far item: 4 bytes), per lane, per warp */
+            const size_t per_cap = (size_t)(th / 32) * 32 * (sizeof(T) + (far ? 4 : 0));
+            long long cu = (long long)((budget - fixed) / per_cap);
+            const long long want = 2 * (min_cap_u > min_cap_g ? min_cap_u : min_cap_g) + 8;
+            if (cu > want) cu = want;
+            cu &= ~1LL;
+            if (cu >= min_cap_u + 4 && cu >= 2 * min_cap_g) {
+                *threads = th;
+                P->cap_u = (int)cu; P->cap_g = (int)(cu / 2);
+                P->capf_u = far ? (int)cu : 0; P->capf_g = far ? (int)(cu / 2) : 0;
+                *smem = fixed + (size_t)cu * per_cap;
+                return true;
+            }
+            if (pass == 0) break; /* two CTAs per SM only at full size */
         }
     }
     return false;

@@ -127,7 +127,7 @@ __global__ void __launch_bounds__(RECIP_THREADS) recip_kernel(RecipArgs<T> A)
 
 /* Tables and stack shapes of the real-space machinery, common to the energy and move kernels. */
 template <typename T> struct PairTabs {
-    const T *pair_tab; int n_bins;   /* [n_bins][PairFmt<T>::NC]                                        */
+    const T *pair_tab; int n_bins;   /* [n_bins][PairFmt<T>::REP][PairFmt<T>::NC]                       */
     T t_safe;                        /* some t inside the table                                         */
     const float *far_tab; int n_far; /* FP64 kernels: [n_far][FarFmt::REP][4] far-shell cubics; 0 = none */
     int key_far;                     /* order key of the far shell's start, INT_MAX = none              */
@@ -152,7 +152,7 @@ constexpr int REAL_MAX_THREADS = 512;
 
 /* Shared-memory carve-up common to the real-space and move kernels. */
 template <typename T> struct RealSmem {
-    T *tab;     /* [n_bins][NC] */
+    T *tab;     /* [n_bins][REP][NC] */
     float *far; /* [n_far][REP][4] */
     T *img;     /* [nimg][3] */
     T *ion;     /* [n_ion][4] = x,y,z,q */
@@ -163,7 +163,7 @@ template <typename T> struct RealSmem {
     __device__ __forceinline__ RealSmem(unsigned char *raw, const PairTabs<T> &P, int nimg, int n_ion, size_t rest_elems)
     {
         tab = reinterpret_cast<T *>(raw);
-        far = reinterpret_cast<float *>(tab + up4((size_t)P.n_bins * PairFmt<T>::NC));
+        far = reinterpret_cast<float *>(tab + up4((size_t)P.n_bins * PairFmt<T>::NC * PairFmt<T>::REP));
         img = reinterpret_cast<T *>(reinterpret_cast<unsigned char *>(far) + far_bytes(P.n_far));
         ion = img + up4(3 * (size_t)nimg);
         rest = ion + up4(4 * (size_t)n_ion);
@@ -172,7 +172,7 @@ template <typename T> struct RealSmem {
     /* bytes before the stacks */
     static size_t fixed_bytes(int n_bins, int n_far, int nimg, int n_ion, size_t rest_elems)
     {
-        return (up4((size_t)n_bins * PairFmt<T>::NC) + up4(3 * (size_t)nimg) + up4(4 * (size_t)n_ion) +
+        return (up4((size_t)n_bins * PairFmt<T>::NC * PairFmt<T>::REP) + up4(3 * (size_t)nimg) + up4(4 * (size_t)n_ion) +
                 up4(rest_elems)) * sizeof(T) + far_bytes(n_far);
     }
     /* bytes of one warp's stacks (the two item kinds of a stack share the same bytes) */
@@ -184,7 +184,7 @@ template <typename T> struct RealSmem {
                                          const T *ion_q, int n_ion, int tid, int nthreads)
     {
         {   /* NC * sizeof(T) is a multiple of 16 */
-            const int n4 = P.n_bins * PairFmt<T>::NC * (int)sizeof(T) / 16;
+            const int n4 = P.n_bins * PairFmt<T>::NC * PairFmt<T>::REP * (int)sizeof(T) / 16;
             const int4 *src = reinterpret_cast<const int4 *>(P.pair_tab);
             int4 *dst = reinterpret_cast<int4 *>(tab);
             for (int t = tid; t < n4; t += nthreads) dst[t] = src[t];
@@ -254,22 +254,29 @@ __device__ __forceinline__ double real_body(const RealArgs<T> &A, RealSmem<T> &S
     {
         const int H = (n - 1) / 2;
         const bool even = (n & 1) == 0;
+        typedef ScanShape<DIM, ORTHO, M, UQ> Shape;
+        constexpr int GROUP = Shape::GROUP;
         PairWalk pw; pw.init(gid, team, n);
         for (;;) {
-            const bool valid = pw.k < H || (even && pw.k == H && pw.i < n / 2);
+            bool valid = pw.k < H || (even && pw.k == H && pw.i < n / 2);
             if (!__any_sync(0xffffffffu, valid)) break;
-            T d[3] = {0, 0, 0};
-            T w = UQ ? q0 * q0 : T(0);
-            if (valid) {
-                const int i = pw.i;
-                int j = i + pw.k + 1;
-                if (j >= n) j -= n;
 #pragma unroll
-                for (int x = 0; x < DIM; x++) d[x] = (sp[x * n + i] - sp[x * n + j]) * A.g.kappa;
-                if (!UQ) w = sq[i] * sq[j];
+            for (int u = 0; u < GROUP; u++) {
+                if (u > 0) valid = pw.k < H || (even && pw.k == H && pw.i < n / 2);
+                T d[3] = {0, 0, 0};
+                T w = UQ ? q0 * q0 : T(0);
+                if (valid) {
+                    const int i = pw.i;
+                    int j = i + pw.k + 1;
+                    if (j >= n) j -= n;
+#pragma unroll
+                    for (int x = 0; x < DIM; x++) d[x] = (sp[x * n + i] - sp[x * n + j]) * A.g.kappa;
+                    if (!UQ) w = sq[i] * sq[j];
+                }
+                scan_pair<T, DIM, ORTHO, M, UQ, false, false, GROUP == 1>(A.g, d, w, valid, st, direct, S.img, A.nimg);
+                pw.next();
             }
-            scan_pair<T, DIM, ORTHO, M, UQ>(A.g, d, w, valid, st, direct, S.img, A.nimg);
-            pw.next();
+            if (GROUP > 1) st.service(Shape::LIMIT);
         }
         st.finish();
         total += st.take() * (UQ ? (double)(q0 * q0) : 1.0);

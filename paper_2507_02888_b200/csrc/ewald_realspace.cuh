@@ -24,8 +24,11 @@
 namespace ewald {
 
 template <typename T> struct PairFmt;
-template <> struct PairFmt<double> { static constexpr int K = 7, DEG = 5, NC = 6, SHIFT = 20 - 7, EBIAS = 1023; };
-template <> struct PairFmt<float> { static constexpr int K = 5, DEG = 3, NC = 4, SHIFT = 23 - 5, EBIAS = 127; };
+/* REP: copies of the table, interleaved [bin][copy][NC]; lane l reads copy l mod REP.  The 16-byte FP32
+ * entries are replicated 8 times: the 8 lanes of a quarter-warp then read 8 different 16-byte columns and
+ * the gather has no bank conflicts (6 KB -> 48 KB; the 61 KB FP64 table cannot afford it). */
+template <> struct PairFmt<double> { static constexpr int K = 7, DEG = 5, NC = 6, SHIFT = 20 - 7, EBIAS = 1023, REP = 1; };
+template <> struct PairFmt<float> { static constexpr int K = 5, DEG = 3, NC = 4, SHIFT = 23 - 5, EBIAS = 127, REP = 8; };
 
 /* Geometry in kappa-scaled units. */
 template <typename T> struct RealGeom {
@@ -76,7 +79,7 @@ __device__ __forceinline__ float pair_f(float t, const float *tab, int bias)
 {
     const int key = order_key(t);
     const float u = t - bin_centre(t, key);
-    const float4 c = reinterpret_cast<const float4 *>(tab)[(key >> PairFmt<float>::SHIFT) - bias];
+    const float4 c = reinterpret_cast<const float4 *>(tab)[((key >> PairFmt<float>::SHIFT) - bias) * PairFmt<float>::REP];
     float p = fmaf(c.w, u, c.z);
     p = fmaf(p, u, c.y);
     return fmaf(p, u, c.x);
@@ -192,7 +195,8 @@ struct LaneStack : StackBase<T, T, UQ, LaneStack<T, UQ, SIGNED>> {
     int bias;
     __device__ __forceinline__ void init(void *warp_mem, int lane, int cap, const T *table, int b, T t_safe)
     {
-        tab = table; bias = b;
+        tab = table + (lane % PairFmt<T>::REP) * PairFmt<T>::NC; /* this lane's copy */
+        bias = b;
         this->init_base(warp_mem, lane, cap, t_safe);
     }
     __device__ __forceinline__ T term(T t, T w) const
@@ -278,13 +282,16 @@ template <int DIM, bool ORTHO, int M, bool UQ> struct ScanShape {
     /* (t, qq) items take twice the bytes, i.e. half the capacity: always once per x-row */
     static constexpr bool WHOLE = ALL <= (UQ ? 9 : 3);
     static constexpr bool PLANE = UQ && !WHOLE && DIM == 3 && ROW == 3;
-    static constexpr int LIMIT = ORTHO ? (WHOLE ? ALL : PLANE ? ROW * ROW : ROW) : IMG_STEP;
+    /* with very few images per pair the energy kernel scans GROUP pairs between two services */
+    static constexpr int GROUP = UQ && ORTHO && WHOLE && ALL <= 4 ? 8 / ALL : 1;
+    static constexpr int LIMIT = ORTHO ? (WHOLE ? ALL * GROUP : PLANE ? ROW * ROW : ROW) : IMG_STEP;
     static constexpr int MIN_CAP = LIMIT + PAIR_R;
 };
 
 /* Phase A for one pair per lane.  d = kappa (r_i - r_j), not yet reduced; w = q_i q_j.  Terms below the
  * table (t < t_min) are evaluated directly into `direct` (weighted by w); the rest go to the stack. */
-template <typename T, int DIM, bool ORTHO, int M, bool UQ, bool SIGNED = false, bool NEG = false>
+template <typename T, int DIM, bool ORTHO, int M, bool UQ, bool SIGNED = false, bool NEG = false,
+          bool SERVICE = true>
 __device__ __forceinline__ void scan_pair(const RealGeom<T> &g, T *d, T w, bool valid,
                                           PairStacks<T, UQ, SIGNED> &st, double &direct, const T *simg, int nimg)
 {
@@ -358,7 +365,7 @@ __device__ __forceinline__ void scan_pair(const RealGeom<T> &g, T *d, T w, bool 
                     }
                 }
             }
-            st.service(Shape::LIMIT);
+            if (SERVICE) st.service(Shape::LIMIT); /* else the caller does, after Shape::GROUP pairs */
         } else {
             /* rolled loops over the y and z images (the stacks are serviced after every x-row) */
 #pragma unroll 1
