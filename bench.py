@@ -42,6 +42,14 @@ def parse():
     return p.parse_args()
 
 
+def recorded_traffic(key, kernel):
+    """DRAM bytes per launch from the committed ncu --set full capture (profiles/), or None."""
+    try:
+        return json.load(open(os.path.join(ROOT, "profiles", "r01b_traffic.json")))[key][kernel]
+    except Exception:
+        return None
+
+
 def measured_peaks():
     try:
         return json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
@@ -203,7 +211,9 @@ def move_leg(torch, E, device, stream, prec, n_steps, flush, hbm_peak_gbs):
     return {"workload": "BASELINE configs[4]: %s" % w.name, "dtype": prec, "moves_per_s": W / t,
             "ms_per_batch_of_%d_moves" % W: t * 1e3, "timed_batches": len(ms), "warmup_batches": warm,
             "roofline": {"kernel": "move", "bound": "hbm", "unit": "GB/s", "achieved": gbs, "peak": hbm_peak_gbs,
-                         "frac": gbs / hbm_peak_gbs, "alg_bytes_per_move": bytes_per_move, "traffic": None},
+                         "frac": gbs / hbm_peak_gbs, "alg_bytes_per_move": bytes_per_move,
+                         "alg_bytes_per_launch": bytes_per_move * W,
+                         "traffic": recorded_traffic("cfg5_%s" % prec, "move")},
             "delta_e_finite": bool(torch.isfinite(d_de).all().item())}
 
 
@@ -354,7 +364,9 @@ def main():
                 "peak_source": "derived: %d SMs x %d %s lanes x 2 x %.0f MHz (sm_max_mhz); the FMA-chain probe "
                                "in extras measures it" % (SM_COUNT, lanes, args.prec, sm_max_hz / 1e6),
                 "achieved": kernels[dominant]["achieved_tflops"], "frac": kernels[dominant]["frac_of_peak"],
-                "traffic": None,
+                "traffic": recorded_traffic("cfg%d_%s" % (args.config, args.prec), dominant),
+                "traffic_note": "DRAM bytes per launch (ncu, profiles/r01b_ncu_summary.md); algorithmic: the positions "
+                                "once = %d bytes" % (soa.nbytes),
                 "note": "algorithmic flops per DESIGN.md section 6; the real-space kernel is limited by "
                         "shared-memory wavefronts (table gathers), see profiles/"}
 
