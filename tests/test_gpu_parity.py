@@ -488,6 +488,34 @@ def test_full_size_config5_moves_sampled_walkers(torch_cuda):
         assert np.abs(E.ewald_get_positions(ctx, int(wk), w.n) - final[wk]).max() == 0
 
 
+def test_largest_paper_system_n1630(torch_cuda):
+    """The paper's largest electron gas (N = 1630) at r_s = 1: positions no longer leave room
+    for the full-size stacks in shared memory, so the launch shapes shrink; 3 walkers against the oracle, FP64
+    and FP32, and one committed move per walker."""
+    n = 1630
+    L = (4.0 * math.pi * n / 3.0) ** (1.0 / 3.0)
+    cell = np.eye(3) * L
+    kappa, rc = 5.4 / L, 1.1 * L
+    gc = 2 * math.pi / L * math.sqrt(97) * (1 + 1e-9)
+    rng = np.random.default_rng(1630)
+    pos = rng.random((3, n, 3)) * L
+    q = -np.ones(n)
+    ctx = E.ewald_setup(3, cell, kappa, gc, rc)
+    for dtype, tol in (("f64", TOL64), ("f32", TOL32)):
+        p = pos if dtype == "f64" else _r32(pos)
+        e_ref, _ = ref.energy_batch(3, cell, kappa, gc, rc, p, q)
+        e, _ = _gpu_energy(torch_cuda, ctx, p, q, dtype, components=False)
+        assert (np.abs(e - e_ref) / np.abs(e_ref)).max() <= tol
+    electron = rng.integers(0, n, (1, 3)).astype(np.int32)
+    new_r = rng.random((1, 3, 3)) * L
+    de_ref, _, _ = ref.move_chain(3, cell, kappa, gc, rc, pos, q, electron, new_r)
+    E.ewald_load_walkers(ctx, n, torch_cuda.from_numpy(E.to_soa(pos)).cuda(), torch_cuda.from_numpy(q).cuda())
+    d_de = torch_cuda.zeros(3, dtype=torch_cuda.float64, device="cuda")
+    E.ewald_move_delta_batch(ctx, torch_cuda.arange(3, dtype=torch_cuda.int32, device="cuda"),
+                             torch_cuda.from_numpy(electron[0]).cuda(), torch_cuda.from_numpy(new_r[0]).cuda(), 1, d_de)
+    _assert_delta(d_de.cpu().numpy()[None, :], de_ref, TOL64)
+
+
 def test_translation_and_permutation_invariance_on_gpu(torch_cuda):
     w = workloads.config(2)
     pos = w.positions(4)
