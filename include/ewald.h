@@ -187,6 +187,11 @@ ewald_status ewald_get_constants(const ewald_ctx *ctx, double *xi_r, double *v_m
  * *flops (2 per FMA), timed with CUDA events on the context's stream.  Synchronises.            */
 ewald_status ewald_probe_fma(ewald_ctx *ctx, ewald_prec prec, int iters, double *flops);
 
+/* Measured ceiling of the octant reciprocal kernel's FMA phase: its inner loop alone (a 4 x 15 outer-product
+ * tile per lane, one broadcast shared-memory load per (cos, sin) pair; no tables, no barriers), one CTA of
+ * `threads` (32..256, multiple of 32) per SM, `iters` iterations of 60 FMAs.  *flops = FLOP/s.  Synchronises. */
+ewald_status ewald_probe_fma_tile(ewald_ctx *ctx, ewald_prec prec, int iters, int threads, double *flops);
+
 /* Per-kernel device timers: when enabled, every kernel launch is bracketed by CUDA events on the
  * context's stream.  ewald_profile_read synchronises, returns and resets the accumulated device
  * milliseconds and launch counts per kernel class:

@@ -1035,6 +1035,34 @@ extern "C" ewald_status ewald_get_positions(ewald_ctx *c, int walker, double *po
     return EWALD_OK;
 }
 
+extern "C" ewald_status ewald_probe_fma_tile(ewald_ctx *c, ewald_prec prec, int iters, int threads, double *flops)
+{
+    if (!c || !flops || iters <= 0 || threads < 32 || threads > 256 || threads % 32) return EWALD_EINVAL;
+    CU_TRY(c, cudaSetDevice(c->device));
+    ewald_status st = ensure(c, &c->stage_e, 64);
+    if (st != EWALD_OK) return st;
+    CU_TRY(c, cudaMemsetAsync(c->stage_e.p, 0, 64, c->stream));
+    const int blocks = c->sm_count; /* one CTA per SM, like recip_oct_kernel */
+    cudaEvent_t e0, e1;
+    CU_TRY(c, cudaEventCreate(&e0));
+    CU_TRY(c, cudaEventCreate(&e1));
+    for (int rep = 0; rep < 2; rep++) { /* first pass warms up */
+        CU_TRY(c, cudaEventRecord(e0, c->stream));
+        if (prec == EWALD_F64)
+            fma_tile_probe_kernel<double><<<blocks, threads, 0, c->stream>>>(iters, (const double *)c->stage_e.p, (double *)c->stage_e.p);
+        else
+            fma_tile_probe_kernel<float><<<blocks, threads, 0, c->stream>>>(iters, (const float *)c->stage_e.p, (float *)c->stage_e.p);
+        CU_TRY(c, cudaEventRecord(e1, c->stream));
+        CU_TRY(c, cudaEventSynchronize(e1));
+    }
+    float ms = 0;
+    CU_TRY(c, cudaEventElapsedTime(&ms, e0, e1));
+    cudaEventDestroy(e0);
+    cudaEventDestroy(e1);
+    *flops = 2.0 * 60.0 * iters * (double)blocks * threads / (ms * 1e-3);
+    return EWALD_OK;
+}
+
 extern "C" ewald_status ewald_probe_fma(ewald_ctx *c, ewald_prec prec, int iters, double *flops)
 {
     if (!c || !flops || iters <= 0) return EWALD_EINVAL;

@@ -24,7 +24,7 @@ SYMBOLS = ["ewald_padded_n", "ewald_setup", "ewald_setup_summary", "ewald_oct_pl
            "ewald_set_fixed_charges", "ewald_energy_batch", "ewald_energy_batch_host",
            "ewald_load_walkers", "ewald_move_delta_batch", "ewald_move_delta_batch_host",
            "ewald_move_delta", "ewald_num_g", "ewald_num_images", "ewald_r_cutoff", "ewald_get_g",
-           "ewald_get_rho", "ewald_get_positions", "ewald_get_constants", "ewald_probe_fma",
+           "ewald_get_rho", "ewald_get_positions", "ewald_get_constants", "ewald_probe_fma", "ewald_probe_fma_tile",
            "ewald_profile_enable", "ewald_profile_read", "ewald_launch_count",
            "ewald_last_error", "ewald_version"]
 
@@ -80,6 +80,7 @@ def load_library():
         "ewald_get_positions": (i, [vp, i, dp]),
         "ewald_get_constants": (i, [vp, dp, dp, dp]),
         "ewald_probe_fma": (i, [vp, i, i, dp]),
+        "ewald_probe_fma_tile": (i, [vp, i, i, i, dp]),
         "ewald_profile_enable": (i, [vp, i]),
         "ewald_profile_read": (i, [vp, dp, ip]),
         "ewald_launch_count": (ctypes.c_longlong, [vp]),
@@ -325,6 +326,13 @@ def ewald_get_constants(ctx):
 def ewald_probe_fma(ctx, prec, iters=4096):
     f = ctypes.c_double()
     _check(ctx, load_library().ewald_probe_fma(ctx.handle, int(prec), int(iters), ctypes.byref(f)))
+    return f.value
+
+
+def ewald_probe_fma_tile(ctx, prec, iters=20000, threads=256):
+    """FLOP/s of the octant kernel's inner loop alone, one CTA of `threads` per SM (its FMA-phase ceiling)."""
+    f = ctypes.c_double()
+    _check(ctx, load_library().ewald_probe_fma_tile(ctx.handle, int(prec), int(iters), int(threads), ctypes.byref(f)))
     return f.value
 
 
