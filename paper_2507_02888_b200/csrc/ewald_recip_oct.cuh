@@ -90,41 +90,55 @@ __device__ __forceinline__ void oct_dispatch_c0(T (&acc)[4][1 + 2 * NPB], bool c
     else oct_fma<T, NPB, NP, false, MODE>(acc, rA, rB, rX, cnt, rowlen);
 }
 
-/* [S1,S2] Phase seeds and power rows of one chunk of particles, for all walkers of the CTA.  Tasks (axis,
- * local walker, particle) are handed out 32 at a time from a shared counter, so warps whose FMA lists are
- * short build most of the next chunk's tables while the long ones still multiply. */
+/* [S1,S2] Phase seeds and power rows of one chunk of particles, for all walkers of the CTA.  A task is one
+ * (local walker, particle): the lane builds the rows of all DIM axes together (DIM independent dependency
+ * chains: sincospi, then the recurrence).  Tasks are handed out 32 at a time from a shared counter, so warps
+ * whose FMA lists are short build most of the next chunk's tables while the long ones still multiply. */
 template <typename T, int DIM>
 __device__ __forceinline__ void oct_build_rows(const OctArgs<T> &A, typename Num<T>::T2 *tab, int *counter, int w0,
                                                int base_p, int cnt, int lane)
 {
     typedef typename Num<T>::T2 T2;
-    const int per_walker = (cnt + 31) & ~31;          /* tasks of one (axis, walker), padded to whole warps */
-    const int n_tasks = DIM * A.wc * per_walker;
+    const int per_walker = (cnt + 31) & ~31;          /* tasks of one walker, padded to whole warps */
+    const int n_tasks = A.wc * per_walker;
+    int nmax_all = A.nmax[0];
+#pragma unroll
+    for (int k = 1; k < DIM; k++) nmax_all = max(nmax_all, A.nmax[k]);
     for (;;) {
         int t0 = 0;
         if (lane == 0) t0 = atomicAdd(counter, 32);
         t0 = __shfl_sync(0xffffffffu, t0, 0);
         if (t0 >= n_tasks) break;
-        const int grp = t0 / per_walker, p = t0 - grp * per_walker + lane; /* grp = axis * wc + walker */
-        const int k = grp / A.wc, wl = grp - k * A.wc;
+        const int wl = t0 / per_walker, p = t0 - wl * per_walker + lane;
         if (p >= cnt || w0 + wl >= A.n_walkers) continue;
         const T *pw = A.pos + (size_t)(w0 + wl) * DIM * A.npad + base_p + p;
-        T s = 0;
+        T x[DIM];
 #pragma unroll
-        for (int x = 0; x < DIM; x++) s += __ldg(pw + x * A.npad) * A.binv[3 * k + x];
-        s -= Num<T>::rint_(s);
-        T sn, cs;
-        Num<T>::sincospi_(2 * s, &sn, &cs);
-        const T scale = k == DIM - 1 ? __ldg(A.q + base_p + p) : T(1);
-        T2 *row = tab + (size_t)wl * A.wstride + (size_t)p * A.rowlen + A.off[k];
-        T2 e; e.x = scale; e.y = 0;
-        if (k > 0) row[0] = e; else row -= 1; /* axis 1 stores n = 1.. only */
-        for (int n = 1; n <= A.nmax[k]; n++) {
-            T2 f;
-            f.x = e.x * cs - e.y * sn;
-            f.y = e.x * sn + e.y * cs;
-            e = f;
-            row[n] = e;
+        for (int k = 0; k < DIM; k++) x[k] = __ldg(pw + k * A.npad);
+        const T qp = __ldg(A.q + base_p + p);
+        T sn[DIM], cs[DIM];
+        T2 e[DIM];
+        T2 *row[DIM];
+#pragma unroll
+        for (int k = 0; k < DIM; k++) {
+            T s = 0;
+#pragma unroll
+            for (int c = 0; c < DIM; c++) s += x[c] * A.binv[3 * k + c];
+            s -= Num<T>::rint_(s);
+            Num<T>::sincospi_(2 * s, &sn[k], &cs[k]);
+            row[k] = tab + (size_t)wl * A.wstride + (size_t)p * A.rowlen + A.off[k];
+            e[k].x = k == DIM - 1 ? qp : T(1); e[k].y = 0;
+            if (k > 0) row[k][0] = e[k]; else row[k] -= 1; /* axis 1 stores n = 1.. only */
+        }
+        for (int n = 1; n <= nmax_all; n++) {
+#pragma unroll
+            for (int k = 0; k < DIM; k++) {
+                T2 f;
+                f.x = e[k].x * cs[k] - e[k].y * sn[k];
+                f.y = e[k].x * sn[k] + e[k].y * cs[k];
+                e[k] = f;
+                if (n <= A.nmax[k]) row[k][n] = f;
+            }
         }
     }
 }
