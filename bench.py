@@ -36,7 +36,8 @@ def parse():
     p.add_argument("--steps", type=int, default=500)
     p.add_argument("--warmup", type=int, default=3)
     p.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    p.add_argument("--config", type=int, default=2, help="BASELINE.json config index (1-based): 1..4 energies, 5 moves")
+    p.add_argument("--config", type=int, default=2,
+                   help="BASELINE.json config index (1-based): 1..4 energies, 5 moves; 6 = NEXT-1 hexagonal cell")
     p.add_argument("--prec", default="f64", choices=["f64", "f32"])
     p.add_argument("--no-extras", action="store_true", help="skip FP32 / move / cpu_baseline legs")
     return p.parse_args()
@@ -218,7 +219,8 @@ def move_leg(torch, E, device, stream, prec, n_steps, flush, hbm_peak_gbs):
 
 
 def workload_config(w, walkers_per_gpu, l2_note):
-    return {"workload": "BASELINE configs[%d]: %s" % (w.index - 1, w.name), "dim": w.dim, "n_particles": w.n,
+    label = "BASELINE configs[%d]" % (w.index - 1) if w.index <= 5 else "SURVEY 8(f) NEXT-1"
+    return {"workload": "%s: %s" % (label, w.name), "dim": w.dim, "n_particles": w.n,
             "n_fixed": 0 if w.ion_q is None else len(w.ion_q), "walkers_per_gpu": walkers_per_gpu,
             "kappa_L": round(w.kappa * w.L, 6), "n2_max": w.n2_max, "r_cutoff_over_L": round(w.r_cutoff / w.L, 6),
             "l2": l2_note, "parallelism": "walkers sharded across GPUs, no data-path collective"}
@@ -351,10 +353,15 @@ def main():
                             frac_of_peak=recip_flops / (kernels["recip"]["ms_per_launch"] * 1e-3) / peak_flops)
     # real-space kernel: algorithmic flops = per pair (displacement, reduction to the cell, image squares and sums)
     # + 12 per pair-image term (u = t - centre, quintic Horner, accumulate), all counted as FP64
-    pairs, terms, n_cand, m_img = count_pair_terms(w, pos[:4])
-    row = 2 * m_img + 1
-    per_pair = 21 + 2 * w.dim * row + (row * row if w.dim == 3 else 0) + n_cand
-    real_flops = (per_pair * pairs + 12.0 * terms) * W
+    if np.count_nonzero(w.cell - np.diag(np.diag(w.cell))) == 0:
+        pairs, terms, n_cand, m_img = count_pair_terms(w, pos[:4])
+        row = 2 * m_img + 1
+        per_pair = 21 + 2 * w.dim * row + (row * row if w.dim == 3 else 0) + n_cand
+    else:   # general cell (image-list scan): 21 flops per pair + 6 per scanned image; terms not counted here
+        n_img = E.ewald_num_images(ctx)
+        pairs = w.n * (w.n - 1) // 2 + w.n * (0 if w.ion_q is None else len(w.ion_q))
+        terms, per_pair = float("nan"), 21 + 6 * n_img
+    real_flops = (per_pair * pairs + (0.0 if terms != terms else 12.0 * terms)) * W
     t_real = kernels["real"]["ms_per_launch"] * 1e-3
     kernels["real"].update(pairs_per_walker=pairs, pair_image_terms_per_walker=terms,
                            pair_image_terms_per_s=terms * W / t_real, alg_flops_per_launch=real_flops,

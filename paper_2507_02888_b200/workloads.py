@@ -35,9 +35,13 @@ class Workload:
     charges: np.ndarray = field(default=None, repr=False)
     ion_pos: np.ndarray = field(default=None, repr=False)
     ion_q: np.ndarray = field(default=None, repr=False)
+    g_cut: float = 0.0    # non-cubic cells: explicit |G| cut-off (inverse bohr); 0 = from n2_max
+    sigma: float = 1.0    # electrons around ions: Gaussian width (bohr)
 
     @property
     def g_cutoff(self):
+        if self.g_cut > 0:
+            return self.g_cut
         # shell membership is decided by the integer n^2 <= n2_max; the next shell is >= 0.5 % away
         return 2.0 * math.pi / self.L * math.sqrt(self.n2_max) * (1.0 + 1e-9)
 
@@ -58,7 +62,7 @@ class Workload:
         # config 4: electron 4I+m sits at ion I plus N(0,1) per component (reading R13)
         per_ion = self.n // len(self.ion_pos)
         base = np.repeat(self.ion_pos, per_ion, axis=0)
-        return base[None, :, :] + rng.standard_normal((nw, self.n, self.dim))
+        return base[None, :, :] + self.sigma * rng.standard_normal((nw, self.n, self.dim))
 
     def moves(self, n_walkers=None, n_steps=None):
         """Config 5 move stream (reading R14): electron [S, W] int32, displacement [S, W, dim] float64."""
@@ -117,8 +121,37 @@ def config(index):
         L = rs * (4.0 * math.pi * n / 3.0) ** (1.0 / 3.0)
         return Workload("heg3d_n1000_moves", 5, 3, n, 4096, L, 5.4 / L, 97, 1.1 * L, ("f64", "f32"),
                         n_steps=100, step_sigma=0.3 * rs, cell=_cubic(L, 3), charges=-np.ones(n))
-    raise ValueError("config index must be 1..5")
+    if index == 6:
+        return hbn_hexagonal()
+    raise ValueError("config index must be 1..6")
+
+
+def hbn_hexagonal():
+    """a slab-like workload in a NON-orthogonal cell, shaped like the paper's
+    9 x 9 hexagonal boron-nitride supercell (synthetic positions, the paper's input deck is
+    not available).  Hexagonal cell a1 = (A, 0, 0), a2 = (-A/2, A sqrt(3)/2, 0), a3 = (0, 0, c) with
+    A = 9 x 4.75 bohr and c = 20 bohr; 81 B (q = +3) and 81 N (q = +5) ions in the plane z = c/2; 648 electrons,
+    4 per ion at the ion plus N(0, 1) per component (neutral cell); kappa = 0.32 / bohr with cut-offs for a
+    truncation of 1e-14 (~25 000 G-vectors).  Exercises the general-cell paths: complex half-set reciprocal
+    kernel, image-list real-space scan, two ion species (so (t, qq) stack items)."""
+    a, reps, c = 4.75, 9, 20.0
+    A = a * reps
+    cell = np.array([[A, 0.0, 0.0], [-0.5 * A, 0.5 * math.sqrt(3.0) * A, 0.0], [0.0, 0.0, c]])
+    prim = np.array([[a, 0.0, 0.0], [-0.5 * a, 0.5 * math.sqrt(3.0) * a, 0.0]])
+    ions, q = [], []
+    for i in range(reps):
+        for j in range(reps):
+            for (f1, f2, qq) in ((1.0 / 3.0, 2.0 / 3.0, 3.0), (2.0 / 3.0, 1.0 / 3.0, 5.0)):
+                xy = (i + f1) * prim[0] + (j + f2) * prim[1]
+                ions.append([xy[0], xy[1], 0.5 * c])
+                q.append(qq)
+    ions, q = np.array(ions), np.array(q)
+    kappa = 0.32
+    x = math.sqrt(-math.log(1e-14))
+    n = 4 * len(ions)
+    return Workload("hbn_9x9_hexagonal", 6, 3, n, 256, A, kappa, 0, x / kappa, ("f64", "f32"),
+                    cell=cell, charges=-np.ones(n), ion_pos=ions, ion_q=q, g_cut=2.0 * kappa * x)
 
 
 def all_configs():
-    return [config(i) for i in range(1, 6)]
+    return [config(i) for i in range(1, 6)]   # the five BASELINE.json configs; config(6) is the NEXT-1 workload

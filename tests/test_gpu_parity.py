@@ -516,6 +516,32 @@ def test_largest_paper_system_n1630(torch_cuda):
     _assert_delta(d_de.cpu().numpy()[None, :], de_ref, TOL64)
 
 
+def test_next1_hexagonal_hbn_workload(torch_cuda):
+    """the hexagonal 9 x 9 hBN-shaped cell (non-orthogonal cell, ~25 000
+    G-vectors, 648 electrons, two ion species): complex half-set reciprocal kernel, image-list real-space scan,
+    (t, qq) stack items.  Energies of 3 walkers in FP64 and FP32, then two committed moves per walker."""
+    w = workloads.config(6)
+    pos = w.positions(3)
+    ctx = _ctx(w)
+    for dtype, tol in (("f64", TOL64), ("f32", TOL32)):
+        p = pos if dtype == "f64" else _r32(pos)
+        e_ref, c_ref = _oracle_energy(w, p)
+        e, c = _gpu_energy(torch_cuda, ctx, p, w.charges, dtype)
+        _assert_energy(e, c, e_ref, c_ref, tol)
+    rng = np.random.default_rng(6)
+    S = 2
+    electron = rng.integers(0, w.n, (S, 3)).astype(np.int32)
+    cur = pos.copy()
+    new_r = np.zeros((S, 3, 3))
+    for s_ in range(S):
+        new_r[s_] = cur[np.arange(3), electron[s_]] + 0.5 * rng.standard_normal((3, 3))
+        cur[np.arange(3), electron[s_]] = new_r[s_]
+    de_ref, _, _ = ref.move_chain(w.dim, w.cell, w.kappa, w.g_cutoff, w.r_cutoff, pos, w.charges, electron, new_r,
+                                  w.ion_pos, w.ion_q)
+    de = _run_moves(torch_cuda, ctx, w, pos, electron, new_r, "f64")
+    _assert_delta(de, de_ref, TOL64)
+
+
 def test_translation_and_permutation_invariance_on_gpu(torch_cuda):
     w = workloads.config(2)
     pos = w.positions(4)

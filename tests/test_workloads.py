@@ -52,3 +52,27 @@ def test_config_cutoffs_are_converged(idx):
     g2, r2 = ora.auto_cutoffs(w.dim, w.cell, k2, 1e-17)
     e2, _ = ora.energy_batch(w.dim, w.cell, k2, g2, r2, pos, w.charges, w.ion_pos, w.ion_q)
     assert e[0] == pytest.approx(e2[0], rel=1e-12)
+
+
+def test_config6_hexagonal_geometry():
+    """NEXT-1 workload: neutral hexagonal cell, B-N nearest-neighbour distance a / sqrt(3), ~25 000 G-vectors."""
+    w = workloads.config(6)
+    assert w.ion_pos.shape == (162, 3) and w.n == 648
+    assert w.ion_q.sum() + w.charges.sum() == 0
+    frac = w.ion_pos @ np.linalg.inv(w.cell)
+    assert frac.min() >= 0 and frac.max() < 1
+    d = w.ion_pos[:, None] - w.ion_pos[None]
+    f = d @ np.linalg.inv(w.cell)
+    d = (f - np.rint(f)) @ w.cell
+    r = np.linalg.norm(d, axis=-1)
+    r[r == 0] = 1e9
+    assert r.min() == pytest.approx(4.75 / np.sqrt(3))
+    ng = ora.num_g(w.dim, w.cell, w.g_cutoff)
+    assert 20000 < ng < 30000
+    # the cut-offs reproduce a converged evaluation at another splitting (one walker)
+    pos = w.positions(1)
+    e, _ = ora.energy_batch(w.dim, w.cell, w.kappa, w.g_cutoff, w.r_cutoff, pos, w.charges, w.ion_pos, w.ion_q)
+    k2 = 0.8 * w.kappa
+    g2, r2 = ora.auto_cutoffs(w.dim, w.cell, k2, 1e-17)
+    e2, _ = ora.energy_batch(w.dim, w.cell, k2, g2, r2, pos, w.charges, w.ion_pos, w.ion_q)
+    assert e[0] == pytest.approx(e2[0], rel=1e-11)
