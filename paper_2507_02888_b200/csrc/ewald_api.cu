@@ -232,7 +232,7 @@ extern "C" ewald_status ewald_setup(ewald_ctx **out, int dim, const double *cell
     }
     if (st == EWALD_OK && t.oct.valid) {
         std::vector<double> wt(t.oct.wt);
-        wt.resize(wt.size() + (size_t)(t.oct.npb + 1) * 2, 0.0); /* the zero-weight dummy item */
+        wt.resize(wt.size() + (size_t)(t.oct.npb + 1) * 4, 0.0); /* the zero-weight dummy item */
         st = upload(c, &c->d_oct_wt, wt);
     }
     if (st != EWALD_OK) { ewald_destroy(c); return st; }
@@ -269,10 +269,8 @@ extern "C" ewald_status ewald_oct_plan_summary(int dim, const double *cell, doub
     const OctPlan &P = t.oct;
     long double ws = 0;
     for (int it = 0; it < P.n_items; it++)
-        for (int j = 0; j <= P.npb; j++) {
-            ws += P.wt[((size_t)it * (P.npb + 1) + j) * 2];
-            if (dim == 2) ws += P.wt[((size_t)it * (P.npb + 1) + j) * 2 + 1];
-        }
+        for (int j = 0; j <= P.npb; j++)
+            for (int cls = 0; cls < 4; cls++) ws += P.wt[((size_t)it * (P.npb + 1) + j) * 4 + cls];
     OctLaunch L;
     make_oct_launch(P, n_walkers_per_cta, 1 << 20, &L);
     if (n_items) *n_items = P.n_items;

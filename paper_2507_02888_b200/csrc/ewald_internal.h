@@ -20,7 +20,7 @@ struct OctPlan {
     int n_items = 0;
     std::vector<int> offA, offB, offX, np, c0; /* [n_items] */
     std::vector<int> col;                      /* [n_items][3] = n2 (2D: n2a), n3 (2D: n2b or -1), first n1 of the block - 1 */
-    std::vector<double> wt;                    /* [n_items][1 + npb][2] */
+    std::vector<double> wt;                    /* [n_items][1 + npb][4] class weights (3D: ++, +-, -+, --; 2D: a+, a-, b+, b-) */
     std::vector<double> tion;                  /* [n_items][1 + 2 npb][4]; empty without fixed charges */
 };
 

@@ -21,20 +21,34 @@ void build_oct_plan(HostTables *t)
 {
     OctPlan &P = t->oct;
     P = OctPlan();
-    if (!t->orthogonal) return; /* |G| must be even in every n_k */
+    /* Any cell: G.r = 2 pi n.s in fractional coordinates, so the eight real sums T_abc(n), n >= 0, give
+     * rho(+-n1, +-n2, +-n3) for every sign choice.  Only the weights depend on the signs when the reciprocal
+     * axes are not orthogonal: rho(-G) = conj rho(G) leaves four classes (p, q) = (s1 s2, s1 s3), each with
+     * its own weight W_pq(n) = 2^nz/4 w(n1, p n2, q n3) (2^nz/8 per sign choice corrects for the choices that
+     * coincide when some n_k = 0; times 2 for G and -G).  2D: two classes p, W_p = 2^nz/2 w(n1, p n2). */
     const int dim = t->dim;
     const size_t ngp = t->g_w2.size();
-    std::map<std::tuple<int, int, int>, double> w; /* full-sphere weight w(G) = w2 / 2 on the octant */
-    for (size_t g = 0; g < ngp; g++) {
-        const int n1 = t->g_n[3 * g], n2 = t->g_n[3 * g + 1], n3 = t->g_n[3 * g + 2];
-        if (n2 < 0 || n3 < 0) continue;
-        w[std::make_tuple(n1, n2, n3)] = 0.5 * t->g_w2[g];
-    }
-    auto weight = [&](int n1, int n2, int n3) -> double { /* w(G) 2^nz, 0 outside the sphere */
+    std::map<std::tuple<int, int, int>, double> w; /* full-sphere weight w(G) = w2 / 2, keyed by the half-set member */
+    for (size_t g = 0; g < ngp; g++)
+        w[std::make_tuple(t->g_n[3 * g], t->g_n[3 * g + 1], t->g_n[3 * g + 2])] = 0.5 * t->g_w2[g];
+    auto w_of = [&](int n1, int n2, int n3) -> double { /* w(G) for any signs, 0 outside the sphere */
+        if (n1 < 0 || (n1 == 0 && (n2 < 0 || (n2 == 0 && n3 < 0)))) { n1 = -n1; n2 = -n2; n3 = -n3; }
         auto it = w.find(std::make_tuple(n1, n2, n3));
-        if (it == w.end()) return 0.0;
+        return it == w.end() ? 0.0 : it->second;
+    };
+    /* class weights of the octant point n >= 0: 3D (++, +-, -+, --) in (p, q); 2D (+, -) in p */
+    auto class_weight = [&](int n1, int n2, int n3, int cls) -> double {
         const int nz = (n1 != 0) + (n2 != 0) + (n3 != 0);
-        return it->second * (double)(1 << nz);
+        if (dim == 3) {
+            const int p = (cls & 2) ? -1 : 1, q = (cls & 1) ? -1 : 1;
+            return w_of(n1, p * n2, q * n3) * (double)(1 << nz) / 4.0;
+        }
+        return w_of(n1, (cls & 1) ? -n2 : n2, 0) * (double)(1 << nz) / 2.0;
+    };
+    auto weight = [&](int n1, int n2, int n3) -> double { /* sum over the classes: non-zero iff the point is used */
+        double sum = 0;
+        for (int cls = 0; cls < (dim == 3 ? 4 : 2); cls++) sum += class_weight(n1, n2, n3, cls);
+        return sum;
     };
     const int nm0 = t->n_max[0], nm1 = t->n_max[1], nm2 = dim == 3 ? t->n_max[2] : 0;
     if (nm1 + nm2 + nm0 + 3 > 0xffff) return;
@@ -85,13 +99,18 @@ void build_oct_plan(HostTables *t)
             P.col.push_back(c.a); P.col.push_back(c.b); P.col.push_back(start);
             for (int j = 0; j <= npb; j++) {
                 const int n1 = j == 0 ? 0 : start + j;
-                double w0 = 0, w1 = 0;
+                double wv[4] = {0, 0, 0, 0};
                 if ((j == 0 && b == 0) || (j >= 1 && j <= np)) {
-                    if (dim == 3) w0 = w1 = weight(n1, c.a, c.b);
-                    else { w0 = weight(n1, c.a, 0); w1 = c.b >= 0 ? weight(n1, c.b, 0) : 0.0; }
+                    if (dim == 3) {
+                        for (int cls = 0; cls < 4; cls++) wv[cls] = class_weight(n1, c.a, c.b, cls);
+                    } else {
+                        for (int cls = 0; cls < 2; cls++) {
+                            wv[cls] = class_weight(n1, c.a, 0, cls);
+                            wv[2 + cls] = c.b >= 0 ? class_weight(n1, c.b, 0, cls) : 0.0;
+                        }
+                    }
                 }
-                P.wt.push_back(w0);
-                P.wt.push_back(w1);
+                for (int cls = 0; cls < 4; cls++) P.wt.push_back(wv[cls]);
             }
         }
     }

@@ -39,7 +39,7 @@ template <typename T> struct OctArgs {
     int nmax[3];
     const int4 *lane;   /* [n_slabs][blockDim.x] {local walker | rank << 8, item, offA | offB << 16, offX} */
     const int *variant; /* [n_slabs][n_warps] NP | C0 << 8 */
-    const double *wt;   /* [n_items][1 + NPB][2]: w(G) 2^nz per entry for products (0,1) and (2,3) */
+    const double *wt;   /* [n_items][1 + NPB][4]: class weights W_pq per entry (ewald_octplan.cpp) */
     const double *tion; /* [n_items][1 + 2 NPB][4] fixed-charge sums, or null */
     double *e_recip;    /* [W][n_slabs] */
     T binv[9];
@@ -201,26 +201,42 @@ __global__ void __launch_bounds__(OctCfg<T, NPB>::MAX_THREADS) recip_oct_kernel(
         __syncthreads();
     }
 
-    /* [S4] E_recip = sum w 2^nz T^2, in FP64; entries of weight zero are padding (never read as values) */
+    /* [S4] E_recip = sum_n sum_classes W_pq(n) |rho_pq(n)|^2 in FP64, with (c = cos, s = sin along axes 1,2,3)
+     *   Re rho_pq = T_ccc - p T_ssc - q T_scs - pq T_css,   Im rho_pq = T_scc + p T_csc + q T_ccs - pq T_sss;
+     * for orthogonal reciprocal axes the four weights are equal and the sum is W sum_abc T_abc^2.
+     * Entries of weight zero are padding (never read as values). */
     double e = 0;
     {
-        const double *wt = A.wt + (size_t)L.y * (NPB + 1) * 2;
+        const double *wt = A.wt + (size_t)L.y * (NPB + 1) * 4;
         const double *ti = A.tion ? A.tion + (size_t)L.y * NE * 4 : nullptr;
 #pragma unroll
         for (int j = 0; j <= NPB; j++) {
-            const double wlo = wt[2 * j], whi = wt[2 * j + 1];
+            double Tc[4], Ts[4];
 #pragma unroll
             for (int k = 0; k < 4; k++) {
-                const double wk = k < 2 ? wlo : whi;
                 if (j == 0) {
-                    double v = (double)acc[k][0];
-                    if (ti) v += ti[k];
-                    e += wk != 0 ? wk * v * v : 0.0;
+                    Tc[k] = (double)acc[k][0]; Ts[k] = 0;
+                    if (ti) Tc[k] += ti[k];
                 } else {
-                    double vc = (double)acc[k][2 * j - 1], vs = (double)acc[k][2 * j];
-                    if (ti) { vc += ti[(2 * j - 1) * 4 + k]; vs += ti[(2 * j) * 4 + k]; }
-                    e += wk != 0 ? wk * (vc * vc + vs * vs) : 0.0;
+                    Tc[k] = (double)acc[k][2 * j - 1]; Ts[k] = (double)acc[k][2 * j];
+                    if (ti) { Tc[k] += ti[(2 * j - 1) * 4 + k]; Ts[k] += ti[(2 * j) * 4 + k]; }
                 }
+            }
+#pragma unroll
+            for (int cls = 0; cls < 4; cls++) {
+                const double wk = wt[4 * j + cls];
+                double re, im;
+                if (MODE == 0) { /* products k: 0 = c2 c3, 1 = c2 s3, 2 = s2 c3, 3 = s2 s3 */
+                    const double p = (cls & 2) ? -1.0 : 1.0, q = (cls & 1) ? -1.0 : 1.0;
+                    re = Tc[0] - p * Ts[2] - q * Ts[1] - p * q * Tc[3];
+                    im = Ts[0] + p * Tc[2] + q * Tc[1] - p * q * Ts[3];
+                } else {         /* two columns: k = 0,1 (c2, s2 of n2 = a) and k = 2,3 (of n2 = b) */
+                    const int o = cls & 2;
+                    const double p = (cls & 1) ? -1.0 : 1.0;
+                    re = Tc[o] - p * Ts[o + 1];
+                    im = Ts[o] + p * Tc[o + 1];
+                }
+                e += wk != 0 ? wk * (re * re + im * im) : 0.0;
             }
         }
     }

@@ -157,11 +157,24 @@ def test_octant_plan_covers_every_g_once():
         assert (ng + 1) / o["fma_per_particle"] > 0.6   # wc = 7: the cut-off wastes < 40 % of the lanes
 
 
-def test_octant_plan_orthorhombic_only():
+def test_octant_plan_any_cell():
+    """The octant plan exists for every cell (fractional coordinates); for a triclinic cell the class weights
+    still add up to the full-sphere weight sum, computed here from the plain definition over all G."""
     cell = np.array([[4.0, 0, 0], [0, 5.0, 0], [0, 0, 6.5]])
     o = E.ewald_oct_plan_summary(3, cell, 0.9, 5.0, 2)
     assert o["n_items"] > 0
-    tri = np.array([[4.0, 0, 0], [1.0, 5.0, 0], [0, 0, 6.5]])
-    with pytest.raises(E.EwaldError) as ei:
-        E.ewald_oct_plan_summary(3, tri, 0.9, 5.0, 2)
-    assert ei.value.status == 4
+    tri = np.array([[4.0, 0, 0], [1.0, 5.0, 0], [0.3, -0.4, 6.5]])
+    kappa, gc = 0.9, 5.0
+    o = E.ewald_oct_plan_summary(3, tri, kappa, gc, 2)
+    b = 2 * math.pi * np.linalg.inv(tri).T      # rows: reciprocal basis
+    vol = abs(np.linalg.det(tri))
+    nm = 8
+    tot = 0.0
+    for n1 in range(-nm, nm + 1):
+        for n2 in range(-nm, nm + 1):
+            for n3 in range(-nm, nm + 1):
+                g = n1 * b[0] + n2 * b[1] + n3 * b[2]
+                g2 = float(g @ g)
+                if 0 < g2 <= gc * gc * (1 + 1e-12):
+                    tot += 2 * math.pi / vol * math.exp(-g2 / (4 * kappa * kappa)) / g2
+    assert abs(o["weight_sum"] - tot) <= 1e-13 * tot

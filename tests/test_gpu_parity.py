@@ -140,14 +140,27 @@ def test_octant_kernel_orthorhombic_cells_and_single_walker(torch_cuda):
             _assert_energy(e, c, e_ref, c_ref, TOL64)
 
 
-def test_octant_kernel_refuses_general_cells(torch_cuda):
-    cell = np.array([[5.0, 0, 0], [1.5, 4.0, 0], [0.3, 0.2, 6.0]])
-    ctx = E.ewald_setup(3, cell, 1.0, 6.0)
-    E.ewald_set_recip_variant(ctx, 2)
-    pos = np.random.default_rng(1).random((2, 5, 3)) @ cell
-    with pytest.raises(E.EwaldError) as ei:
-        _gpu_energy(torch_cuda, ctx, pos, -np.ones(5), "f64")
-    assert ei.value.status == 4
+@pytest.mark.parametrize("dim", [2, 3])
+def test_octant_kernel_on_general_cells(torch_cuda, dim):
+    """Non-orthogonal cells: the octant kernel (class weights per sign choice) and the complex half-set kernel
+    both match the oracle, mixed charges and fixed ions included."""
+    rng = np.random.default_rng(40 + dim)
+    cell = (np.array([[5.0, 0, 0], [1.5, 4.0, 0], [0.3, 0.2, 6.0]]) if dim == 3 else np.array([[5.0, 0.0], [-2.0, 4.5]]))
+    kappa = 0.95
+    gc, rc = ref.auto_cutoffs(dim, cell, kappa, 1e-17)
+    n = 23
+    q = rng.choice([-1.0, 1.0, 2.0], size=n)
+    pos = (rng.random((5, n, dim)) * 1.4 - 0.2) @ cell
+    ion_pos = rng.random((3, dim)) @ cell
+    ion_q = np.array([2.0, -1.0, 0.5])
+    e_ref, c_ref = ref.energy_batch(dim, cell, kappa, gc, rc, pos, q, ion_pos, ion_q)
+    ctx = E.ewald_setup(dim, cell, kappa, gc, rc)
+    E.ewald_set_fixed_charges(ctx, ion_pos, ion_q)
+    scale = np.abs(c_ref).max(axis=1)
+    for variant in (2, 1, 0):
+        E.ewald_set_recip_variant(ctx, variant)
+        e, c = _gpu_energy(torch_cuda, ctx, pos, q, "f64")
+        assert (np.abs(c - c_ref) / scale[:, None]).max() <= TOL64, variant
 
 
 @pytest.mark.parametrize("idx", [2, 3])
