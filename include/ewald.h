@@ -81,10 +81,9 @@ ewald_status ewald_setup_summary(int dim, const double cell[9], double gamma, do
                                  double r_cutoff, int *num_g, int *num_images, int n_max[3],
                                  double *xi_r, double *v_m);
 
-/* Host-only summary of the work plan of the octant-form reciprocal kernel (orthorhombic cells; else
- * EWALD_ESTATE): items per walker, n1 pairs per block, warps of a CTA of n_walkers_per_cta walkers,
- * the sum of all octant weights w(G_n) 2^nz (must equal the full-sphere sum of w(G): the plan covers
- * every G exactly once) and the FMA + product operations the kernel executes per particle and walker
+/* Host-only summary of the work plan of the octant-form reciprocal kernel (any cell): items per walker,
+ * n1 pairs per block, warps of a CTA of n_walkers_per_cta walkers, the sum of all class weights of the
+ * octant points (must equal the full-sphere sum of w(G): the plan covers every G exactly once) and the FMA + product operations the kernel executes per particle and walker
  * (to compare with the algorithmic N_G + 1).  Any output pointer may be null. */
 ewald_status ewald_oct_plan_summary(int dim, const double cell[9], double gamma, double g_cutoff,
                                     int n_walkers_per_cta, int *n_items, int *npb, int *n_warps,
@@ -102,9 +101,9 @@ ewald_status ewald_pair_table_eval(ewald_prec prec, double t_max, int n, const d
 ewald_status ewald_set_stream(ewald_ctx *ctx, void *stream);
 
 /* Which reciprocal-space kernel ewald_energy_batch uses (both compute the same E_recip; for tests
- * and measurements): 0 = automatic (octant real-product form on orthorhombic cells, complex
- * half-set form otherwise), 1 = complex half-set form, 2 = octant form (EWALD_ESTATE at the next
- * energy call if the cell is not orthorhombic). */
+ * and measurements): 0 = automatic (the octant real-product form), 1 = complex half-set form,
+ * 2 = octant form (EWALD_ESTATE at the next energy call if no plan could be built: G indices beyond
+ * 16 bits). */
 ewald_status ewald_set_recip_variant(ewald_ctx *ctx, int variant);
 
 /* How the FP64 real-space kernels treat the far shell of the real-lattice sum of Eq. 3:

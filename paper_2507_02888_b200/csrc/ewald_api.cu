@@ -710,7 +710,7 @@ static ewald_status energy_batch_t(ewald_ctx *c, int W, int n, const T *pos, con
     }
     CU_TRY(c, cudaGetLastError());
     const bool oct = c->recip_variant != 1 && c->t.oct.valid;
-    if (c->recip_variant == 2 && !oct) return fail(c, EWALD_ESTATE, "octant kernel needs an orthorhombic cell");
+    if (c->recip_variant == 2 && !oct) return fail(c, EWALD_ESTATE, "octant kernel: no plan for this G set");
     ewald_status st = oct ? launch_recip_oct<T>(c, W, n, pos, q, &n_slabs)
                           : launch_recip<T>(c, W, n, pos, q, nullptr, &n_slabs);
     if (st != EWALD_OK) return st;

@@ -10,7 +10,7 @@
 
 namespace ewald {
 
-/* Host plan of the octant-form reciprocal kernel (ewald_recip_oct.cuh; orthorhombic cells only).
+/* Host plan of the octant-form reciprocal kernel (ewald_recip_oct.cuh; any cell).
  * An item is a column (n2, n3) -- in 2D a pair of n2 values -- with a block of <= npb consecutive
  * n1 >= 1 (block 0 also carries n1 = 0).  Offsets are in (cos,sin)-pair units within a table row. */
 struct OctPlan {

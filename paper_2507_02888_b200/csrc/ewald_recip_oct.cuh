@@ -1,13 +1,14 @@
 /* ewald_recip_oct.cuh -- [S1-S4] reciprocal-space energy in the octant (real-product) form.
  *
- * For an orthorhombic cell G.r = 2 pi sum_k n_k s_k (s = fractional coordinates) and Eq. 8
+ * In any cell G.r = 2 pi sum_k n_k s_k (s = fractional coordinates) and Eq. 8
  * factorises exp(iG.r) into per-axis powers.  Taking real and imaginary parts per axis,
  * the eight real sums over particles
  *     T_abc(n) = sum_i q_i t^a(2 pi n1 s_i1) t^b(2 pi n2 s_i2) t^c(2 pi n3 s_i3),  t in {cos, sin}, n_k >= 0
  * give rho(+-n1, +-n2, +-n3) for all sign choices, and summing |rho|^2 over the sign choices leaves
  *     E_recip = sum_{n >= 0, n != 0} w(G_n) 2^{nz(n)} sum_abc T_abc(n)^2
- * (nz = number of non-zero n_k; every cross term cancels).  One real FMA per (particle, G of the
- * full sphere): the algorithmic count 2 N N_G flops per walker, half of the complex half-set form.
+ * (nz = number of non-zero n_k; every cross term cancels) when the reciprocal axes are orthogonal; else the
+ * four sign classes of an octant point carry their own weights (S4 below, ewald_octplan.cpp).  One real FMA
+ * per (particle, G of the full sphere): the algorithmic count 2 N N_G flops per walker, half of the complex half-set form.
  *
  * Work decomposition (host plan, ewald_octplan.cpp):
  *   row    per (walker, particle): the "powers ... computed and buffered" of PAPER.md:157, in shared

@@ -194,7 +194,7 @@ def ewald_setup_summary(dim, cell, gamma, g_cutoff, r_cutoff=0.0):
 
 
 def ewald_oct_plan_summary(dim, cell, gamma, g_cutoff, n_walkers_per_cta=1):
-    """Host-only: work plan of the octant-form reciprocal kernel (orthorhombic cells)."""
+    """Host-only: work plan of the octant-form reciprocal kernel (any cell)."""
     c = _cell9(cell, dim)
     ni, nb, nw = ctypes.c_int(), ctypes.c_int(), ctypes.c_int()
     ws, fm = ctypes.c_double(), ctypes.c_double()
