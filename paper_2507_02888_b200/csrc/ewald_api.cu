@@ -573,6 +573,14 @@ static bool real_ortho(const ewald_ctx *c)
     return true;
 }
 
+template <typename T> static void fill_species(const ewald_ctx *c, PairTabs<T> *P)
+{
+    P->ion_uniform = c->t.ion_uniform ? 1 : 0;
+    P->n_species = c->t.ion_uniform ? (int)c->t.sp_start.size() - 1 : 0;
+    for (int s = 0; s < 5; s++)
+        P->sp_start[s] = s < (int)c->t.sp_start.size() && c->t.ion_uniform ? c->t.sp_start[s] : c->t.n_ion;
+}
+
 /* Fills the table part of PairTabs and returns the bytes of shared memory the tables take. */
 template <typename T> static void fill_pair_tabs(const ewald_ctx *c, const double *qinfo, PairTabs<T> *P);
 template <> void fill_pair_tabs<float>(const ewald_ctx *c, const double *qinfo, PairTabs<float> *P)
@@ -580,7 +588,8 @@ template <> void fill_pair_tabs<float>(const ewald_ctx *c, const double *qinfo, 
     const PairTable &pt = c->t.pair32;
     P->pair_tab = c->d_pairf; P->n_bins = pt.n_bins; P->t_safe = (float)pt.t_min;
     P->far_tab = nullptr; P->n_far = 0; P->key_far = 0x7fffffff;
-    P->qinfo = qinfo; P->ion_uniform = c->t.ion_uniform ? 1 : 0;
+    P->qinfo = qinfo;
+    fill_species(c, P);
     P->capf_u = P->capf_g = 0;
 }
 template <> void fill_pair_tabs<double>(const ewald_ctx *c, const double *qinfo, PairTabs<double> *P)
@@ -593,7 +602,8 @@ template <> void fill_pair_tabs<double>(const ewald_ctx *c, const double *qinfo,
     P->n_bins = far && near_bins < pt.n_bins ? near_bins : pt.n_bins;
     P->far_tab = far ? c->d_far : nullptr; P->n_far = far ? c->t.n_far : 0;
     P->key_far = far ? host_key((double)FAR_T0) : 0x7fffffff;
-    P->qinfo = qinfo; P->ion_uniform = c->t.ion_uniform ? 1 : 0;
+    P->qinfo = qinfo;
+    fill_species(c, P);
     P->capf_u = P->capf_g = 0;
 }
 

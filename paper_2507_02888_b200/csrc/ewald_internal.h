@@ -43,6 +43,7 @@ struct PairTable {
 constexpr int PAIR_K64 = 7, PAIR_DEG64 = 5;  /* FP64: 128 bins per octave, quintic: rel. error < 1e-16 */
 constexpr int PAIR_K32 = 5, PAIR_DEG32 = 3;  /* FP32:  32 bins per octave, cubic:   rel. error < 3e-9  */
 constexpr int FAR_T0 = 16, FAR_KB = 3, FAR_REP = 8; /* far shell of the FP64 kernels (FarFmt)       */
+constexpr int MAX_SPECIES = 4;               /* distinct fixed charges the bare-t real-space path handles  */
 constexpr int PAIR_EMIN = -6;                /* t < 2^-6 (kappa r < 1/8) takes the direct formula      */
 
 /* Everything ewald_setup computes on the host, in long double, before rounding (PAPER.md:359:
@@ -78,7 +79,8 @@ struct HostTables {
     std::vector<double> ion_pos; /* [n_ion][3] */
     std::vector<double> ion_q;
     std::vector<double> ion_rho; /* [ngp][2], sum_I q_I exp(iG.r_I)                              */
-    bool ion_uniform = true;     /* no fixed charges, or all of them equal */
+    bool ion_uniform = true;     /* at most MAX_SPECIES distinct fixed charges */
+    std::vector<int> sp_start;   /* [n_species + 1] first ion of each species (ions are kept grouped by charge) */
     double ion_q2 = 0, ion_qsum = 0, ion_real = 0; /* sum q^2, sum q, sum_{I<J} q_I q_J psi(r_IJ) */
     OctPlan oct;
 };

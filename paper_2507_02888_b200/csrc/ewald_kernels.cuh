@@ -132,7 +132,8 @@ template <typename T> struct PairTabs {
     const float *far_tab; int n_far; /* FP64 kernels: [n_far][FarFmt::REP][4] far-shell cubics; 0 = none */
     int key_far;                     /* order key of the far shell's start, INT_MAX = none              */
     const double *qinfo;             /* device [4]: sum q^2, sum q, all-equal flag, q_0                  */
-    int ion_uniform;                 /* no fixed charges, or all of them equal                          */
+    int ion_uniform;                 /* at most 4 distinct fixed charges (species)                      */
+    int n_species, sp_start[5];      /* ions [sp_start[s], sp_start[s+1]) carry one charge each         */
     int cap_u, cap_g;                /* near-stack capacity per lane: bare t items / (t, qq) items      */
     int capf_u, capf_g;              /* far-stack capacity per lane                                     */
 };
@@ -241,7 +242,7 @@ struct PairWalk {
 
 template <typename T, int DIM, bool ORTHO, int M, bool UQ>
 __device__ __forceinline__ double real_body(const RealArgs<T> &A, RealSmem<T> &S, const T *sp, const T *sq,
-                                            int tile, T q0, T qion0)
+                                            int tile, T q0)
 {
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, n = A.n;
     PairStacks<T, UQ, false> st;
@@ -281,11 +282,14 @@ __device__ __forceinline__ double real_body(const RealArgs<T> &A, RealSmem<T> &S
         st.finish();
         total += st.take() * (UQ ? (double)(q0 * q0) : 1.0);
     }
-    /* mobile particles against the fixed charges */
-    if (A.n_ion > 0) {
+    /* mobile particles against the fixed charges: with bare-t items one segment per species */
+    for (int s = 0; s < (UQ ? A.P.n_species : (A.n_ion > 0 ? 1 : 0)); s++) {
+        const int k0 = UQ ? A.P.sp_start[s] : 0, k1 = UQ ? A.P.sp_start[s + 1] : A.n_ion;
+        const T qion0 = S.ion[4 * k0 + 3];
         PairWalk pw; pw.init(gid, team, n);
+        pw.k += k0;
         for (;;) {
-            const bool valid = pw.k < A.n_ion;
+            const bool valid = pw.k < k1;
             if (!__any_sync(0xffffffffu, valid)) break;
             T d[3] = {0, 0, 0};
             T w = UQ ? q0 * qion0 : T(0);
@@ -323,10 +327,10 @@ __global__ void __launch_bounds__(REAL_MAX_THREADS) real_kernel(RealArgs<T> A)
     __syncthreads();
 
     const bool uq = A.P.qinfo[2] != 0.0 && A.P.ion_uniform;
-    const T q0 = (T)A.P.qinfo[3], qion0 = A.n_ion > 0 ? S.ion[3] : T(0);
+    const T q0 = (T)A.P.qinfo[3];
     double acc;
-    if (uq) acc = real_body<T, DIM, ORTHO, M, true>(A, S, sp, sq, tile, q0, qion0);
-    else acc = real_body<T, DIM, ORTHO, M, false>(A, S, sp, sq, tile, q0, qion0);
+    if (uq) acc = real_body<T, DIM, ORTHO, M, true>(A, S, sp, sq, tile, q0);
+    else acc = real_body<T, DIM, ORTHO, M, false>(A, S, sp, sq, tile, q0);
     acc = block_sum(acc, red);
     if (tid == 0) A.partial[(size_t)w * A.n_tiles + tile] = acc * (double)A.g.kappa;
 }
@@ -408,18 +412,22 @@ constexpr int MOVE_THREADS = 256;
  * (or 1 with the common charge applied here when UQ). */
 template <typename T, int DIM, bool ORTHO, int M, bool UQ>
 __device__ __forceinline__ double move_real(const MoveArgs<T> &A, RealSmem<T> &S, const T *pw, int k,
-                                            const T *r_old, const T *r_new, T q0, T qion0)
+                                            const T *r_old, const T *r_new, T q0)
 {
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     PairStacks<T, UQ, true> st;
     init_stacks(st, S, A.P, A.g.bias, warp, lane);
     __syncwarp();
     double total = 0, direct = 0;
-    for (int seg = 0; seg < 2; seg++) {
-        const int cnt = seg == 0 ? A.n : A.n_ion;
-        for (int base = 0; base < cnt; base += 32) {
+    /* segment 0: the mobile partners; then the fixed charges, one segment per species with bare-t items */
+    const int n_seg = 1 + (UQ ? A.P.n_species : (A.n_ion > 0 ? 1 : 0));
+    for (int seg = 0; seg < n_seg; seg++) {
+        const int j0 = seg == 0 || !UQ ? 0 : A.P.sp_start[seg - 1];
+        const int cnt = seg == 0 ? A.n : (UQ ? A.P.sp_start[seg] : A.n_ion);
+        const T qion0 = seg == 0 ? T(0) : S.ion[4 * j0 + 3];
+        for (int base = j0; base < cnt; base += 32) {
             const int j = base + lane;
-            const bool valid = j < cnt && (seg == 1 || j != k);
+            const bool valid = j < cnt && (seg >= 1 || j != k);
             T rj[3] = {0, 0, 0};
             T w = UQ ? T(1) : T(0);
             if (valid) {
@@ -442,7 +450,7 @@ __device__ __forceinline__ double move_real(const MoveArgs<T> &A, RealSmem<T> &S
             scan_pair<T, DIM, ORTHO, M, UQ, true, false>(A.g, dn, w, valid, st, direct, S.img, A.nimg);
             scan_pair<T, DIM, ORTHO, M, UQ, true, true>(A.g, dold, UQ ? w : -w, valid, st, direct, S.img, A.nimg);
         }
-        if (cnt > 0) st.finish();
+        if (cnt > j0) st.finish();
         const double wseg = UQ ? (double)(seg == 0 ? q0 : qion0) : 1.0;
         total += (st.take() + direct) * wseg;
         direct = 0;
@@ -463,7 +471,7 @@ __global__ void __launch_bounds__(MOVE_MAX_THREADS) move_kernel(MoveArgs<T> A)
     S.fill(A.P, A.img, A.nimg, A.ion_pos, A.ion_q, A.n_ion, tid, blockDim.x);
     __syncthreads();
     const bool uq = A.P.qinfo[2] != 0.0 && A.P.ion_uniform;
-    const T q0 = (T)A.P.qinfo[3], qion0 = A.n_ion > 0 ? S.ion[3] : T(0);
+    const T q0 = (T)A.P.qinfo[3];
 
     for (int m = blockIdx.x * n_warps + warp; m < A.n_moves; m += gridDim.x * n_warps) {
         const int w = A.walker[m], k = A.electron[m];
@@ -522,8 +530,8 @@ __global__ void __launch_bounds__(MOVE_MAX_THREADS) move_kernel(MoveArgs<T> A)
 
         /* [S7c] Delta E_real = q_k sum_{j != k} q_j [psi(r'-r_j) - psi(r-r_j)] */
         double accr;
-        if (uq) accr = move_real<T, DIM, ORTHO, M, true>(A, S, pw, k, r_old, r_new, q0, qion0);
-        else accr = move_real<T, DIM, ORTHO, M, false>(A, S, pw, k, r_old, r_new, q0, qion0);
+        if (uq) accr = move_real<T, DIM, ORTHO, M, true>(A, S, pw, k, r_old, r_new, q0);
+        else accr = move_real<T, DIM, ORTHO, M, false>(A, S, pw, k, r_old, r_new, q0);
         acc += (double)qk * accr * (double)A.g.kappa;
         acc = warp_sum(acc); /* its shuffles also order every lane's read of r_old before the commit */
         if (lane == 0) {

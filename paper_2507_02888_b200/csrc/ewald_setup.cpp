@@ -5,6 +5,7 @@
  * tables are "numerically sensitive and are always performed using DP"; "much of the
  * data required can be moved to the GPU once, at the outset").
  */
+#include <algorithm>
 #include <cmath>
 #include <cstdint>
 #include <cstring>
@@ -303,6 +304,7 @@ ewald_status build_tables(int dim, const double *cell, double kappa_d, double g_
     t->ion_pos.clear(); t->ion_q.clear(); t->ion_rho.clear();
     t->ion_q2 = t->ion_qsum = t->ion_real = 0;
     t->ion_uniform = true;
+    t->sp_start.assign(1, 0);
     build_oct_plan(t);
     return EWALD_OK;
 }
@@ -315,20 +317,31 @@ ewald_status build_fixed_charges(HostTables *t, int n_ion, const double *pos, co
     const size_t ngp = t->g_w2.size();
     t->n_ion = n_ion;
     t->ion_pos.assign((size_t)3 * n_ion, 0.0);
-    t->ion_q.assign(q, q + n_ion);
+    t->ion_q.assign((size_t)n_ion, 0.0);
     t->ion_rho.assign(2 * ngp, 0.0);
-    for (int i = 0; i < n_ion; i++)
+    /* the fixed charges are kept grouped by charge value ("species"; stable order inside a group): the
+     * real-space kernels then treat every species as one segment with a single charge product */
+    std::vector<int> order(n_ion);
+    for (int i = 0; i < n_ion; i++) order[i] = i;
+    std::stable_sort(order.begin(), order.end(), [&](int x, int y) { return q[x] < q[y]; });
+    t->sp_start.clear();
+    for (int k = 0; k < n_ion; k++) {
+        const int i = order[k];
+        t->ion_q[k] = q[i];
+        if (k == 0 || q[i] != q[order[k - 1]]) t->sp_start.push_back(k);
         for (int x = 0; x < dim; x++) {
             if (!std::isfinite(pos[(size_t)i * dim + x])) { *err = "non-finite ion position"; return EWALD_EINVAL; }
-            t->ion_pos[3 * i + x] = pos[(size_t)i * dim + x];
+            t->ion_pos[3 * k + x] = pos[(size_t)i * dim + x];
         }
+    }
+    t->sp_start.push_back(n_ion);
+    q = t->ion_q.data(); /* from here on: the grouped order */
     real q2 = 0, qs = 0;
     for (int i = 0; i < n_ion; i++) { q2 += (real)q[i] * q[i]; qs += q[i]; }
     t->ion_q2 = (double)q2;
     t->ion_qsum = (double)qs;
-    t->ion_uniform = true; /* one ion species: the real-space kernels keep bare t on their stacks */
-    for (int i = 1; i < n_ion; i++)
-        if (q[i] != q[0]) t->ion_uniform = false;
+    /* up to MAX_SPECIES species: the real-space kernels keep bare t on their stacks */
+    t->ion_uniform = (int)t->sp_start.size() - 1 <= MAX_SPECIES;
 
     /* rho_ion(G) = sum_I q_I exp(2 pi i n.s_I) with s = fractional coordinates */
     std::vector<real> s((size_t)3 * n_ion);
