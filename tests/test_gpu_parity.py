@@ -287,6 +287,45 @@ def test_uniform_charges_cutoff_reaching_two_far_images(torch_cuda):
             assert (np.abs(de - de_ref[s_]) / np.maximum(np.abs(de_ref[s_]), scale)).max() <= TOL64
 
 
+@pytest.mark.parametrize("mixed", [False, True])
+def test_cubic_cell_two_ion_species_energies_and_moves(torch_cuda, mixed):
+    """Cubic cell with |m| <= 1 images, far shell present (kappa r_c = 6.1 > 4), fixed charges of two species.
+    mixed = False: equal mobile charges -> bare-t stacks, one segment per species, signed items in the moves.
+    mixed = True: unequal mobile charges -> (t, qq) items everywhere, far shell included."""
+    rng = np.random.default_rng(77 + mixed)
+    L = 7.0
+    cell = np.eye(3) * L
+    rc = 1.25 * L
+    kappa = 6.1 / rc
+    gc, _ = ref.auto_cutoffs(3, cell, kappa, 1e-17)
+    n = 37
+    q = rng.choice([-1.0, 1.0, -2.0], size=n) if mixed else -np.ones(n)
+    pos = rng.random((4, n, 3)) * L
+    ion_pos = rng.random((7, 3)) * L
+    ion_q = np.array([3.0, 5.0, 3.0, 5.0, 5.0, 3.0, 3.0])
+    e_ref, c_ref = ref.energy_batch(3, cell, kappa, gc, rc, pos, q, ion_pos, ion_q)
+    ctx = E.ewald_setup(3, cell, kappa, gc, rc)
+    E.ewald_set_fixed_charges(ctx, ion_pos, ion_q)
+    scale = np.abs(c_ref).max(axis=1)
+    for dtype, tol in (("f64", TOL64), ("f32", TOL32)):
+        p = pos if dtype == "f64" else _r32(pos)
+        er, cr = (e_ref, c_ref) if dtype == "f64" else ref.energy_batch(3, cell, kappa, gc, rc, p, q, ion_pos, ion_q)
+        e, c = _gpu_energy(torch_cuda, ctx, p, q, dtype)
+        assert (np.abs(c - cr) / np.abs(cr).max(axis=1)[:, None]).max() <= tol
+    S = 3
+    electron = rng.integers(0, n, (S, 4)).astype(np.int32)
+    new_r = rng.random((S, 4, 3)) * L
+    de_ref, _, _ = ref.move_chain(3, cell, kappa, gc, rc, pos, q, electron, new_r, ion_pos, ion_q)
+    E.ewald_load_walkers(ctx, n, torch_cuda.from_numpy(E.to_soa(pos)).cuda(), torch_cuda.from_numpy(q).cuda())
+    d_w = torch_cuda.arange(4, dtype=torch_cuda.int32, device="cuda")
+    for s_ in range(S):
+        d_de = torch_cuda.zeros(4, dtype=torch_cuda.float64, device="cuda")
+        E.ewald_move_delta_batch(ctx, d_w, torch_cuda.from_numpy(electron[s_]).cuda(),
+                                 torch_cuda.from_numpy(new_r[s_]).cuda(), 1, d_de)
+        de = d_de.cpu().numpy()
+        assert (np.abs(de - de_ref[s_]) / np.maximum(np.abs(de_ref[s_]), scale)).max() <= TOL64
+
+
 def test_fixed_charges_equal_mobile_charges(torch_cuda):
     """Ions passed as fixed charges give the same energy as the same ions passed as mobile particles."""
     rng = np.random.default_rng(11)
