@@ -257,12 +257,15 @@ __device__ __forceinline__ double real_body(const RealArgs<T> &A, RealSmem<T> &S
         const bool even = (n & 1) == 0;
         typedef ScanShape<DIM, ORTHO, M, UQ> Shape;
         constexpr int GROUP = Shape::GROUP;
+        /* image-list path with few images: IMG_STEP / nimg pairs between two services */
+        const int list_group = !ORTHO && A.nimg > 0 && 2 * A.nimg <= IMG_STEP ? IMG_STEP / A.nimg : 1;
+        const int group = ORTHO ? GROUP : list_group;
         PairWalk pw; pw.init(gid, team, n);
         for (;;) {
             bool valid = pw.k < H || (even && pw.k == H && pw.i < n / 2);
             if (!__any_sync(0xffffffffu, valid)) break;
 #pragma unroll
-            for (int u = 0; u < GROUP; u++) {
+            for (int u = 0; u < (ORTHO ? GROUP : group); u++) {
                 if (u > 0) valid = pw.k < H || (even && pw.k == H && pw.i < n / 2);
                 T d[3] = {0, 0, 0};
                 T w = UQ ? q0 * q0 : T(0);
@@ -274,10 +277,11 @@ __device__ __forceinline__ double real_body(const RealArgs<T> &A, RealSmem<T> &S
                     for (int x = 0; x < DIM; x++) d[x] = (sp[x * n + i] - sp[x * n + j]) * A.g.kappa;
                     if (!UQ) w = sq[i] * sq[j];
                 }
-                scan_pair<T, DIM, ORTHO, M, UQ, false, false, GROUP == 1>(A.g, d, w, valid, st, direct, S.img, A.nimg);
+                scan_pair<T, DIM, ORTHO, M, UQ, false, false, GROUP == 1>(A.g, d, w, valid, st, direct, S.img, A.nimg,
+                                                                          group == 1);
                 pw.next();
             }
-            if (GROUP > 1) st.service(Shape::LIMIT);
+            if (group > 1) st.service(Shape::LIMIT);
         }
         st.finish();
         total += st.take() * (UQ ? (double)(q0 * q0) : 1.0);

@@ -293,9 +293,11 @@ template <int DIM, bool ORTHO, int M, bool UQ> struct ScanShape {
 template <typename T, int DIM, bool ORTHO, int M, bool UQ, bool SIGNED = false, bool NEG = false,
           bool SERVICE = true>
 __device__ __forceinline__ void scan_pair(const RealGeom<T> &g, T *d, T w, bool valid,
-                                          PairStacks<T, UQ, SIGNED> &st, double &direct, const T *simg, int nimg)
+                                          PairStacks<T, UQ, SIGNED> &st, double &direct, const T *simg, int nimg,
+                                          bool list_service = true)
 {
-    /* NEG (move kernel, old position): the term enters with a minus sign -- in w for (t, w) items (the
+    /* list_service = false (image-list path, few images): the caller services the stacks after several pairs.
+     * NEG (move kernel, old position): the term enters with a minus sign -- in w for (t, w) items (the
      * caller passes -w), in the sign bit of t for bare-t items */
     constexpr bool FLIP = NEG && UQ && SIGNED;
     typedef ScanShape<DIM, ORTHO, M, UQ> Shape;
@@ -402,20 +404,19 @@ __device__ __forceinline__ void scan_pair(const RealGeom<T> &g, T *d, T w, bool 
             for (int k = 0; k < DIM; k++) d[x] = fma(-f[k], g.a[3 * k + x], d[x]);
         }
         for (int m0 = 0; m0 < nimg; m0 += IMG_STEP) {
-#pragma unroll
-            for (int u = 0; u < IMG_STEP; u++) {
-                const int m = m0 + u;
-                const bool in = valid && m < nimg;
-                const int mm = m < nimg ? m : 0;
+            const int m1 = min(m0 + IMG_STEP, nimg); /* uniform trip count: no work for images that do not exist */
+#pragma unroll 4
+            for (int m = m0; m < m1; m++) {
+                const bool in = valid;
                 T t = 0;
 #pragma unroll
-                for (int x = 0; x < DIM; x++) { const T v = d[x] - simg[3 * mm + x]; t = fma(v, v, t); }
+                for (int x = 0; x < DIM; x++) { const T v = d[x] - simg[3 * m + x]; t = fma(v, v, t); }
                 const int key = order_key(t);
                 const bool tiny = in && key < g.key_min;
                 if (tiny) direct += (double)((FLIP ? -w : w) * pair_f_direct(t));
                 st.template push<FLIP>(in && !tiny && key <= g.key_rc, t, key, w);
             }
-            st.service(Shape::LIMIT);
+            if (list_service) st.service(Shape::LIMIT);
         }
     }
 }
