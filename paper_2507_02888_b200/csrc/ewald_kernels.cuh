@@ -257,8 +257,8 @@ __device__ __forceinline__ double real_body(const RealArgs<T> &A, RealSmem<T> &S
         const bool even = (n & 1) == 0;
         typedef ScanShape<DIM, ORTHO, M, UQ> Shape;
         constexpr int GROUP = Shape::GROUP;
-        /* image-list path with few images: IMG_STEP / nimg pairs between two services */
-        const int list_group = !ORTHO && A.nimg > 0 && 2 * A.nimg <= IMG_STEP ? IMG_STEP / A.nimg : 1;
+        /* image-list path with few images: LIMIT / nimg pairs between two services */
+        const int list_group = !ORTHO && A.nimg > 0 && 2 * A.nimg <= Shape::LIMIT ? Shape::LIMIT / A.nimg : 1;
         const int group = ORTHO ? GROUP : list_group;
         PairWalk pw; pw.init(gid, team, n);
         for (;;) {

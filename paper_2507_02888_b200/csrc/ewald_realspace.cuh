@@ -284,7 +284,8 @@ template <int DIM, bool ORTHO, int M, bool UQ> struct ScanShape {
     static constexpr bool PLANE = UQ && !WHOLE && DIM == 3 && ROW == 3;
     /* with very few images per pair the energy kernel scans GROUP pairs between two services */
     static constexpr int GROUP = UQ && ORTHO && WHOLE && ALL <= 4 ? 8 / ALL : 1;
-    static constexpr int LIMIT = ORTHO ? (WHOLE ? ALL * GROUP : PLANE ? ROW * ROW : ROW) : IMG_STEP;
+    /* image-list path: (t, qq) items have half the capacity, so half the images between two services */
+    static constexpr int LIMIT = ORTHO ? (WHOLE ? ALL * GROUP : PLANE ? ROW * ROW : ROW) : (UQ ? IMG_STEP : IMG_STEP / 2);
     static constexpr int MIN_CAP = LIMIT + PAIR_R;
 };
 
@@ -403,8 +404,8 @@ __device__ __forceinline__ void scan_pair(const RealGeom<T> &g, T *d, T w, bool 
 #pragma unroll
             for (int k = 0; k < DIM; k++) d[x] = fma(-f[k], g.a[3 * k + x], d[x]);
         }
-        for (int m0 = 0; m0 < nimg; m0 += IMG_STEP) {
-            const int m1 = min(m0 + IMG_STEP, nimg); /* uniform trip count: no work for images that do not exist */
+        for (int m0 = 0; m0 < nimg; m0 += Shape::LIMIT) {
+            const int m1 = min(m0 + Shape::LIMIT, nimg); /* uniform trip count: no work for images that do not exist */
 #pragma unroll 4
             for (int m = m0; m < m1; m++) {
                 const bool in = valid;
