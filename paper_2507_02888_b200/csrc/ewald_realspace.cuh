@@ -277,15 +277,15 @@ constexpr int IMG_STEP = 8;
 template <int DIM, bool ORTHO, int M, bool UQ> struct ScanShape {
     static constexpr int ROW = 2 * M + 1;
     static constexpr int ALL = DIM == 3 ? ROW * ROW * ROW : ROW * ROW;
-    /* the stacks are serviced once per pair (few images), after every group of <= 9 candidates (|m| <= 1 in
-     * 3D, see scan_pair), else once per x-row: small LIMIT = small stacks = more warps per SM */
+    /* the stacks are serviced once per pair (few images), after the 8 core and after the 12 one-far candidates
+     * (|m| <= 1 in 3D, see scan_pair), else once per x-row: small LIMIT = small stacks = more warps per SM */
     /* (t, qq) items take twice the bytes, i.e. half the capacity: always once per x-row */
     static constexpr bool WHOLE = ALL <= (UQ ? 9 : 3);
     static constexpr bool PLANE = UQ && !WHOLE && DIM == 3 && ROW == 3;
     /* with very few images per pair the energy kernel scans GROUP pairs between two services */
     static constexpr int GROUP = UQ && ORTHO && WHOLE && ALL <= 4 ? 8 / ALL : 1;
     /* image-list path: (t, qq) items have half the capacity, so half the images between two services */
-    static constexpr int LIMIT = ORTHO ? (WHOLE ? ALL * GROUP : PLANE ? ROW * ROW : ROW) : (UQ ? IMG_STEP : IMG_STEP / 2);
+    static constexpr int LIMIT = ORTHO ? (WHOLE ? ALL * GROUP : PLANE ? 12 : ROW) : (UQ ? IMG_STEP : IMG_STEP / 2);
     static constexpr int MIN_CAP = LIMIT + PAIR_R;
 };
 
@@ -328,7 +328,6 @@ __device__ __forceinline__ void scan_pair(const RealGeom<T> &g, T *d, T w, bool 
         st.service(Shape::LIMIT);
 #pragma unroll
         for (int c = 0; c < 4; c++) { cand(2, c & 1, c >> 1, valid); cand(c & 1, 2, c >> 1, valid); }
-        st.service(Shape::LIMIT);
 #pragma unroll
         for (int c = 0; c < 4; c++) cand(c & 1, c >> 1, 2, valid);
         if (g.multi_far) {
