@@ -594,6 +594,56 @@ def test_next1_hexagonal_hbn_workload(torch_cuda):
     _assert_delta(de, de_ref, TOL64)
 
 
+@pytest.mark.parametrize("seed", list(range(24)))
+def test_randomised_small_systems(torch_cuda, seed):
+    """Seeded random small systems across the code paths: 2D/3D; cubic, orthorhombic and general cells; image
+    ranges 0..3; equal or mixed mobile charges; 0..6 fixed charges of 1..6 species (more than 4 species fall back
+    to (t, qq) items); energies in FP64 and FP32 and two moves per walker (one committed, one not)."""
+    rng = np.random.default_rng(1000 + seed)
+    dim = 2 + seed % 2
+    kind = (seed // 2) % 3
+    sides = np.array([4.0 + 3.0 * rng.random() for _ in range(dim)])
+    if kind == 0:
+        cell = np.eye(dim) * sides[0]
+    elif kind == 1:
+        cell = np.diag(sides)
+    else:
+        cell = np.diag(sides) + rng.uniform(-0.2, 0.2, (dim, dim)) * sides.min()
+    kappa = float(rng.choice([0.45, 0.7, 1.0, 1.6, 2.4])) * 6.0 / sides.min() / 2.0
+    gc, rc = ref.auto_cutoffs(dim, cell, kappa, 1e-17)
+    n = int(rng.integers(1, 41))
+    q = -np.ones(n) if rng.random() < 0.5 else rng.choice([-1.0, 1.0, 2.0, -0.5], size=n)
+    n_ion = int(rng.integers(0, 7))
+    ion_pos = rng.random((n_ion, dim)) @ cell if n_ion else None
+    ion_q = rng.choice([1.0, 2.0, 3.0, 4.0, 5.0, 6.0], size=n_ion) if n_ion else None
+    W = 3
+    pos = (rng.random((W, n, dim)) * 1.5 - 0.25) @ cell
+    ctx = E.ewald_setup(dim, cell, kappa, gc, rc)
+    if n_ion:
+        E.ewald_set_fixed_charges(ctx, ion_pos, ion_q)
+    for dtype, tol in (("f64", TOL64), ("f32", TOL32)):
+        p = pos if dtype == "f64" else _r32(pos)
+        e_ref, c_ref = ref.energy_batch(dim, cell, kappa, gc, rc, p, q, ion_pos, ion_q)
+        e, c = _gpu_energy(torch_cuda, ctx, p, q, dtype)
+        scale = np.abs(c_ref).max(axis=1)
+        assert (np.abs(c - c_ref) / scale[:, None]).max() <= tol, (dtype, seed)
+    electron = rng.integers(0, n, (2, W)).astype(np.int32)
+    new_r = (rng.random((2, W, dim)) * 1.2 - 0.1) @ cell
+    # step 0 is not committed, step 1 is: the oracle chain therefore starts both from the loaded positions
+    de0, _, _ = ref.move_chain(dim, cell, kappa, gc, rc, pos, q, electron[:1], new_r[:1], ion_pos, ion_q)
+    de1, _, _ = ref.move_chain(dim, cell, kappa, gc, rc, pos, q, electron[1:], new_r[1:], ion_pos, ion_q)
+    E.ewald_load_walkers(ctx, n, torch_cuda.from_numpy(E.to_soa(pos)).cuda(), torch_cuda.from_numpy(q).cuda())
+    d_w = torch_cuda.arange(W, dtype=torch_cuda.int32, device="cuda")
+    e_ref, c_ref = ref.energy_batch(dim, cell, kappa, gc, rc, pos, q, ion_pos, ion_q)
+    scale = np.abs(c_ref).max(axis=1)
+    for s_, (commit, want) in enumerate(((0, de0[0]), (1, de1[0]))):
+        d_de = torch_cuda.zeros(W, dtype=torch_cuda.float64, device="cuda")
+        E.ewald_move_delta_batch(ctx, d_w, torch_cuda.from_numpy(electron[s_]).cuda(),
+                                 torch_cuda.from_numpy(new_r[s_]).cuda(), commit, d_de)
+        de = d_de.cpu().numpy()
+        assert (np.abs(de - want) / np.maximum(np.abs(want), scale)).max() <= TOL64, (s_, seed)
+
+
 def test_translation_and_permutation_invariance_on_gpu(torch_cuda):
     w = workloads.config(2)
     pos = w.positions(4)
