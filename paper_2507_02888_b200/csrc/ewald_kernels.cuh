@@ -1,14 +1,17 @@
 /* ewald_kernels.cuh -- device code of the B200 Ewald library (sm_100a).
  *
  * Kernels (SURVEY.md section 8(a) step names in brackets):
- *   recip_kernel   [S1-S4]  phase seeds exp(2 pi i s_k) by sincospi, power tables by complex
- *                           recurrence in shared memory (Eq. 8: "powers of these
+ *   recip_kernel   [S1-S4]  complex half-set form: phase seeds exp(2 pi i s_k) by sincospi, power tables by
+ *                           complex recurrence in shared memory (Eq. 8: "powers of these
  *                           exponentials are computed and buffered"), rho(G) on the half set,
- *                           E_recip = sum_{G+} 2 w(G) |rho(G)|^2; optionally stores rho(G)
- *   real_kernel    [S5]     sum_{i<j} q_i q_j sum_R erfc(kappa|r_ij-R|)/|r_ij-R| (real-lattice sum
- *                           of Eq. 3) plus mobile-ion pairs
- *   combine_kernel [S6]     adds partial sums and the constants of Eqs. 3-4
- *   move_kernel    [S7a-d]  single-particle move: Delta E and patch of the stored rho(G)
+ *                           E_recip = sum_{G+} 2 w(G) |rho(G)|^2; stores rho(G) for ewald_load_walkers.
+ *                           (The energy path uses recip_oct_kernel, ewald_recip_oct.cuh.)
+ *   real_kernel    [S5]     sum_{i<j} q_i q_j sum_R erfc(kappa|r_ij-R|)/|r_ij-R| (real-lattice sum of
+ *                           Eq. 3) plus mobile-ion pairs; machinery in ewald_realspace.cuh
+ *   combine_kernel [S6]     adds partial sums and the constants of Eqs. 3-4; charge_sums_kernel gives
+ *                           sum q^2, sum q and the all-equal flag of the mobile charges
+ *   move_kernel    [S7a-d]  single-particle moves, one warp per move: Delta E and patch of the stored rho(G)
+ *   fma_probe_kernel, fma_tile_probe_kernel   measurement helpers (roofline denominators)
  * The paper's version-2 loop structure (real-lattice loop || reciprocal-lattice loop, then a
  * combining loop) is kept as three kernels; everything inside them is new.
  */
