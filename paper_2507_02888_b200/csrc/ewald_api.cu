@@ -158,6 +158,7 @@ template <typename T> static void fill_geom(const HostTables &t, RealGeom<T> *g)
     g->kappa = (T)t.kappa;
     g->m_shift = t.m_shift;
     g->multi_far = 0;
+    g->outer_far = 0; /* set by set_outer_far once the far shell is known to be on */
     {
         const double rc2 = t.r_cutoff * t.r_cutoff * (1 + 1e-5);
         for (int j = 0; j < 3; j++)
@@ -563,6 +564,19 @@ static ewald_status launch_recip_oct(ewald_ctx *c, int W, int n, const T *pos, c
     return EWALD_OK;
 }
 
+/* With the far shell on and every (kappa L_k)^2 >= FAR_T0, a candidate that has a far image on some axis lies in
+ * the far shell whatever the other components are: the scan then touches the far stack only for those. */
+template <typename T> static void set_outer_far(const ewald_ctx *c, const PairTabs<T> &P, RealGeom<T> *g)
+{
+    g->outer_far = 0;
+    if (P.n_far <= 0) return;
+    for (int k = 0; k < c->t.dim; k++) {
+        const double l = c->t.a[4 * k] * c->t.kappa;
+        if (l * l < FAR_T0 * (1 + 1e-9)) return;
+    }
+    g->outer_far = 1;
+}
+
 /* The orthorhombic image scan needs boxes that reach the cut-off within +-2 images and that are wide enough
  * for only the un-shifted image to fall below the pair table (kappa L_k / 2 > sqrt(t_min)). */
 static bool real_ortho(const ewald_ctx *c)
@@ -664,6 +678,7 @@ static ewald_status launch_real(ewald_ctx *c, int W, int n, const T *pos, const 
     A.ion_pos = Tabs<T>::ion_pos(c); A.ion_q = Tabs<T>::ion_q(c); A.n_ion = c->t.n_ion;
     fill_pair_tabs<T>(c, (const double *)c->qsums.p, &A.P);
     fill_geom(c->t, &A.g);
+    set_outer_far(c, A.P, &A.g);
     const bool ortho = real_ortho(c);
     if (ortho) A.nimg = 0; /* the orthorhombic path does not read the image list */
     const size_t fixed = RealSmem<T>::fixed_bytes(A.P.n_bins, A.P.n_far, A.nimg, A.n_ion, (size_t)(c->t.dim + 1) * n);
@@ -844,6 +859,7 @@ static ewald_status move_batch_t(ewald_ctx *c, int n_moves, const int *walker, c
     A.walker = walker; A.electron = electron; A.new_r = new_r; A.commit = commit; A.delta_e = delta_e;
     for (int i = 0; i < 9; i++) A.binv[i] = (T)c->t.binv[i];
     fill_geom(c->t, &A.g);
+    set_outer_far(c, A.P, &A.g);
     const bool ortho = real_ortho(c);
     if (ortho) A.nimg = 0;
     /* one warp per move; the CTA size follows from the shared memory the stacks need */

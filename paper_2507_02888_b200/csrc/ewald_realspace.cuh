@@ -42,6 +42,7 @@ template <typename T> struct RealGeom {
     int bias;    /* bin index = (key >> SHIFT) - bias             */
     int m_shift; /* images -m_shift..m_shift scanned per axis (orthorhombic path) */
     int multi_far; /* 3D, m_shift = 1: some L_j^2 + L_k^2 < kappa^2 r_c^2, i.e. two far images can be in range */
+    int outer_far; /* every (kappa L_k)^2 >= 16: a candidate with a far image always belongs to the far shell */
 };
 
 /* Positive floating-point numbers order like their leading bits.  FP64 uses the high word: ties within
@@ -249,6 +250,7 @@ template <typename T, bool UQ, bool SIGNED> struct PairStacks;
 template <bool UQ, bool SIGNED> struct PairStacks<float, UQ, SIGNED> {
     LaneStack<float, UQ, SIGNED> nr;
     template <bool FLIP> __device__ __forceinline__ void push(bool ok, float t, int, float w) { nr.push(ok, FLIP ? -t : t, w); }
+    template <bool FLIP> __device__ __forceinline__ void push_far(bool ok, float t, int key, float w) { push<FLIP>(ok, t, key, w); }
     __device__ __forceinline__ void service(int limit) { nr.service(limit); }
     __device__ __forceinline__ void finish() { nr.finish(); }
     __device__ __forceinline__ double take() { const double v = nr.sum; nr.sum = 0; return v; }
@@ -262,6 +264,11 @@ template <bool UQ, bool SIGNED> struct PairStacks<double, UQ, SIGNED> {
         const bool far = key >= key_far;
         nr.push(ok && !far, FLIP ? -t : t, w);
         fr.push(ok && far, far_fixed(t) | (FLIP ? 0x80000000u : 0u), (float)w);
+    }
+    /* for candidates known to lie in the far shell (t >= T0): no near-stack instructions at all */
+    template <bool FLIP> __device__ __forceinline__ void push_far(bool ok, double t, int, double w)
+    {
+        fr.push(ok, far_fixed(t) | (FLIP ? 0x80000000u : 0u), (float)w);
     }
     /* key_far is uniform over the grid: the far stack is either used by every lane or by none */
     __device__ __forceinline__ bool has_far() const { return key_far != 0x7fffffff; }
@@ -323,13 +330,25 @@ __device__ __forceinline__ void scan_pair(const RealGeom<T> &g, T *d, T w, bool 
             const int key = order_key(t);
             st.template push<FLIP>(ok && key <= g.key_rc, t, key, w);
         };
+        auto cand_far = [&](int i, int j, int k, bool ok) { /* t >= 16 is known: far stack only */
+            const T t = a[0][i] + (a[1][j] + a[2][k]);
+            const int key = order_key(t);
+            st.template push_far<FLIP>(ok && key <= g.key_rc, t, key, w);
+        };
 #pragma unroll
         for (int c = 0; c < 8; c++) cand(c & 1, (c >> 1) & 1, c >> 2, c == 0 ? central_ok : valid);
         st.service(Shape::LIMIT);
+        if (g.outer_far) { /* uniform over the grid */
 #pragma unroll
-        for (int c = 0; c < 4; c++) { cand(2, c & 1, c >> 1, valid); cand(c & 1, 2, c >> 1, valid); }
+            for (int c = 0; c < 4; c++) { cand_far(2, c & 1, c >> 1, valid); cand_far(c & 1, 2, c >> 1, valid); }
 #pragma unroll
-        for (int c = 0; c < 4; c++) cand(c & 1, c >> 1, 2, valid);
+            for (int c = 0; c < 4; c++) cand_far(c & 1, c >> 1, 2, valid);
+        } else {
+#pragma unroll
+            for (int c = 0; c < 4; c++) { cand(2, c & 1, c >> 1, valid); cand(c & 1, 2, c >> 1, valid); }
+#pragma unroll
+            for (int c = 0; c < 4; c++) cand(c & 1, c >> 1, 2, valid);
+        }
         if (g.multi_far) {
             st.service(Shape::LIMIT);
 #pragma unroll
