@@ -252,6 +252,7 @@ template <bool UQ, bool SIGNED> struct PairStacks<float, UQ, SIGNED> {
     template <bool FLIP> __device__ __forceinline__ void push(bool ok, float t, int, float w) { nr.push(ok, FLIP ? -t : t, w); }
     template <bool FLIP> __device__ __forceinline__ void push_far(bool ok, float t, int key, float w) { push<FLIP>(ok, t, key, w); }
     __device__ __forceinline__ void service(int limit) { nr.service(limit); }
+    __device__ __forceinline__ void service_far(int limit) { nr.service(limit); } /* no far stack in FP32 */
     __device__ __forceinline__ void finish() { nr.finish(); }
     __device__ __forceinline__ double take() { const double v = nr.sum; nr.sum = 0; return v; }
 };
@@ -273,6 +274,8 @@ template <bool UQ, bool SIGNED> struct PairStacks<double, UQ, SIGNED> {
     /* key_far is uniform over the grid: the far stack is either used by every lane or by none */
     __device__ __forceinline__ bool has_far() const { return key_far != 0x7fffffff; }
     __device__ __forceinline__ void service(int limit) { nr.service(limit); if (has_far()) fr.service(limit); }
+    /* after a group that pushed on the far stack only (push_far) */
+    __device__ __forceinline__ void service_far(int limit) { fr.service(limit); }
     __device__ __forceinline__ void finish() { nr.finish(); if (has_far()) fr.finish(); }
     __device__ __forceinline__ double take() { const double v = nr.sum + fr.sum; nr.sum = 0; fr.sum = 0; return v; }
 };
@@ -343,6 +346,7 @@ __device__ __forceinline__ void scan_pair(const RealGeom<T> &g, T *d, T w, bool 
             for (int c = 0; c < 4; c++) { cand_far(2, c & 1, c >> 1, valid); cand_far(c & 1, 2, c >> 1, valid); }
 #pragma unroll
             for (int c = 0; c < 4; c++) cand_far(c & 1, c >> 1, 2, valid);
+            if (!g.multi_far) st.service_far(Shape::LIMIT);
         } else {
 #pragma unroll
             for (int c = 0; c < 4; c++) { cand(2, c & 1, c >> 1, valid); cand(c & 1, 2, c >> 1, valid); }
@@ -355,7 +359,7 @@ __device__ __forceinline__ void scan_pair(const RealGeom<T> &g, T *d, T w, bool 
             for (int c = 0; c < 2; c++) { cand(2, 2, c, valid); cand(2, c, 2, valid); cand(c, 2, 2, valid); }
             cand(2, 2, 2, valid);
         }
-        st.service(Shape::LIMIT);
+        if (!g.outer_far || g.multi_far) st.service(Shape::LIMIT);
     } else if (ORTHO) {
         constexpr int ROW = Shape::ROW;
         T sq[DIM][ROW];
