@@ -158,7 +158,7 @@ template <typename T> static void fill_geom(const HostTables &t, RealGeom<T> *g)
     g->kappa = (T)t.kappa;
     g->m_shift = t.m_shift;
     g->multi_far = 0;
-    g->outer_far = 0; /* set by set_outer_far once the far shell is known to be on */
+    g->outer_far = 0; g->far_once = 0; /* set by set_outer_far once the far shell and the capacities are known */
     {
         const double rc2 = t.r_cutoff * t.r_cutoff * (1 + 1e-5);
         for (int j = 0; j < 3; j++)
@@ -569,12 +569,16 @@ static ewald_status launch_recip_oct(ewald_ctx *c, int W, int n, const T *pos, c
 template <typename T> static void set_outer_far(const ewald_ctx *c, const PairTabs<T> &P, RealGeom<T> *g)
 {
     g->outer_far = 0;
+    g->far_once = 0;
     if (P.n_far <= 0) return;
     for (int k = 0; k < c->t.dim; k++) {
         const double l = c->t.a[4 * k] * c->t.kappa;
         if (l * l < FAR_T0 * (1 + 1e-9)) return;
     }
     g->outer_far = 1;
+    /* ... and if the far stack holds all 20 candidates of a pair plus a round, it is serviced once per pair
+     * (call after real_shape has fixed the capacities) */
+    g->far_once = !g->multi_far && P.capf_u >= 20 + PAIR_R;
 }
 
 /* The orthorhombic image scan needs boxes that reach the cut-off within +-2 images and that are wide enough
@@ -637,18 +641,22 @@ static bool real_shape(const ewald_ctx *c, size_t fixed, int min_cap_u, int min_
         const size_t budget = pass == 0 ? (half < full ? half : full) : full;
         for (int th = max_threads; th >= 32; th /= 2) {
             if (fixed >= budget) break;
-            /* bytes per unit of capacity: near item + (far item: 4 bytes), per lane, per warp */
-            const size_t per_cap = (size_t)(th / 32) * 32 * (sizeof(T) + (far ? 4 : 0));
-            long long cu = (long long)((budget - fixed) / per_cap);
-            const long long want = 2 * (min_cap_u > min_cap_g ? min_cap_u : min_cap_g) + 8;
-            if (cu > want) cu = want;
-            cu &= ~1LL;
-            if (cu >= min_cap_u + 4 && cu >= 2 * min_cap_g) {
-                *threads = th;
-                P->cap_u = (int)cu; P->cap_g = (int)(cu / 2);
-                P->capf_u = far ? (int)cu : 0; P->capf_g = far ? (int)(cu / 2) : 0;
-                *smem = fixed + (size_t)cu * per_cap;
-                return true;
+            /* bytes per unit of capacity: one near item + ff far items of 4 bytes, per lane, per warp.  ff = 2 (the
+             * far stack twice as deep: it receives twice the terms and can be serviced once per pair) if that
+             * fits, else 1 */
+            for (int ff = far ? 2 : 1; ff >= 1; ff--) {
+                const size_t per_cap = (size_t)(th / 32) * 32 * (sizeof(T) + (far ? 4 * ff : 0));
+                long long cu = (long long)((budget - fixed) / per_cap);
+                const long long want = 2 * (min_cap_u > min_cap_g ? min_cap_u : min_cap_g) + 8;
+                if (cu > want) cu = want;
+                cu &= ~1LL;
+                if (cu >= min_cap_u && cu >= 2 * min_cap_g) {
+                    *threads = th;
+                    P->cap_u = (int)cu; P->cap_g = (int)(cu / 2);
+                    P->capf_u = far ? ff * (int)cu : 0; P->capf_g = far ? ff * (int)cu / 2 : 0;
+                    *smem = fixed + (size_t)cu * per_cap;
+                    return true;
+                }
             }
             if (pass == 0) break; /* two CTAs per SM only at full size */
         }
@@ -678,7 +686,6 @@ static ewald_status launch_real(ewald_ctx *c, int W, int n, const T *pos, const 
     A.ion_pos = Tabs<T>::ion_pos(c); A.ion_q = Tabs<T>::ion_q(c); A.n_ion = c->t.n_ion;
     fill_pair_tabs<T>(c, (const double *)c->qsums.p, &A.P);
     fill_geom(c->t, &A.g);
-    set_outer_far(c, A.P, &A.g);
     const bool ortho = real_ortho(c);
     if (ortho) A.nimg = 0; /* the orthorhombic path does not read the image list */
     const size_t fixed = RealSmem<T>::fixed_bytes(A.P.n_bins, A.P.n_far, A.nimg, A.n_ion, (size_t)(c->t.dim + 1) * n);
@@ -686,6 +693,7 @@ static ewald_status launch_real(ewald_ctx *c, int W, int n, const T *pos, const 
     if (!real_shape<T>(c, fixed, real_min_cap(c, ortho, true), real_min_cap(c, ortho, false), REAL_MAX_THREADS, &A.P,
                        &threads, &smem))
         return fail(c, EWALD_ERANGE, "real-space kernel: problem too large for shared memory");
+    set_outer_far(c, A.P, &A.g);
 
     const long long H = (n - 1) / 2;
     const long long total = (long long)n * H + ((n & 1) ? 0 : n / 2) + (long long)n * c->t.n_ion;
@@ -859,7 +867,6 @@ static ewald_status move_batch_t(ewald_ctx *c, int n_moves, const int *walker, c
     A.walker = walker; A.electron = electron; A.new_r = new_r; A.commit = commit; A.delta_e = delta_e;
     for (int i = 0; i < 9; i++) A.binv[i] = (T)c->t.binv[i];
     fill_geom(c->t, &A.g);
-    set_outer_far(c, A.P, &A.g);
     const bool ortho = real_ortho(c);
     if (ortho) A.nimg = 0;
     /* one warp per move; the CTA size follows from the shared memory the stacks need */
@@ -872,6 +879,7 @@ static ewald_status move_batch_t(ewald_ctx *c, int n_moves, const int *walker, c
                              &smem) && threads == th;
     }
     if (!fits) return fail(c, EWALD_ERANGE, "move kernel: tables too large for shared memory");
+    set_outer_far(c, A.P, &A.g);
     const int warps = threads / 32;
     int grid = (n_moves + warps - 1) / warps;
     if (grid > c->sm_count) grid = c->sm_count; /* persistent CTAs: the tables are staged once per CTA */

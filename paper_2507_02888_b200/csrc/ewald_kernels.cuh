@@ -182,7 +182,7 @@ template <typename T> struct RealSmem {
     /* bytes of one warp's stacks (the two item kinds of a stack share the same bytes) */
     static __host__ __device__ size_t warp_stack_bytes(const PairTabs<T> &P)
     {
-        return (size_t)P.cap_u * 32 * sizeof(T) + (size_t)P.capf_u * 32 * 4;
+        return (size_t)P.cap_u * 32 * sizeof(T) + (size_t)P.capf_u * 32 * 4; /* capf_u = 2 cap_u or 0 */
     }
     __device__ __forceinline__ void fill(const PairTabs<T> &P, const T *gimg, int nimg, const T *ion_pos,
                                          const T *ion_q, int n_ion, int tid, int nthreads)

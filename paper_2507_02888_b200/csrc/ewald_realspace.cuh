@@ -43,6 +43,7 @@ template <typename T> struct RealGeom {
     int m_shift; /* images -m_shift..m_shift scanned per axis (orthorhombic path) */
     int multi_far; /* 3D, m_shift = 1: some L_j^2 + L_k^2 < kappa^2 r_c^2, i.e. two far images can be in range */
     int outer_far; /* every (kappa L_k)^2 >= 16: a candidate with a far image always belongs to the far shell */
+    int far_once;  /* outer_far, no multi_far, and the far stack is deep enough for one service per pair */
 };
 
 /* Positive floating-point numbers order like their leading bits.  FP64 uses the high word: ties within
@@ -253,6 +254,7 @@ template <bool UQ, bool SIGNED> struct PairStacks<float, UQ, SIGNED> {
     template <bool FLIP> __device__ __forceinline__ void push_far(bool ok, float t, int key, float w) { push<FLIP>(ok, t, key, w); }
     __device__ __forceinline__ void service(int limit) { nr.service(limit); }
     __device__ __forceinline__ void service_far(int limit) { nr.service(limit); } /* no far stack in FP32 */
+    __device__ __forceinline__ void service_near(int limit) { nr.service(limit); }
     __device__ __forceinline__ void finish() { nr.finish(); }
     __device__ __forceinline__ double take() { const double v = nr.sum; nr.sum = 0; return v; }
 };
@@ -276,6 +278,7 @@ template <bool UQ, bool SIGNED> struct PairStacks<double, UQ, SIGNED> {
     __device__ __forceinline__ void service(int limit) { nr.service(limit); if (has_far()) fr.service(limit); }
     /* after a group that pushed on the far stack only (push_far) */
     __device__ __forceinline__ void service_far(int limit) { fr.service(limit); }
+    __device__ __forceinline__ void service_near(int limit) { nr.service(limit); }
     __device__ __forceinline__ void finish() { nr.finish(); if (has_far()) fr.finish(); }
     __device__ __forceinline__ double take() { const double v = nr.sum + fr.sum; nr.sum = 0; fr.sum = 0; return v; }
 };
@@ -297,6 +300,7 @@ template <int DIM, bool ORTHO, int M, bool UQ> struct ScanShape {
     /* image-list path: (t, qq) items have half the capacity, so half the images between two services */
     static constexpr int LIMIT = ORTHO ? (WHOLE ? ALL * GROUP : PLANE ? 12 : ROW) : (UQ ? IMG_STEP : IMG_STEP / 2);
     static constexpr int MIN_CAP = LIMIT + PAIR_R;
+    static constexpr int FAR_LIMIT = 20; /* PLANE, fast variant: all 20 candidates between two far services */
 };
 
 /* Phase A for one pair per lane.  d = kappa (r_i - r_j), not yet reduced; w = q_i q_j.  Terms below the
@@ -340,13 +344,17 @@ __device__ __forceinline__ void scan_pair(const RealGeom<T> &g, T *d, T w, bool 
         };
 #pragma unroll
         for (int c = 0; c < 8; c++) cand(c & 1, (c >> 1) & 1, c >> 2, c == 0 ? central_ok : valid);
-        st.service(Shape::LIMIT);
-        if (g.outer_far) { /* uniform over the grid */
+        /* fast = far-image candidates are far-shell terms and there are 12 of them (uniform over the grid):
+         * the near stack sees the 8 core candidates only, the far stack (twice the capacity) is serviced once
+         * per pair, after all 20 */
+        const bool fast = g.far_once != 0;
+        if (fast) st.service_near(8); else st.service(Shape::LIMIT);
+        if (g.outer_far) {
 #pragma unroll
             for (int c = 0; c < 4; c++) { cand_far(2, c & 1, c >> 1, valid); cand_far(c & 1, 2, c >> 1, valid); }
 #pragma unroll
             for (int c = 0; c < 4; c++) cand_far(c & 1, c >> 1, 2, valid);
-            if (!g.multi_far) st.service_far(Shape::LIMIT);
+            if (fast) st.service_far(Shape::FAR_LIMIT);
         } else {
 #pragma unroll
             for (int c = 0; c < 4; c++) { cand(2, c & 1, c >> 1, valid); cand(c & 1, 2, c >> 1, valid); }
