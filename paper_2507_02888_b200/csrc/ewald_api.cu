@@ -881,14 +881,19 @@ static ewald_status move_batch_t(ewald_ctx *c, int n_moves, const int *walker, c
     if (!fits) return fail(c, EWALD_ERANGE, "move kernel: tables too large for shared memory");
     set_outer_far(c, A.P, &A.g);
     const int warps = threads / 32;
-    int grid = (n_moves + warps - 1) / warps;
-    if (grid > c->sm_count) grid = c->sm_count; /* persistent CTAs: the tables are staged once per CTA */
+    const int want_grid = (n_moves + warps - 1) / warps;
     ewald_status st;
+    /* persistent CTAs (the tables are staged once per CTA): as many as the SMs hold at once */
 #define EWALD_LAUNCH_MOVE(DIM, ORTHO, M)                                                          \
     do {                                                                                          \
         if ((st = allow_smem(c, move_kernel<T, DIM, ORTHO, M>, smem)) != EWALD_OK) return st;     \
+        int per_sm = 1;                                                                           \
+        CU_TRY(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, move_kernel<T, DIM, ORTHO, M>, threads, \
+                                                                smem));                           \
+        if (per_sm < 1) per_sm = 1;                                                               \
+        const int grid = want_grid < c->sm_count * per_sm ? want_grid : c->sm_count * per_sm;     \
         ProfScope ps(c, 3);                                                                       \
-        move_kernel<T, DIM, ORTHO, M><<<grid, threads, smem, c->stream>>>(A);             \
+        move_kernel<T, DIM, ORTHO, M><<<grid, threads, smem, c->stream>>>(A);                     \
     } while (0)
     const int m = c->t.m_shift;
     if (c->t.dim == 3) {
