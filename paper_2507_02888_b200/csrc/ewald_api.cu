@@ -454,7 +454,7 @@ static ewald_status oct_launch_any(ewald_ctx *c, const OctArgs<T> &A, int grid, 
 
 template <typename T> static int oct_max_threads(int npb)
 {
-    return sizeof(T) == 8 ? (npb >= 6 ? 256 : 384) : (npb >= 6 ? 384 : 512);
+    return sizeof(T) == 8 ? (npb >= 6 ? 256 : 384) : (npb >= 6 ? 224 : 512);
 }
 
 /* Shared-memory shape of a CTA of wc walkers: particles per chunk, slab stride, bytes. */

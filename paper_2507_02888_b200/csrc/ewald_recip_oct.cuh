@@ -49,7 +49,8 @@ template <typename T> struct OctArgs {
 /* Threads per CTA the register file allows: 4 (1 + 2 NPB) accumulators per lane (doubles take two
  * registers each): FP64 NPB = 7 needs ~254 registers -> 256 threads; NPB <= 5 fits 168 -> 384. */
 template <typename T, int NPB> struct OctCfg {
-    static constexpr int MAX_THREADS = sizeof(T) == 8 ? (NPB >= 6 ? 256 : 384) : (NPB >= 6 ? 384 : 512);
+    static constexpr int MAX_THREADS = sizeof(T) == 8 ? (NPB >= 6 ? 256 : 384) : (NPB >= 6 ? 224 : 512);
+    static constexpr int MIN_CTAS = sizeof(T) == 4 && NPB >= 6 ? 2 : 1; /* FP32: two CTAs of 7 warps per SM */
 };
 
 /* One chunk of particles for one lane: acc[k][e] += p_k * X1_e. */
@@ -145,7 +146,7 @@ __device__ __forceinline__ void oct_build_rows(const OctArgs<T> &A, typename Num
 }
 
 template <typename T, int DIM, int NPB>
-__global__ void __launch_bounds__(OctCfg<T, NPB>::MAX_THREADS) recip_oct_kernel(OctArgs<T> A)
+__global__ void __launch_bounds__(OctCfg<T, NPB>::MAX_THREADS, OctCfg<T, NPB>::MIN_CTAS) recip_oct_kernel(OctArgs<T> A)
 {
     typedef typename Num<T>::T2 T2;
     constexpr int MODE = DIM == 3 ? 0 : 1;
