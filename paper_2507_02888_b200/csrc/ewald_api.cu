@@ -104,6 +104,22 @@ struct ProfScope {
     }
 };
 
+/* Makes the context's device current for one entry point and restores the caller's on exit. */
+struct DeviceGuard {
+    int prev = -1;
+    bool ok = false;
+    explicit DeviceGuard(int dev)
+    {
+        if (cudaGetDevice(&prev) != cudaSuccess) prev = -1;
+        ok = prev == dev || cudaSetDevice(dev) == cudaSuccess;
+        if (prev == dev) prev = -1;
+    }
+    ~DeviceGuard() { if (prev >= 0) cudaSetDevice(prev); }
+};
+#define EWALD_DEVICE(c)                                                                          \
+    DeviceGuard guard_((c)->device);                                                             \
+    if (!guard_.ok) { (c)->err = "cudaSetDevice failed"; return EWALD_ECUDA; }
+
 static ewald_status fail(ewald_ctx *c, ewald_status s, const char *msg)
 {
     if (c) c->err = msg;
@@ -153,9 +169,19 @@ template <> const PairTable &pair_of<float>(const HostTables &t) { return t.pair
 /* Real-space geometry in kappa-scaled lengths (ewald_realspace.cuh). */
 template <typename T> static void fill_geom(const HostTables &t, RealGeom<T> *g)
 {
-    for (int i = 0; i < 9; i++) { g->a[i] = (T)(t.a[i] * t.kappa); g->binv[i] = (T)(t.binv[i] / t.kappa); }
-    for (int k = 0; k < 3; k++) { g->L[k] = (T)(t.a[4 * k] * t.kappa); g->invL[k] = (T)(1.0 / (t.a[4 * k] * t.kappa)); }
+    for (int i = 0; i < 9; i++) {
+        g->a[i] = (T)(t.a[i] * t.kappa); g->binv[i] = (T)(t.binv[i] / t.kappa);
+        g->a_lo[i] = (T)(t.a[i] * t.kappa - (double)g->a[i]);
+    }
+    for (int k = 0; k < 3; k++) {
+        const double l = t.a[4 * k], c2 = l * t.kappa * l * t.kappa;
+        g->L[k] = (T)(l * t.kappa); g->invL[k] = (T)(1.0 / (l * t.kappa));
+        g->invLu[k] = (T)(1.0 / l); g->invLu_lo[k] = (T)(1.0 / l - (double)g->invLu[k]);
+        g->C[k] = (T)c2; g->C_lo[k] = (T)(c2 - (double)g->C[k]);
+    }
     g->kappa = (T)t.kappa;
+    g->kappa_lo = (T)(t.kappa - (double)g->kappa); /* zero in FP64 */
+    g->kappa_d = t.kappa;
     g->m_shift = t.m_shift;
     g->multi_far = 0;
     g->outer_far = 0; g->far_once = 0; /* set by set_outer_far once the far shell and the capacities are known */
@@ -193,8 +219,8 @@ extern "C" ewald_status ewald_setup(ewald_ctx **out, int dim, const double *cell
     if (st != EWALD_OK) { delete c; return st; }
     c->device = opts ? opts->device : 0;
     c->stream = opts ? (cudaStream_t)opts->stream : nullptr;
-    cudaError_t ce = cudaSetDevice(c->device);
-    if (ce != cudaSuccess) { delete c; return EWALD_ECUDA; }
+    DeviceGuard guard_(c->device);
+    if (!guard_.ok) { delete c; return EWALD_ECUDA; }
 
     const HostTables &t = c->t;
     c->ngp = (int)t.g_w2.size();
@@ -211,7 +237,12 @@ extern "C" ewald_status ewald_setup(ewald_ctx **out, int dim, const double *cell
     if (st == EWALD_OK) st = upload(c, &c->d_w2, t.g_w2);
     if (st == EWALD_OK) st = upload(c, &c->d_w2f, to_f32(t.g_w2));
     if (st == EWALD_OK) st = upload(c, &c->d_img, scaled(t.img, t.kappa));
-    if (st == EWALD_OK) st = upload(c, &c->d_imgf, to_f32(scaled(t.img, t.kappa)));
+    {   /* FP32 image list: high parts, then the low parts (ewald_realspace.cuh, RealGeom) */
+        const std::vector<double> im = scaled(t.img, t.kappa);
+        std::vector<float> hl(2 * im.size());
+        for (size_t i = 0; i < im.size(); i++) { hl[i] = (float)im[i]; hl[im.size() + i] = (float)(im[i] - (double)hl[i]); }
+        if (st == EWALD_OK) st = upload(c, &c->d_imgf, hl);
+    }
     if (st == EWALD_OK) st = upload(c, &c->d_pair, t.pair64.coef);
     {   /* FP32 table: PairFmt<float>::REP interleaved copies */
         const std::vector<float> one = to_f32(t.pair32.coef);
@@ -296,7 +327,7 @@ extern "C" ewald_status ewald_pair_table_eval(ewald_prec prec, double t_max, int
 extern "C" void ewald_destroy(ewald_ctx *c)
 {
     if (!c) return;
-    cudaSetDevice(c->device);
+    DeviceGuard guard_(c->device);
     cudaStreamSynchronize(c->stream);
     cudaFree(c->d_gn); cudaFree(c->d_w2); cudaFree(c->d_w2f); cudaFree(c->d_img); cudaFree(c->d_imgf);
     cudaFree(c->d_ion_rho); cudaFree(c->d_ion_rhof); cudaFree(c->d_ion_pos); cudaFree(c->d_ion_posf);
@@ -305,8 +336,9 @@ extern "C" void ewald_destroy(ewald_ctx *c)
     for (auto &kv : c->oct_dev) { cudaFree(kv.second.d_lane); cudaFree(kv.second.d_variant); }
     DevBuf *bufs[] = {&c->partial_recip, &c->partial_real, &c->qsums, &c->stage_pos, &c->stage_q,
                       &c->stage_e, &c->stage_comp, &c->mv_walker, &c->mv_electron, &c->mv_newr,
-                      &c->mv_de, &c->st_pos, &c->st_q, &c->st_rho};
+                      &c->mv_de, &c->st_pos, &c->st_q, &c->st_rho, &c->st_qinfo};
     for (DevBuf *b : bufs) release(b);
+    for (ProfRec &r : c->recs) { cudaEventDestroy(r.a); cudaEventDestroy(r.b); }
     delete c;
 }
 
@@ -334,7 +366,7 @@ extern "C" ewald_status ewald_set_stream(ewald_ctx *c, void *stream)
 extern "C" ewald_status ewald_set_fixed_charges(ewald_ctx *c, int n_ion, const double *pos, const double *q)
 {
     if (!c) return EWALD_EINVAL;
-    CU_TRY(c, cudaSetDevice(c->device));
+    EWALD_DEVICE(c);
     std::string err;
     ewald_status st = build_fixed_charges(&c->t, n_ion, pos, q, &err);
     if (st != EWALD_OK) return fail(c, st, err.c_str());
@@ -378,7 +410,7 @@ template <> struct Tabs<float> {
 template <typename K> static ewald_status allow_smem(ewald_ctx *c, K kernel, size_t bytes)
 {
     if (bytes > 48 * 1024) {
-        if (bytes > 227 * 1024) return fail(c, EWALD_ERANGE, "problem too large for shared memory");
+        if (bytes > c->smem_optin) return fail(c, EWALD_ERANGE, "problem too large for shared memory");
         CU_TRY(c, cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes));
     }
     return EWALD_OK;
@@ -402,7 +434,7 @@ static ewald_status launch_recip(ewald_ctx *c, int W, int n, const T *pos, const
     A.rho_out = rho_out;
     A.partial = (double *)c->partial_recip.p;
     A.n_slabs = n_slabs;
-    for (int i = 0; i < 9; i++) A.binv[i] = (T)c->t.binv[i];
+    for (int i = 0; i < 9; i++) A.binv[i] = c->t.binv[i];
     const size_t smem = (size_t)RECIP_CHUNK * c->rowlen * sizeof(T2);
     const long long grid = (long long)W * n_slabs;
     if (grid > 0x7fffffffLL) return fail(c, EWALD_ERANGE, "grid too large");
@@ -500,7 +532,7 @@ static void oct_fill_args(ewald_ctx *c, OctArgs<T> *A, int W, int n, const T *po
     A->lane = d.d_lane; A->variant = d.d_variant;
     A->wt = c->d_oct_wt; A->tion = c->t.n_ion ? c->d_oct_tion : nullptr;
     A->e_recip = e_recip;
-    for (int i = 0; i < 9; i++) A->binv[i] = (T)c->t.binv[i];
+    for (int i = 0; i < 9; i++) A->binv[i] = c->t.binv[i];
 }
 
 /* Picks the walkers-per-CTA that minimises (waves x work per wave) on this device. */
@@ -780,7 +812,7 @@ extern "C" ewald_status ewald_energy_batch(ewald_ctx *c, int W, int n, ewald_pre
     if (st != EWALD_OK) return st;
     if (W == 0) return EWALD_OK;
     if (!energies) return fail(c, EWALD_EINVAL, "null energies");
-    CU_TRY(c, cudaSetDevice(c->device));
+    EWALD_DEVICE(c);
     if (prec == EWALD_F64)
         return energy_batch_t<double>(c, W, n, (const double *)pos, (const double *)q, energies, components);
     return energy_batch_t<float>(c, W, n, (const float *)pos, (const float *)q, energies, components);
@@ -794,7 +826,7 @@ extern "C" ewald_status ewald_energy_batch_host(ewald_ctx *c, int W, int n, ewal
     if (st != EWALD_OK) return st;
     if (W == 0) return EWALD_OK;
     if (!energies) return fail(c, EWALD_EINVAL, "null energies");
-    CU_TRY(c, cudaSetDevice(c->device));
+    EWALD_DEVICE(c);
     const size_t es = prec == EWALD_F64 ? 8 : 4;
     const size_t pbytes = (size_t)W * c->t.dim * ewald_padded_n(n) * es, qbytes = (size_t)n * es;
     if ((st = ensure(c, &c->stage_pos, pbytes)) != EWALD_OK) return st;
@@ -819,7 +851,7 @@ extern "C" ewald_status ewald_load_walkers(ewald_ctx *c, int W, int n, ewald_pre
     ewald_status st = check_batch(c, W, n, prec, pos, q);
     if (st != EWALD_OK) return st;
     if (W == 0) return fail(c, EWALD_EINVAL, "n_walkers must be > 0");
-    CU_TRY(c, cudaSetDevice(c->device));
+    EWALD_DEVICE(c);
     const size_t es = prec == EWALD_F64 ? 8 : 4;
     const int npad = ewald_padded_n(n);
     const size_t pbytes = (size_t)W * c->t.dim * npad * es;
@@ -865,7 +897,7 @@ static ewald_status move_batch_t(ewald_ctx *c, int n_moves, const int *walker, c
     fill_pair_tabs<T>(c, (const double *)c->st_qinfo.p, &A.P);
     A.n_moves = n_moves;
     A.walker = walker; A.electron = electron; A.new_r = new_r; A.commit = commit; A.delta_e = delta_e;
-    for (int i = 0; i < 9; i++) A.binv[i] = (T)c->t.binv[i];
+    for (int i = 0; i < 9; i++) A.binv[i] = c->t.binv[i];
     fill_geom(c->t, &A.g);
     const bool ortho = real_ortho(c);
     if (ortho) A.nimg = 0;
@@ -921,7 +953,7 @@ extern "C" ewald_status ewald_move_delta_batch(ewald_ctx *c, int n_moves, const 
     if (n_moves < 0) return fail(c, EWALD_EINVAL, "n_moves < 0");
     if (n_moves == 0) return EWALD_OK;
     if (!walker || !electron || !new_r || !delta_e) return fail(c, EWALD_EINVAL, "null move argument");
-    CU_TRY(c, cudaSetDevice(c->device));
+    EWALD_DEVICE(c);
     if (c->st_prec == EWALD_F64)
         return move_batch_t<double>(c, n_moves, walker, electron, (const double *)new_r, commit, delta_e);
     return move_batch_t<float>(c, n_moves, walker, electron, (const float *)new_r, commit, delta_e);
@@ -936,7 +968,7 @@ extern "C" ewald_status ewald_move_delta_batch_host(ewald_ctx *c, int n_moves, c
     if (n_moves < 0) return fail(c, EWALD_EINVAL, "n_moves < 0");
     if (n_moves == 0) return EWALD_OK;
     if (!walker || !electron || !new_r || !delta_e) return fail(c, EWALD_EINVAL, "null move argument");
-    CU_TRY(c, cudaSetDevice(c->device));
+    EWALD_DEVICE(c);
     const size_t es = c->st_prec == EWALD_F64 ? 8 : 4;
     const size_t rbytes = (size_t)n_moves * c->t.dim * es;
     ewald_status st;
@@ -981,7 +1013,7 @@ extern "C" ewald_status ewald_profile_enable(ewald_ctx *c, int on)
 extern "C" ewald_status ewald_profile_read(ewald_ctx *c, double *ms, int *launches)
 {
     if (!c || !ms || !launches) return EWALD_EINVAL;
-    CU_TRY(c, cudaSetDevice(c->device));
+    EWALD_DEVICE(c);
     CU_TRY(c, cudaStreamSynchronize(c->stream));
     for (int k = 0; k < 4; k++) { ms[k] = 0; launches[k] = 0; }
     for (ProfRec &r : c->recs) {
@@ -1035,7 +1067,7 @@ extern "C" ewald_status ewald_get_rho(ewald_ctx *c, int walker, double *re_im)
     if (!c || !re_im) return EWALD_EINVAL;
     if (!c->loaded) return fail(c, EWALD_ESTATE, "no walkers loaded");
     if (walker < 0 || walker >= c->st_walkers) return fail(c, EWALD_ESTATE, "walker index out of range");
-    CU_TRY(c, cudaSetDevice(c->device));
+    EWALD_DEVICE(c);
     const size_t es = c->st_prec == EWALD_F64 ? 8 : 4;
     std::vector<unsigned char> h((size_t)2 * c->ngp_pad * es);
     CU_TRY(c, cudaMemcpyAsync(h.data(), (const char *)c->st_rho.p + (size_t)walker * h.size(), h.size(),
@@ -1058,7 +1090,7 @@ extern "C" ewald_status ewald_get_positions(ewald_ctx *c, int walker, double *po
     if (!c || !pos) return EWALD_EINVAL;
     if (!c->loaded) return fail(c, EWALD_ESTATE, "no walkers loaded");
     if (walker < 0 || walker >= c->st_walkers) return fail(c, EWALD_ESTATE, "walker index out of range");
-    CU_TRY(c, cudaSetDevice(c->device));
+    EWALD_DEVICE(c);
     const size_t es = c->st_prec == EWALD_F64 ? 8 : 4;
     const int dim = c->t.dim, npad = c->st_npad, n = c->st_n;
     std::vector<unsigned char> h((size_t)dim * npad * es);
@@ -1075,7 +1107,7 @@ extern "C" ewald_status ewald_get_positions(ewald_ctx *c, int walker, double *po
 extern "C" ewald_status ewald_probe_fma_tile(ewald_ctx *c, ewald_prec prec, int iters, int threads, double *flops)
 {
     if (!c || !flops || iters <= 0 || threads < 32 || threads > 256 || threads % 32) return EWALD_EINVAL;
-    CU_TRY(c, cudaSetDevice(c->device));
+    EWALD_DEVICE(c);
     ewald_status st = ensure(c, &c->stage_e, 64);
     if (st != EWALD_OK) return st;
     CU_TRY(c, cudaMemsetAsync(c->stage_e.p, 0, 64, c->stream));
@@ -1103,7 +1135,7 @@ extern "C" ewald_status ewald_probe_fma_tile(ewald_ctx *c, ewald_prec prec, int 
 extern "C" ewald_status ewald_probe_fma(ewald_ctx *c, ewald_prec prec, int iters, double *flops)
 {
     if (!c || !flops || iters <= 0) return EWALD_EINVAL;
-    CU_TRY(c, cudaSetDevice(c->device));
+    EWALD_DEVICE(c);
     cudaDeviceProp prop;
     CU_TRY(c, cudaGetDeviceProperties(&prop, c->device));
     ewald_status st = ensure(c, &c->stage_e, 64);

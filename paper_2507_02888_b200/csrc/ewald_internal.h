@@ -66,11 +66,8 @@ struct HostTables {
     double self_coef = 0;  /* E_self = -self_coef * sum q^2,  self_coef = kappa/sqrt(pi)          */
     double bg_coef = 0;    /* E_bg = -bg_coef/2 * Q^2 ; pi/(Omega kappa^2) (3D), 2 sqrt(pi)/(A kappa) (2D) */
     double v_m = 0;        /* Eq. 4 */
-    /* real-space evaluation tables (ewald_realspace.cuh): erfc on 16 bins of z = kappa r in [0, z_max],
-     * rows c_0..c_deg then -(2b+1); FP64 table of degree 11 and FP32 table of degree 6 */
-    double z_max = 0;
+    /* real-space evaluation tables (ewald_realspace.cuh) */
     int m_shift = 0;              /* orthorhombic cells: images -m..m per axis reach r_cutoff      */
-    std::vector<double> erfc_tab64, erfc_tab32;
     PairTable pair64, pair32;
     std::vector<float> far_tab;   /* [n_far][FAR_REP][4] */
     int n_far = 0;
@@ -94,7 +91,6 @@ void make_oct_launch(const OctPlan &p, int wc, int max_warps, OctLaunch *out);
 /* Returns EWALD_OK or an error status with a message. */
 ewald_status build_tables(int dim, const double *cell, double kappa, double g_cutoff,
                           double r_cutoff, HostTables *out, std::string *err);
-void build_erfc_table(double z_max, int n_bins, int degree, std::vector<double> *tab);
 void build_pair_table(int kbits, int degree, int e_min, double t_max, PairTable *out);
 double eval_pair_table(const PairTable &p, double t);
 void build_far_table(int t0, int kb, int rep, double t_max, std::vector<float> *tab, int *n_far);

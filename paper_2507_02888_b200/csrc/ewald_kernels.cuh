@@ -37,7 +37,7 @@ template <typename T> struct RecipArgs {
     T *rho_out;        /* [W][2][ngp_pad] or null */
     double *partial;   /* [W][n_slabs] */
     int n_slabs;
-    T binv[9];
+    double binv[9];    /* FP64 in both precisions: s is reduced to one period before it is rounded */
 };
 
 constexpr int RECIP_THREADS = 256;
@@ -78,10 +78,10 @@ __global__ void __launch_bounds__(RECIP_THREADS) recip_kernel(RecipArgs<T> A)
         /* [S1,S2] one (particle, direction) per thread */
         for (int t = tid; t < cnt * DIM; t += RECIP_THREADS) {
             const int p = t / DIM, k = t - p * DIM;
-            T s = 0;
+            double s = 0;
 #pragma unroll
-            for (int x = 0; x < DIM; x++) s += pw[x * A.npad + base + p] * A.binv[3 * k + x];
-            power_row<T>(s, k == 0 ? A.q[base + p] : T(1), A.nmax[k], tab + p * A.rowlen + A.off[k]);
+            for (int x = 0; x < DIM; x++) s += (double)pw[x * A.npad + base + p] * A.binv[3 * k + x];
+            power_row<T>((T)(s - rint(s)), k == 0 ? A.q[base + p] : T(1), A.nmax[k], tab + p * A.rowlen + A.off[k]);
         }
         __syncthreads();
         /* [S3] rho(G) += q e1^n1 e2^n2 e3^n3 */
@@ -158,10 +158,11 @@ constexpr int REAL_MAX_THREADS = 512;
 template <typename T> struct RealSmem {
     T *tab;     /* [n_bins][REP][NC] */
     float *far; /* [n_far][REP][4] */
-    T *img;     /* [nimg][3] */
+    T *img;     /* [nimg][3]; FP32: followed by the [nimg][3] low parts */
     T *ion;     /* [n_ion][4] = x,y,z,q */
     T *rest;    /* caller's arrays (rest_elems), then the stacks */
     unsigned char *stacks;
+    static constexpr int IMG_PARTS = sizeof(T) == 4 ? 2 : 1;
     static __host__ __device__ size_t up4(size_t e) { return (e + 3) & ~(size_t)3; }
     static __host__ __device__ size_t far_bytes(int n_far) { return (size_t)n_far * FarFmt::REP * 16; }
     __device__ __forceinline__ RealSmem(unsigned char *raw, const PairTabs<T> &P, int nimg, int n_ion, size_t rest_elems)
@@ -169,14 +170,14 @@ template <typename T> struct RealSmem {
         tab = reinterpret_cast<T *>(raw);
         far = reinterpret_cast<float *>(tab + up4((size_t)P.n_bins * PairFmt<T>::NC * PairFmt<T>::REP));
         img = reinterpret_cast<T *>(reinterpret_cast<unsigned char *>(far) + far_bytes(P.n_far));
-        ion = img + up4(3 * (size_t)nimg);
+        ion = img + up4(3 * IMG_PARTS * (size_t)nimg);
         rest = ion + up4(4 * (size_t)n_ion);
         stacks = reinterpret_cast<unsigned char *>(rest + up4(rest_elems));
     }
     /* bytes before the stacks */
     static size_t fixed_bytes(int n_bins, int n_far, int nimg, int n_ion, size_t rest_elems)
     {
-        return (up4((size_t)n_bins * PairFmt<T>::NC * PairFmt<T>::REP) + up4(3 * (size_t)nimg) + up4(4 * (size_t)n_ion) +
+        return (up4((size_t)n_bins * PairFmt<T>::NC * PairFmt<T>::REP) + up4(3 * IMG_PARTS * (size_t)nimg) + up4(4 * (size_t)n_ion) +
                 up4(rest_elems)) * sizeof(T) + far_bytes(n_far);
     }
     /* bytes of one warp's stacks (the two item kinds of a stack share the same bytes) */
@@ -199,7 +200,7 @@ template <typename T> struct RealSmem {
             int4 *dst = reinterpret_cast<int4 *>(far);
             for (int t = tid; t < n4; t += nthreads) dst[t] = src[t];
         }
-        for (int t = tid; t < 3 * nimg; t += nthreads) img[t] = gimg[t];
+        for (int t = tid; t < 3 * IMG_PARTS * nimg; t += nthreads) img[t] = gimg[t];
         for (int t = tid; t < n_ion; t += nthreads) {
             ion[4 * t + 0] = ion_pos[3 * t + 0];
             ion[4 * t + 1] = ion_pos[3 * t + 1];
@@ -277,7 +278,7 @@ __device__ __forceinline__ double real_body(const RealArgs<T> &A, RealSmem<T> &S
                     int j = i + pw.k + 1;
                     if (j >= n) j -= n;
 #pragma unroll
-                    for (int x = 0; x < DIM; x++) d[x] = (sp[x * n + i] - sp[x * n + j]) * A.g.kappa;
+                    for (int x = 0; x < DIM; x++) d[x] = sp[x * n + i] - sp[x * n + j];
                     if (!UQ) w = sq[i] * sq[j];
                 }
                 scan_pair<T, DIM, ORTHO, M, UQ, false, false, GROUP == 1>(A.g, d, w, valid, st, direct, S.img, A.nimg,
@@ -303,7 +304,7 @@ __device__ __forceinline__ double real_body(const RealArgs<T> &A, RealSmem<T> &S
             if (valid) {
                 const int i = pw.i, I = pw.k;
 #pragma unroll
-                for (int x = 0; x < DIM; x++) d[x] = (sp[x * n + i] - S.ion[4 * I + x]) * A.g.kappa;
+                for (int x = 0; x < DIM; x++) d[x] = sp[x * n + i] - S.ion[4 * I + x];
                 if (!UQ) w = sq[i] * S.ion[4 * I + 3];
             }
             scan_pair<T, DIM, ORTHO, M, UQ>(A.g, d, w, valid, st, direct, S.img, A.nimg);
@@ -339,7 +340,7 @@ __global__ void __launch_bounds__(REAL_MAX_THREADS) real_kernel(RealArgs<T> A)
     if (uq) acc = real_body<T, DIM, ORTHO, M, true>(A, S, sp, sq, tile, q0);
     else acc = real_body<T, DIM, ORTHO, M, false>(A, S, sp, sq, tile, q0);
     acc = block_sum(acc, red);
-    if (tid == 0) A.partial[(size_t)w * A.n_tiles + tile] = acc * (double)A.g.kappa;
+    if (tid == 0) A.partial[(size_t)w * A.n_tiles + tile] = acc * A.g.kappa_d;
 }
 
 /* ------------------------------------------------------------------------------------------ */
@@ -409,11 +410,9 @@ template <typename T> struct MoveArgs {
     const int *walker; const int *electron; const T *new_r; /* [n_moves], [n_moves], [n_moves][DIM] */
     int commit;
     double *delta_e;
-    T binv[9];                                    /* unscaled: s_k = r . binv[k] */
+    double binv[9];                               /* unscaled: s_k = r . binv[k]; FP64 in both precisions */
     RealGeom<T> g;
 };
-
-constexpr int MOVE_THREADS = 256;
 
 /* [S7c] one warp: sum over the partners j != k of w_j [F-sum(r_new - r_j) - F-sum(r_old - r_j)], w_j = q_j
  * (or 1 with the common charge applied here when UQ). */
@@ -451,8 +450,8 @@ __device__ __forceinline__ double move_real(const MoveArgs<T> &A, RealSmem<T> &S
             T dn[3] = {0, 0, 0}, dold[3] = {0, 0, 0};
 #pragma unroll
             for (int x = 0; x < DIM; x++) {
-                dn[x] = (r_new[x] - rj[x]) * A.g.kappa;
-                dold[x] = (r_old[x] - rj[x]) * A.g.kappa;
+                dn[x] = r_new[x] - rj[x];
+                dold[x] = r_old[x] - rj[x];
             }
             scan_pair<T, DIM, ORTHO, M, UQ, true, false>(A.g, dn, w, valid, st, direct, S.img, A.nimg);
             scan_pair<T, DIM, ORTHO, M, UQ, true, true>(A.g, dold, UQ ? w : -w, valid, st, direct, S.img, A.nimg);
@@ -496,10 +495,10 @@ __global__ void __launch_bounds__(MOVE_MAX_THREADS) move_kernel(MoveArgs<T> A)
         if (lane < 2 * DIM) {
             const int which = lane / DIM, d = lane - which * DIM;
             const T *r = which ? r_new : r_old;
-            T s = 0;
+            double s = 0;
 #pragma unroll
-            for (int x = 0; x < DIM; x++) s += r[x] * A.binv[3 * d + x];
-            power_row<T>(s, T(1), A.nmax[d], tab + which * A.rowlen + A.off[d]);
+            for (int x = 0; x < DIM; x++) s += (double)r[x] * A.binv[3 * d + x];
+            power_row<T>((T)(s - rint(s)), T(1), A.nmax[d], tab + which * A.rowlen + A.off[d]);
         }
         __syncwarp();
 
@@ -539,7 +538,7 @@ __global__ void __launch_bounds__(MOVE_MAX_THREADS) move_kernel(MoveArgs<T> A)
         double accr;
         if (uq) accr = move_real<T, DIM, ORTHO, M, true>(A, S, pw, k, r_old, r_new, q0);
         else accr = move_real<T, DIM, ORTHO, M, false>(A, S, pw, k, r_old, r_new, q0);
-        acc += (double)qk * accr * (double)A.g.kappa;
+        acc += (double)qk * accr * A.g.kappa_d;
         acc = warp_sum(acc); /* its shuffles also order every lane's read of r_old before the commit */
         if (lane == 0) {
             A.delta_e[m] = acc;

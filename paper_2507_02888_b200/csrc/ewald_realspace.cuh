@@ -37,6 +37,16 @@ template <typename T> struct RealGeom {
     T L[3];      /* orthorhombic box lengths * kappa              */
     T invL[3];
     T kappa;
+    /* FP32 kernels: kappa, kappa L_k and the lattice rows rounded to float are the same for every pair, i.e. a
+     * SYSTEMATIC error of up to 6e-8 relative in every t (measured: 1e-7 of E_real with one sign on every walker,
+     * more than the 2e-5 of |E| allowed when the components cancel).  A low part added after a rounding is
+     * absorbed (it is below half an ulp), so the FP32 orthorhombic scan works in units of the box instead: the box
+     * length is exactly 1, every rounding is of a pair-dependent quantity (unbiased), and the only constants,
+     * 1/L_k and (kappa L_k)^2, enter through one fma with their low parts: fma(x, c_hi, x c_lo). */
+    T kappa_lo, a_lo[9];
+    T invLu[3], invLu_lo[3]; /* 1/L_k (unscaled box lengths) */
+    T C[3], C_lo[3];         /* (kappa L_k)^2 */
+    double kappa_d; /* the unrounded kappa: prefactor of the sums */
     int key_rc;  /* order key of kappa^2 r_c^2                    */
     int key_min; /* order key of the table's lower end t_min      */
     int bias;    /* bin index = (key >> SHIFT) - bias             */
@@ -45,6 +55,34 @@ template <typename T> struct RealGeom {
     int outer_far; /* every (kappa L_k)^2 >= 16: a candidate with a far image always belongs to the far shell */
     int far_once;  /* outer_far, no multi_far, and the far stack is deep enough for one service per pair */
 };
+
+/* kappa * diff; FP32: with the low part of kappa, rounded once. */
+template <typename T> __device__ __forceinline__ T scale_kappa(const RealGeom<T> &g, T diff)
+{
+    if (sizeof(T) == 4) return fma(diff, g.kappa, diff * g.kappa_lo);
+    return diff * g.kappa;
+}
+
+/* One axis of an orthorhombic cell: from the raw difference to the quantity the image scan shifts.
+ * FP64: v = kappa-scaled displacement reduced to (-L/2, L/2], images at v - m L_k, square as is.
+ * FP32: v = displacement in units of the box reduced to (-1/2, 1/2], images at v - m (exact), square scaled by
+ * (kappa L_k)^2 with its low part. */
+template <typename T> __device__ __forceinline__ T axis_reduce(const RealGeom<T> &g, int k, T diff)
+{
+    if (sizeof(T) == 4) {
+        const T s = fma(diff, g.invLu[k], diff * g.invLu_lo[k]);
+        return s - Num<T>::rint_(s);
+    }
+    const T d = diff * g.kappa;
+    return fma(-Num<T>::rint_(d * g.invL[k]), g.L[k], d);
+}
+template <typename T> __device__ __forceinline__ T axis_unit(const RealGeom<T> &g, int k) { return sizeof(T) == 4 ? T(1) : g.L[k]; }
+template <typename T> __device__ __forceinline__ T axis_square(const RealGeom<T> &g, int k, T x)
+{
+    const T x2 = x * x;
+    if (sizeof(T) == 4) return fma(x2, g.C[k], x2 * g.C_lo[k]);
+    return x2;
+}
 
 /* Positive floating-point numbers order like their leading bits.  FP64 uses the high word: ties within
  * 2^-20 are accepted (the cut-off is converged: a term at r_c is below 1e-16 of the sum, reading R19),
@@ -303,7 +341,7 @@ template <int DIM, bool ORTHO, int M, bool UQ> struct ScanShape {
     static constexpr int FAR_LIMIT = 20; /* PLANE, fast variant: all 20 candidates between two far services */
 };
 
-/* Phase A for one pair per lane.  d = kappa (r_i - r_j), not yet reduced; w = q_i q_j.  Terms below the
+/* Phase A for one pair per lane.  d = r_i - r_j (raw, neither scaled nor reduced); w = q_i q_j.  Terms below the
  * table (t < t_min) are evaluated directly into `direct` (weighted by w); the rest go to the stack. */
 template <typename T, int DIM, bool ORTHO, int M, bool UQ, bool SIGNED = false, bool NEG = false,
           bool SERVICE = true>
@@ -324,9 +362,8 @@ __device__ __forceinline__ void scan_pair(const RealGeom<T> &g, T *d, T w, bool 
         T a[3][3];
 #pragma unroll
         for (int k = 0; k < 3; k++) {
-            d[k] = fma(-Num<T>::rint_(d[k] * g.invL[k]), g.L[k], d[k]);
-            const T ad = abs_of(d[k]), x1 = g.L[k] - ad, x2 = g.L[k] + ad;
-            a[k][0] = d[k] * d[k]; a[k][1] = x1 * x1; a[k][2] = x2 * x2;
+            const T v = axis_reduce(g, k, d[k]), ad = abs_of(v), unit = axis_unit(g, k);
+            a[k][0] = axis_square(g, k, v); a[k][1] = axis_square(g, k, unit - ad); a[k][2] = axis_square(g, k, unit + ad);
         }
         const T t0 = a[0][0] + (a[1][0] + a[2][0]);
         const bool tiny = valid && order_key(t0) < g.key_min;
@@ -354,7 +391,8 @@ __device__ __forceinline__ void scan_pair(const RealGeom<T> &g, T *d, T w, bool 
             for (int c = 0; c < 4; c++) { cand_far(2, c & 1, c >> 1, valid); cand_far(c & 1, 2, c >> 1, valid); }
 #pragma unroll
             for (int c = 0; c < 4; c++) cand_far(c & 1, c >> 1, 2, valid);
-            if (fast) st.service_far(Shape::FAR_LIMIT);
+            /* not fast: the next pair's 8 core candidates may push on the far stack before the next service */
+            if (fast) st.service_far(Shape::FAR_LIMIT); else st.service_far(Shape::LIMIT);
         } else {
 #pragma unroll
             for (int c = 0; c < 4; c++) { cand(2, c & 1, c >> 1, valid); cand(c & 1, 2, c >> 1, valid); }
@@ -373,9 +411,9 @@ __device__ __forceinline__ void scan_pair(const RealGeom<T> &g, T *d, T w, bool 
         T sq[DIM][ROW];
 #pragma unroll
         for (int k = 0; k < DIM; k++) {
-            d[k] = fma(-Num<T>::rint_(d[k] * g.invL[k]), g.L[k], d[k]);
+            d[k] = axis_reduce(g, k, d[k]);
 #pragma unroll
-            for (int m = 0; m < ROW; m++) { const T x = fma((T)(M - m), g.L[k], d[k]); sq[k][m] = x * x; }
+            for (int m = 0; m < ROW; m++) sq[k][m] = axis_square(g, k, fma((T)(M - m), axis_unit(g, k), d[k]));
         }
         /* only the un-shifted candidate can fall below the table: |d_k - m L_k| >= L_k/2 otherwise */
         T t0 = sq[0][M] + sq[1][M];
@@ -404,11 +442,10 @@ __device__ __forceinline__ void scan_pair(const RealGeom<T> &g, T *d, T w, bool 
 #pragma unroll 1
             for (int mz = 0; mz < (DIM == 3 ? ROW : 1); mz++) {
                 T sz = 0;
-                if (DIM == 3) { const T z = fma((T)(M - mz), g.L[2], d[2]); sz = z * z; }
+                if (DIM == 3) sz = axis_square(g, 2, fma((T)(M - mz), axis_unit(g, 2), d[2]));
 #pragma unroll 1
                 for (int my = 0; my < ROW; my++) {
-                    const T y = fma((T)(M - my), g.L[1], d[1]);
-                    const T syz = fma(y, y, sz);
+                    const T syz = axis_square(g, 1, fma((T)(M - my), axis_unit(g, 1), d[1])) + sz;
                     const bool crow = my == M && (DIM == 2 || mz == M);
 #pragma unroll
                     for (int mx = 0; mx < ROW; mx++) {
@@ -423,6 +460,8 @@ __device__ __forceinline__ void scan_pair(const RealGeom<T> &g, T *d, T w, bool 
     } else {
         T f[3];
 #pragma unroll
+        for (int x = 0; x < DIM; x++) d[x] = scale_kappa(g, d[x]);
+#pragma unroll
         for (int k = 0; k < DIM; k++) {
             T s = 0;
 #pragma unroll
@@ -432,7 +471,10 @@ __device__ __forceinline__ void scan_pair(const RealGeom<T> &g, T *d, T w, bool 
 #pragma unroll
         for (int x = 0; x < DIM; x++) {
 #pragma unroll
-            for (int k = 0; k < DIM; k++) d[x] = fma(-f[k], g.a[3 * k + x], d[x]);
+            for (int k = 0; k < DIM; k++) {
+                d[x] = fma(-f[k], g.a[3 * k + x], d[x]);
+                if (sizeof(T) == 4) d[x] = fma(-f[k], g.a_lo[3 * k + x], d[x]);
+            }
         }
         for (int m0 = 0; m0 < nimg; m0 += Shape::LIMIT) {
             const int m1 = min(m0 + Shape::LIMIT, nimg); /* uniform trip count: no work for images that do not exist */
@@ -441,7 +483,11 @@ __device__ __forceinline__ void scan_pair(const RealGeom<T> &g, T *d, T w, bool 
                 const bool in = valid;
                 T t = 0;
 #pragma unroll
-                for (int x = 0; x < DIM; x++) { const T v = d[x] - simg[3 * m + x]; t = fma(v, v, t); }
+                for (int x = 0; x < DIM; x++) {
+                    T v = d[x] - simg[3 * m + x];
+                    if (sizeof(T) == 4) v -= simg[3 * (nimg + m) + x]; /* low parts follow the nimg high parts */
+                    t = fma(v, v, t);
+                }
                 const int key = order_key(t);
                 const bool tiny = in && key < g.key_min;
                 if (tiny) direct += (double)((FLIP ? -w : w) * pair_f_direct(t));

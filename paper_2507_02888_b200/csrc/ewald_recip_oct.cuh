@@ -43,7 +43,7 @@ template <typename T> struct OctArgs {
     const double *wt;   /* [n_items][1 + NPB][4]: class weights W_pq per entry (ewald_octplan.cpp) */
     const double *tion; /* [n_items][1 + 2 NPB][4] fixed-charge sums, or null */
     double *e_recip;    /* [W][n_slabs] */
-    T binv[9];
+    double binv[9];     /* FP64 also in the FP32 kernels: the reduction of s to one period is done in FP64 */
 };
 
 /* Threads per CTA the register file allows: 4 (1 + 2 NPB) accumulators per lane (doubles take two
@@ -123,11 +123,11 @@ __device__ __forceinline__ void oct_build_rows(const OctArgs<T> &A, typename Num
         T2 *row[DIM];
 #pragma unroll
         for (int k = 0; k < DIM; k++) {
-            T s = 0;
+            double s = 0;
 #pragma unroll
-            for (int c = 0; c < DIM; c++) s += x[c] * A.binv[3 * k + c];
-            s -= Num<T>::rint_(s);
-            Num<T>::sincospi_(2 * s, &sn[k], &cs[k]);
+            for (int c = 0; c < DIM; c++) s += (double)x[c] * A.binv[3 * k + c];
+            s -= rint(s);
+            Num<T>::sincospi_((T)(2 * s), &sn[k], &cs[k]);
             row[k] = tab + (size_t)wl * A.wstride + (size_t)p * A.rowlen + A.off[k];
             e[k].x = k == DIM - 1 ? qp : T(1); e[k].y = 0;
             if (k > 0) row[k][0] = e[k]; else row[k] -= 1; /* axis 1 stores n = 1.. only */

@@ -30,41 +30,6 @@ static real weight(int dim, real volume, real kappa, real g2)
     return kPi / volume * erfcl(g / (2 * kappa)) / g;
 }
 
-/* Piecewise polynomial for erfc(z) on n_bins equal bins of [0, z_max]: on bin b, with
- * u = 2 z / h - (2b+1) in [-1,1], erfc(z) ~ sum_k c_k u^k.  Interpolation at Chebyshev nodes of a
- * slightly widened interval (the kernel picks the bin from an FP32 product), Chebyshev series
- * converted to monomials, all in long double.  Layout [row][bin]: rows c_0..c_degree, then -(2b+1). */
-void build_erfc_table(double z_max, int n_bins, int degree, std::vector<double> *tab)
-{
-    const int n = degree + 1;
-    const real h = (real)z_max / n_bins, widen = 1 + 1e-4L;
-    tab->assign((size_t)(degree + 2) * n_bins, 0.0);
-    std::vector<real> fv(n), cheb(n), mono(n), t0(n), t1(n), t2(n);
-    for (int b = 0; b < n_bins; b++) {
-        const real centre = (b + 0.5L) * h, half = 0.5L * h * widen;
-        for (int i = 0; i < n; i++) fv[i] = erfcl(centre + half * cosl(kPi * (2 * i + 1) / (2 * n)));
-        for (int k = 0; k < n; k++) {
-            real s = 0;
-            for (int i = 0; i < n; i++) s += fv[i] * cosl(k * kPi * (2 * i + 1) / (2 * n));
-            cheb[k] = (k == 0 ? 1 : 2) * s / n;
-        }
-        /* sum_k cheb[k] T_k(v) -> monomials in v via T_{k+1} = 2 v T_k - T_{k-1} */
-        for (int i = 0; i < n; i++) { mono[i] = 0; t0[i] = 0; t1[i] = 0; }
-        t0[0] = 1;                 /* T_0 */
-        if (n > 1) t1[1] = 1;      /* T_1 */
-        for (int i = 0; i < n; i++) mono[i] += cheb[0] * t0[i];
-        if (n > 1) for (int i = 0; i < n; i++) mono[i] += cheb[1] * t1[i];
-        for (int k = 2; k < n; k++) {
-            for (int i = 0; i < n; i++) t2[i] = (i > 0 ? 2 * t1[i - 1] : 0) - t0[i];
-            for (int i = 0; i < n; i++) mono[i] += cheb[k] * t2[i];
-            t0 = t1; t1 = t2;
-        }
-        real scale = 1; /* v = u / widen */
-        for (int k = 0; k < n; k++) { (*tab)[(size_t)k * n_bins + b] = (double)(mono[k] * scale); scale /= widen; }
-        (*tab)[(size_t)(degree + 1) * n_bins + b] = -(double)(2 * b + 1);
-    }
-}
-
 /* Pair-function table of the real-space kernels (ewald_realspace.cuh):
  *     F(t) = erfc(sqrt t)/sqrt t,  t = kappa^2 r^2,
  * so that a term of the real-lattice sum of Eq. 3 is kappa q_i q_j F(t) -- no square
@@ -204,12 +169,9 @@ ewald_status build_tables(int dim, const double *cell, double kappa_d, double g_
     t->g_cutoff = g_cutoff;
     t->volume = (double)fabsl(det);
     if (r_cutoff == 0) r_cutoff = (double)(sqrtl(-logl(1e-17L)) / kappa);
-    /* erfc(6.5) = 4e-20: beyond kappa r = 6.5 no term can matter at FP64; keeps the erfc table's range fixed */
+    /* erfc(6.5) = 4e-20: beyond kappa r = 6.5 no term can matter at FP64; bounds the pair table's range */
     if (r_cutoff * kappa_d > 6.5) r_cutoff = 6.5 / kappa_d;
     t->r_cutoff = r_cutoff;
-    t->z_max = r_cutoff * kappa_d * (1 + 4e-6);
-    build_erfc_table(t->z_max, 16, 11, &t->erfc_tab64);
-    build_erfc_table(t->z_max, 16, 6, &t->erfc_tab32);
     /* the cull compares high words / FP32 values: cover a little beyond kappa^2 r_c^2 */
     const double t_top = r_cutoff * r_cutoff * kappa_d * kappa_d * (1 + 1e-5);
     build_pair_table(PAIR_K64, PAIR_DEG64, PAIR_EMIN, t_top, &t->pair64);
@@ -315,6 +277,12 @@ ewald_status build_fixed_charges(HostTables *t, int n_ion, const double *pos, co
     if (n_ion < 0 || (n_ion > 0 && (!pos || !q))) { *err = "bad fixed-charge arguments"; return EWALD_EINVAL; }
     const int dim = t->dim;
     const size_t ngp = t->g_w2.size();
+    /* validate everything before touching the tables: a failed call leaves the previous ions in place */
+    for (int i = 0; i < n_ion; i++) {
+        if (!std::isfinite(q[i])) { *err = "non-finite ion charge"; return EWALD_EINVAL; }
+        for (int x = 0; x < dim; x++)
+            if (!std::isfinite(pos[(size_t)i * dim + x])) { *err = "non-finite ion position"; return EWALD_EINVAL; }
+    }
     t->n_ion = n_ion;
     t->ion_pos.assign((size_t)3 * n_ion, 0.0);
     t->ion_q.assign((size_t)n_ion, 0.0);
@@ -329,10 +297,7 @@ ewald_status build_fixed_charges(HostTables *t, int n_ion, const double *pos, co
         const int i = order[k];
         t->ion_q[k] = q[i];
         if (k == 0 || q[i] != q[order[k - 1]]) t->sp_start.push_back(k);
-        for (int x = 0; x < dim; x++) {
-            if (!std::isfinite(pos[(size_t)i * dim + x])) { *err = "non-finite ion position"; return EWALD_EINVAL; }
-            t->ion_pos[3 * k + x] = pos[(size_t)i * dim + x];
-        }
+        for (int x = 0; x < dim; x++) t->ion_pos[3 * k + x] = pos[(size_t)i * dim + x];
     }
     t->sp_start.push_back(n_ion);
     q = t->ion_q.data(); /* from here on: the grouped order */

@@ -2,11 +2,13 @@
 seeded inputs (paper_2507_02888_b200.workloads).  Tolerances are BASELINE.json's: 1e-11 relative
 per walker (FP64), 2e-5 (FP32); Delta E per reading R12: tol * max(|dE|, rms dE of the step).
 
-FP32 (reading R16): the FP32 path receives the seeded positions rounded to float32, and the
-oracle is evaluated on exactly those rounded values (they are representable in FP64), i.e. both sides see
-the same inputs.  Rounding the inputs alone moves the energy of a walker with a close pair by more than
-2e-5 (measured 6.4e-5 on config 3), so a comparison on unrounded inputs would test the rounding of the
-input, not the kernels.
+FP32 (reading R16): the FP32 entry points take float32 positions, so the caller rounds the seeded
+FP64 positions.  Two comparisons are made and both are reported:
+  * against the oracle on exactly the rounded values (representable in FP64): both sides see the same inputs;
+    this isolates the kernels' own FP32 arithmetic and is asserted at 2e-5 everywhere;
+  * against the oracle on the UNROUNDED seeded inputs (SURVEY reading 16): measured per config by
+    test_fp32_against_oracle_on_unrounded_inputs, printed, and asserted against the bound DESIGN.md R16 states
+    for each config (the rounding of a close pair's coordinates to 2^-24 L dominates it, not the kernels).
 """
 import math
 
@@ -283,8 +285,7 @@ def test_uniform_charges_cutoff_reaching_two_far_images(torch_cuda):
             d_de = torch_cuda.zeros(4, dtype=torch_cuda.float64, device="cuda")
             E.ewald_move_delta_batch(ctx, d_w, torch_cuda.from_numpy(electron[s_]).cuda(),
                                      torch_cuda.from_numpy(new_r[s_]).cuda(), 1, d_de)
-            de = d_de.cpu().numpy()
-            assert (np.abs(de - de_ref[s_]) / np.maximum(np.abs(de_ref[s_]), scale)).max() <= TOL64
+            _assert_delta(d_de.cpu().numpy()[None, :], de_ref[s_][None, :], TOL64, 1e-3 * scale)
 
 
 @pytest.mark.parametrize("mixed", [False, True])
@@ -322,8 +323,7 @@ def test_cubic_cell_two_ion_species_energies_and_moves(torch_cuda, mixed):
         d_de = torch_cuda.zeros(4, dtype=torch_cuda.float64, device="cuda")
         E.ewald_move_delta_batch(ctx, d_w, torch_cuda.from_numpy(electron[s_]).cuda(),
                                  torch_cuda.from_numpy(new_r[s_]).cuda(), 1, d_de)
-        de = d_de.cpu().numpy()
-        assert (np.abs(de - de_ref[s_]) / np.maximum(np.abs(de_ref[s_]), scale)).max() <= TOL64
+        _assert_delta(d_de.cpu().numpy()[None, :], de_ref[s_][None, :], TOL64, 1e-3 * scale)
 
 
 def test_fixed_charges_equal_mobile_charges(torch_cuda):
@@ -394,10 +394,14 @@ def _run_moves(torch, ctx, w, pos0, electron, new_r, dtype):
     return de
 
 
-def _assert_delta(de, de_ref, tol):
+def _assert_delta(de, de_ref, tol, floor=0.0):
+    """Reading R12: |dE - dE_ref| <= tol * max(|dE_ref|, rms of dE_ref over the step's batch).  `floor` guards the
+    degenerate small systems only (a lone particle in a periodic cell has dE = 0 exactly): it is 1e-3 of the
+    walker's largest energy component there, i.e. an absolute error of 1e-14 of that component at FP64."""
     rms = np.sqrt((de_ref ** 2).mean(axis=1, keepdims=True))
-    err = np.abs(de - de_ref) / np.maximum(np.abs(de_ref), rms)
+    err = np.abs(de - de_ref) / np.maximum(np.maximum(np.abs(de_ref), rms), floor)
     assert err.max() <= tol, "max Delta-E error %.3e > %.1e" % (err.max(), tol)
+    return float(err.max())
 
 
 @pytest.mark.parametrize("dtype,tol", [("f64", TOL64), ("f32", TOL32)])
@@ -486,20 +490,32 @@ def test_state_errors(torch_cuda):
     assert np.array_equal(E.ewald_get_rho(ctx, 1), before)
 
 
+N_SAMPLE = 256   # walkers the oracle checks one by one in the full-size tests (>= 256)
+
+
+def _sample(n_walkers, k=N_SAMPLE, seed=2):
+    """First, last and k - 2 seeded-random other walkers."""
+    rng = np.random.default_rng(seed)
+    mid = rng.choice(np.arange(1, n_walkers - 1), size=min(k, n_walkers) - 2, replace=False)
+    return np.sort(np.concatenate([[0, n_walkers - 1], mid]))
+
+
 def test_full_size_config2_sampled_walkers(torch_cuda):
     """BASELINE configs[1] at its full size (1024 walkers), in the launch configuration bench.py
-    times; the oracle checks a sample of walkers one by one."""
+    times; the oracle checks 256 walkers one by one, FP64 and FP32."""
     w = workloads.config(2)
     pos = w.positions()
     ctx = _ctx(w)
-    sample = np.array([0, 1, 511, 777, 1023])
+    sample = _sample(w.n_walkers)
     for dtype, tol in (("f64", TOL64), ("f32", TOL32)):
         if dtype == "f32":
             pos = _r32(pos)
         e_ref, _ = _oracle_energy(w, pos[sample])
         e, _ = _gpu_energy(torch_cuda, ctx, pos, w.charges, dtype, components=False)
         assert np.all(np.isfinite(e))
-        assert (np.abs(e[sample] - e_ref) / np.abs(e_ref)).max() <= tol
+        rel = np.abs(e[sample] - e_ref) / np.abs(e_ref)
+        print("config 2 %s: max rel err over %d walkers %.3e" % (dtype, len(sample), rel.max()))
+        assert rel.max() <= tol
         # property that holds at any size: identical walkers give identical energies
         e2, _ = _gpu_energy(torch_cuda, ctx, pos[::-1].copy(), w.charges, dtype, components=False)
         assert np.array_equal(e2[::-1], e)
@@ -508,36 +524,112 @@ def test_full_size_config2_sampled_walkers(torch_cuda):
 @pytest.mark.parametrize("idx", [3, 4])
 def test_full_size_configs_3_and_4_sampled_walkers(torch_cuda, idx):
     """BASELINE configs[2] and configs[3] at their full sizes (1024 / 4096 walkers), in the launch
-    configuration bench.py --config 3 / 4 times; the oracle checks a sample of walkers one by one."""
+    configuration bench.py --config 3 / 4 times; the oracle checks 256 walkers one by one (FP64; FP32: 64)."""
     w = workloads.config(idx)
     pos = w.positions()
     ctx = _ctx(w)
-    sample = np.array([0, 1, w.n_walkers // 2 + 3, w.n_walkers - 1])
-    for dtype, tol in (("f64", TOL64), ("f32", TOL32)):
+    for dtype, tol, k in (("f64", TOL64, N_SAMPLE), ("f32", TOL32, 64)):
+        sample = _sample(w.n_walkers, k)
         p = pos if dtype == "f64" else _r32(pos)
         e_ref, _ = _oracle_energy(w, p[sample])
         e, _ = _gpu_energy(torch_cuda, ctx, p, w.charges, dtype, components=False)
         assert np.all(np.isfinite(e))
-        assert (np.abs(e[sample] - e_ref) / np.abs(e_ref)).max() <= tol
+        rel = np.abs(e[sample] - e_ref) / np.abs(e_ref)
+        print("config %d %s: max rel err over %d walkers %.3e" % (idx, dtype, len(sample), rel.max()))
+        assert rel.max() <= tol
 
 
-def test_full_size_config5_moves_sampled_walkers(torch_cuda):
-    """BASELINE configs[4] at its full size: 4096 walkers with stored rho(G), batches of 4096 committed moves
-    (the launch configuration bench.py times), 6 steps; walkers are independent, so the oracle runs the
-    chains of a sample of walkers and compares their Delta E, final rho(G) and positions."""
+# Bound on the error of the stored FP32 rho(G) after 100 patches, in units of N (DESIGN.md R16).  The loaded rho is
+# an FP32 sum of N unit phasors (|rho| ~ sqrt N, error a few ulps); each patch adds q delta(G) (|delta| <= 2) and
+# rounds to 2^-24 |rho| ~ 2e-6 at N = 1000: 100 patches random-walk to ~ 2e-5, the worst of 1979 G-vectors to
+# ~ 1e-4 absolute = 1e-7 N.  Asserted with a factor 3 of margin; the measured value is printed.
+RHO32_DRIFT = 3e-7
+
+
+@pytest.mark.parametrize("dtype,tol", [("f64", TOL64), ("f32", TOL32)])
+def test_full_size_config5_100_steps(torch_cuda, dtype, tol):
+    """BASELINE configs[4] at its stated size: 4096 walkers with stored rho(G), 100 committed steps per walker in
+    batches of 4096 moves (the launch configuration bench.py times), FP64 and FP32.  Walkers are independent, so
+    the oracle runs the 100-step chains of 16 sampled walkers: Delta E of every step, final rho(G) and final
+    positions; and sum Delta E + E_0 is checked against a fresh ewald_energy_batch of the final configuration
+    for ALL walkers (with the oracle's energies on the sample)."""
     w = workloads.config(5)
-    W, S = w.n_walkers, 6
+    W, S = w.n_walkers, w.n_steps
+    assert (W, S) == (4096, 100)
     pos0, electron, new_r, final = _move_inputs(w, W, S)
+    if dtype == "f32":
+        pos0, new_r, final = _r32(pos0), _r32(new_r), _r32(final)
     ctx = _ctx(w)
-    de = _run_moves(torch_cuda, ctx, w, pos0, electron, new_r, "f64")
+    de = _run_moves(torch_cuda, ctx, w, pos0, electron, new_r, dtype)
     assert np.all(np.isfinite(de))
-    sample = np.array([0, 2047, 4095])
+    sample = _sample(W, 16, seed=5)
     de_ref, pos_ref, rho_ref = ref.move_chain(w.dim, w.cell, w.kappa, w.g_cutoff, w.r_cutoff, pos0[sample],
                                               w.charges, electron[:, sample], new_r[:, sample], want_rho=True)
-    _assert_delta(de[:, sample], de_ref, TOL64)
+    err = _assert_delta(de[:, sample], de_ref, tol)
+    drift = 0.0
     for k, wk in enumerate(sample):
-        assert np.abs(E.ewald_get_rho(ctx, int(wk)) - rho_ref[k]).max() <= 1e-12 * w.n
+        d = np.abs(E.ewald_get_rho(ctx, int(wk)) - rho_ref[k]).max() / w.n
+        drift = max(drift, d)
         assert np.abs(E.ewald_get_positions(ctx, int(wk), w.n) - final[wk]).max() == 0
+    print("config 5 %s: max Delta-E error (R12) %.3e over 16 walkers x 100 steps; stored rho drift %.3e N"
+          % (dtype, err, drift))
+    assert drift <= (1e-12 if dtype == "f64" else RHO32_DRIFT)
+    # sum of the steps + E_0 = energy of the final configuration (all 4096 walkers, GPU; oracle on the sample)
+    e0, _ = _gpu_energy(torch_cuda, ctx, pos0, w.charges, dtype, components=False)
+    e1, _ = _gpu_energy(torch_cuda, ctx, final, w.charges, dtype, components=False)
+    closure = np.abs(e0 + de.sum(axis=0) - e1) / np.abs(e1)
+    e1_ref, _ = _oracle_energy(w, final[sample])
+    print("config 5 %s: closure |E0 + sum dE - E1|/|E1| max %.3e; E1 vs oracle %.3e"
+          % (dtype, closure.max(), (np.abs(e1[sample] - e1_ref) / np.abs(e1_ref)).max()))
+    assert (np.abs(e1[sample] - e1_ref) / np.abs(e1_ref)).max() <= tol
+    # 100 steps each within tol * max(|dE|, rms dE) of the oracle; the sum is compared at 10 tol of |E|
+    assert closure.max() <= 10 * tol
+
+
+# Measured bound of the FP32 path against the oracle on the UNROUNDED seeded inputs (DESIGN.md R16): the kernels'
+# own error (<= 2e-5, asserted everywhere else on the rounded inputs) plus the effect of rounding the coordinates
+# to float32 (half an ulp of up to L: 2^-25 L), which a close pair amplifies by L / r_min.
+FP32_UNROUNDED_BOUND = {1: 2e-5, 2: 2e-5, 3: 2e-4, 4: 2e-5, 5: 2e-5}
+
+
+@pytest.mark.parametrize("idx", [1, 2, 3, 4, 5])
+def test_fp32_against_oracle_on_unrounded_inputs(torch_cuda, idx):
+    """SURVEY reading 16 as a measured diagnostic: FP32 path on float32(positions) against the oracle on the
+    unrounded FP64 positions, beside the same comparison on the rounded positions."""
+    w = workloads.config(idx)
+    nw = {1: 8, 2: 64, 3: 64, 4: 32, 5: 8}[idx]
+    pos = w.positions(nw)
+    e_un, _ = _oracle_energy(w, pos)
+    e_rd, _ = _oracle_energy(w, _r32(pos))
+    e, _ = _gpu_energy(torch_cuda, _ctx(w), pos, w.charges, "f32", components=False)   # to_soa rounds
+    rel_un = np.abs(e - e_un) / np.abs(e_un)
+    rel_rd = np.abs(e - e_rd) / np.abs(e_rd)
+    rel_in = np.abs(e_rd - e_un) / np.abs(e_un)
+    print("config %d FP32, %d walkers: vs oracle(unrounded) max %.3e | vs oracle(rounded) max %.3e | "
+          "input rounding alone (oracle vs oracle) max %.3e" % (idx, nw, rel_un.max(), rel_rd.max(), rel_in.max()))
+    assert rel_rd.max() <= TOL32
+    assert rel_un.max() <= FP32_UNROUNDED_BOUND[idx]
+
+
+def test_far_stack_headroom_n1000_wide_cutoff(torch_cuda):
+    """N = 1000 in FP64 leaves room for an 18-deep far stack only (outer_far without far_once): between two
+    services a lane can push 12 one-far candidates and then the next pair's 8 core candidates.  kappa L = 4.6 with
+    r_c = 6.5 / kappa fills the far shell as densely as the geometry allows (the far stack overflowed
+    into the next warp's near stack here)."""
+    n = 1000
+    L = (4.0 * math.pi * n / 3.0) ** (1.0 / 3.0)
+    cell = np.eye(3) * L
+    kappa = 4.6 / L
+    rc = 6.5 / kappa
+    gc = 2 * math.pi / L * math.sqrt(61) * (1 + 1e-9)
+    rng = np.random.default_rng(4600)
+    pos = rng.random((2, n, 3)) * L
+    q = -np.ones(n)
+    ctx = E.ewald_setup(3, cell, kappa, gc, rc)
+    e_ref, c_ref = ref.energy_batch(3, cell, kappa, gc, rc, pos, q)
+    e, c = _gpu_energy(torch_cuda, ctx, pos, q, "f64")
+    assert (np.abs(c[:, 1] - c_ref[:, 1]) / np.abs(c_ref[:, 1])).max() <= 1e-12
+    _assert_energy(e, c, e_ref, c_ref, TOL64)
 
 
 def test_largest_paper_system_n1630(torch_cuda):
@@ -640,8 +732,7 @@ def test_randomised_small_systems(torch_cuda, seed):
         d_de = torch_cuda.zeros(W, dtype=torch_cuda.float64, device="cuda")
         E.ewald_move_delta_batch(ctx, d_w, torch_cuda.from_numpy(electron[s_]).cuda(),
                                  torch_cuda.from_numpy(new_r[s_]).cuda(), commit, d_de)
-        de = d_de.cpu().numpy()
-        assert (np.abs(de - want) / np.maximum(np.abs(want), scale)).max() <= TOL64, (s_, seed)
+        _assert_delta(d_de.cpu().numpy()[None, :], want[None, :], TOL64, 1e-3 * scale)
 
 
 def test_translation_and_permutation_invariance_on_gpu(torch_cuda):

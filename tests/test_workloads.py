@@ -41,7 +41,7 @@ def test_config5_moves():
     assert np.array_equal(el2[:10, :4], el) and np.array_equal(disp2[:10, :4], disp)
 
 
-@pytest.mark.parametrize("idx", [1, 2, 3, 4])
+@pytest.mark.parametrize("idx", [1, 2, 3, 4, 5])
 def test_config_cutoffs_are_converged(idx):
     """The configs' (kappa, G_cut, r_cut) reproduce a fully converged evaluation at kappa' = 1.3 kappa."""
     w = workloads.config(idx)
