@@ -577,19 +577,29 @@ def test_full_size_config5_100_steps(torch_cuda, dtype, tol):
     # sum of the steps + E_0 = energy of the final configuration (all 4096 walkers, GPU; oracle on the sample)
     e0, _ = _gpu_energy(torch_cuda, ctx, pos0, w.charges, dtype, components=False)
     e1, _ = _gpu_energy(torch_cuda, ctx, final, w.charges, dtype, components=False)
-    closure = np.abs(e0 + de.sum(axis=0) - e1) / np.abs(e1)
+    # Denominators as in reading R12: uniform-random N = 1000 walkers have E between -2 and -180 Ha (close pairs)
+    # out of components of +-3300 Ha, so a walker's own |E| can be 1e-3 of what the arithmetic handles; FP64 keeps
+    # the per-walker |E| all the same.
     e1_ref, _ = _oracle_energy(w, final[sample])
-    print("config 5 %s: closure |E0 + sum dE - E1|/|E1| max %.3e; E1 vs oracle %.3e"
-          % (dtype, closure.max(), (np.abs(e1[sample] - e1_ref) / np.abs(e1_ref)).max()))
-    assert (np.abs(e1[sample] - e1_ref) / np.abs(e1_ref)).max() <= tol
-    # 100 steps each within tol * max(|dE|, rms dE) of the oracle; the sum is compared at 10 tol of |E|
+    rms = np.sqrt((e1_ref ** 2).mean())
+    den_all = np.abs(e1) if dtype == "f64" else np.maximum(np.abs(e1), rms)
+    den = np.abs(e1_ref) if dtype == "f64" else np.maximum(np.abs(e1_ref), rms)
+    closure = np.abs(e0 + de.sum(axis=0) - e1) / den_all
+    e1_err = np.abs(e1[sample] - e1_ref) / den
+    print("config 5 %s: closure |E0 + sum dE - E1| / den max %.3e; E1 vs oracle %.3e (per-walker |E|: %.3e)"
+          % (dtype, closure.max(), e1_err.max(), (np.abs(e1[sample] - e1_ref) / np.abs(e1_ref)).max()))
+    assert e1_err.max() <= tol
+    # 100 steps each within tol * max(|dE|, rms dE) of the oracle; the sum is compared at 10 tol
     assert closure.max() <= 10 * tol
 
 
 # Measured bound of the FP32 path against the oracle on the UNROUNDED seeded inputs (R16): the kernels'
 # own error (<= 2e-5, asserted everywhere else on the rounded inputs) plus the effect of rounding the coordinates
 # to float32 (half an ulp of up to L: 2^-25 L), which a close pair amplifies by L / r_min.
-FP32_UNROUNDED_BOUND = {1: 2e-5, 2: 2e-5, 3: 2e-4, 4: 2e-5, 5: 2e-5}
+# Config 3 (2D, L = 188 bohr, 450 particles): the closest pair of a walker sits at ~0.05 bohr while half an ulp of a
+# coordinate is 5.6e-6 bohr, so input rounding ALONE moves E by up to 4.2e-4 (oracle vs oracle, 64 walkers, printed);
+# the kernels' own error stays <= 2e-5.  The test asserts that the excess over the input-rounding effect is <= 2e-5.
+FP32_UNROUNDED_BOUND = {1: 2e-5, 2: 2e-5, 3: 1e-3, 4: 2e-5, 5: 2e-5}
 
 
 @pytest.mark.parametrize("idx", [1, 2, 3, 4, 5])
@@ -609,6 +619,7 @@ def test_fp32_against_oracle_on_unrounded_inputs(torch_cuda, idx):
           "input rounding alone (oracle vs oracle) max %.3e" % (idx, nw, rel_un.max(), rel_rd.max(), rel_in.max()))
     assert rel_rd.max() <= TOL32
     assert rel_un.max() <= FP32_UNROUNDED_BOUND[idx]
+    assert (rel_un - rel_in).max() <= TOL32   # what the kernels add on top of the caller's rounding
 
 
 def test_far_stack_headroom_n1000_wide_cutoff(torch_cuda):
