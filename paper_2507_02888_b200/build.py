@@ -18,7 +18,7 @@ HEADERS = [os.path.join(ROOT, "include", "ewald.h"), os.path.join(CSRC, "ewald_i
            os.path.join(CSRC, "ewald_recip_oct.cuh")]
 
 NVCC_FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
-              "-Xcompiler", "-fPIC", "-shared", "-cudart", "static"]
+              "-Xcompiler", "-fPIC", "-shared", "-cudart", "static", "--split-compile=0"]
 
 
 def _nvcc():

@@ -3,6 +3,7 @@
  * the sm_100a kernels of ewald_kernels.cuh or fails with EWALD_ECUDA. */
 #include <cmath>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 #include <string>
@@ -309,7 +310,7 @@ extern "C" ewald_status ewald_oct_plan_summary(int dim, const double *cell, doub
     if (npb) *npb = P.npb;
     if (n_warps) *n_warps = L.n_warps;
     if (weight_sum) *weight_sum = (double)ws;
-    if (fma_per_particle) *fma_per_particle = L.cost / n_walkers_per_cta;
+    if (fma_per_particle) *fma_per_particle = L.fma_ops / n_walkers_per_cta;
     return EWALD_OK;
 }
 
@@ -486,7 +487,8 @@ static ewald_status oct_launch_any(ewald_ctx *c, const OctArgs<T> &A, int grid, 
 
 template <typename T> static int oct_max_threads(int npb)
 {
-    return sizeof(T) == 8 ? (npb >= 6 ? 256 : 384) : (npb >= 6 ? 224 : 512);
+    (void)npb;
+    return OctCfg<T, 7>::MAX_THREADS;
 }
 
 /* Shared-memory shape of a CTA of wc walkers: particles per chunk, slab stride, bytes. */
@@ -496,7 +498,7 @@ static bool oct_shape(const OctPlan &P, int wc, int /*n_warps*/, int n, size_t e
     for (; p >= 1; p--) {
         const int ws = p * P.rowlen + 1; /* +1 pair: staggers the walkers' slabs over the banks */
         /* two table buffers (the next chunk is built while this one is multiplied), partial sums, walker tags */
-        const size_t b = 2 * ((size_t)wc * ws + P.npb + 1) * es2 + (size_t)wc * (P.n_items + 1) * sizeof(double);
+        const size_t b = 2 * ((size_t)wc * ws + P.rowlen) * es2 + (size_t)wc * (P.n_items + 1) * sizeof(double);
         if (b <= 200 * 1024) { *pc = p; *wstride = ws; *smem = b; return true; }
     }
     return false;
@@ -540,6 +542,10 @@ template <typename T>
 static ewald_status oct_choose(ewald_ctx *c, int W, int n, int *wc_out)
 {
     const long long key = (long long)W | ((long long)n << 24) | ((long long)(sizeof(T) == 4) << 60);
+    if (const char *ov = getenv("EWALD_OCT_WC")) { /* tuning runs only */
+        const int wc = atoi(ov);
+        if (wc >= 1 && wc <= 16 && wc <= W) { *wc_out = wc; return EWALD_OK; }
+    }
     auto it = c->oct_choice.find(key);
     if (it != c->oct_choice.end()) { *wc_out = it->second; return EWALD_OK; }
     const OctPlan &P = c->t.oct;

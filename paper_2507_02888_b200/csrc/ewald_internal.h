@@ -11,26 +11,31 @@
 namespace ewald {
 
 /* Host plan of the octant-form reciprocal kernel (ewald_recip_oct.cuh; any cell).
- * An item is a column (n2, n3) -- in 2D a pair of n2 values -- with a block of <= npb consecutive
- * n1 >= 1 (block 0 also carries n1 = 0).  Offsets are in (cos,sin)-pair units within a table row. */
+ * A table row of one (walker, particle) holds the (cos, sin) pairs X1[0..nmax1] (times q), X2[0..nmax2],
+ * X3[0..nmax3].  An item is a block of <= npb consecutive n1 >= 1 (block 0 also carries n1 = 0) of
+ *   OCT_FULL  one column (n2 > 0, n3 > 0): four products X2[n2] (x) X3[n3] per particle, or
+ *   OCT_PAIR  two half columns -- (n2, 0), (0, n3) or (0, 0); in 2D any two n2 -- with two products each.
+ * Offsets are in pair units within a row. */
+constexpr int OCT_FULL = 0, OCT_PAIR = 1, OCT_EMPTY = 2;
 struct OctPlan {
     bool valid = false;
     int dim = 3, npb = 0;
     int rowlen = 0, off[3] = {0, 0, 0};
     int n_items = 0;
-    std::vector<int> offA, offB, offX, np, c0; /* [n_items] */
-    std::vector<int> col;                      /* [n_items][3] = n2 (2D: n2a), n3 (2D: n2b or -1), first n1 of the block - 1 */
-    std::vector<double> wt;                    /* [n_items][1 + npb][4] class weights (3D: ++, +-, -+, --; 2D: a+, a-, b+, b-) */
+    std::vector<int> kind, offA, offB, offX, np, c0; /* [n_items] */
+    std::vector<int> col;                      /* [n_items][5] = axis and n of half A, of half B (axis -1: none), first n1 of the block - 1 */
+    std::vector<double> wt;                    /* [n_items][1 + npb][4] class weights (FULL: ++, +-, -+, --; PAIR: A+, A-, B+, B-) */
     std::vector<double> tion;                  /* [n_items][1 + 2 npb][4]; empty without fixed charges */
 };
 
-/* Lane assignment of one CTA of `wc` walkers: items of all its walkers sorted by block length. */
+/* Lane assignment of the CTAs of one group of `wc` walkers (make_oct_launch). */
 struct OctLaunch {
     int wc = 0, n_warps = 0, n_slabs = 1; /* warps per CTA; CTAs per walker group */
     int rank_stride = 1;        /* most lanes any walker has in one CTA */
-    double cost = 0;            /* executed FMA + product operations per particle, whole CTA */
+    double cost = 0;            /* FP64 operations per particle the group is charged: 128 n_slabs x its busiest sub-partition */
+    double fma_ops = 0;         /* FMA + product operations per particle actually executed, whole group */
     std::vector<int> lane;      /* [n_slabs][32 n_warps][4] = local walker | rank << 8, item, offA | offB << 16, offX */
-    std::vector<int> variant;   /* [n_slabs][n_warps] np | c0 << 8 */
+    std::vector<int> variant;   /* [n_slabs][n_warps] np | c0 << 8 | kind << 16 */
 };
 
 /* Pair-function table F(t) = erfc(sqrt t)/sqrt t on bins cut from the bits of t (ewald_setup.cpp). */

@@ -1,9 +1,9 @@
 /* ewald_octplan.cpp -- host plan for the octant-form reciprocal kernel (ewald_recip_oct.cuh).
  *
- * From the G+ list of ewald_setup (Eq. 3's reciprocal sum) builds, for orthorhombic
- * cells, the non-negative octant n >= 0 with weights w(G_n) 2^nz, cut into items (column, n1 block),
- * and the per-CTA lane assignment that keeps every warp at one block length.  Long double where
- * values are computed (setup always in DP or better).
+ * From the G+ list of ewald_setup (Eq. 3's reciprocal sum) builds the non-negative octant
+ * n >= 0 with the class weights of every octant point, cut into items (column(s), n1 block), and the per-CTA
+ * lane assignment: warps of one block length, dealt to the four sub-partitions of an SM so that they carry
+ * equal FP64 work.  Long double where values are computed (setup always in DP or better).
  */
 #include <algorithm>
 #include <cmath>
@@ -50,6 +50,13 @@ void build_oct_plan(HostTables *t)
         for (int cls = 0; cls < (dim == 3 ? 4 : 2); cls++) sum += class_weight(n1, n2, n3, cls);
         return sum;
     };
+    /* A half column is a column with one phase only: (n2, 0) [axis 1], (0, n3) [axis 2]; in 2D every column.
+     * Its two sign classes s = +-: the class weights of the point summed over the sign that does not matter. */
+    auto half_weight = [&](int n1, int axis, int n, int s) -> double {
+        if (dim == 2) return class_weight(n1, n, 0, s);
+        if (axis == 1) return class_weight(n1, n, 0, 2 * s) + class_weight(n1, n, 0, 2 * s + 1);
+        return class_weight(n1, 0, n, s) + class_weight(n1, 0, n, 2 + s);
+    };
     const int nm0 = t->n_max[0], nm1 = t->n_max[1], nm2 = dim == 3 ? t->n_max[2] : 0;
     if (nm1 + nm2 + nm0 + 3 > 0xffff) return;
     const int nblk_max = std::max(1, (nm0 + 6) / 7);
@@ -57,56 +64,70 @@ void build_oct_plan(HostTables *t)
     if (npb < 4) npb = 4;
     P.dim = dim;
     P.npb = npb;
+    /* table row of one (walker, particle): X1[0..nm0] (carries q), X2[0..nm1], X3[0..nm2] as (cos, sin) pairs */
     P.off[0] = 0;
-    P.off[1] = nm0;
-    P.off[2] = nm0 + nm1 + 1;
+    P.off[1] = nm0 + 1;
+    P.off[2] = nm0 + nm1 + 2;
     P.rowlen = dim == 3 ? P.off[2] + nm2 + 1 : P.off[2];
+    P.rowlen |= 1; /* odd number of 16-byte pairs: 32 lanes that write (or read) the same entry of 32 consecutive rows hit 32 different bank groups */
 
-    /* columns: (a, b, n1max_a, n1max_b); 3D: a = n2, b = n3; 2D: a, b = two n2 values (b = -1: none) */
-    struct Col { int a, b, m; };
-    std::vector<Col> cols;
     auto n1max_of = [&](int n2, int n3) {
         int m = -1;
         for (int n1 = 0; n1 <= nm0; n1++)
             if ((n1 == 0 && n2 == 0 && n3 == 0) || weight(n1, n2, n3) != 0.0) m = n1;
         return m;
     };
+    /* columns: FULL (n2 > 0 and n3 > 0: four products X2 (x) X3) and half columns, paired two to an item */
+    struct Col { int kind, aa, an, ba, bn, m; }; /* kind, half A (axis, n), half B (axis, n; axis -1: none), n1max */
+    struct Half { int m, axis, n; };
+    std::vector<Col> cols;
+    std::vector<Half> halves;
     if (dim == 3) {
         for (int n2 = 0; n2 <= nm1; n2++)
             for (int n3 = 0; n3 <= nm2; n3++) {
                 const int m = n1max_of(n2, n3);
-                if (m >= 0) cols.push_back({n2, n3, m});
+                if (m < 0) continue;
+                if (n2 > 0 && n3 > 0) cols.push_back({OCT_FULL, 1, n2, 2, n3, m});
+                else halves.push_back({m, n3 > 0 ? 2 : 1, n3 > 0 ? n3 : n2});
             }
     } else {
-        std::vector<std::pair<int, int>> v; /* (-n1max, n2) */
         for (int n2 = 0; n2 <= nm1; n2++) {
             const int m = n1max_of(n2, 0);
-            if (m >= 0) v.push_back({-m, n2});
+            if (m >= 0) halves.push_back({m, 1, n2});
         }
-        std::sort(v.begin(), v.end());
-        for (size_t i = 0; i < v.size(); i += 2)
-            cols.push_back({v[i].second, i + 1 < v.size() ? v[i + 1].second : -1, -v[i].first});
     }
+    std::sort(halves.begin(), halves.end(), [](const Half &x, const Half &y) {
+        if (x.m != y.m) return x.m > y.m;
+        if (x.axis != y.axis) return x.axis < y.axis;
+        return x.n < y.n;
+    });
+    for (size_t i = 0; i < halves.size(); i += 2) {
+        const bool two = i + 1 < halves.size();
+        cols.push_back({OCT_PAIR, halves[i].axis, halves[i].n, two ? halves[i + 1].axis : -1, two ? halves[i + 1].n : 0,
+                        halves[i].m});
+    }
+    auto half_off = [&](int axis, int n) { return P.off[axis] + n; };
     for (const Col &c : cols) {
         const int nblk = std::max(1, (c.m + npb - 1) / npb);
         for (int b = 0; b < nblk; b++) {
             const int start = b * npb, np = std::max(0, std::min(npb, c.m - start));
-            P.offA.push_back(P.off[1] + c.a);
-            P.offB.push_back(dim == 3 ? P.off[2] + c.b : P.off[1] + (c.b >= 0 ? c.b : c.a));
-            P.offX.push_back(P.off[0] + start);
+            P.kind.push_back(c.kind);
+            P.offA.push_back(half_off(c.aa, c.an));
+            P.offB.push_back(c.ba >= 0 ? half_off(c.ba, c.bn) : half_off(c.aa, c.an));
+            P.offX.push_back(P.off[0] + start); /* pairs j = 1..np at offX + j; block 0 also reads offX + 0 = (q, 0) */
             P.np.push_back(np);
             P.c0.push_back(b == 0);
-            P.col.push_back(c.a); P.col.push_back(c.b); P.col.push_back(start);
+            P.col.push_back(c.aa); P.col.push_back(c.an); P.col.push_back(c.ba); P.col.push_back(c.bn); P.col.push_back(start);
             for (int j = 0; j <= npb; j++) {
                 const int n1 = j == 0 ? 0 : start + j;
                 double wv[4] = {0, 0, 0, 0};
                 if ((j == 0 && b == 0) || (j >= 1 && j <= np)) {
-                    if (dim == 3) {
-                        for (int cls = 0; cls < 4; cls++) wv[cls] = class_weight(n1, c.a, c.b, cls);
+                    if (c.kind == OCT_FULL) {
+                        for (int cls = 0; cls < 4; cls++) wv[cls] = class_weight(n1, c.an, c.bn, cls);
                     } else {
-                        for (int cls = 0; cls < 2; cls++) {
-                            wv[cls] = class_weight(n1, c.a, 0, cls);
-                            wv[2 + cls] = c.b >= 0 ? class_weight(n1, c.b, 0, cls) : 0.0;
+                        for (int s = 0; s < 2; s++) {
+                            wv[s] = half_weight(n1, c.aa, c.an, s);
+                            wv[2 + s] = c.ba >= 0 ? half_weight(n1, c.ba, c.bn, s) : 0.0;
                         }
                     }
                 }
@@ -118,13 +139,15 @@ void build_oct_plan(HostTables *t)
     P.valid = P.n_items > 0;
 }
 
-/* T_abc of the fixed charges per item entry, laid out like the kernel's accumulators. */
+/* T_abc of the fixed charges per item entry, laid out like the kernel's accumulators: entry e = 0 is n1 = 0
+ * (cos only), e = 2j - 1 / 2j the cos / sin of n1 = start + j; products k as in the kernel (FULL: c2c3, c2s3,
+ * s2c3, s2s3; PAIR: cos, sin of half A, cos, sin of half B). */
 void fill_oct_ion(HostTables *t)
 {
     OctPlan &P = t->oct;
     P.tion.clear();
     if (!P.valid || t->n_ion == 0) return;
-    const int ne = 1 + 2 * P.npb, dim = t->dim;
+    const int ne = 1 + 2 * P.npb;
     P.tion.assign((size_t)P.n_items * ne * 4, 0.0);
     std::vector<real> s((size_t)3 * t->n_ion);
     for (int i = 0; i < t->n_ion; i++)
@@ -139,7 +162,8 @@ void fill_oct_ion(HostTables *t)
         return which ? sinl(2 * kPi * ph) : cosl(2 * kPi * ph);
     };
     for (int it = 0; it < P.n_items; it++) {
-        const int a = P.col[3 * it], b = P.col[3 * it + 1], start = P.col[3 * it + 2];
+        const int *c = &P.col[5 * it];
+        const int aa = c[0], an = c[1], ba = c[2], bn = c[3], start = c[4];
         for (int e = 0; e < ne; e++) {
             const int j = (e + 1) / 2, n1 = e == 0 ? 0 : start + j, which1 = e == 0 ? 0 : (e % 2 == 0);
             if (e == 0 && !P.c0[it]) continue;
@@ -148,8 +172,8 @@ void fill_oct_ion(HostTables *t)
                 real sum = 0;
                 for (int i = 0; i < t->n_ion; i++) {
                     real pr;
-                    if (dim == 3) pr = cs(i, 1, a, k >> 1) * cs(i, 2, b, k & 1);
-                    else pr = k < 2 ? cs(i, 1, a, k & 1) : (b >= 0 ? cs(i, 1, b, k & 1) : 0);
+                    if (P.kind[it] == OCT_FULL) pr = cs(i, aa, an, k >> 1) * cs(i, ba, bn, k & 1);
+                    else pr = k < 2 ? cs(i, aa, an, k & 1) : (ba >= 0 ? cs(i, ba, bn, k & 1) : 0);
                     sum += (real)t->ion_q[i] * pr * cs(i, 0, n1, which1);
                 }
                 P.tion[((size_t)it * ne + e) * 4 + k] = (double)sum;
@@ -158,57 +182,97 @@ void fill_oct_ion(HostTables *t)
     }
 }
 
+/* Lane assignment of the CTAs of one group of `wc` walkers.  The (walker, item) lanes are sorted by kind and
+ * block length and cut into warps (a warp never mixes kinds and runs the block length of its longest lane).
+ * The warps are then dealt to n_slabs CTAs x 4 sub-partitions, longest first to the least loaded bin (warp w of
+ * a CTA runs on sub-partition w mod 4): the FMA phase of a CTA lasts as long as its busiest sub-partition. */
 void make_oct_launch(const OctPlan &P, int wc, int max_warps, OctLaunch *L)
 {
-    struct Key { int len, wl, item; };
+    struct Key { int kind, len, wl, item; };
     std::vector<Key> v;
     v.reserve((size_t)wc * P.n_items);
     for (int wl = 0; wl < wc; wl++)
-        for (int it = 0; it < P.n_items; it++) v.push_back({2 * P.np[it] + P.c0[it], wl, it});
+        for (int it = 0; it < P.n_items; it++) v.push_back({P.kind[it], 2 * P.np[it] + P.c0[it], wl, it});
     std::sort(v.begin(), v.end(), [](const Key &x, const Key &y) {
+        if (x.kind != y.kind) return x.kind < y.kind;
         if (x.len != y.len) return x.len > y.len;
         if (x.wl != y.wl) return x.wl < y.wl;
         return x.item < y.item;
     });
-    /* the sorted list is cut into n_slabs CTAs of n_warps warps each (one CTA when it fits) */
-    const int total_warps = (int)((v.size() + 31) / 32);
-    const int n_slabs = (total_warps + max_warps - 1) / max_warps;
-    const int per_cta = (total_warps + n_slabs - 1) / n_slabs;
-    const int n_warps = per_cta * n_slabs; /* padded: trailing warps hold dummy items only */
+    struct Warp { size_t first, count; int kind, np, c0; double cost; };
+    std::vector<Warp> warps;
+    for (size_t i = 0; i < v.size();) {
+        size_t j = i;
+        int np = 0, c0 = 0;
+        while (j < v.size() && j - i < 32 && v[j].kind == v[i].kind) {
+            np = std::max(np, P.np[v[j].item]);
+            c0 = std::max(c0, P.c0[v[j].item]);
+            j++;
+        }
+        /* FP64 operations per particle of one lane: the tile's FMAs and the products */
+        warps.push_back({i, j - i, v[i].kind, np, c0, 4.0 * (2 * np + c0) + (v[i].kind == OCT_FULL ? 4.0 : 0.0)});
+        i = j;
+    }
+    max_warps = std::max(4, max_warps);
+    const int total = (int)warps.size();
+    const int n_slabs = std::max(1, (total + max_warps - 1) / max_warps);
+    const int n_bins = 4 * n_slabs;
+    auto bin_cap = [&](int b) { return (max_warps - (b & 3) + 3) / 4; }; /* warps w = b mod 4, + 4, ... below max_warps */
+    std::vector<std::vector<int>> bins(n_bins);
+    std::vector<double> load(n_bins, 0.0);
+    std::vector<int> order(total);
+    for (int i = 0; i < total; i++) order[i] = i;
+    std::stable_sort(order.begin(), order.end(), [&](int a, int b) { return warps[a].cost > warps[b].cost; });
+    for (int wi : order) {
+        int best = -1;
+        for (int b = 0; b < n_bins; b++)
+            if ((int)bins[b].size() < bin_cap(b) && (best < 0 || load[b] < load[best])) best = b;
+        bins[best].push_back(wi);
+        load[best] += warps[wi].cost;
+    }
+    int per_cta = 4;
+    for (int b = 0; b < n_bins; b++)
+        if (!bins[b].empty()) per_cta = std::max(per_cta, 4 * ((int)bins[b].size() - 1) + (b & 3) + 1);
     L->wc = wc;
     L->n_warps = per_cta;
     L->n_slabs = n_slabs;
-    L->lane.assign((size_t)n_warps * 32 * 4, 0);
-    L->variant.assign(n_warps, 0);
-    L->cost = 0;
-    /* padding lanes repeat the list's last entry with item = a zero-weight dummy: item index n_items */
-    /* rank = position of a lane among the lanes of its walker inside its CTA: the kernel adds a walker's
-     * lane sums in rank order, so the result does not depend on where in the batch the walker sits */
-    std::vector<int> next_rank((size_t)wc, 0);
-    L->rank_stride = 1;
-    for (int wp = 0; wp < n_warps; wp++) {
-        if (wp % per_cta == 0) std::fill(next_rank.begin(), next_rank.end(), 0);
-        int np = 0, c0 = 0;
-        for (int l = 0; l < 32; l++) {
-            const size_t i = (size_t)wp * 32 + l;
-            int *o = &L->lane[i * 4];
-            if (i < v.size()) {
-                const Key &k = v[i];
-                const int rank = next_rank[k.wl]++;
-                if (rank + 1 > L->rank_stride) L->rank_stride = rank + 1;
-                o[0] = k.wl | (rank << 8); o[1] = k.item;
-                o[2] = P.offA[k.item] | (P.offB[k.item] << 16);
-                o[3] = P.offX[k.item];
-                np = std::max(np, P.np[k.item]);
-                c0 = std::max(c0, P.c0[k.item]);
-            } else {
-                o[0] = 0 | (0xffffff << 8); o[1] = P.n_items; /* dummy item: all weights zero, no rank */
-                o[2] = P.offA[0] | (P.offB[0] << 16);
-                o[3] = P.offX[0];
+    L->lane.assign((size_t)n_slabs * per_cta * 32 * 4, 0);
+    L->variant.assign((size_t)n_slabs * per_cta, OCT_EMPTY << 16);
+    L->cost = 32.0 * 4.0 * n_slabs * *std::max_element(load.begin(), load.end());
+    L->fma_ops = 0;
+    /* rank = position of the item in the sorted item list (the same for every walker): the kernel adds a
+     * walker's lane sums in rank order, so the result does not depend on where in the batch the walker sits */
+    std::vector<int> item_rank((size_t)P.n_items, 0);
+    {
+        int r = 0;
+        for (const Key &k : v)
+            if (k.wl == 0) item_rank[k.item] = r++;
+    }
+    L->rank_stride = P.n_items;
+    for (int s = 0; s < n_slabs; s++) {
+        for (int wp = 0; wp < per_cta; wp++) {
+            const std::vector<int> &bin = bins[4 * s + (wp & 3)];
+            const int slot = wp >> 2;
+            const Warp *W = slot < (int)bin.size() ? &warps[bin[slot]] : nullptr;
+            if (W) {
+                L->variant[(size_t)s * per_cta + wp] = W->np | (W->c0 << 8) | (W->kind << 16);
+                L->fma_ops += 32.0 * W->cost;
+            }
+            for (int l = 0; l < 32; l++) {
+                int *o = &L->lane[(((size_t)s * per_cta + wp) * 32 + l) * 4];
+                if (W && (size_t)l < W->count) {
+                    const Key &k = v[W->first + l];
+                    const int rank = item_rank[k.item];
+                    o[0] = k.wl | (rank << 8); o[1] = k.item;
+                    o[2] = P.offA[k.item] | (P.offB[k.item] << 16);
+                    o[3] = P.offX[k.item];
+                } else { /* dummy item (index n_items): all weights zero, no rank */
+                    o[0] = 0 | (0xffffff << 8); o[1] = P.n_items;
+                    o[2] = P.offA[0] | (P.offB[0] << 16);
+                    o[3] = P.offX[0];
+                }
             }
         }
-        L->variant[wp] = np | (c0 << 8);
-        if ((size_t)wp * 32 < v.size()) L->cost += 32.0 * (4.0 * (2 * np + c0) + (P.dim == 3 ? 4.0 : 0.0));
     }
 }
 

@@ -12,84 +12,131 @@
  *
  * Work decomposition (host plan, ewald_octplan.cpp):
  *   row    per (walker, particle): the "powers ... computed and buffered" of PAPER.md:157, in shared
- *          memory as (cos, sin) pairs: X1[n=1..], X2[n=0..], X3[n=0..] (the last axis carries q_i)
- *   item   a column (n2, n3) and a block of <= NPB consecutive n1 (plus n1 = 0 in the first block);
- *          in 2D a pair of n2 values
- *   lane   owns one (walker, item) for the whole kernel: 4 products p = X2 (x) X3 (unique per lane)
- *          times the X1 pairs of the block (one broadcast LDS.128 per pair) -> 4 x (1 + 2 NP) register
- *          accumulators, 4 (1 + 2 NP) FMA per 2 + NP shared-memory loads
- *   warp   32 lanes of equal block length: the items of all walkers of the CTA are sorted by length, so
- *          the spherical cut-off costs no divergent lanes
+ *          memory as (cos, sin) pairs: X1[n = 0..] (times q_i), X2[n = 0..], X3[n = 0..]
+ *   item   a block of <= NPB consecutive n1 (plus n1 = 0 in the first block) of either one column
+ *          (n2 > 0, n3 > 0) with its four products X2 (x) X3 [FULL], or two half columns ((n2, 0), (0, n3),
+ *          (0, 0); in 2D any n2) with their two products each [PAIR]: no product that is identically zero
+ *   lane   owns one (walker, item) for the whole kernel: 4 products (unique per lane) times the X1 pairs of
+ *          the block (one broadcast LDS.128 per pair) -> 4 x (1 + 2 NP) register accumulators.  The loop is
+ *          software-pipelined by hand: the pairs of particle p + 1 are loaded while those of p are multiplied
+ *          (a DFMA needs its LDS operand 30 cycles after issue; with one product held in the operand reuse
+ *          cache a DFMA reads two register operands and issues every 2 cycles, profiles/r02_fp64_pipe.md)
+ *   warp   32 lanes of one kind and block length: the items of all walkers of the CTA are sorted, so the
+ *          spherical cut-off costs no divergent lanes; warps are dealt to the four sub-partitions (warp mod 4)
+ *          so that each carries the same number of FP64 operations
  */
 #pragma once
 #include "ewald_kernels_common.cuh"
 
 namespace ewald {
 
+constexpr int OCT_KIND_FULL = 0, OCT_KIND_PAIR = 1, OCT_KIND_EMPTY = 2; /* = OCT_FULL, ... of ewald_internal.h */
+
 template <typename T> struct OctArgs {
     const T *pos;       /* [W][DIM][npad] */
     const T *q;         /* [n] */
     int n, npad, n_walkers;
     int wc;             /* walkers per CTA */
-    int n_slabs;        /* CTAs per walker group: the sorted item list is cut into slabs */
+    int n_slabs;        /* CTAs per walker group: the warp list is dealt to n_slabs CTAs */
     int pc;             /* particles per chunk */
     int rank_stride;    /* most lanes any walker has in one CTA */
     int rowlen;         /* (cos,sin) pairs per (walker, particle) row */
     int wstride;        /* pairs per walker slab (pc * rowlen + bank stagger) */
-    int off[3];         /* pair offset of X1 (n = 1..), X2 (n = 0..), X3 (n = 0..) within a row */
+    int off[3];         /* pair offset of X1, X2, X3 (each n = 0..) within a row */
     int nmax[3];
     const int4 *lane;   /* [n_slabs][blockDim.x] {local walker | rank << 8, item, offA | offB << 16, offX} */
-    const int *variant; /* [n_slabs][n_warps] NP | C0 << 8 */
-    const double *wt;   /* [n_items][1 + NPB][4]: class weights W_pq per entry (ewald_octplan.cpp) */
+    const int *variant; /* [n_slabs][n_warps] NP | C0 << 8 | kind << 16 */
+    const double *wt;   /* [n_items][1 + NPB][4]: class weights per entry (ewald_octplan.cpp) */
     const double *tion; /* [n_items][1 + 2 NPB][4] fixed-charge sums, or null */
     double *e_recip;    /* [W][n_slabs] */
     double binv[9];     /* FP64 also in the FP32 kernels: the reduction of s to one period is done in FP64 */
 };
 
-/* Threads per CTA the register file allows: 4 (1 + 2 NPB) accumulators per lane (doubles take two
- * registers each): FP64 NPB = 7 needs ~254 registers -> 256 threads; NPB <= 5 fits 168 -> 384. */
+/* Threads per CTA the register file allows: 4 (1 + 2 NPB) accumulators per lane (doubles take two registers
+ * each) plus the prefetched pairs of the next particle. */
+#ifndef EWALD_OCT_THREADS64
+#define EWALD_OCT_THREADS64 384
+#endif
+#ifndef EWALD_OCT_THREADS32
+#define EWALD_OCT_THREADS32 512
+#endif
 template <typename T, int NPB> struct OctCfg {
-    static constexpr int MAX_THREADS = sizeof(T) == 8 ? (NPB >= 6 ? 256 : 384) : (NPB >= 6 ? 224 : 512);
-    static constexpr int MIN_CTAS = sizeof(T) == 4 && NPB >= 6 ? 2 : 1; /* FP32: two CTAs of 7 warps per SM */
+    static constexpr int MAX_THREADS = sizeof(T) == 8 ? EWALD_OCT_THREADS64 : EWALD_OCT_THREADS32;
+    /* registers per thread when MAX_THREADS are resident: 64 K registers, allocated 8 at a time per thread */
+    static constexpr int MAX_REGS = (65536 / MAX_THREADS) / 8 * 8 > 255 ? 255 : (65536 / MAX_THREADS) / 8 * 8;
 };
 
-/* One chunk of particles for one lane: acc[k][e] += p_k * X1_e. */
-template <typename T, int NPB, int NP, bool C0, int MODE>
+/* Prefetch distance of the pipelined loop in (cos, sin) pairs: the pairs of a particle form a sequence of
+ * LEN = NP + C0 entries; a ring of D registers pairs holds the next D of them, D a divisor of LEN so that the
+ * ring is in the same state at the start of every particle.  D = 4 pairs = 32 DFMAs ahead of use. */
+__host__ __device__ constexpr int oct_ring(int len)
+{
+    return len <= 5 ? (len < 1 ? 1 : len) : len % 4 == 0 ? 4 : len % 3 == 0 ? 3 : len;
+}
+
+/* One chunk of particles for one lane: acc[k][e] += p_k * X1_e, software-pipelined over the particles. */
+template <typename T, int NPB, int NP, bool C0, int KIND>
 __device__ __forceinline__ void oct_fma(T (&acc)[4][1 + 2 * NPB], const typename Num<T>::T2 *rA,
                                         const typename Num<T>::T2 *rB, const typename Num<T>::T2 *rX,
                                         int cnt, int rowlen)
 {
     typedef typename Num<T>::T2 T2;
-#pragma unroll 2
+    constexpr int FIRST = C0 ? 0 : 1, LEN = NP + 1 - FIRST, D = oct_ring(LEN);
+    if (LEN == 0) return;
+    T2 a = *rA, b = *rB, ring[D];
+#pragma unroll
+    for (int i = 0; i < D; i++) ring[i] = rX[FIRST + i];
     for (int p = 0; p < cnt; p++) {
-        const T2 a = *rA, b = *rB;
+        /* the row after the chunk's last one is read but never used: the buffers carry a row of slack */
         T pr[4];
-        if (MODE == 0) { pr[0] = a.x * b.x; pr[1] = a.x * b.y; pr[2] = a.y * b.x; pr[3] = a.y * b.y; }
+        if (KIND == OCT_KIND_FULL) { pr[0] = a.x * b.x; pr[1] = a.x * b.y; pr[2] = a.y * b.x; pr[3] = a.y * b.y; }
         else { pr[0] = a.x; pr[1] = a.y; pr[2] = b.x; pr[3] = b.y; }
-        if (C0) {
+        rA += rowlen; rB += rowlen;
+        a = *rA; b = *rB;
 #pragma unroll
-            for (int k = 0; k < 4; k++) acc[k][0] += pr[k];
-        }
+        for (int i = 0; i < LEN; i++) {
+            const int j = FIRST + i;               /* pair index: n1 = block start + j; j = 0 is X1[0] = (q, 0) */
+            const T2 c = ring[i % D];
+            ring[i % D] = i + D < LEN ? rX[j + D] : rX[rowlen + j + D - LEN];
+            if (j == 0) {
 #pragma unroll
-        for (int j = 0; j < NP; j++) {
-            const T2 cs = rX[j];
+                for (int k = 0; k < 4; k++) acc[k][0] = fma(pr[k], c.x, acc[k][0]);
+            } else {
 #pragma unroll
-            for (int k = 0; k < 4; k++) {
-                acc[k][1 + 2 * j] = fma(pr[k], cs.x, acc[k][1 + 2 * j]);
-                acc[k][2 + 2 * j] = fma(pr[k], cs.y, acc[k][2 + 2 * j]);
+                for (int k = 0; k < 4; k++) {
+                    acc[k][2 * j - 1] = fma(pr[k], c.x, acc[k][2 * j - 1]);
+                    acc[k][2 * j] = fma(pr[k], c.y, acc[k][2 * j]);
+                }
             }
         }
-        rA += rowlen; rB += rowlen; rX += rowlen;
+        rX += rowlen;
     }
 }
 
-template <typename T, int NPB, int MODE, int NP>
+template <typename T, int NPB, int KIND, int NP>
 __device__ __forceinline__ void oct_dispatch_c0(T (&acc)[4][1 + 2 * NPB], bool c0,
                                                 const typename Num<T>::T2 *rA, const typename Num<T>::T2 *rB,
                                                 const typename Num<T>::T2 *rX, int cnt, int rowlen)
 {
-    if (c0) oct_fma<T, NPB, NP, true, MODE>(acc, rA, rB, rX, cnt, rowlen);
-    else oct_fma<T, NPB, NP, false, MODE>(acc, rA, rB, rX, cnt, rowlen);
+    if (c0) oct_fma<T, NPB, NP, true, KIND>(acc, rA, rB, rX, cnt, rowlen);
+    else oct_fma<T, NPB, NP, false, KIND>(acc, rA, rB, rX, cnt, rowlen);
+}
+
+template <typename T, int NPB, int KIND>
+__device__ __forceinline__ void oct_dispatch_np(T (&acc)[4][1 + 2 * NPB], int np, bool c0,
+                                                const typename Num<T>::T2 *rA, const typename Num<T>::T2 *rB,
+                                                const typename Num<T>::T2 *rX, int cnt, int rowlen)
+{
+    switch (np) {
+#define EWALD_OCT_CASE(NP)                                                                              \
+    case NP:                                                                                            \
+        if (NP <= NPB) oct_dispatch_c0<T, NPB, KIND, (NP <= NPB ? NP : 0)>(acc, c0, rA, rB, rX, cnt, rowlen); \
+        break;
+        EWALD_OCT_CASE(0) EWALD_OCT_CASE(1) EWALD_OCT_CASE(2) EWALD_OCT_CASE(3)
+        EWALD_OCT_CASE(4) EWALD_OCT_CASE(5) EWALD_OCT_CASE(6) EWALD_OCT_CASE(7)
+#undef EWALD_OCT_CASE
+    default: break;
+    }
 }
 
 /* [S1,S2] Phase seeds and power rows of one chunk of particles, for all walkers of the CTA.  A task is one
@@ -129,8 +176,8 @@ __device__ __forceinline__ void oct_build_rows(const OctArgs<T> &A, typename Num
             s -= rint(s);
             Num<T>::sincospi_((T)(2 * s), &sn[k], &cs[k]);
             row[k] = tab + (size_t)wl * A.wstride + (size_t)p * A.rowlen + A.off[k];
-            e[k].x = k == DIM - 1 ? qp : T(1); e[k].y = 0;
-            if (k > 0) row[k][0] = e[k]; else row[k] -= 1; /* axis 1 stores n = 1.. only */
+            e[k].x = k == 0 ? qp : T(1); e[k].y = 0; /* the first axis carries q: X1[0] = (q, 0) */
+            row[k][0] = e[k];
         }
         for (int n = 1; n <= nmax_all; n++) {
 #pragma unroll
@@ -146,14 +193,14 @@ __device__ __forceinline__ void oct_build_rows(const OctArgs<T> &A, typename Num
 }
 
 template <typename T, int DIM, int NPB>
-__global__ void __launch_bounds__(OctCfg<T, NPB>::MAX_THREADS, OctCfg<T, NPB>::MIN_CTAS) recip_oct_kernel(OctArgs<T> A)
+__global__ void __maxnreg__((OctCfg<T, NPB>::MAX_REGS)) recip_oct_kernel(OctArgs<T> A)
 {
     typedef typename Num<T>::T2 T2;
-    constexpr int MODE = DIM == 3 ? 0 : 1;
     constexpr int NE = 1 + 2 * NPB;
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    /* two table buffers [wc][wstride] (+ slack), then the per-thread partial sums and walker tags */
-    const size_t buf_pairs = (size_t)A.wc * A.wstride + NPB + 1;
+    /* two table buffers [wc][wstride] plus a row of slack (the pipelined loop reads one row ahead), then the
+     * per-lane partial sums */
+    const size_t buf_pairs = (size_t)A.wc * A.wstride + A.rowlen;
     T2 *tab0 = reinterpret_cast<T2 *>(smem_raw);
     double *part = reinterpret_cast<double *>(tab0 + 2 * buf_pairs); /* [wc][rank_stride] lane sums by rank */
     __shared__ int counter[2];
@@ -165,8 +212,8 @@ __global__ void __launch_bounds__(OctCfg<T, NPB>::MAX_THREADS, OctCfg<T, NPB>::M
     const int rank = (int)((unsigned)L.x >> 8);
     L.x &= 255;
     const int var = A.variant[slab * (nthreads >> 5) + warp];
-    const int np = var & 255;
-    const bool c0 = (var >> 8) != 0;
+    const int np = var & 255, kind = var >> 16;
+    const bool c0 = ((var >> 8) & 255) != 0;
     if (tid < 2) counter[tid] = 0;
 
     T acc[4][NE];
@@ -186,16 +233,8 @@ __global__ void __launch_bounds__(OctCfg<T, NPB>::MAX_THREADS, OctCfg<T, NPB>::M
         const T2 *lane_base = tab + (size_t)L.x * A.wstride;
         const T2 *baseA = lane_base + (L.z & 0xffff), *baseB = lane_base + (L.z >> 16), *baseX = lane_base + L.w;
         /* [S3] */
-        switch (np) {
-#define EWALD_OCT_CASE(NP)                                                                              \
-    case NP:                                                                                            \
-        if (NP <= NPB) oct_dispatch_c0<T, NPB, MODE, (NP <= NPB ? NP : 0)>(acc, c0, baseA, baseB, baseX, cnt, A.rowlen); \
-        break;
-            EWALD_OCT_CASE(0) EWALD_OCT_CASE(1) EWALD_OCT_CASE(2) EWALD_OCT_CASE(3)
-            EWALD_OCT_CASE(4) EWALD_OCT_CASE(5) EWALD_OCT_CASE(6) EWALD_OCT_CASE(7)
-#undef EWALD_OCT_CASE
-        default: break;
-        }
+        if (DIM == 3 && kind == OCT_KIND_FULL) oct_dispatch_np<T, NPB, OCT_KIND_FULL>(acc, np, c0, baseA, baseB, baseX, cnt, A.rowlen);
+        else if (kind == OCT_KIND_PAIR) oct_dispatch_np<T, NPB, OCT_KIND_PAIR>(acc, np, c0, baseA, baseB, baseX, cnt, A.rowlen);
         /* the next chunk's tables go to the other buffer (read last in the previous pass) */
         if (base_p + A.pc < A.n)
             oct_build_rows<T, DIM>(A, tab0 + (size_t)((it + 1) & 1) * buf_pairs, &counter[it & 1], w0, base_p + A.pc,
@@ -203,12 +242,15 @@ __global__ void __launch_bounds__(OctCfg<T, NPB>::MAX_THREADS, OctCfg<T, NPB>::M
         __syncthreads();
     }
 
-    /* [S4] E_recip = sum_n sum_classes W_pq(n) |rho_pq(n)|^2 in FP64, with (c = cos, s = sin along axes 1,2,3)
+    /* [S4] E_recip = sum_n sum_classes W(n) |rho(n)|^2 in FP64.  FULL items (products k: 0 = c2 c3, 1 = c2 s3,
+     * 2 = s2 c3, 3 = s2 s3; c = cos, s = sin along axes 1, 2, 3), classes (p, q) = signs of n2, n3 relative to n1:
      *   Re rho_pq = T_ccc - p T_ssc - q T_scs - pq T_css,   Im rho_pq = T_scc + p T_csc + q T_ccs - pq T_sss;
-     * for orthogonal reciprocal axes the four weights are equal and the sum is W sum_abc T_abc^2.
+     * PAIR items (k = 0,1: cos, sin of half column A; k = 2,3: of B), classes p = sign of the half column's n:
+     *   Re rho_p = T_cc - p T_ss,   Im rho_p = T_sc + p T_cs.
+     * For orthogonal reciprocal axes the class weights are equal and the sum is W sum_abc T_abc^2.
      * Entries of weight zero are padding (never read as values). */
     double e = 0;
-    {
+    if (kind != OCT_KIND_EMPTY) {
         const double *wt = A.wt + (size_t)L.y * (NPB + 1) * 4;
         const double *ti = A.tion ? A.tion + (size_t)L.y * NE * 4 : nullptr;
 #pragma unroll
@@ -228,11 +270,11 @@ __global__ void __launch_bounds__(OctCfg<T, NPB>::MAX_THREADS, OctCfg<T, NPB>::M
             for (int cls = 0; cls < 4; cls++) {
                 const double wk = wt[4 * j + cls];
                 double re, im;
-                if (MODE == 0) { /* products k: 0 = c2 c3, 1 = c2 s3, 2 = s2 c3, 3 = s2 s3 */
+                if (DIM == 3 && kind == OCT_KIND_FULL) {
                     const double p = (cls & 2) ? -1.0 : 1.0, q = (cls & 1) ? -1.0 : 1.0;
                     re = Tc[0] - p * Ts[2] - q * Ts[1] - p * q * Tc[3];
                     im = Ts[0] + p * Tc[2] + q * Tc[1] - p * q * Ts[3];
-                } else {         /* two columns: k = 0,1 (c2, s2 of n2 = a) and k = 2,3 (of n2 = b) */
+                } else {
                     const int o = cls & 2;
                     const double p = (cls & 1) ? -1.0 : 1.0;
                     re = Tc[o] - p * Ts[o + 1];

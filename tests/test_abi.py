@@ -151,10 +151,11 @@ def test_octant_plan_covers_every_g_once():
             o = E.ewald_oct_plan_summary(w.dim, w.cell, w.kappa, w.g_cutoff, wc)
             want = _full_sphere_weight_sum(w.dim, w.L, w.kappa, w.n2_max)
             assert abs(o["weight_sum"] - want) <= 1e-13 * want
-            assert 4 <= o["npb"] <= 7 and o["n_warps"] == -(-wc * o["n_items"] // 32)
+            # warps never mix item kinds and are dealt to the four sub-partitions
+            assert 4 <= o["npb"] <= 7 and o["n_warps"] >= max(4, -(-wc * o["n_items"] // 32))
             # executed FMA + products per particle can never be below the algorithmic N_G + 1
             assert o["fma_per_particle"] >= ng + 1
-        assert (ng + 1) / o["fma_per_particle"] > 0.6   # wc = 7: the cut-off wastes < 40 % of the lanes
+        assert (ng + 1) / o["fma_per_particle"] > 0.7    # wc = 7: products + padding cost < 43 % of the algorithmic FMAs (config 1; 22 % on config 2)
 
 
 def test_octant_plan_any_cell():
