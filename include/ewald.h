@@ -89,6 +89,15 @@ ewald_status ewald_oct_plan_summary(int dim, const double cell[9], double gamma,
                                     int n_walkers_per_cta, int *n_items, int *npb, int *n_warps,
                                     double *weight_sum, double *fma_per_particle);
 
+/* Host-only summary of the plan of the tensor-core (FP64 DMMA) form of the octant kernel: the structure-factor
+ * sums of Eq. 8 as a contraction over the particles, cut into slots of 8 columns x 2 M-tiles
+ * of 4 n1 values.  n_slots per walker; walkers_per_pass = the most walkers one CTA pass can hold (0: the plan does
+ * not fit 12 warps x 3 slots, the FMA-pipe form is used); weight_sum as above (covers every G exactly once);
+ * dmma_per_quad = m8n8k4 instructions per four particles and walker.  Any output pointer may be null. */
+ewald_status ewald_mma_plan_summary(int dim, const double cell[9], double gamma, double g_cutoff,
+                                    int *n_slots, int *walkers_per_pass, double *weight_sum,
+                                    double *dmma_per_quad);
+
 /* Host-only evaluation of the pair-function table the real-space kernels read,
  *     F(t) = erfc(sqrt t)/sqrt t,  t = kappa^2 |r_ij - R|^2   (a term of the real-lattice sum of Eq. 3,
  * PAPER.md:117, is kappa q_i q_j F(t)): a piecewise polynomial in t on bins cut from the binary format of
@@ -101,7 +110,9 @@ ewald_status ewald_pair_table_eval(ewald_prec prec, double t_max, int n, const d
 ewald_status ewald_set_stream(ewald_ctx *ctx, void *stream);
 
 /* Which reciprocal-space kernel ewald_energy_batch uses (both compute the same E_recip; for tests
- * and measurements): 0 = automatic (the octant real-product form), 1 = complex half-set form,
+ * and measurements): 0 = automatic (FP64: the octant form on the FP64 tensor cores when its plan fits, else
+ * and in FP32 the octant form on the FMA pipe), 1 = complex half-set form, 3 = tensor-core octant form (FP64;
+ * EWALD_ESTATE at the next energy call when its plan does not fit),
  * 2 = octant form (EWALD_ESTATE at the next energy call if no plan could be built: G indices beyond
  * 16 bits). */
 ewald_status ewald_set_recip_variant(ewald_ctx *ctx, int variant);

@@ -13,6 +13,7 @@
 #include "ewald_internal.h"
 #include "ewald_kernels.cuh"
 #include "ewald_recip_oct.cuh"
+#include "ewald_recip_mma.cuh"
 #include <map>
 
 using namespace ewald;
@@ -36,10 +37,19 @@ struct OctDev {
     size_t smem = 0;
 };
 
+/* Device copy of one MmaLaunch. */
+struct MmaDev {
+    MmaLaunch L;
+    int2 *d_lane = nullptr;
+    int4 *d_meta = nullptr;
+};
+
 struct ewald_ctx {
     bool prof = false;
-    int recip_variant = 0;                 /* 0 auto, 1 complex half-set kernel, 2 octant kernel */
+    int recip_variant = 0;                 /* 0 auto, 1 complex half-set kernel, 2 octant FMA-pipe kernel, 3 octant DMMA kernel */
     double *d_oct_wt = nullptr, *d_oct_tion = nullptr;
+    double *d_mma_wt = nullptr, *d_mma_tion = nullptr;
+    std::map<int, MmaDev> mma_dev;         /* key: warps per walker */
     std::map<long long, OctDev> oct_dev;   /* key: wc | prec << 16 */
     std::map<long long, int> oct_choice;   /* key: W | prec << 40 | n << 41 ... -> wc */
     std::vector<ProfRec> recs;
@@ -268,6 +278,7 @@ extern "C" ewald_status ewald_setup(ewald_ctx **out, int dim, const double *cell
         wt.resize(wt.size() + (size_t)(t.oct.npb + 1) * 4, 0.0); /* the zero-weight dummy item */
         st = upload(c, &c->d_oct_wt, wt);
     }
+    if (st == EWALD_OK && t.mma.valid) st = upload(c, &c->d_mma_wt, t.mma.wt);
     if (st != EWALD_OK) { ewald_destroy(c); return st; }
     *out = c;
     return EWALD_OK;
@@ -314,6 +325,30 @@ extern "C" ewald_status ewald_oct_plan_summary(int dim, const double *cell, doub
     return EWALD_OK;
 }
 
+extern "C" ewald_status ewald_mma_plan_summary(int dim, const double *cell, double gamma, double g_cutoff,
+                                               int *n_slots, int *walkers_per_pass, double *weight_sum,
+                                               double *dmma_per_quad)
+{
+    HostTables t;
+    std::string err;
+    ewald_status st = build_tables(dim, cell, gamma, g_cutoff, 0.0, &t, &err);
+    if (st != EWALD_OK) return st;
+    if (!t.mma.valid) return EWALD_ESTATE;
+    long double ws = 0;
+    for (double v : t.mma.wt) ws += v;
+    int cap = 0;
+    for (int nw = MMA_WARPS; nw >= 1 && !cap; nw--) {
+        MmaLaunch L;
+        make_mma_launch(t.mma, MMA_WARPS / nw, &L);
+        if (L.valid) cap = nw;
+    }
+    if (n_slots) *n_slots = (int)t.mma.slots.size();
+    if (walkers_per_pass) *walkers_per_pass = cap;
+    if (weight_sum) *weight_sum = (double)ws;
+    if (dmma_per_quad) *dmma_per_quad = t.mma.dmma_per_quad;
+    return EWALD_OK;
+}
+
 extern "C" ewald_status ewald_pair_table_eval(ewald_prec prec, double t_max, int n, const double *t, double *value)
 {
     if (!(t_max > 0) || n < 0 || (n > 0 && (!t || !value))) return EWALD_EINVAL;
@@ -333,7 +368,8 @@ extern "C" void ewald_destroy(ewald_ctx *c)
     cudaFree(c->d_gn); cudaFree(c->d_w2); cudaFree(c->d_w2f); cudaFree(c->d_img); cudaFree(c->d_imgf);
     cudaFree(c->d_ion_rho); cudaFree(c->d_ion_rhof); cudaFree(c->d_ion_pos); cudaFree(c->d_ion_posf);
     cudaFree(c->d_ion_q); cudaFree(c->d_ion_qf); cudaFree(c->d_pair); cudaFree(c->d_pairf); cudaFree(c->d_far);
-    cudaFree(c->d_oct_wt); cudaFree(c->d_oct_tion);
+    cudaFree(c->d_oct_wt); cudaFree(c->d_oct_tion); cudaFree(c->d_mma_wt); cudaFree(c->d_mma_tion);
+    for (auto &kv : c->mma_dev) { cudaFree(kv.second.d_lane); cudaFree(kv.second.d_meta); }
     for (auto &kv : c->oct_dev) { cudaFree(kv.second.d_lane); cudaFree(kv.second.d_variant); }
     DevBuf *bufs[] = {&c->partial_recip, &c->partial_real, &c->qsums, &c->stage_pos, &c->stage_q,
                       &c->stage_e, &c->stage_comp, &c->mv_walker, &c->mv_electron, &c->mv_newr,
@@ -345,7 +381,7 @@ extern "C" void ewald_destroy(ewald_ctx *c)
 
 extern "C" ewald_status ewald_set_recip_variant(ewald_ctx *c, int variant)
 {
-    if (!c || variant < 0 || variant > 2) return EWALD_EINVAL;
+    if (!c || variant < 0 || variant > 3) return EWALD_EINVAL;
     c->recip_variant = variant;
     return EWALD_OK;
 }
@@ -384,6 +420,7 @@ extern "C" ewald_status ewald_set_fixed_charges(ewald_ctx *c, int n_ion, const d
         if (!ti.empty()) ti.resize(ti.size() + (size_t)(1 + 2 * t.oct.npb) * 4, 0.0);
         st = upload(c, &c->d_oct_tion, ti);
     }
+    if (st == EWALD_OK) st = upload(c, &c->d_mma_tion, t.mma.tion);
     c->loaded = false; /* a stored rho(G) would no longer match */
     return st;
 }
@@ -602,6 +639,95 @@ static ewald_status launch_recip_oct(ewald_ctx *c, int W, int n, const T *pos, c
     return EWALD_OK;
 }
 
+/* ---- octant kernel on the FP64 tensor cores (ewald_recip_mma.cuh): launch shape and launch ------------ */
+
+static ewald_status get_mma_dev(ewald_ctx *c, int wpw, MmaDev **out)
+{
+    auto it = c->mma_dev.find(wpw);
+    if (it == c->mma_dev.end()) {
+        MmaDev d;
+        make_mma_launch(c->t.mma, wpw, &d.L);
+        if (d.L.valid) {
+            CU_TRY(c, cudaMalloc((void **)&d.d_lane, d.L.lane.size() * sizeof(int)));
+            CU_TRY(c, cudaMemcpy(d.d_lane, d.L.lane.data(), d.L.lane.size() * sizeof(int), cudaMemcpyHostToDevice));
+            CU_TRY(c, cudaMalloc((void **)&d.d_meta, d.L.meta.size() * sizeof(int)));
+            CU_TRY(c, cudaMemcpy(d.d_meta, d.L.meta.data(), d.L.meta.size() * sizeof(int), cudaMemcpyHostToDevice));
+        }
+        it = c->mma_dev.emplace(wpw, d).first;
+    }
+    *out = &it->second;
+    return EWALD_OK;
+}
+
+/* true when the tensor-core kernel can take this problem (a plan exists and some split of the warps fits) */
+static ewald_status mma_max_walkers(ewald_ctx *c, int *nw_cap)
+{
+    *nw_cap = 0;
+    if (!c->t.mma.valid) return EWALD_OK;
+    for (int nw = MMA_WARPS; nw >= 1; nw--) {
+        MmaDev *d;
+        ewald_status st = get_mma_dev(c, MMA_WARPS / nw, &d);
+        if (st != EWALD_OK) return st;
+        if (d->L.valid) { *nw_cap = nw; return EWALD_OK; }
+    }
+    return EWALD_OK;
+}
+
+static ewald_status launch_recip_mma(ewald_ctx *c, int W, int n, const double *pos, const double *q, int *n_slabs_out)
+{
+    const MmaPlan &M = c->t.mma;
+    int nw_cap = 0;
+    ewald_status st = mma_max_walkers(c, &nw_cap);
+    if (st != EWALD_OK) return st;
+    if (nw_cap < 1) return fail(c, EWALD_ESTATE, "tensor-core octant kernel: the plan does not fit");
+    if ((st = ensure(c, &c->partial_recip, (size_t)W * sizeof(double))) != EWALD_OK) return st;
+    /* walkers per CTA so that the grid is one wave; shared memory bounds the walkers of a pass */
+    const int pc = 32, qstride = 4 * M.rowlen, wstride = (pc / 4) * qstride;
+    const size_t slab_bytes = (size_t)wstride * sizeof(double2);
+    const size_t part_bytes = (size_t)MMA_WARPS * 2 * M.slots.size() * sizeof(double);
+    const size_t avail = (c->smem_optin < 200 * 1024 ? c->smem_optin : 200 * 1024) - part_bytes;
+    int nw_pass = (int)(avail / (2 * slab_bytes));
+    if (nw_pass > nw_cap) nw_pass = nw_cap;
+    if (nw_pass < 1) return fail(c, EWALD_ERANGE, "tensor-core octant kernel: shared memory");
+    int wpc = (W + c->sm_count - 1) / c->sm_count;          /* walkers per CTA */
+    if (wpc > MMA_MAX_PASS * nw_pass) wpc = MMA_MAX_PASS * nw_pass;
+    const int n_pass = (wpc + nw_pass - 1) / nw_pass;
+    MmaArgs A;
+    A.pos = pos; A.q = q; A.n = n; A.npad = ewald_padded_n(n); A.n_walkers = W;
+    A.walkers_per_cta = wpc; A.n_pass = n_pass;
+    int nw_max = 0, first = 0;
+    for (int p = 0; p < n_pass; p++) { /* passes as equal as possible: 7 walkers = 4 + 3 */
+        const int nw = (wpc - first + (n_pass - p) - 1) / (n_pass - p);
+        MmaDev *d;
+        if ((st = get_mma_dev(c, MMA_WARPS / nw, &d)) != EWALD_OK) return st;
+        if (!d->L.valid) return fail(c, EWALD_ESTATE, "tensor-core octant kernel: pass shape");
+        A.pass[p].first = first; A.pass[p].nw = nw; A.pass[p].wpw = MMA_WARPS / nw;
+        A.pass[p].lane = d->d_lane; A.pass[p].meta = d->d_meta;
+        first += nw;
+        if (nw > nw_max) nw_max = nw;
+    }
+    A.pc = pc; A.rowlen = M.rowlen; A.qstride = qstride; A.wstride = wstride;
+    for (int k = 0; k < 3; k++) { A.off[k] = M.off[k]; A.nmax[k] = c->t.n_max[k]; }
+    A.n_slots = (int)M.slots.size();
+    A.wt = c->d_mma_wt; A.tion = c->t.n_ion ? c->d_mma_tion : nullptr;
+    A.e_recip = (double *)c->partial_recip.p;
+    for (int i = 0; i < 9; i++) A.binv[i] = c->t.binv[i];
+    const size_t smem = 2 * (size_t)nw_max * slab_bytes + (size_t)nw_max * 2 * M.slots.size() * sizeof(double);
+    const int grid = (W + wpc - 1) / wpc;
+    if (c->t.dim == 3) {
+        if ((st = allow_smem(c, recip_mma_kernel<3>, smem)) != EWALD_OK) return st;
+        ProfScope ps(c, 0);
+        recip_mma_kernel<3><<<grid, MMA_THREADS, smem, c->stream>>>(A, nw_max);
+    } else {
+        if ((st = allow_smem(c, recip_mma_kernel<2>, smem)) != EWALD_OK) return st;
+        ProfScope ps(c, 0);
+        recip_mma_kernel<2><<<grid, MMA_THREADS, smem, c->stream>>>(A, nw_max);
+    }
+    CU_TRY(c, cudaGetLastError());
+    *n_slabs_out = 1;
+    return EWALD_OK;
+}
+
 /* With the far shell on and every (kappa L_k)^2 >= FAR_T0, a candidate that has a far image on some axis lies in
  * the far shell whatever the other components are: the scan then touches the far stack only for those. */
 template <typename T> static void set_outer_far(const ewald_ctx *c, const PairTabs<T> &P, RealGeom<T> *g)
@@ -770,6 +896,30 @@ static ewald_status launch_real(ewald_ctx *c, int W, int n, const T *pos, const 
     return EWALD_OK;
 }
 
+/* FP64: the tensor-core form of the octant kernel (variant 0 or 3) when its plan fits; FP32 and variant 2: the
+ * FMA-pipe form; variant 1 or no octant plan: the complex half-set kernel. */
+template <typename T>
+static ewald_status launch_recip_any(ewald_ctx *c, bool oct, int W, int n, const T *pos, const T *q, int *n_slabs);
+template <>
+ewald_status launch_recip_any<double>(ewald_ctx *c, bool oct, int W, int n, const double *pos, const double *q, int *n_slabs)
+{
+    if (!oct) return launch_recip<double>(c, W, n, pos, q, nullptr, n_slabs);
+    if (c->recip_variant != 2) {
+        int nw_cap = 0;
+        ewald_status st = mma_max_walkers(c, &nw_cap);
+        if (st != EWALD_OK) return st;
+        if (nw_cap >= 1) return launch_recip_mma(c, W, n, pos, q, n_slabs);
+        if (c->recip_variant == 3) return fail(c, EWALD_ESTATE, "tensor-core octant kernel: the plan does not fit");
+    }
+    return launch_recip_oct<double>(c, W, n, pos, q, n_slabs);
+}
+template <>
+ewald_status launch_recip_any<float>(ewald_ctx *c, bool oct, int W, int n, const float *pos, const float *q, int *n_slabs)
+{
+    if (!oct) return launch_recip<float>(c, W, n, pos, q, nullptr, n_slabs);
+    return launch_recip_oct<float>(c, W, n, pos, q, n_slabs);
+}
+
 template <typename T>
 static ewald_status energy_batch_t(ewald_ctx *c, int W, int n, const T *pos, const T *q,
                                    double *energies, double *components)
@@ -781,9 +931,8 @@ static ewald_status energy_batch_t(ewald_ctx *c, int W, int n, const T *pos, con
     }
     CU_TRY(c, cudaGetLastError());
     const bool oct = c->recip_variant != 1 && c->t.oct.valid;
-    if (c->recip_variant == 2 && !oct) return fail(c, EWALD_ESTATE, "octant kernel: no plan for this G set");
-    ewald_status st = oct ? launch_recip_oct<T>(c, W, n, pos, q, &n_slabs)
-                          : launch_recip<T>(c, W, n, pos, q, nullptr, &n_slabs);
+    if (c->recip_variant >= 2 && !oct) return fail(c, EWALD_ESTATE, "octant kernel: no plan for this G set");
+    ewald_status st = launch_recip_any<T>(c, oct, W, n, pos, q, &n_slabs);
     if (st != EWALD_OK) return st;
     st = launch_real<T>(c, W, n, pos, q, &n_tiles);
     if (st != EWALD_OK) return st;

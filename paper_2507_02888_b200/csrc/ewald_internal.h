@@ -38,6 +38,35 @@ struct OctLaunch {
     std::vector<int> variant;   /* [n_slabs][n_warps] np | c0 << 8 | kind << 16 */
 };
 
+/* Host plan of the FP64 tensor-core form of the octant kernel (ewald_recip_mma.cuh): the structure-factor sums
+ * T[entry][product] = sum_i X1_entry(i) P_product(i) are a contraction over the particles, done by m8n8k4 DMMAs.
+ * A group is 8 columns of one kind (FULL: (n2 > 0, n3 > 0), four products; HALF: one phase, two products);
+ * a slot is what one warp accumulates in one set of registers: a FULL group or two HALF groups, times the M-tiles
+ * t0, t0 + 1 (M-tile t = the X1 doubles 8t..8t+7 = cos/sin of n1 = 4t..4t+3). */
+constexpr int MMA_SMAX = 3;     /* slots per warp */
+constexpr int MMA_WARPS = 12;   /* warps per CTA */
+struct MmaSlot {
+    int kind = OCT_FULL;        /* OCT_FULL or OCT_PAIR (two HALF groups) */
+    int t0 = 0, nt = 1;         /* first M-tile, number of M-tiles (1 or 2) */
+    int ax[2][8], n[2][8];      /* FULL: [0] = (axis 1, n2), [1] = (axis 2, n3) of column c; PAIR: half column c of group A / B; axis -1: none */
+};
+struct MmaPlan {
+    bool valid = false;
+    int dim = 3, rowlen = 0, off[3] = {0, 0, 0};
+    std::vector<MmaSlot> slots;
+    std::vector<double> wt;     /* [n_slots][2 tiles][4 n1][8 columns][4 classes] */
+    std::vector<double> tion;   /* [n_slots][2 tiles][8 doubles][8 columns][4 products]; empty without fixed charges */
+    double dmma_per_quad = 0;   /* DMMAs per four particles and walker */
+};
+/* Slots of one walker dealt to `wpw` warps (all slots of a warp share t0, at most MMA_SMAX each). */
+struct MmaLaunch {
+    int wpw = 0;
+    bool valid = false;
+    double max_dmma = 0;        /* DMMAs per quad of the busiest warp */
+    std::vector<int> lane;      /* [wpw][MMA_SMAX][32][2]: offsets (in pairs, within a quad block) of the lane's two operands */
+    std::vector<int> meta;      /* [wpw][MMA_SMAX][4]: kind (OCT_EMPTY: none), t0, nt, slot index */
+};
+
 /* Pair-function table F(t) = erfc(sqrt t)/sqrt t on bins cut from the bits of t (ewald_setup.cpp). */
 struct PairTable {
     int kbits = 0, degree = 0, e_min = 0; /* 2^kbits bins per binary octave, from 2^e_min upwards   */
@@ -85,12 +114,15 @@ struct HostTables {
     std::vector<int> sp_start;   /* [n_species + 1] first ion of each species (ions are kept grouped by charge) */
     double ion_q2 = 0, ion_qsum = 0, ion_real = 0; /* sum q^2, sum q, sum_{I<J} q_I q_J psi(r_IJ) */
     OctPlan oct;
+    MmaPlan mma;
 };
 
 struct HostTables;
 void build_oct_plan(HostTables *t);
 void fill_oct_ion(HostTables *t);
 void make_oct_launch(const OctPlan &p, int wc, int max_warps, OctLaunch *out);
+void fill_mma_ion(HostTables *t);
+void make_mma_launch(const MmaPlan &p, int wpw, MmaLaunch *out);
 
 
 /* Returns EWALD_OK or an error status with a message. */

@@ -137,6 +137,89 @@ void build_oct_plan(HostTables *t)
     }
     P.n_items = (int)P.np.size();
     P.valid = P.n_items > 0;
+
+    /* ---- the tensor-core (DMMA) form of the same sums: groups of 8 columns, M-tiles of 4 n1 values ---- */
+    MmaPlan &M = t->mma;
+    M = MmaPlan();
+    M.dim = dim; M.rowlen = P.rowlen;
+    for (int k = 0; k < 3; k++) M.off[k] = P.off[k];
+    struct MCol { int ax0, n0, ax1, n1, m; };  /* FULL: (1, n2, 2, n3); HALF: (axis, n, -1, 0) */
+    auto tiles_of = [](int m) { return m / 4 + 1; };
+    /* two columns that share a quarter-warp read two 64-byte chunks (entry x 4 particles) of one operand in one
+     * LDS.128: without bank conflict when the entries are equal or differ in parity */
+    auto compatible = [&](const MCol &x, const MCol &y) {
+        auto ok = [&](int ax, int a, int bx, int b) {
+            const int ea = P.off[ax] + a, eb = P.off[bx] + b; /* entries within a table row */
+            return ea == eb || ((ea + eb) & 1) != 0;
+        };
+        return ok(x.ax0, x.n0, y.ax0, y.n0) && (x.ax1 < 0 || ok(x.ax1, x.n1, y.ax1, y.n1));
+    };
+    auto make_groups = [&](std::vector<MCol> v) {
+        std::stable_sort(v.begin(), v.end(), [&](const MCol &x, const MCol &y) { return tiles_of(x.m) > tiles_of(y.m); });
+        std::vector<std::vector<MCol>> groups;
+        for (size_t i = 0; i < v.size(); i += 8) {
+            std::vector<MCol> g(v.begin() + i, v.begin() + std::min(v.size(), i + 8));
+            /* greedy pairing for the quarter-warps */
+            std::vector<MCol> out;
+            std::vector<bool> used(g.size(), false);
+            for (size_t a = 0; a < g.size(); a++) {
+                if (used[a]) continue;
+                used[a] = true;
+                out.push_back(g[a]);
+                size_t best = g.size();
+                for (size_t b = a + 1; b < g.size(); b++)
+                    if (!used[b] && compatible(g[a], g[b])) { best = b; break; }
+                if (best == g.size())
+                    for (size_t b = a + 1; b < g.size(); b++)
+                        if (!used[b]) { best = b; break; }
+                if (best < g.size()) { used[best] = true; out.push_back(g[best]); }
+            }
+            groups.push_back(out);
+        }
+        return groups;
+    };
+    std::vector<MCol> fullc, halfc;
+    for (const Col &c : cols)
+        if (c.kind == OCT_FULL) fullc.push_back({1, c.an, 2, c.bn, c.m});
+    for (const Half &h : halves) halfc.push_back({h.axis, h.n, -1, 0, h.m});
+    const auto fgroups = make_groups(fullc), hgroups = make_groups(halfc);
+    auto group_tiles = [&](const std::vector<MCol> &g) { int tl = 1; for (const MCol &c : g) tl = std::max(tl, tiles_of(c.m)); return tl; };
+    auto push_slot = [&](int kind, const std::vector<MCol> *ga, const std::vector<MCol> *gb, int t0, int nt) {
+        MmaSlot S;
+        S.kind = kind; S.t0 = t0; S.nt = nt;
+        for (int c = 0; c < 8; c++) {
+            S.ax[0][c] = S.ax[1][c] = -1; S.n[0][c] = S.n[1][c] = 0;
+            if (kind == OCT_FULL) {
+                if (c < (int)ga->size()) { S.ax[0][c] = 1; S.n[0][c] = (*ga)[c].n0; S.ax[1][c] = 2; S.n[1][c] = (*ga)[c].n1; }
+            } else {
+                if (c < (int)ga->size()) { S.ax[0][c] = (*ga)[c].ax0; S.n[0][c] = (*ga)[c].n0; }
+                if (gb && c < (int)gb->size()) { S.ax[1][c] = (*gb)[c].ax0; S.n[1][c] = (*gb)[c].n0; }
+            }
+        }
+        for (int tile = 0; tile < 2; tile++)
+            for (int l = 0; l < 4; l++) {
+                const int n1 = 4 * (t0 + tile) + l;
+                for (int c = 0; c < 8; c++)
+                    for (int cls = 0; cls < 4; cls++) {
+                        double wv = 0;
+                        if (tile < nt && n1 <= nm0) {
+                            if (kind == OCT_FULL) { if (S.ax[0][c] >= 0) wv = class_weight(n1, S.n[0][c], S.n[1][c], cls); }
+                            else if (S.ax[cls >> 1][c] >= 0) wv = half_weight(n1, S.ax[cls >> 1][c], S.n[cls >> 1][c], cls & 1);
+                        }
+                        M.wt.push_back(wv);
+                    }
+            }
+        M.slots.push_back(S);
+        M.dmma_per_quad += 4.0 * nt;
+    };
+    for (const auto &g : fgroups)
+        for (int t0 = 0; t0 < group_tiles(g); t0 += 2) push_slot(OCT_FULL, &g, nullptr, t0, std::min(2, group_tiles(g) - t0));
+    for (size_t i = 0; i < hgroups.size(); i += 2) {
+        const std::vector<MCol> *ga = &hgroups[i], *gb = i + 1 < hgroups.size() ? &hgroups[i + 1] : nullptr;
+        const int tl = std::max(group_tiles(*ga), gb ? group_tiles(*gb) : 1);
+        for (int t0 = 0; t0 < tl; t0 += 2) push_slot(OCT_PAIR, ga, gb, t0, std::min(2, tl - t0));
+    }
+    M.valid = !M.slots.empty() && dim >= 2;
 }
 
 /* T_abc of the fixed charges per item entry, laid out like the kernel's accumulators: entry e = 0 is n1 = 0
@@ -274,6 +357,155 @@ void make_oct_launch(const OctPlan &P, int wc, int max_warps, OctLaunch *L)
             }
         }
     }
+}
+
+} // namespace ewald
+
+namespace ewald {
+
+/* Fixed-charge sums laid out like the DMMA accumulators: [slot][tile][X1 double d][column][product]. */
+void fill_mma_ion(HostTables *t)
+{
+    MmaPlan &M = t->mma;
+    M.tion.clear();
+    if (!M.valid || t->n_ion == 0) return;
+    M.tion.assign(M.slots.size() * 2 * 8 * 8 * 4, 0.0);
+    std::vector<real> s((size_t)3 * t->n_ion);
+    for (int i = 0; i < t->n_ion; i++)
+        for (int k = 0; k < 3; k++) {
+            real v = 0;
+            for (int x = 0; x < 3; x++) v += (real)t->ion_pos[3 * i + x] * (real)t->binv[3 * k + x];
+            s[3 * i + k] = v - nearbyintl(v);
+        }
+    auto cs = [&](int i, int k, int n, int which) -> real {
+        real ph = n * s[3 * i + k];
+        ph -= nearbyintl(ph);
+        return which ? sinl(2 * kPi * ph) : cosl(2 * kPi * ph);
+    };
+    for (size_t si = 0; si < M.slots.size(); si++) {
+        const MmaSlot &S = M.slots[si];
+        for (int tile = 0; tile < S.nt; tile++)
+            for (int d = 0; d < 8; d++) {
+                const int idx = 8 * (S.t0 + tile) + d, n1 = idx >> 1, which1 = idx & 1;
+                if (n1 > t->n_max[0]) continue;
+                for (int c = 0; c < 8; c++)
+                    for (int k = 0; k < 4; k++) {
+                        real sum = 0;
+                        for (int i = 0; i < t->n_ion; i++) {
+                            real pr = 0;
+                            if (S.kind == OCT_FULL) {
+                                if (S.ax[0][c] >= 0) pr = cs(i, 1, S.n[0][c], k >> 1) * cs(i, 2, S.n[1][c], k & 1);
+                            } else if (S.ax[k >> 1][c] >= 0) {
+                                pr = cs(i, S.ax[k >> 1][c], S.n[k >> 1][c], k & 1);
+                            }
+                            sum += (real)t->ion_q[i] * pr * cs(i, 0, n1, which1);
+                        }
+                        M.tion[(((si * 2 + tile) * 8 + d) * 8 + c) * 4 + k] = (double)sum;
+                    }
+            }
+    }
+}
+
+/* Deals the slots of one walker to wpw warps: longest first to the least loaded warp that still has room and
+ * whose slots start at the same M-tile (the warp loads the X1 operand of a quad once for all its slots). */
+void make_mma_launch(const MmaPlan &M, int wpw, MmaLaunch *L)
+{
+    L->wpw = wpw;
+    L->valid = false;
+    L->lane.assign((size_t)wpw * MMA_SMAX * 32 * 2, 0);
+    L->meta.assign((size_t)wpw * MMA_SMAX * 4, 0);
+    for (int w = 0; w < wpw; w++)
+        for (int s = 0; s < MMA_SMAX; s++) L->meta[((size_t)w * MMA_SMAX + s) * 4] = OCT_EMPTY;
+    /* classes of slots by first M-tile: the fewest warps each class needs, spare warps to the class with the most
+     * work per warp; inside a class longest slot first to the least loaded warp */
+    std::map<int, std::vector<int>> classes;
+    for (size_t i = 0; i < M.slots.size(); i++) classes[M.slots[i].t0].push_back((int)i);
+    std::map<int, int> n_w;
+    std::map<int, double> work;
+    int used = 0;
+    for (auto &kv : classes) {
+        n_w[kv.first] = ((int)kv.second.size() + MMA_SMAX - 1) / MMA_SMAX;
+        used += n_w[kv.first];
+        double wk = 0;
+        for (int si : kv.second) wk += 4.0 * M.slots[si].nt;
+        work[kv.first] = wk;
+    }
+    if (used > wpw) return; /* does not fit */
+    for (; used < wpw; used++) {
+        int best = -1;
+        for (auto &kv : classes)
+            if (n_w[kv.first] < (int)kv.second.size() && (best < 0 || work[kv.first] / n_w[kv.first] > work[best] / n_w[best]))
+                best = kv.first;
+        if (best < 0) break;
+        n_w[best]++;
+    }
+    /* a piece = (slot, mask of its tiles): whole slots first, two-tile slots may be split to even the loads */
+    struct Piece { int slot, mask; };
+    std::vector<std::vector<Piece>> bins(wpw);
+    std::vector<double> load(wpw, 0.0);
+    std::vector<int> win(wpw, 0); /* first M-tile of the warp's two-tile window */
+    int w_first = 0;
+    for (auto &kv : classes) {
+        std::vector<int> order(kv.second);
+        std::stable_sort(order.begin(), order.end(), [&](int a, int b) { return M.slots[a].nt > M.slots[b].nt; });
+        const int w_end = w_first + n_w[kv.first];
+        for (int w = w_first; w < w_end; w++) win[w] = kv.first;
+        for (int si : order) {
+            int best = -1;
+            for (int w = w_first; w < w_end; w++)
+                if ((int)bins[w].size() < MMA_SMAX && (best < 0 || load[w] < load[best])) best = w;
+            if (best < 0) return;
+            bins[best].push_back({si, M.slots[si].nt > 1 ? 3 : 1});
+            load[best] += 4.0 * M.slots[si].nt;
+        }
+        /* the busiest warp of the class hands one tile of a two-tile slot to the idlest one while that helps */
+        for (int guard = 0; guard < 64; guard++) {
+            int hi = w_first, lo = w_first;
+            for (int w = w_first; w < w_end; w++) {
+                if (load[w] > load[hi]) hi = w;
+                if (load[w] < load[lo]) lo = w;
+            }
+            if (load[hi] - load[lo] < 8.0 || (int)bins[lo].size() >= MMA_SMAX) break;
+            size_t k = 0;
+            while (k < bins[hi].size() && bins[hi][k].mask != 3) k++;
+            if (k == bins[hi].size()) break;
+            bins[hi][k].mask = 1;
+            bins[lo].push_back({bins[hi][k].slot, 2});
+            load[hi] -= 4.0; load[lo] += 4.0;
+        }
+        w_first = w_end;
+    }
+    /* heaviest warps first, so that warp w mod 4 (the sub-partition) sees every weight class in turn */
+    {
+        std::vector<int> perm(wpw);
+        for (int w = 0; w < wpw; w++) perm[w] = w;
+        std::stable_sort(perm.begin(), perm.end(), [&](int a, int b) { return load[a] > load[b]; });
+        std::vector<std::vector<Piece>> b2(wpw);
+        std::vector<double> l2(wpw);
+        std::vector<int> w2(wpw);
+        for (int w = 0; w < wpw; w++) { b2[w] = bins[perm[w]]; l2[w] = load[perm[w]]; w2[w] = win[perm[w]]; }
+        bins.swap(b2); load.swap(l2); win.swap(w2);
+    }
+    L->max_dmma = 0;
+    for (int w = 0; w < wpw; w++) {
+        L->max_dmma = std::max(L->max_dmma, load[w]);
+        for (size_t s = 0; s < bins[w].size(); s++) {
+            const int si = bins[w][s].slot;
+            const MmaSlot &S = M.slots[si];
+            int *meta = &L->meta[((size_t)w * MMA_SMAX + s) * 4];
+            /* kind, the warp's window, tile mask within the window, slot | first tile of the slot << 16 */
+            meta[0] = S.kind; meta[1] = win[w]; meta[2] = bins[w][s].mask << (S.t0 - win[w]); meta[3] = si | (S.t0 << 16);
+            for (int lane = 0; lane < 32; lane++) {
+                const int kk = lane & 3, c = lane >> 2;
+                int *o = &L->lane[(((size_t)w * MMA_SMAX + s) * 32 + lane) * 2];
+                for (int h = 0; h < 2; h++) {
+                    const int ax = S.ax[h][c] >= 0 ? S.ax[h][c] : 1, n = S.ax[h][c] >= 0 ? S.n[h][c] : 0;
+                    o[h] = (M.off[ax] + n) * 4 + kk;
+                }
+            }
+        }
+    }
+    L->valid = true;
 }
 
 } // namespace ewald

@@ -354,6 +354,7 @@ ewald_status build_fixed_charges(HostTables *t, int n_ion, const double *pos, co
         }
     t->ion_real = (double)e;
     fill_oct_ion(t);
+    fill_mma_ion(t);
     return EWALD_OK;
 }
 

@@ -18,7 +18,7 @@ _STATUS = {0: "EWALD_OK", 1: "EWALD_EINVAL", 2: "EWALD_ESINGULAR", 3: "EWALD_ERA
            4: "EWALD_ESTATE", 5: "EWALD_ECUDA", 6: "EWALD_ENOMEM"}
 
 # every symbol include/ewald.h declares (checked by tests/test_abi.py against the header text)
-SYMBOLS = ["ewald_padded_n", "ewald_setup", "ewald_setup_summary", "ewald_oct_plan_summary",
+SYMBOLS = ["ewald_padded_n", "ewald_setup", "ewald_setup_summary", "ewald_oct_plan_summary", "ewald_mma_plan_summary",
            "ewald_pair_table_eval",
            "ewald_destroy", "ewald_set_stream", "ewald_set_recip_variant", "ewald_set_real_variant",
            "ewald_set_fixed_charges", "ewald_energy_batch", "ewald_energy_batch_host",
@@ -61,6 +61,7 @@ def load_library():
         "ewald_setup_summary": (i, [i, dp, d, d, d, ip, ip, ip, dp, dp]),
         "ewald_pair_table_eval": (i, [i, d, i, dp, dp]),
         "ewald_oct_plan_summary": (i, [i, dp, d, d, i, ip, ip, ip, dp, dp]),
+        "ewald_mma_plan_summary": (i, [i, dp, d, d, ip, ip, dp, dp]),
         "ewald_destroy": (None, [vp]),
         "ewald_set_stream": (i, [vp, vp]),
         "ewald_set_recip_variant": (i, [vp, i]),
@@ -205,6 +206,18 @@ def ewald_oct_plan_summary(dim, cell, gamma, g_cutoff, n_walkers_per_cta=1):
         raise EwaldError(st, "ewald_oct_plan_summary failed")
     return dict(n_items=ni.value, npb=nb.value, n_warps=nw.value, weight_sum=ws.value,
                 fma_per_particle=fm.value)
+
+
+def ewald_mma_plan_summary(dim, cell, gamma, g_cutoff):
+    """Host-only: plan of the tensor-core form of the octant kernel (any cell)."""
+    c = _cell9(cell, dim)
+    ns, wp = ctypes.c_int(), ctypes.c_int()
+    ws, dq = ctypes.c_double(), ctypes.c_double()
+    st = load_library().ewald_mma_plan_summary(dim, _dp(c), float(gamma), float(g_cutoff), ctypes.byref(ns),
+                                               ctypes.byref(wp), ctypes.byref(ws), ctypes.byref(dq))
+    if st != 0:
+        raise EwaldError(st, "ewald_mma_plan_summary failed")
+    return {"n_slots": ns.value, "walkers_per_pass": wp.value, "weight_sum": ws.value, "dmma_per_quad": dq.value}
 
 
 def ewald_pair_table_eval(prec, t_max, t):

@@ -105,15 +105,16 @@ def test_both_real_space_variants_match_oracle(torch_cuda, idx):
 
 @pytest.mark.parametrize("idx", [1, 2, 3, 4])
 def test_both_reciprocal_kernels_match_oracle(torch_cuda, idx):
-    """Octant real-product form (variant 2) and complex half-set form (variant 1), FP64 and FP32, on
-    walker counts that leave the last CTA of the octant kernel partly empty."""
+    """Octant real-product form on the FMA pipe (variant 2) and on the FP64 tensor cores (variant 3; FP32 has no
+    such form and takes the FMA-pipe kernel) and complex half-set form (variant 1), FP64 and FP32, on walker
+    counts that leave the last CTA partly empty."""
     w = workloads.config(idx)
     nw = {1: 8, 2: 9, 3: 11, 4: 5}[idx]
     pos = w.positions(nw)
     e_ref, c_ref = _oracle_energy(w, pos)
     e32_ref, c32_ref = _oracle_energy(w, _r32(pos))
     ctx = _ctx(w)
-    for variant in (1, 2):
+    for variant in (1, 2, 3):
         E.ewald_set_recip_variant(ctx, variant)
         e, c = _gpu_energy(torch_cuda, ctx, pos, w.charges, "f64")
         _assert_energy(e, c, e_ref, c_ref, TOL64)
@@ -122,7 +123,7 @@ def test_both_reciprocal_kernels_match_oracle(torch_cuda, idx):
         assert (np.abs(e - e32_ref) / np.abs(e32_ref)).max() <= TOL32
         assert (np.abs(c[:, 0] - c32_ref[:, 0]) / np.abs(c32_ref[:, 0])).max() <= TOL32
     with pytest.raises(E.EwaldError):
-        E.ewald_set_recip_variant(ctx, 3)
+        E.ewald_set_recip_variant(ctx, 4)
 
 
 def test_octant_kernel_orthorhombic_cells_and_single_walker(torch_cuda):
@@ -136,10 +137,11 @@ def test_octant_kernel_orthorhombic_cells_and_single_walker(torch_cuda):
             q = rng.choice([-1.0, 2.0], size=n)
             e_ref, c_ref = ref.energy_batch(dim, cell, kappa, gc, rc, pos, q)
             ctx = E.ewald_setup(dim, cell, kappa, gc, rc)
-            E.ewald_set_recip_variant(ctx, 2)
-            e, c = _gpu_energy(torch_cuda, ctx, pos, q, "f64")
-            assert (np.abs(c[:, 0] - c_ref[:, 0]) / np.abs(c_ref[:, 0])).max() <= 1e-12
-            _assert_energy(e, c, e_ref, c_ref, TOL64)
+            for variant in (2, 3):
+                E.ewald_set_recip_variant(ctx, variant)
+                e, c = _gpu_energy(torch_cuda, ctx, pos, q, "f64")
+                assert (np.abs(c[:, 0] - c_ref[:, 0]) / np.abs(c_ref[:, 0])).max() <= 1e-12
+                _assert_energy(e, c, e_ref, c_ref, TOL64)
 
 
 @pytest.mark.parametrize("dim", [2, 3])
@@ -159,7 +161,7 @@ def test_octant_kernel_on_general_cells(torch_cuda, dim):
     ctx = E.ewald_setup(dim, cell, kappa, gc, rc)
     E.ewald_set_fixed_charges(ctx, ion_pos, ion_q)
     scale = np.abs(c_ref).max(axis=1)
-    for variant in (2, 1, 0):
+    for variant in (3, 2, 1, 0):
         E.ewald_set_recip_variant(ctx, variant)
         e, c = _gpu_energy(torch_cuda, ctx, pos, q, "f64")
         assert (np.abs(c - c_ref) / scale[:, None]).max() <= TOL64, variant
