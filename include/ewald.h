@@ -197,10 +197,10 @@ ewald_status ewald_get_constants(const ewald_ctx *ctx, double *xi_r, double *v_m
  * *flops (2 per FMA), timed with CUDA events on the context's stream.  Synchronises.            */
 ewald_status ewald_probe_fma(ewald_ctx *ctx, ewald_prec prec, int iters, double *flops);
 
-/* Measured ceiling of the octant reciprocal kernel's FMA phase: its inner loop alone (a 4 x 15 outer-product
- * tile per lane, one broadcast shared-memory load per (cos, sin) pair; no tables, no barriers), one CTA of
- * `threads` (32..256, multiple of 32) per SM, `iters` iterations of 60 FMAs.  *flops = FLOP/s.  Synchronises. */
-ewald_status ewald_probe_fma_tile(ewald_ctx *ctx, ewald_prec prec, int iters, int threads, double *flops);
+/* FP64 tensor-core probe (the roofline denominator of the tensor-core form of the reciprocal kernel): every warp
+ * of one 256-thread CTA per SM issues `iters` rounds of 32 independent m8n8k4 DMMAs; *flops = FLOP/s (512 per
+ * DMMA).  On B200 it measures the same 37 TFLOP/s as the FP64 FMA chain.  Synchronises. */
+ewald_status ewald_probe_dmma(ewald_ctx *ctx, int iters, double *flops);
 
 /* Per-kernel device timers: when enabled, every kernel launch is bracketed by CUDA events on the
  * context's stream.  ewald_profile_read synchronises, returns and resets the accumulated device

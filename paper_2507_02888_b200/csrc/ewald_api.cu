@@ -3,7 +3,6 @@
  * the sm_100a kernels of ewald_kernels.cuh or fails with EWALD_ECUDA. */
 #include <cmath>
 #include <cstdio>
-#include <cstdlib>
 #include <cstring>
 #include <new>
 #include <string>
@@ -579,10 +578,6 @@ template <typename T>
 static ewald_status oct_choose(ewald_ctx *c, int W, int n, int *wc_out)
 {
     const long long key = (long long)W | ((long long)n << 24) | ((long long)(sizeof(T) == 4) << 60);
-    if (const char *ov = getenv("EWALD_OCT_WC")) { /* tuning runs only */
-        const int wc = atoi(ov);
-        if (wc >= 1 && wc <= 16 && wc <= W) { *wc_out = wc; return EWALD_OK; }
-    }
     auto it = c->oct_choice.find(key);
     if (it != c->oct_choice.end()) { *wc_out = it->second; return EWALD_OK; }
     const OctPlan &P = c->t.oct;
@@ -685,11 +680,12 @@ static ewald_status launch_recip_mma(ewald_ctx *c, int W, int n, const double *p
     const int pc = 32, qstride = 4 * M.rowlen, wstride = (pc / 4) * qstride;
     const size_t slab_bytes = (size_t)wstride * sizeof(double2);
     const size_t part_bytes = (size_t)MMA_WARPS * 2 * M.slots.size() * sizeof(double);
-    const size_t avail = (c->smem_optin < 200 * 1024 ? c->smem_optin : 200 * 1024) - part_bytes;
+    const size_t avail = (c->smem_optin < 200 * 1024 ? c->smem_optin : 200 * 1024) / MMA_CTAS_PER_SM - 1024 - part_bytes;
     int nw_pass = (int)(avail / (2 * slab_bytes));
     if (nw_pass > nw_cap) nw_pass = nw_cap;
     if (nw_pass < 1) return fail(c, EWALD_ERANGE, "tensor-core octant kernel: shared memory");
-    int wpc = (W + c->sm_count - 1) / c->sm_count;          /* walkers per CTA */
+    const int slots = c->sm_count * MMA_CTAS_PER_SM;
+    int wpc = (W + slots - 1) / slots;                      /* walkers per CTA */
     if (wpc > MMA_MAX_PASS * nw_pass) wpc = MMA_MAX_PASS * nw_pass;
     const int n_pass = (wpc + nw_pass - 1) / nw_pass;
     MmaArgs A;
@@ -1259,23 +1255,20 @@ extern "C" ewald_status ewald_get_positions(ewald_ctx *c, int walker, double *po
     return EWALD_OK;
 }
 
-extern "C" ewald_status ewald_probe_fma_tile(ewald_ctx *c, ewald_prec prec, int iters, int threads, double *flops)
+extern "C" ewald_status ewald_probe_dmma(ewald_ctx *c, int iters, double *flops)
 {
-    if (!c || !flops || iters <= 0 || threads < 32 || threads > 256 || threads % 32) return EWALD_EINVAL;
+    if (!c || !flops || iters <= 0) return EWALD_EINVAL;
     EWALD_DEVICE(c);
     ewald_status st = ensure(c, &c->stage_e, 64);
     if (st != EWALD_OK) return st;
     CU_TRY(c, cudaMemsetAsync(c->stage_e.p, 0, 64, c->stream));
-    const int blocks = c->sm_count; /* one CTA per SM, like recip_oct_kernel */
+    const int blocks = c->sm_count, threads = 256;
     cudaEvent_t e0, e1;
     CU_TRY(c, cudaEventCreate(&e0));
     CU_TRY(c, cudaEventCreate(&e1));
     for (int rep = 0; rep < 2; rep++) { /* first pass warms up */
         CU_TRY(c, cudaEventRecord(e0, c->stream));
-        if (prec == EWALD_F64)
-            fma_tile_probe_kernel<double><<<blocks, threads, 0, c->stream>>>(iters, (const double *)c->stage_e.p, (double *)c->stage_e.p);
-        else
-            fma_tile_probe_kernel<float><<<blocks, threads, 0, c->stream>>>(iters, (const float *)c->stage_e.p, (float *)c->stage_e.p);
+        dmma_probe_kernel<<<blocks, threads, 0, c->stream>>>(iters, (const double *)c->stage_e.p, (double *)c->stage_e.p);
         CU_TRY(c, cudaEventRecord(e1, c->stream));
         CU_TRY(c, cudaEventSynchronize(e1));
     }
@@ -1283,7 +1276,7 @@ extern "C" ewald_status ewald_probe_fma_tile(ewald_ctx *c, ewald_prec prec, int 
     CU_TRY(c, cudaEventElapsedTime(&ms, e0, e1));
     cudaEventDestroy(e0);
     cudaEventDestroy(e1);
-    *flops = 2.0 * 60.0 * iters * (double)blocks * threads / (ms * 1e-3);
+    *flops = 2.0 * 256.0 * 32.0 * iters * (double)blocks * (threads / 32) / (ms * 1e-3);
     return EWALD_OK;
 }
 

@@ -11,7 +11,7 @@
  *   combine_kernel [S6]     adds partial sums and the constants of Eqs. 3-4; charge_sums_kernel gives
  *                           sum q^2, sum q and the all-equal flag of the mobile charges
  *   move_kernel    [S7a-d]  single-particle moves, one warp per move: Delta E and patch of the stored rho(G)
- *   fma_probe_kernel, fma_tile_probe_kernel   measurement helpers (roofline denominators)
+ *   fma_probe_kernel   measurement helper (roofline denominator); dmma_probe_kernel in ewald_recip_mma.cuh
  * The paper's version-2 loop structure (real-lattice loop || reciprocal-lattice loop, then a
  * combining loop) is kept as three kernels; everything inside them is new.
  */
@@ -565,44 +565,6 @@ __global__ void __launch_bounds__(256) fma_probe_kernel(int iters, T a, T b, T *
         }
     }
     T s = x0 + x1 + x2 + x3 + x4 + x5 + x6 + x7;
-    if (s == T(123456789)) sink[0] = s;
-}
-
-/* Register-tile probe: the inner loop of recip_oct_kernel alone -- a 4 x 15 outer-product FMA tile per lane
- * fed by one broadcast LDS.128 per (cos, sin) pair, no tables to build, no barriers.  What it reaches is the
- * ceiling of that kernel's FMA phase for a given number of warps per SM. */
-template <typename T>
-__global__ void __launch_bounds__(256) fma_tile_probe_kernel(int iters, const T *in, T *sink)
-{
-    typedef typename Num<T>::T2 T2;
-    __shared__ T2 tab[32 * 8];
-    for (int i = threadIdx.x; i < 32 * 8; i += blockDim.x) { T2 v; v.x = in[i & 7]; v.y = in[(i + 3) & 7]; tab[i] = v; }
-    __syncthreads();
-    T acc[4][15];
-#pragma unroll
-    for (int k = 0; k < 4; k++)
-#pragma unroll
-        for (int e = 0; e < 15; e++) acc[k][e] = 0;
-    const T pr[4] = {in[0], in[1], in[2], in[3]};
-    for (int it = 0; it < iters; it++) {
-        const T2 *row = tab + (it & 31) * 8;
-#pragma unroll
-        for (int k = 0; k < 4; k++) acc[k][0] += pr[k];
-#pragma unroll
-        for (int j = 0; j < 7; j++) {
-            const T2 cs = row[j];
-#pragma unroll
-            for (int k = 0; k < 4; k++) {
-                acc[k][1 + 2 * j] = fma(pr[k], cs.x, acc[k][1 + 2 * j]);
-                acc[k][2 + 2 * j] = fma(pr[k], cs.y, acc[k][2 + 2 * j]);
-            }
-        }
-    }
-    T s = 0;
-#pragma unroll
-    for (int k = 0; k < 4; k++)
-#pragma unroll
-        for (int e = 0; e < 15; e++) s += acc[k][e];
     if (s == T(123456789)) sink[0] = s;
 }
 

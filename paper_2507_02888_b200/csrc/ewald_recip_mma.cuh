@@ -28,6 +28,7 @@ namespace ewald {
 constexpr int MMA_KIND_FULL = 0, MMA_KIND_PAIR = 1, MMA_KIND_EMPTY = 2; /* = OCT_FULL, OCT_PAIR, OCT_EMPTY */
 constexpr int MMA_S = 3;        /* = MMA_SMAX of ewald_internal.h */
 constexpr int MMA_THREADS = 384;
+constexpr int MMA_CTAS_PER_SM = 1;  /* two CTAs of 6 warps per SM were measured slower (config 2: 99 vs 89 us) */
 constexpr int MMA_MAX_PASS = 16;
 
 struct MmaPassDev {
@@ -130,7 +131,17 @@ __device__ __forceinline__ void mma_chunk(double (&acc)[MMA_S][4][2][2], const d
 }
 
 template <int DIM>
-__global__ void __launch_bounds__(MMA_THREADS, 1) recip_mma_kernel(MmaArgs A, int nw_max)
+__device__ __forceinline__ void mma_chunk_ns(int ns, double (&acc)[MMA_S][4][2][2], const double2 *tw, int nq, int qstride,
+                                             int oA0, int oA1, const int2 (&lo)[MMA_S], const bool (&full)[MMA_S],
+                                             const bool (&use0)[MMA_S], const bool (&use1)[MMA_S])
+{
+    if (ns == 3) mma_chunk<DIM, 3>(acc, tw, nq, qstride, oA0, oA1, lo, full, use0, use1);
+    else if (ns == 2) mma_chunk<DIM, 2>(acc, tw, nq, qstride, oA0, oA1, lo, full, use0, use1);
+    else if (ns == 1) mma_chunk<DIM, 1>(acc, tw, nq, qstride, oA0, oA1, lo, full, use0, use1);
+}
+
+template <int DIM>
+__global__ void __launch_bounds__(MMA_THREADS, MMA_CTAS_PER_SM) recip_mma_kernel(MmaArgs A, int nw_max)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const size_t buf_pairs = (size_t)nw_max * A.wstride;
@@ -180,20 +191,17 @@ __global__ void __launch_bounds__(MMA_THREADS, 1) recip_mma_kernel(MmaArgs A, in
             const int cnt = min(A.pc, A.n - base_p);
             const bool more = base_p + A.pc < A.n;
             double2 *next = tab0 + (size_t)((it + 1) & 1) * buf_pairs;
-            /* half of the warps of a sub-partition build the next chunk's tables first, the others last: the
-             * latency-bound table code overlaps the DMMA stream of the other warps */
-            const bool build_first = ((warp >> 2) & 1) != 0;
-            if (more && build_first)
-                mma_build_rows<DIM>(A, next, w0, nw, base_p + A.pc, min(A.pc, A.n - base_p - A.pc), warp, n_warps, lane);
-            if (active) { /* [S3] */
-                const double2 *tw = tab0 + (size_t)(it & 1) * buf_pairs + (size_t)wl * A.wstride;
-                const int nq = (cnt + 3) >> 2;
-                if (ns == 3) mma_chunk<DIM, 3>(acc, tw, nq, A.qstride, oA0, oA1, lo, full, use0, use1);
-                else if (ns == 2) mma_chunk<DIM, 2>(acc, tw, nq, A.qstride, oA0, oA1, lo, full, use0, use1);
-                else if (ns == 1) mma_chunk<DIM, 1>(acc, tw, nq, A.qstride, oA0, oA1, lo, full, use0, use1);
-            }
-            if (more && !build_first)
-                mma_build_rows<DIM>(A, next, w0, nw, base_p + A.pc, min(A.pc, A.n - base_p - A.pc), warp, n_warps, lane);
+            /* The table code is latency-bound (global loads, sincospi, a recurrence) and hardly uses the FP64 pipe:
+             * of the three warps of a sub-partition one builds its share of the next chunk's tables before its
+             * DMMAs, one half-way through and one after them, so that two warps always feed the tensor pipe. */
+            const int phase = (warp >> 2) % 3;
+            const int next_cnt = more ? min(A.pc, A.n - base_p - A.pc) : 0;
+            const double2 *tw = tab0 + (size_t)(it & 1) * buf_pairs + (size_t)wl * A.wstride;
+            const int nq = (cnt + 3) >> 2, nq0 = phase == 0 ? 0 : phase == 1 ? nq >> 1 : nq;
+            if (active && nq0 > 0) mma_chunk_ns<DIM>(ns, acc, tw, nq0, A.qstride, oA0, oA1, lo, full, use0, use1);
+            if (more) mma_build_rows<DIM>(A, next, w0, nw, base_p + A.pc, next_cnt, warp, n_warps, lane);
+            if (active && nq0 < nq)
+                mma_chunk_ns<DIM>(ns, acc, tw + (size_t)nq0 * A.qstride, nq - nq0, A.qstride, oA0, oA1, lo, full, use0, use1);
             __syncthreads();
         }
 
@@ -259,6 +267,27 @@ __global__ void __launch_bounds__(MMA_THREADS, 1) recip_mma_kernel(MmaArgs A, in
         }
         __syncthreads();
     }
+}
+
+/* FP64 tensor-core probe: 32 independent m8n8k4 DMMAs per warp and round (the roofline denominator of
+ * recip_mma_kernel; on B200 it equals the DFMA-chain peak of fma_probe_kernel). */
+__global__ void __launch_bounds__(256) dmma_probe_kernel(int iters, const double *in, double *sink)
+{
+    double c[8][2], a[4], b[4];
+#pragma unroll
+    for (int u = 0; u < 8; u++) { c[u][0] = 0; c[u][1] = 0; }
+#pragma unroll
+    for (int u = 0; u < 4; u++) { a[u] = in[u] + threadIdx.x; b[u] = in[u + 4] + 1; }
+    for (int i = 0; i < iters; i++) {
+#pragma unroll
+        for (int r = 0; r < 4; r++)
+#pragma unroll
+            for (int u = 0; u < 8; u++) dmma8x8x4(c[u][0], c[u][1], a[(u + r) & 3], b[u & 3]);
+    }
+    double s = 0;
+#pragma unroll
+    for (int u = 0; u < 8; u++) s += c[u][0] + c[u][1];
+    if (s == 123456789.0) sink[0] = s;
 }
 
 } // namespace ewald

@@ -24,7 +24,7 @@ SYMBOLS = ["ewald_padded_n", "ewald_setup", "ewald_setup_summary", "ewald_oct_pl
            "ewald_set_fixed_charges", "ewald_energy_batch", "ewald_energy_batch_host",
            "ewald_load_walkers", "ewald_move_delta_batch", "ewald_move_delta_batch_host",
            "ewald_move_delta", "ewald_num_g", "ewald_num_images", "ewald_r_cutoff", "ewald_get_g",
-           "ewald_get_rho", "ewald_get_positions", "ewald_get_constants", "ewald_probe_fma", "ewald_probe_fma_tile",
+           "ewald_get_rho", "ewald_get_positions", "ewald_get_constants", "ewald_probe_fma", "ewald_probe_dmma",
            "ewald_profile_enable", "ewald_profile_read", "ewald_launch_count",
            "ewald_last_error", "ewald_version"]
 
@@ -81,7 +81,7 @@ def load_library():
         "ewald_get_positions": (i, [vp, i, dp]),
         "ewald_get_constants": (i, [vp, dp, dp, dp]),
         "ewald_probe_fma": (i, [vp, i, i, dp]),
-        "ewald_probe_fma_tile": (i, [vp, i, i, i, dp]),
+        "ewald_probe_dmma": (i, [vp, i, dp]),
         "ewald_profile_enable": (i, [vp, i]),
         "ewald_profile_read": (i, [vp, dp, ip]),
         "ewald_launch_count": (ctypes.c_longlong, [vp]),
@@ -155,6 +155,30 @@ def _dev_ptr(t, what):
 
 def _host_ptr(a):
     return None if a is None else ctypes.c_void_p(a.ctypes.data)
+
+
+def _dtype_name(t):
+    return str(t.dtype).replace("torch.", "")
+
+
+def _expect(t, what, dtype, shape):
+    """Argument check of the binding (no arithmetic): dtype and shape of a tensor / array, None allowed."""
+    if t is None:
+        return
+    if _dtype_name(t) != dtype:
+        raise TypeError("%s must be %s, got %s" % (what, dtype, _dtype_name(t)))
+    if tuple(t.shape) != tuple(shape):
+        raise ValueError("%s must have shape %s, got %s" % (what, tuple(shape), tuple(t.shape)))
+
+
+def _check_batch(ctx, n_particles, positions, charges, energies=None, components=None):
+    if len(positions.shape) != 3 or positions.shape[1] != ctx.dim or positions.shape[2] != ewald_padded_n(n_particles):
+        raise ValueError("positions must have shape [W, %d, %d] (SoA, n padded to 4), got %s"
+                         % (ctx.dim, ewald_padded_n(n_particles), tuple(positions.shape)))
+    _prec_of(positions.dtype)
+    _expect(charges, "charges", _dtype_name(positions), (n_particles,))
+    _expect(energies, "energies", "float64", (positions.shape[0],))
+    _expect(components, "components", "float64", (positions.shape[0], 4))
 
 
 def ewald_padded_n(n):
@@ -256,6 +280,7 @@ def ewald_set_fixed_charges(ctx, pos, q):
 
 def ewald_energy_batch(ctx, n_particles, positions, charges, energies, components=None):
     """positions: CUDA tensor [W, dim, n_pad]; charges: CUDA [n]; energies: CUDA float64 [W]."""
+    _check_batch(ctx, n_particles, positions, charges, energies, components)
     w = positions.shape[0]
     _check(ctx, load_library().ewald_energy_batch(
         ctx.handle, w, n_particles, _prec_of(positions.dtype), _dev_ptr(positions, "positions"),
@@ -264,28 +289,41 @@ def ewald_energy_batch(ctx, n_particles, positions, charges, energies, component
 
 def ewald_energy_batch_host(ctx, n_particles, positions, charges, energies, components=None):
     """Same with numpy arrays (positions [W, dim, n_pad]); copies inside the call, synchronises."""
+    _check_batch(ctx, n_particles, positions, charges, energies, components)
     w = positions.shape[0]
-    assert positions.flags.c_contiguous and charges.dtype == positions.dtype and energies.dtype == np.float64
+    if not (positions.flags.c_contiguous and charges.flags.c_contiguous and energies.flags.c_contiguous):
+        raise TypeError("host arrays must be C-contiguous")
     _check(ctx, load_library().ewald_energy_batch_host(
         ctx.handle, w, n_particles, _prec_of(positions.dtype), _host_ptr(positions), _host_ptr(charges),
         _host_ptr(energies), _host_ptr(components)))
 
 
 def ewald_load_walkers(ctx, n_particles, positions, charges):
+    _check_batch(ctx, n_particles, positions, charges)
+    ctx.loaded = (positions.shape[0], n_particles, _dtype_name(positions))
     _check(ctx, load_library().ewald_load_walkers(
         ctx.handle, positions.shape[0], n_particles, _prec_of(positions.dtype),
         _dev_ptr(positions, "positions"), _dev_ptr(charges, "charges")))
 
 
 def ewald_move_delta_batch(ctx, walker, electron, new_r, commit, delta_e):
-    """walker, electron: CUDA int32 [M]; new_r: CUDA [M, dim]; delta_e: CUDA float64 [M]."""
+    """walker, electron: CUDA int32 [M]; new_r: CUDA [M, dim] in the loaded precision; delta_e: CUDA float64 [M]."""
+    m = walker.shape[0]
+    _expect(walker, "walker", "int32", (m,))
+    _expect(electron, "electron", "int32", (m,))
+    _expect(new_r, "new_r", getattr(ctx, "loaded", (0, 0, _dtype_name(new_r)))[2], (m, ctx.dim))
+    _expect(delta_e, "delta_e", "float64", (m,))
     _check(ctx, load_library().ewald_move_delta_batch(
         ctx.handle, walker.shape[0], _dev_ptr(walker, "walker"), _dev_ptr(electron, "electron"),
         _dev_ptr(new_r, "new_r"), int(commit), _dev_ptr(delta_e, "delta_e")))
 
 
 def ewald_move_delta_batch_host(ctx, walker, electron, new_r, commit, delta_e):
-    assert walker.dtype == np.int32 and electron.dtype == np.int32 and delta_e.dtype == np.float64
+    m = walker.shape[0]
+    _expect(walker, "walker", "int32", (m,))
+    _expect(electron, "electron", "int32", (m,))
+    _expect(new_r, "new_r", getattr(ctx, "loaded", (0, 0, _dtype_name(new_r)))[2], (m, ctx.dim))
+    _expect(delta_e, "delta_e", "float64", (m,))
     _check(ctx, load_library().ewald_move_delta_batch_host(
         ctx.handle, walker.shape[0], _host_ptr(walker), _host_ptr(electron), _host_ptr(new_r),
         int(commit), _host_ptr(delta_e)))
@@ -324,6 +362,9 @@ def ewald_get_rho(ctx, walker):
 
 
 def ewald_get_positions(ctx, walker, n_particles):
+    loaded = getattr(ctx, "loaded", None)
+    if loaded is not None and n_particles != loaded[1]:
+        raise ValueError("n_particles = %d, but %d particles per walker are loaded" % (n_particles, loaded[1]))
     out = np.zeros((n_particles, ctx.dim))
     _check(ctx, load_library().ewald_get_positions(ctx.handle, int(walker), _dp(out)))
     return out
@@ -342,14 +383,11 @@ def ewald_probe_fma(ctx, prec, iters=4096):
     return f.value
 
 
-def ewald_probe_fma_tile(ctx, prec, iters=20000, threads=256):
-    """FLOP/s of the octant kernel's inner loop alone, one CTA of `threads` per SM (its FMA-phase ceiling)."""
+def ewald_probe_dmma(ctx, iters=4096):
+    """FLOP/s of the FP64 tensor cores (m8n8k4 DMMA), the denominator of the tensor-core reciprocal kernel."""
     f = ctypes.c_double()
-    _check(ctx, load_library().ewald_probe_fma_tile(ctx.handle, int(prec), int(iters), int(threads), ctypes.byref(f)))
+    _check(ctx, load_library().ewald_probe_dmma(ctx.handle, int(iters), ctypes.byref(f)))
     return f.value
-
-
-KERNEL_CLASSES = ("recip", "real", "combine", "move")
 
 
 def ewald_profile_enable(ctx, on=True):
