@@ -46,7 +46,7 @@ def parse():
 def recorded_traffic(key, kernel):
     """DRAM bytes per launch from the committed ncu --set full capture (profiles/), or None."""
     try:
-        return json.load(open(os.path.join(ROOT, "profiles", "r01b_traffic.json")))[key][kernel]
+        return json.load(open(os.path.join(ROOT, "profiles", "r02_traffic.json")))[key][kernel]
     except Exception:
         return None
 
@@ -146,28 +146,125 @@ def run_reference(args, rank):
 
 def count_pair_terms(w, pos):
     """Pairs and pair-image terms (|r_ij - R| < r_c) per walker of an orthorhombic workload, counted with
-    numpy on a few walkers: the unit count of the real-space kernel's roofline."""
+    numpy on a few walkers: the unit count of the real-space kernel's roofline.
+    Returns pairs, terms, terms of the far shell (kappa^2 r^2 >= 16, evaluated in FP32 by the FP64 kernel),
+    images per axis."""
     sides = np.diag(w.cell)[:w.dim]
     m = int(math.floor(w.r_cutoff / sides.min() + 0.5 - 1e-12))
     shifts = np.array(np.meshgrid(*[np.arange(-m, m + 1)] * w.dim, indexing="ij")).reshape(w.dim, -1).T * sides
-    terms = []
+    terms, far = [], []
     for p in pos:
         others = [p] if w.ion_pos is None else [p, w.ion_pos]
-        cnt = 0
+        cnt = cnt_far = 0
         for k, o in enumerate(others):
             d = p[:, None, :] - o[None, :, :]
             d -= np.rint(d / sides) * sides
             r2 = ((d[:, :, None, :] - shifts[None, None, :, :]) ** 2).sum(-1)
             inside = r2 < w.r_cutoff ** 2
+            outer = inside & (r2 * w.kappa ** 2 >= 16.0)
             if k == 0:
                 iu = np.triu_indices(len(p), 1)
-                cnt += int(inside[iu].sum())
+                cnt += int(inside[iu].sum()); cnt_far += int(outer[iu].sum())
             else:
-                cnt += int(inside.sum())
-        terms.append(cnt)
+                cnt += int(inside.sum()); cnt_far += int(outer.sum())
+        terms.append(cnt); far.append(cnt_far)
     n_ion = 0 if w.ion_pos is None else len(w.ion_pos)
     pairs = w.n * (w.n - 1) // 2 + w.n * n_ion
-    return pairs, float(np.mean(terms)), (2 * m + 1) ** w.dim, m
+    return pairs, float(np.mean(terms)), float(np.mean(far)), m
+
+
+def real_space_work(w, pos, n_images):
+    """Algorithmic work of the real-space kernel per walker: pairs, pair-image terms, and a
+    flop count in FP64 equivalents -- per pair 12 (displacement and reduction to the cell) + 5 per axis image
+    square + 2 per enumerated candidate (20 in 3D with one image per side, else (2M+1)^dim); per near term
+    (kappa^2 r^2 < 16) 12 FP64 flops (u, quintic Horner, accumulate); per far term 8 FP32 flops = 4 FP64
+    equivalents (the FP64 kernel evaluates the far shell by an FP32 cubic; FP32 peak = 2 x FP64 peak)."""
+    n_ion = 0 if w.ion_q is None else len(w.ion_q)
+    if np.count_nonzero(w.cell - np.diag(np.diag(w.cell))) == 0:
+        pairs, terms, far, m_img = count_pair_terms(w, pos[:4])
+        row = 2 * m_img + 1
+        n_cand = 20 if (w.dim == 3 and m_img == 1) else row ** w.dim
+        per_pair = 12 + 5 * w.dim * row + 2 * n_cand
+        flops = per_pair * pairs + 12.0 * (terms - far) + 4.0 * far
+        return {"pairs_per_walker": pairs, "pair_image_terms_per_walker": terms, "far_shell_terms_per_walker": far,
+                "candidates_per_pair": n_cand, "alg_flops_per_walker_fp64_equiv": flops}
+    pairs = w.n * (w.n - 1) // 2 + w.n * n_ion   # general cell: the image list is scanned, terms not counted here
+    return {"pairs_per_walker": pairs, "pair_image_terms_per_walker": None, "images_scanned_per_pair": n_images,
+            "alg_flops_per_walker_fp64_equiv": (21 + 6 * n_images) * pairs}
+
+
+def kernel_report(E, ctx, w, pos, prec, W, prof, n_prof, peak_tf):
+    """Per-kernel device times (CUDA events inside the library, on its launch stream) and what SURVEY 8(d) asks
+    for each kernel: reciprocal = algorithmic 2 N N_G flops per walker over the measured FMA-chain peak;
+    real space = pair-image terms/s and FP64-equivalent flops over the same peak."""
+    kernels = {}
+    for name, (ms, cnt) in prof.items():
+        if cnt:
+            kernels[name] = {"ms_per_launch": ms / cnt, "launches_per_step": cnt / n_prof}
+    step_ms = sum(k["ms_per_launch"] * k["launches_per_step"] for k in kernels.values())
+    for k in kernels.values():
+        k["share_of_step"] = k["ms_per_launch"] * k["launches_per_step"] / step_ms
+    n_g = E.ewald_num_g(ctx)
+    recip_flops = 2.0 * w.n * n_g * W
+    t_rec = kernels["recip"]["ms_per_launch"] * 1e-3
+    kernels["recip"].update(alg_flops_per_launch=recip_flops, achieved_tflops=recip_flops / t_rec / 1e12,
+                            frac_of_peak=recip_flops / t_rec / 1e12 / peak_tf)
+    work = real_space_work(w, pos, E.ewald_num_images(ctx))
+    t_real = kernels["real"]["ms_per_launch"] * 1e-3
+    real_flops = work["alg_flops_per_walker_fp64_equiv"] * W * (1.0 if prec == "f64" else 0.5)
+    kernels["real"].update(work)
+    if work["pair_image_terms_per_walker"] is not None:
+        kernels["real"]["pair_image_terms_per_s"] = work["pair_image_terms_per_walker"] * W / t_real
+    kernels["real"].update(alg_flops_per_launch=real_flops, achieved_tflops=real_flops / t_real / 1e12,
+                           frac_of_peak=real_flops / t_real / 1e12 / peak_tf)
+    return kernels
+
+
+def energy_leg(torch, E, device, stream, idx, prec, steps, flush, peak_tf, n_oracle):
+    """One energy workload, device-resident: walker-energies/s (CUDA events per step, L2 flushed in between),
+    per-kernel times, and parity of the first n_oracle walkers against the oracle (same inputs as the GPU got)."""
+    w = workloads.config(idx)
+    W = w.n_walkers
+    npdt = np.float64 if prec == "f64" else np.float32
+    pos = w.positions(W)
+    ctx = E.ewald_setup(w.dim, w.cell, w.kappa, w.g_cutoff, w.r_cutoff, device=device, stream=stream)
+    if w.ion_pos is not None:
+        E.ewald_set_fixed_charges(ctx, w.ion_pos, w.ion_q)
+    soa = E.to_soa(pos, npdt)
+    d_pos = torch.from_numpy(soa).cuda()
+    d_q = torch.from_numpy(w.charges.astype(npdt)).cuda()
+    d_e = torch.zeros(W, dtype=torch.float64, device="cuda")
+    for _ in range(3):
+        E.ewald_energy_batch(ctx, w.n, d_pos, d_q, d_e)
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
+    for a, b in ev:
+        flush.zero_()
+        a.record()
+        E.ewald_energy_batch(ctx, w.n, d_pos, d_q, d_e)
+        b.record()
+    torch.cuda.synchronize()
+    ms = sum(a.elapsed_time(b) for a, b in ev) / steps
+    n_prof = min(steps, 20)
+    E.ewald_profile_enable(ctx, True)
+    for _ in range(n_prof):
+        flush.zero_()
+        E.ewald_energy_batch(ctx, w.n, d_pos, d_q, d_e)
+    prof = E.ewald_profile_read(ctx)
+    E.ewald_profile_enable(ctx, False)
+    kernels = kernel_report(E, ctx, w, pos, prec, W, prof, n_prof, peak_tf)
+    out = {"workload": workload_config(w, W, "flushed")["workload"], "dtype": prec, "walkers": W, "value": W / (ms * 1e-3),
+           "unit": UNIT, "ms_per_step": ms, "steps": steps,
+           "kernels": {k: {kk: v[kk] for kk in ("ms_per_launch", "share_of_step", "frac_of_peak", "achieved_tflops",
+                                                "pair_image_terms_per_s") if kk in v} for k, v in kernels.items()}}
+    if n_oracle:
+        from oracle import ewald_ref as ref
+        sample = pos[:n_oracle] if prec == "f64" else pos[:n_oracle].astype(np.float32).astype(np.float64)
+        e_ref, _ = ref.energy_batch(w.dim, w.cell, w.kappa, w.g_cutoff, w.r_cutoff, sample, w.charges, w.ion_pos, w.ion_q)
+        got = d_e.cpu().numpy()[:n_oracle]
+        out["parity_max_rel_err_vs_oracle"] = float((np.abs(got - e_ref) / np.abs(e_ref)).max())
+        out["parity_walkers"] = int(n_oracle)
+    E.ewald_destroy(ctx)
+    return out
 
 
 def move_leg(torch, E, device, stream, prec, n_steps, flush, hbm_peak_gbs):
@@ -209,13 +306,23 @@ def move_leg(torch, E, device, stream, prec, n_steps, flush, hbm_peak_gbs):
     bytes_per_move = 2 * ngp * 2 * es + w.dim * w.n * es
     gbs = bytes_per_move * W / t / 1e9
     E.ewald_destroy(ctx)
+    # parity of the timed moves themselves: the chains of the first 4 walkers against the oracle (reading R12)
+    from oracle import ewald_ref as ref
+    k = 4
+    r32 = (lambda a: a) if prec == "f64" else (lambda a: a.astype(np.float32).astype(np.float64))
+    de_ref, _, _ = ref.move_chain(w.dim, w.cell, w.kappa, w.g_cutoff, w.r_cutoff, r32(pos0[:k]), w.charges,
+                                  electron[:, :k], r32(new_r[:, :k]))
+    de = d_de.cpu().numpy()[:, :k]
+    rms = np.sqrt((de_ref ** 2).mean(axis=1, keepdims=True))
+    parity = float((np.abs(de - de_ref) / np.maximum(np.abs(de_ref), rms)).max())
     return {"workload": "BASELINE configs[4]: %s" % w.name, "dtype": prec, "moves_per_s": W / t,
             "ms_per_batch_of_%d_moves" % W: t * 1e3, "timed_batches": len(ms), "warmup_batches": warm,
             "roofline": {"kernel": "move", "bound": "hbm", "unit": "GB/s", "achieved": gbs, "peak": hbm_peak_gbs,
                          "frac": gbs / hbm_peak_gbs, "alg_bytes_per_move": bytes_per_move,
                          "alg_bytes_per_launch": bytes_per_move * W,
                          "traffic": recorded_traffic("cfg5_%s" % prec, "move")},
-            "delta_e_finite": bool(torch.isfinite(d_de).all().item())}
+            "delta_e_finite": bool(torch.isfinite(d_de).all().item()),
+            "parity_max_err_vs_oracle_R12": parity, "parity_walkers": k, "parity_steps": S}
 
 
 def workload_config(w, walkers_per_gpu, l2_note):
@@ -326,6 +433,12 @@ def main():
            "d2h_bytes_per_step": int(h_e.numel() * 8)}
     assert np.array_equal(h_e.numpy(), d_e.cpu().numpy())
 
+    # ---- roofline denominators measured in this run: FMA-chain (and DMMA) probes of the library ----------
+    peaks = measured_peaks()
+    chain = {"f64": E.ewald_probe_fma(ctx, E.EWALD_F64, 2048) / 1e12, "f32": E.ewald_probe_fma(ctx, E.EWALD_F32, 4096) / 1e12}
+    dmma_tf = E.ewald_probe_dmma(ctx, 2048) / 1e12
+    peak_tf = chain[args.prec]
+
     # ---- per-kernel device times (CUDA events inside the library, on its launch stream) -----
     n_prof = min(args.steps, 50)
     E.ewald_profile_enable(ctx, True)
@@ -334,48 +447,21 @@ def main():
         step()
     prof = E.ewald_profile_read(ctx)
     E.ewald_profile_enable(ctx, False)
-    peaks = measured_peaks()
-    sm_max_hz = 1e6 * float(peaks.get("sm_max_mhz", 1965.0))
-    lanes = FP64_LANES if args.prec == "f64" else FP32_LANES
-    peak_flops = SM_COUNT * lanes * 2 * sm_max_hz      # derived ALU peak
-    n_g = E.ewald_num_g(ctx)
-    kernels = {}
-    for name, (ms, cnt) in prof.items():
-        if cnt:
-            kernels[name] = {"ms_per_launch": ms / cnt, "launches_per_step": cnt / n_prof}
-    step_ms = sum(k["ms_per_launch"] * k["launches_per_step"] for k in kernels.values())
-    for k in kernels.values():
-        k["share_of_step"] = k["ms_per_launch"] * k["launches_per_step"] / step_ms
-    # reciprocal kernel: algorithmic flops = 2 N N_G per walker (1 FMA per particle and G of the full sphere)
-    recip_flops = 2.0 * w.n * n_g * W
-    kernels["recip"].update(alg_flops_per_launch=recip_flops,
-                            achieved_tflops=recip_flops / (kernels["recip"]["ms_per_launch"] * 1e-3) / 1e12,
-                            frac_of_peak=recip_flops / (kernels["recip"]["ms_per_launch"] * 1e-3) / peak_flops)
-    # real-space kernel: algorithmic flops = per pair (displacement, reduction to the cell, image squares and sums)
-    # + 12 per pair-image term (u = t - centre, quintic Horner, accumulate), all counted as FP64
-    if np.count_nonzero(w.cell - np.diag(np.diag(w.cell))) == 0:
-        pairs, terms, n_cand, m_img = count_pair_terms(w, pos[:4])
-        row = 2 * m_img + 1
-        per_pair = 21 + 2 * w.dim * row + (row * row if w.dim == 3 else 0) + n_cand
-    else:   # general cell (image-list scan): 21 flops per pair + 6 per scanned image; terms not counted here
-        n_img = E.ewald_num_images(ctx)
-        pairs = w.n * (w.n - 1) // 2 + w.n * (0 if w.ion_q is None else len(w.ion_q))
-        terms, per_pair = float("nan"), 21 + 6 * n_img
-    real_flops = (per_pair * pairs + (0.0 if terms != terms else 12.0 * terms)) * W
-    t_real = kernels["real"]["ms_per_launch"] * 1e-3
-    kernels["real"].update(pairs_per_walker=pairs, pair_image_terms_per_walker=terms,
-                           pair_image_terms_per_s=terms * W / t_real, alg_flops_per_launch=real_flops,
-                           achieved_tflops=real_flops / t_real / 1e12, frac_of_peak=real_flops / t_real / peak_flops)
+    kernels = kernel_report(E, ctx, w, pos, args.prec, W, prof, n_prof, peak_tf)
     dominant = max(("recip", "real"), key=lambda k: kernels[k]["share_of_step"])
-    roofline = {"kernel": dominant, "bound": "alu", "unit": "TFLOP/s", "peak": peak_flops / 1e12,
-                "peak_source": "derived: %d SMs x %d %s lanes x 2 x %.0f MHz (sm_max_mhz); the FMA-chain probe "
-                               "in extras measures it" % (SM_COUNT, lanes, args.prec, sm_max_hz / 1e6),
+    sm_max_mhz = float(peaks.get("sm_max_mhz", 1965.0))
+    lanes = FP64_LANES if args.prec == "f64" else FP32_LANES
+    roofline = {"kernel": dominant, "bound": "alu", "unit": "TFLOP/s", "peak": peak_tf,
+                "peak_source": "measured in this run: %s FMA-chain probe of the library (ewald_probe_fma); derived "
+                               "%d SMs x %d lanes x 2 x %.0f MHz = %.2f; FP64 tensor (DMMA) probe %.2f"
+                               % (args.prec, SM_COUNT, lanes, sm_max_mhz, SM_COUNT * lanes * 2 * sm_max_mhz * 1e-6, dmma_tf),
                 "achieved": kernels[dominant]["achieved_tflops"], "frac": kernels[dominant]["frac_of_peak"],
                 "traffic": recorded_traffic("cfg%d_%s" % (args.config, args.prec), dominant),
-                "traffic_note": "DRAM bytes per launch (ncu, profiles/r01b_ncu_summary.md); algorithmic: the positions "
-                                "once = %d bytes" % (soa.nbytes),
-                "note": "algorithmic flops per DESIGN.md section 6; the real-space kernel is limited by "
-                        "shared-memory wavefronts (table gathers), see profiles/"}
+                "traffic_note": "DRAM bytes per launch (ncu --set full, profiles/r02_traffic.json); algorithmic: the "
+                                "positions once = %d bytes" % (soa.nbytes),
+                "note": "real-space kernel: FP64-equivalent algorithmic flops (DESIGN.md section 6: enumerated candidates, "
+                        "near terms FP64, far-shell terms FP32 at half weight); it is limited by shared-memory "
+                        "wavefronts, see profiles/ and kernels.real.pair_image_terms_per_s"}
 
     out = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
            "warmup": max(args.warmup, 3), "ms_per_step": ms_total / args.steps, "higher_is_better": True,
@@ -385,16 +471,7 @@ def main():
            "kernels": kernels, "wall_s_timed_region": t_wall}
 
     if rank == 0 and not args.no_extras:
-        extras = {}
-        try:
-            extras["fma_chain_tflops"] = {"f64": E.ewald_probe_fma(ctx, E.EWALD_F64, 2048) / 1e12,
-                                          "f32": E.ewald_probe_fma(ctx, E.EWALD_F32, 4096) / 1e12}
-            # ceiling of the octant kernel's FMA phase: its 4 x 15 register tile alone, 7 and 8 warps per SM
-            pe = E.EWALD_F64 if args.prec == "f64" else E.EWALD_F32
-            extras["recip_tile_ceiling_tflops"] = {"threads_224": E.ewald_probe_fma_tile(ctx, pe, 20000, 224) / 1e12,
-                                                   "threads_256": E.ewald_probe_fma_tile(ctx, pe, 20000, 256) / 1e12}
-        except Exception as ex:  # the probe is informative only
-            extras["fma_chain_tflops"] = str(ex)
+        extras = {"fma_chain_tflops": chain, "dmma_tflops": dmma_tf}
         # the other precision of the same workload (BASELINE configs[1] is quoted in FP64 and FP32)
         other = "f32" if args.prec == "f64" else "f64"
         o_np, o_t = (np.float32, torch.float32) if other == "f32" else (np.float64, torch.float64)
@@ -416,6 +493,10 @@ def main():
         # single-move Delta-E/s (BASELINE.json's second metric), both precisions
         hbm = float(peaks.get("hbm_gbs", 6542.1))
         extras["single_move"] = [move_leg(torch, E, local, stream, p, 100, flush, hbm) for p in ("f64", "f32")]
+        # the other workloads of BASELINE.json (configs 1, 3, 4) and SURVEY 8(f) NEXT-1 (config 6), short runs
+        extras["per_config"] = [energy_leg(torch, E, local, stream, idx, p, 30, flush, chain[p], n_or)
+                                for idx, p, n_or in ((1, "f64", 8), (3, "f64", 16), (3, "f32", 16), (4, "f64", 16),
+                                                     (6, "f64", 2))]
         out["extras"] = extras
     if rank == 0 and world == 1 and not args.no_extras:
         from oracle import ewald_ref as ref

@@ -390,6 +390,9 @@ def ewald_probe_dmma(ctx, iters=4096):
     return f.value
 
 
+KERNEL_CLASSES = ("recip", "real", "combine", "move")
+
+
 def ewald_profile_enable(ctx, on=True):
     _check(ctx, load_library().ewald_profile_enable(ctx.handle, int(bool(on))))
 
