@@ -153,5 +153,41 @@ def hbn_hexagonal():
                     cell=cell, charges=-np.ones(n), ion_pos=ions, ion_q=q, g_cut=2.0 * kappa * x)
 
 
+class JastrowWorkload:
+    """the homogeneous two-body Jastrow terms u (Eq. 6) and p
+    (Eq. 7) on the electron gas of a BASELINE energy config.  Inputs only: the integer G vectors of
+    the first n_stars stars of the cubic (square) cell -- a star = the G related by permutations and sign changes of
+    (n1, n2, n3), one G of each +-G pair kept -- seeded coefficients a_m decaying like 1/|n|^2, and a seeded
+    polynomial u with N_u = 8, C = 3 and L_u = 0.49 L (below half the distance to the nearest lattice point,
+    PAPER.md:151).  They stand in for CASINO's optimised Jastrow parameters, which are not available."""
+
+    def __init__(self, base_index=2, n_stars=15, n_u=8, C=3, seed=250702888 + 70):
+        w = config(base_index)
+        self.base, self.dim, self.cell, self.L, self.n, self.n_walkers = w, w.dim, w.cell, w.L, w.n, w.n_walkers
+        rng = np.random.Generator(np.random.PCG64(seed))
+        m = 6
+        rngs = [range(-m, m + 1)] * w.dim + [range(0, 1)] * (3 - w.dim)
+        stars = {}
+        for n1 in rngs[0]:
+            for n2 in rngs[1]:
+                for n3 in rngs[2]:
+                    v = (n1, n2, n3)
+                    if v == (0, 0, 0) or next(c for c in v if c != 0) < 0:   # keep one G of each +-G pair
+                        continue
+                    key = (n1 * n1 + n2 * n2 + n3 * n3, tuple(sorted(abs(c) for c in v)))
+                    stars.setdefault(key, []).append(v)
+        keys = sorted(stars)[:n_stars]
+        self.g_n = np.array([v for k in keys for v in stars[k]], dtype=np.int32)
+        self.star = np.array([i for i, k in enumerate(keys) for _ in stars[k]], dtype=np.int32)
+        self.a = np.array([0.05 * rng.uniform(0.5, 1.5) / k[0] for k in keys])
+        self.n_stars = len(keys)
+        self.C, self.L_u = C, 0.49 * w.L
+        # u(r) = (r - L_u)^C sum alpha_l r^l: coefficients so that every term is O(0.1) at r ~ L_u / 2
+        self.alpha = np.array([0.1 * rng.uniform(-1, 1) / (0.5 * self.L_u) ** (l + C) for l in range(n_u + 1)])
+
+    def positions(self, n_walkers=None):
+        return self.base.positions(n_walkers)
+
+
 def all_configs():
     return [config(i) for i in range(1, 6)]   # the five BASELINE.json configs; config(6) is the NEXT-1 workload
