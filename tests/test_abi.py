@@ -30,6 +30,20 @@ def test_header_symbols_all_exported():
     assert sorted(E.SYMBOLS) == declared, "binding's symbol list differs from the header"
 
 
+def test_jastrow_header_symbols_exported_and_bound():
+    """include/jastrow.h: every declared call is exported by the library and has a
+    binding of the same name."""
+    from paper_2507_02888_b200 import jastrow as J
+    text = re.sub(r"/\*.*?\*/", "", open(os.path.join(ROOT, "include", "jastrow.h")).read(), flags=re.S)
+    declared = sorted(set(re.findall(r"\b(jastrow_[a-z0-9_]+)\s*\(", text)))
+    lib = ctypes.CDLL(E.load_library()._name)
+    assert len(declared) == 8 and declared == sorted(J.SYMBOLS)
+    for name in declared:
+        assert hasattr(lib, name), "library does not export %s" % name
+        if name != "jastrow_last_error":
+            assert hasattr(J, name), "python binding lacks %s" % name
+
+
 def test_binding_has_same_names():
     for name in _declared_symbols():
         if name in ("ewald_last_error", "ewald_destroy"):
@@ -155,6 +169,10 @@ def test_octant_plan_covers_every_g_once():
             assert 4 <= o["npb"] <= 7 and o["n_warps"] >= max(4, -(-wc * o["n_items"] // 32))
             # executed FMA + products per particle can never be below the algorithmic N_G + 1
             assert o["fma_per_particle"] >= ng + 1
+        # the tensor-core plan covers the same set: weights, and 64 FMAs per DMMA and particle >= N_G + 1
+        m = E.ewald_mma_plan_summary(w.dim, w.cell, w.kappa, w.g_cutoff)
+        assert abs(m["weight_sum"] - want) <= 1e-13 * want and m["walkers_per_pass"] >= 1
+        assert ng + 1 <= 64 * m["dmma_per_quad"] <= 1.6 * (ng + 1)
         assert (ng + 1) / o["fma_per_particle"] > 0.7    # wc = 7: products + padding cost < 43 % of the algorithmic FMAs (config 1; 22 % on config 2)
 
 
