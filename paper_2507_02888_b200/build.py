@@ -11,8 +11,8 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 ROOT = os.path.dirname(HERE)
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libewald_b200.so")
-SOURCES = ["ewald_api.cu", "jastrow_api.cu", "ewald_setup.cpp", "ewald_octplan.cpp"]
-HEADERS = [os.path.join(ROOT, "include", "ewald.h"), os.path.join(ROOT, "include", "jastrow.h"),
+SOURCES = ["ewald_api.cu", "jastrow_api.cu", "blip_api.cu", "ewald_setup.cpp", "ewald_octplan.cpp"]
+HEADERS = [os.path.join(ROOT, "include", "ewald.h"), os.path.join(ROOT, "include", "jastrow.h"), os.path.join(ROOT, "include", "blip.h"),
            os.path.join(CSRC, "ewald_internal.h"), os.path.join(CSRC, "jastrow_kernels.cuh"),
            os.path.join(CSRC, "ewald_recip_mma.cuh"),
            os.path.join(CSRC, "ewald_kernels.cuh"),

@@ -189,5 +189,25 @@ class JastrowWorkload:
         return self.base.positions(n_walkers)
 
 
+class BlipWorkload:
+    """orbitals in a blip basis on the electron gas of BASELINE configs[1] (N = 250,
+    so 125 doubly occupied orbitals), a 24^3 blip grid, seeded N(0, 1) coefficients smoothed over neighbouring grid
+    points (they stand in for the plane-wave orbitals CASINO re-represents, which are not available).
+    A batch = the positions of all electrons of n_walkers walkers."""
+
+    def __init__(self, base_index=2, n_orb=125, grid=(24, 24, 24), seed=250702888 + 90):
+        w = config(base_index)
+        self.base, self.cell, self.n, self.n_walkers, self.n_orb, self.grid = w, w.cell, w.n, w.n_walkers, n_orb, grid
+        rng = np.random.Generator(np.random.PCG64(seed))
+        c = rng.standard_normal((n_orb,) + tuple(grid))
+        for ax in (1, 2, 3):
+            c = 0.5 * c + 0.25 * (np.roll(c, 1, axis=ax) + np.roll(c, -1, axis=ax))
+        self.coef = c
+
+    def points(self, n_walkers=None):
+        """All electron positions of the first n_walkers walkers as [P, 3]."""
+        return self.base.positions(n_walkers).reshape(-1, 3)
+
+
 def all_configs():
     return [config(i) for i in range(1, 6)]   # the five BASELINE.json configs; config(6) is the NEXT-1 workload

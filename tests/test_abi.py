@@ -44,6 +44,19 @@ def test_jastrow_header_symbols_exported_and_bound():
             assert hasattr(J, name), "python binding lacks %s" % name
 
 
+def test_blip_header_symbols_exported_and_bound():
+    """include/blip.h."""
+    from paper_2507_02888_b200 import blip as B
+    text = re.sub(r"/\*.*?\*/", "", open(os.path.join(ROOT, "include", "blip.h")).read(), flags=re.S)
+    declared = sorted(set(re.findall(r"\b(blip_[a-z0-9_]+)\s*\(", text)))
+    lib = ctypes.CDLL(E.load_library()._name)
+    assert len(declared) == 6 and declared == sorted(B.SYMBOLS)
+    for name in declared:
+        assert hasattr(lib, name), "library does not export %s" % name
+        if name != "blip_last_error":
+            assert hasattr(B, name), "python binding lacks %s" % name
+
+
 def test_binding_has_same_names():
     for name in _declared_symbols():
         if name in ("ewald_last_error", "ewald_destroy"):
