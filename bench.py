@@ -267,6 +267,111 @@ def energy_leg(torch, E, device, stream, idx, prec, steps, flush, peak_tf, n_ora
     return out
 
 
+def jastrow_leg(torch, device, stream, flush, chain_tf, steps=20):
+    """u + p Jastrow terms (value, gradient, Laplacian) of all 1024 walkers of
+    BASELINE configs[1] per launch; algorithmic flops per walker: p term 14 N N_G (structure
+    factor) + 24 N N_G (per-particle derivatives), u term 20 per ordered pair + 80 per pair inside L_u."""
+    from oracle import jastrow_ref as jr
+    from paper_2507_02888_b200 import ewald as E, jastrow as J
+    j = workloads.JastrowWorkload(base_index=2, n_stars=15)
+    out = []
+    pos = j.positions()
+    W, n = pos.shape[0], j.n
+    npad = E.ewald_padded_n(n)
+    inside = (4.0 / 3.0) * math.pi * j.L_u ** 3 / j.L ** 3
+    flops = 38.0 * n * len(j.g_n) + n * (n - 1) * (20.0 + 80.0 * inside)
+    k = 4
+    t0 = time.perf_counter()
+    want = jr.batch(3, j.cell, pos[:k], j.alpha, j.L_u, j.C, j.g_n, j.star, j.a)
+    t_or = time.perf_counter() - t0
+    for prec in ("f64", "f32"):
+        npdt = np.float64 if prec == "f64" else np.float32
+        ctx = J.jastrow_setup(3, j.cell, alpha=j.alpha, l_u=j.L_u, c_exp=j.C, g_n=j.g_n, star=j.star, a=j.a,
+                              device=device, stream=stream)
+        d_pos = torch.from_numpy(E.to_soa(pos, npdt)).cuda()
+        val = torch.zeros(W, dtype=torch.float64, device="cuda")
+        grad = torch.zeros((W, 3, npad), dtype=torch.float64, device="cuda")
+        lap = torch.zeros((W, npad), dtype=torch.float64, device="cuda")
+        for _ in range(3):
+            J.jastrow_batch(ctx, n, d_pos, val, grad, lap)
+        J.jastrow_profile_enable(ctx, True)
+        for _ in range(steps):
+            flush.zero_()
+            J.jastrow_batch(ctx, n, d_pos, val, grad, lap)
+        ms, cnt = J.jastrow_profile_read(ctx)
+        t = ms / cnt * 1e-3
+        g = grad.cpu().numpy()[:k, :, :n].transpose(0, 2, 1)
+        err = max(float((np.abs(val.cpu().numpy()[:k] - want[0]) / np.abs(want[0])).max()),
+                  float((np.abs(g - want[1]).max(axis=(1, 2)) / np.abs(want[1]).max(axis=(1, 2))).max()),
+                  float((np.abs(lap.cpu().numpy()[:k, :n] - want[2]).max(axis=1) / np.abs(want[2]).max(axis=1)).max()))
+        peak = chain_tf[prec]
+        out.append({"workload": "u + p Jastrow terms on BASELINE configs[1] (N = 250, 1024 walkers, %d stars / %d G, N_u = %d)"
+                                % (j.n_stars, len(j.g_n), len(j.alpha) - 1), "dtype": prec,
+                    "walker_evaluations_per_s": W / t, "ms_per_launch": t * 1e3,
+                    "roofline": {"kernel": "jastrow", "bound": "alu", "unit": "TFLOP/s", "achieved": flops * W / t / 1e12,
+                                 "peak": peak, "frac": flops * W / t / 1e12 / peak, "alg_flops_per_walker": flops,
+                                 "traffic": None},
+                    "parity_max_rel_err_vs_oracle": err, "parity_walkers": k, "parity_inputs": "oracle on the FP64 positions",
+                    "cpu_baseline": {"value": k / t_or, "unit": "walker-evaluations/s", "kind": "oracle (pair by pair, O(N^2 N_G))",
+                                     "cores": jr._load().jastrow_ref_max_threads(), "sample": "%d walkers, %.1f s" % (k, t_or)}})
+        J.jastrow_destroy(ctx)
+    return out
+
+
+def blip_leg(torch, device, stream, flush, hbm_gbs, steps=10):
+    """125 blip orbitals (24^3 grid) at the 256 000 electron positions of the 1024 walkers of
+    BASELINE configs[1] per launch: value, gradient, Laplacian.  Algorithmic bytes per position: the gather of
+    64 x n_orb coefficients (served by L2: the table is 14 MB in FP64) + the 5 n_orb doubles written to HBM."""
+    from oracle import blip_ref as br
+    from paper_2507_02888_b200 import blip as B
+    wl = workloads.BlipWorkload()
+    pts = wl.points()
+    P = len(pts)
+    npad = (P + 3) & ~3
+    k = 32
+    t0 = time.perf_counter()
+    want = br.evaluate(wl.cell, wl.coef, pts[:k])
+    t_or = time.perf_counter() - t0
+    out = []
+    for prec in ("f64", "f32"):
+        npdt, es = (np.float64, 8) if prec == "f64" else (np.float32, 4)
+        ctx = B.blip_setup(wl.cell, wl.coef, device=device, stream=stream)
+        soa = np.zeros((3, npad), dtype=npdt)
+        soa[:, :P] = pts.T
+        d_pts = torch.from_numpy(soa).cuda()
+        psi = torch.zeros((P, wl.n_orb), dtype=torch.float64, device="cuda")
+        grad = torch.zeros((P, 3, wl.n_orb), dtype=torch.float64, device="cuda")
+        lap = torch.zeros((P, wl.n_orb), dtype=torch.float64, device="cuda")
+        for _ in range(2):
+            B.blip_eval_batch(ctx, P, d_pts, psi, grad, lap)
+        B.blip_profile_enable(ctx, True)
+        for _ in range(steps):
+            flush.zero_()
+            B.blip_eval_batch(ctx, P, d_pts, psi, grad, lap)
+        ms, cnt = B.blip_profile_read(ctx)
+        t = ms / cnt * 1e-3
+        got = (psi[:k].cpu().numpy(), grad[:k].cpu().numpy(), lap[:k].cpu().numpy())
+        err = max(float((np.abs(g - w_).reshape(k, -1).max(axis=1) / np.abs(w_).reshape(k, -1).max(axis=1)).max())
+                  for g, w_ in zip(got, want))
+        gather = 64.0 * wl.n_orb * es * P
+        written = 5.0 * wl.n_orb * 8 * P
+        out.append({"workload": "%d blip orbitals on a %dx%dx%d grid at %d positions (1024 walkers x 250 electrons)"
+                                % ((wl.n_orb,) + tuple(wl.grid) + (P,)), "dtype": prec,
+                    "orbital_evaluations_per_s": P * wl.n_orb / t, "ms_per_launch": t * 1e3,
+                    "roofline": {"kernel": "blip", "bound": "hbm", "unit": "GB/s", "achieved": written / t / 1e9,
+                                 "peak": hbm_gbs, "frac": written / t / 1e9 / hbm_gbs,
+                                 "alg_bytes_written_per_launch": written, "l2_gather_bytes_per_launch": gather,
+                                 "l2_gather_gbs": gather / t / 1e9, "traffic": None,
+                                 "note": "HBM: the outputs (5 doubles per position and orbital); the coefficient gather is "
+                                         "served by L2"},
+                    "achieved_tflops": 10.0 * 64 * wl.n_orb * P / t / 1e12,
+                    "parity_max_rel_err_vs_oracle": err, "parity_positions": k,
+                    "cpu_baseline": {"value": k * wl.n_orb / t_or, "unit": "orbital-evaluations/s", "kind": "oracle (every grid point)",
+                                     "cores": "OpenMP", "sample": "%d positions, %.1f s" % (k, t_or)}})
+        B.blip_destroy(ctx)
+    return out
+
+
 def move_leg(torch, E, device, stream, prec, n_steps, flush, hbm_peak_gbs):
     """BASELINE configs[4]: 3D HEG N = 1000, 4096 walkers with stored rho(G); each step moves one seeded-random
     electron per walker by a Gaussian step (reading R14), always committed.  Returns moves/s (device-resident,
@@ -497,6 +602,9 @@ def main():
         extras["per_config"] = [energy_leg(torch, E, local, stream, idx, p, 30, flush, chain[p], n_or)
                                 for idx, p, n_or in ((1, "f64", 8), (3, "f64", 16), (3, "f32", 16), (4, "f64", 16),
                                                      (6, "f64", 2))]
+        # SURVEY 8(f) NEXT-2/3 (Jastrow u and p terms) and NEXT-4 (blip orbitals), each with parity and its roofline
+        extras["next"] = {"jastrow": jastrow_leg(torch, local, stream, flush, chain),
+                          "blip": blip_leg(torch, local, stream, flush, hbm)}
         out["extras"] = extras
     if rank == 0 and world == 1 and not args.no_extras:
         from oracle import ewald_ref as ref
