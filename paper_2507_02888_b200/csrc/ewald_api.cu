@@ -52,6 +52,7 @@ struct ewald_ctx {
     std::map<long long, OctDev> oct_dev;   /* key: wc | prec << 16 */
     std::map<long long, int> oct_choice;   /* key: W | prec << 40 | n << 41 ... -> wc */
     std::vector<ProfRec> recs;
+    std::vector<void *> retired;           /* outgrown scratch buffers, freed at destroy */
     long long launches = 0; /* kernels launched since setup */
     HostTables t;
     int device = 0;
@@ -136,10 +137,12 @@ static ewald_status fail(ewald_ctx *c, ewald_status s, const char *msg)
     return s;
 }
 
+/* Grows a scratch buffer without synchronising the stream: kernels already enqueued may still use the old
+ * allocation, so it is retired (freed by ewald_destroy or the next synchronising call), not freed here. */
 static ewald_status ensure(ewald_ctx *c, DevBuf *b, size_t bytes)
 {
     if (bytes <= b->cap) return EWALD_OK;
-    if (b->p) { CU_TRY(c, cudaStreamSynchronize(c->stream)); CU_TRY(c, cudaFree(b->p)); b->p = nullptr; b->cap = 0; }
+    if (b->p) { c->retired.push_back(b->p); b->p = nullptr; b->cap = 0; }
     size_t want = bytes + bytes / 4 + 256;
     CU_TRY(c, cudaMalloc(&b->p, want));
     b->cap = want;
@@ -375,6 +378,7 @@ extern "C" void ewald_destroy(ewald_ctx *c)
                       &c->mv_de, &c->st_pos, &c->st_q, &c->st_rho, &c->st_qinfo};
     for (DevBuf *b : bufs) release(b);
     for (ProfRec &r : c->recs) { cudaEventDestroy(r.a); cudaEventDestroy(r.b); }
+    for (void *p : c->retired) cudaFree(p);
     delete c;
 }
 
@@ -848,7 +852,7 @@ static ewald_status launch_real(ewald_ctx *c, int W, int n, const T *pos, const 
     fill_geom(c->t, &A.g);
     const bool ortho = real_ortho(c);
     if (ortho) A.nimg = 0; /* the orthorhombic path does not read the image list */
-    const size_t fixed = RealSmem<T>::fixed_bytes(A.P.n_bins, A.P.n_far, A.nimg, A.n_ion, (size_t)(c->t.dim + 1) * n);
+    const size_t fixed = RealSmem<T>::fixed_bytes(A.P.n_bins, A.P.n_far, A.nimg, A.n_ion, (size_t)c->t.dim * ewald_padded_n(n) + n);
     int threads = 0; size_t smem = 0;
     if (!real_shape<T>(c, fixed, real_min_cap(c, ortho, true), real_min_cap(c, ortho, false), REAL_MAX_THREADS, &A.P,
                        &threads, &smem))

@@ -278,7 +278,7 @@ __device__ __forceinline__ double real_body(const RealArgs<T> &A, RealSmem<T> &S
                     int j = i + pw.k + 1;
                     if (j >= n) j -= n;
 #pragma unroll
-                    for (int x = 0; x < DIM; x++) d[x] = sp[x * n + i] - sp[x * n + j];
+                    for (int x = 0; x < DIM; x++) d[x] = sp[x * A.npad + i] - sp[x * A.npad + j];
                     if (!UQ) w = sq[i] * sq[j];
                 }
                 scan_pair<T, DIM, ORTHO, M, UQ, false, false, GROUP == 1>(A.g, d, w, valid, st, direct, S.img, A.nimg,
@@ -304,7 +304,7 @@ __device__ __forceinline__ double real_body(const RealArgs<T> &A, RealSmem<T> &S
             if (valid) {
                 const int i = pw.i, I = pw.k;
 #pragma unroll
-                for (int x = 0; x < DIM; x++) d[x] = sp[x * n + i] - S.ion[4 * I + x];
+                for (int x = 0; x < DIM; x++) d[x] = sp[x * A.npad + i] - S.ion[4 * I + x];
                 if (!UQ) w = sq[i] * S.ion[4 * I + 3];
             }
             scan_pair<T, DIM, ORTHO, M, UQ>(A.g, d, w, valid, st, direct, S.img, A.nimg);
@@ -320,18 +320,21 @@ template <typename T, int DIM, bool ORTHO, int M>
 __global__ void __launch_bounds__(REAL_MAX_THREADS) real_kernel(RealArgs<T> A)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    RealSmem<T> S(smem_raw, A.P, A.nimg, A.n_ion, (size_t)(DIM + 1) * A.n);
-    T *sp = S.rest;             /* [DIM][n] positions (unscaled: differences are taken first) */
-    T *sq = sp + DIM * A.n;     /* [n] charges */
-    __shared__ double red[32];
+    RealSmem<T> S(smem_raw, A.P, A.nimg, A.n_ion, (size_t)DIM * A.npad + A.n);
+    T *sp = S.rest;                 /* [DIM][npad] positions (unscaled: differences are taken first) */
+    T *sq = sp + DIM * A.npad;      /* [n] charges */
+    /* static shared memory stays a multiple of 128 bytes: the dynamic part (tables, lane stacks whose rows are
+     * 128 / 256 bytes) keeps its 128-byte alignment; red[32] holds the mbarrier of the bulk copy */
+    __shared__ __align__(128) double red[48];
+    uint64_t *bar = reinterpret_cast<uint64_t *>(&red[32]);
     const int w = blockIdx.x / A.n_tiles, tile = blockIdx.x - w * A.n_tiles, tid = threadIdx.x;
-    const T *pw = A.pos + (size_t)w * DIM * A.npad;
-    for (int t = tid; t < A.n; t += blockDim.x) {
-#pragma unroll
-        for (int x = 0; x < DIM; x++) sp[x * A.n + t] = pw[x * A.npad + t];
-        sq[t] = A.q[t];
-    }
+    /* the walker's SoA block [DIM][npad] is contiguous: one TMA bulk copy stages it while the threads copy the tables */
+    if (tid == 0) tma_barrier_init(bar);
+    __syncthreads();
+    if (tid == 0) tma_load_1d(sp, A.pos + (size_t)w * DIM * A.npad, (unsigned)(DIM * A.npad * sizeof(T)), bar);
+    for (int t = tid; t < A.n; t += blockDim.x) sq[t] = A.q[t];
     S.fill(A.P, A.img, A.nimg, A.ion_pos, A.ion_q, A.n_ion, tid, blockDim.x);
+    tma_wait(bar, 0);
     __syncthreads();
 
     const bool uq = A.P.qinfo[2] != 0.0 && A.P.ion_uniform;

@@ -44,6 +44,30 @@ __device__ __forceinline__ double block_sum(double v, double *red)
     return v;
 }
 
+/* ---- TMA bulk copy global -> shared (cp.async.bulk, SASS UBLKCP) completing on an mbarrier ---------------
+ * One thread initialises the barrier (then __syncthreads), one thread issues the copy, every thread that reads the
+ * data waits on the barrier's phase.  bytes: multiple of 16; source and destination 16-byte aligned. */
+__device__ __forceinline__ unsigned smem_u32(const void *p) { return (unsigned)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void tma_barrier_init(uint64_t *bar)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(smem_u32(bar)) : "memory");
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+}
+__device__ __forceinline__ void tma_load_1d(void *dst_smem, const void *src_gmem, unsigned bytes, uint64_t *bar)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                 ::"r"(smem_u32(dst_smem)), "l"(src_gmem), "r"(bytes), "r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void tma_wait(uint64_t *bar, unsigned parity)
+{
+    unsigned done;
+    do {
+        asm volatile("{ .reg .pred p; mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2; selp.u32 %0, 1, 0, p; }"
+                     : "=r"(done) : "r"(smem_u32(bar)), "r"(parity) : "memory");
+    } while (!done);
+}
+
 /* Power table of one point for one direction: tab[n] = scale * exp(2 pi i s)^n, n = 0..nmax. */
 template <typename T>
 __device__ __forceinline__ void power_row(T s, T scale, int nmax, typename Num<T>::T2 *tab)

@@ -20,7 +20,7 @@
  *          the block (one broadcast LDS.128 per pair) -> 4 x (1 + 2 NP) register accumulators.  The loop is
  *          software-pipelined by hand: the pairs of particle p + 1 are loaded while those of p are multiplied
  *          (a DFMA needs its LDS operand 30 cycles after issue; with one product held in the operand reuse
- *          cache a DFMA reads two register operands and issues every 2 cycles, profiles/r02_fp64_pipe.md)
+ *          cache a DFMA reads two register operands and issues every 2 cycles, profiles/r02_recip_summary.md)
  *   warp   32 lanes of one kind and block length: the items of all walkers of the CTA are sorted, so the
  *          spherical cut-off costs no divergent lanes; warps are dealt to the four sub-partitions (warp mod 4)
  *          so that each carries the same number of FP64 operations
