@@ -681,10 +681,10 @@ static ewald_status launch_recip_mma(ewald_ctx *c, int W, int n, const double *p
     if (nw_cap < 1) return fail(c, EWALD_ESTATE, "tensor-core octant kernel: the plan does not fit");
     if ((st = ensure(c, &c->partial_recip, (size_t)W * sizeof(double))) != EWALD_OK) return st;
     /* walkers per CTA so that the grid is one wave; shared memory bounds the walkers of a pass */
-    const int pc = 32, qstride = 4 * M.rowlen, wstride = (pc / 4) * qstride;
+    const int pc = 32, qstride = 4 * M.rowlen, wstride = (pc / 4) * qstride; /* 64-particle chunks: -1 to -3 % only, twice the shared memory */
     const size_t slab_bytes = (size_t)wstride * sizeof(double2);
     const size_t part_bytes = (size_t)MMA_WARPS * 2 * M.slots.size() * sizeof(double);
-    const size_t avail = (c->smem_optin < 200 * 1024 ? c->smem_optin : 200 * 1024) / MMA_CTAS_PER_SM - 1024 - part_bytes;
+    const size_t avail = c->smem_optin / MMA_CTAS_PER_SM - 2048 - part_bytes;
     int nw_pass = (int)(avail / (2 * slab_bytes));
     if (nw_pass > nw_cap) nw_pass = nw_cap;
     if (nw_pass < 1) return fail(c, EWALD_ERANGE, "tensor-core octant kernel: shared memory");

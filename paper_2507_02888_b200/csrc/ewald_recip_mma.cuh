@@ -224,22 +224,25 @@ __global__ void __launch_bounds__(MMA_THREADS, MMA_CTAS_PER_SM) recip_mma_kernel
                 for (int tile = 0; tile < 2; tile++) {
                     if (!(tile ? use1[s] : use0[s])) continue;
                     const int st = st0[s] + tile; /* tile index within the slot's own tables (0 or 1) */
+                    double wk[4], t0v[4], t1v[4];
+#pragma unroll
+                    for (int cls = 0; cls < 4; cls++) wk[cls] = __ldg(wt + ((st * 4 + n1l) * 8 + col) * 4 + cls);
+#pragma unroll
+                    for (int k = 0; k < 4; k++) {
+                        t0v[k] = ti ? __ldg(ti + ((st * 8 + r) * 8 + 2 * kk) * 4 + k) : 0.0;
+                        t1v[k] = ti ? __ldg(ti + ((st * 8 + r) * 8 + 2 * kk + 1) * 4 + k) : 0.0;
+                    }
                     double e = 0;
                     double Tc[4], Ts[4];
 #pragma unroll
                     for (int k = 0; k < 4; k++) {
-                        double own0 = acc[s][k][tile][0], own1 = acc[s][k][tile][1];
-                        if (ti) {
-                            own0 += ti[((st * 8 + r) * 8 + 2 * kk) * 4 + k];
-                            own1 += ti[((st * 8 + r) * 8 + 2 * kk + 1) * 4 + k];
-                        }
+                        const double own0 = acc[s][k][tile][0] + t0v[k], own1 = acc[s][k][tile][1] + t1v[k];
                         const double recv = __shfl_xor_sync(0xffffffffu, odd ? own0 : own1, 4);
                         Tc[k] = odd ? recv : own0;
                         Ts[k] = odd ? own1 : recv;
                     }
 #pragma unroll
                     for (int cls = 0; cls < 4; cls++) {
-                        const double wk = wt[((st * 4 + n1l) * 8 + col) * 4 + cls];
                         double re, im;
                         if (DIM == 3 && kind[s] == MMA_KIND_FULL) {
                             const double p = (cls & 2) ? -1.0 : 1.0, q = (cls & 1) ? -1.0 : 1.0;
@@ -251,7 +254,7 @@ __global__ void __launch_bounds__(MMA_THREADS, MMA_CTAS_PER_SM) recip_mma_kernel
                             re = Tc[o] - p * Ts[o + 1];
                             im = Ts[o] + p * Tc[o + 1];
                         }
-                        e += wk != 0 ? wk * (re * re + im * im) : 0.0;
+                        e += wk[cls] != 0 ? wk[cls] * (re * re + im * im) : 0.0;
                     }
                     /* one sum per (slot, tile): the same lanes in the same order whichever warp holds it */
                     e = warp_sum(e);
