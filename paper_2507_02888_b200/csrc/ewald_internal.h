@@ -76,7 +76,10 @@ struct PairTable {
 };
 constexpr int PAIR_K64 = 7, PAIR_DEG64 = 5;  /* FP64: 128 bins per octave, quintic: rel. error < 1e-16 */
 constexpr int PAIR_K32 = 5, PAIR_DEG32 = 3;  /* FP32:  32 bins per octave, cubic:   rel. error < 3e-9  */
-constexpr int FAR_T0 = 16, FAR_KB = 3, FAR_REP = 8; /* far shell of the FP64 kernels (FarFmt)       */
+#ifndef EWALD_FAR_T0
+#define EWALD_FAR_T0 13
+#endif
+constexpr int FAR_T0 = EWALD_FAR_T0, FAR_KB = 3, FAR_REP = 8; /* far shell of the FP64 kernels (FarFmt) */
 constexpr int MAX_SPECIES = 4;               /* distinct fixed charges the bare-t real-space path handles  */
 constexpr int PAIR_EMIN = -6;                /* t < 2^-6 (kappa r < 1/8) takes the direct formula      */
 

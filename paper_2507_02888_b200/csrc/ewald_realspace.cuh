@@ -52,7 +52,7 @@ template <typename T> struct RealGeom {
     int bias;    /* bin index = (key >> SHIFT) - bias             */
     int m_shift; /* images -m_shift..m_shift scanned per axis (orthorhombic path) */
     int multi_far; /* 3D, m_shift = 1: some L_j^2 + L_k^2 < kappa^2 r_c^2, i.e. two far images can be in range */
-    int outer_far; /* every (kappa L_k)^2 >= 16: a candidate with a far image always belongs to the far shell */
+    int outer_far; /* every (kappa L_k)^2 >= T0: a candidate with a far image always belongs to the far shell */
     int far_once;  /* outer_far, no multi_far, and the far stack is deep enough for one service per pair */
 };
 
@@ -248,9 +248,10 @@ struct LaneStack : StackBase<T, T, UQ, LaneStack<T, UQ, SIGNED>> {
 };
 
 /* ---- the far shell (FP64 kernels only) ------------------------------------------------------------
- * Terms with t >= 16 are below F(16) = 3.9e-9 each, and their total is < 4e-5 of a sum of order N^2/2:
- * FP32 arithmetic on them (relative error ~1e-7) changes the sum by < 4e-12 in the worst, fully
- * coherent case and ~3e-14 for random rounding (DESIGN.md section 5.2 derives both).  They are kept as
+ * Terms with t >= T0 = 13 are below F(13) = 9.6e-8 each (a few 1e-4 of a sum of order N^2/2 in all):
+ * FP32 arithmetic on them (relative error ~1e-7 per term; the table's u^2 coefficient is chosen at setup so
+ * that the error averages to zero over a bin, ewald_setup.cpp build_far_table) changes E by 4e-13 relative on
+ * config 2 (measured).  They are kept as
  * 32-bit fixed point x = round(t 2^25) (one FP64 add with 2^27 puts it in the low word; resolution
  * 3e-8 in t, so F keeps 3e-8 relative), evaluated by an FP32 cubic on bins of width 1/8 in t whose index
  * and local variable are bit fields of x, from a table replicated 8 times so that the 8 lanes of a
@@ -260,7 +261,10 @@ struct FarFmt {
     static constexpr int KB = 3;            /* 2^KB bins per unit of t                             */
     static constexpr int MB = S - KB;       /* bits of x inside a bin                              */
     static constexpr int REP = 8;           /* table copies                                        */
-    static constexpr int T0 = 16;           /* the far shell starts at t = T0                      */
+#ifndef EWALD_FAR_T0
+#define EWALD_FAR_T0 13
+#endif
+    static constexpr int T0 = EWALD_FAR_T0; /* the far shell starts at t = T0                      */
 };
 __device__ __forceinline__ unsigned far_fixed(double t) { return (unsigned)__double2loint(t + 134217728.0 /* 2^27 */); }
 
@@ -374,7 +378,7 @@ __device__ __forceinline__ void scan_pair(const RealGeom<T> &g, T *d, T w, bool 
             const int key = order_key(t);
             st.template push<FLIP>(ok && key <= g.key_rc, t, key, w);
         };
-        auto cand_far = [&](int i, int j, int k, bool ok) { /* t >= 16 is known: far stack only */
+        auto cand_far = [&](int i, int j, int k, bool ok) { /* t >= T0 is known: far stack only */
             const T t = a[0][i] + (a[1][j] + a[2][k]);
             const int key = order_key(t);
             st.template push_far<FLIP>(ok && key <= g.key_rc, t, key, w);

@@ -106,7 +106,22 @@ void build_far_table(int t0, int kb, int rep, double t_max, std::vector<float> *
         }
         /* T0 = 1, T1 = v, T2 = 2v^2 - 1, T3 = 4v^3 - 3v; v = 2u */
         const real m0 = cheb[0] - cheb[2], m1 = cheb[1] - 3 * cheb[3], m2 = 2 * cheb[2], m3 = 4 * cheb[3];
-        const float c[4] = {(float)m0, (float)(2 * m1), (float)(4 * m2), (float)(8 * m3)};
+        float c[4] = {(float)m0, (float)(2 * m1), (float)(4 * m2), (float)(8 * m3)};
+        /* The same rounded coefficients serve every term that falls in the bin, so the rounding of c0 to float
+         * (3e-8 relative) and the mean of the cubic's truncation error are SYSTEMATIC over a walker's ~1e5 far
+         * terms.  The u^2 coefficient is re-chosen so that the mean of the float polynomial over the bin,
+         * c0 + c2/12, equals the mean of F over the bin (composite Simpson, long double): the error of a term
+         * stays <= ~1e-7 F pointwise but averages to zero for terms spread over the bin. */
+        {
+            const int ns = 64;
+            real acc = 0;
+            for (int i = 0; i <= ns; i++) {
+                const real t = mid + width * ((real)i / ns - 0.5L), z = sqrtl(t);
+                acc += (i == 0 || i == ns ? 1 : (i & 1) ? 4 : 2) * erfcl(z) / z;
+            }
+            const real mean_f = acc / (3 * ns);
+            c[2] = (float)(12 * (mean_f - (real)c[0]));
+        }
         for (int r = 0; r < rep; r++)
             for (int k = 0; k < 4; k++) (*tab)[((size_t)b * rep + r) * 4 + k] = c[k];
     }
