@@ -103,7 +103,7 @@ __device__ __forceinline__ void mma_chunk(double (&acc)[MMA_S][4][2][2], const d
                                           int oA0, int oA1, const int2 (&lo)[MMA_S], const bool (&full)[MMA_S],
                                           const bool (&use0)[MMA_S], const bool (&use1)[MMA_S])
 {
-#pragma unroll 2
+#pragma unroll 2 /* 1: measured 2 % slower */
     for (int q = 0; q < nq; q++) {
         const double2 *qb = tw + (size_t)q * qstride;
         const double *qd = reinterpret_cast<const double *>(qb);
