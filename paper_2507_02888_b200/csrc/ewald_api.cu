@@ -74,7 +74,7 @@ struct ewald_ctx {
     int sm_count = 148; size_t smem_optin = 227 * 1024;
 
     /* scratch */
-    DevBuf partial_recip, partial_real, qsums;
+    DevBuf partial_recip, partial_real, qsums, done;
     DevBuf stage_pos, stage_q, stage_e, stage_comp;           /* *_host entry points */
     DevBuf mv_walker, mv_electron, mv_newr, mv_de;
 
@@ -373,7 +373,7 @@ extern "C" void ewald_destroy(ewald_ctx *c)
     cudaFree(c->d_oct_wt); cudaFree(c->d_oct_tion); cudaFree(c->d_mma_wt); cudaFree(c->d_mma_tion);
     for (auto &kv : c->mma_dev) { cudaFree(kv.second.d_lane); cudaFree(kv.second.d_meta); }
     for (auto &kv : c->oct_dev) { cudaFree(kv.second.d_lane); cudaFree(kv.second.d_variant); }
-    DevBuf *bufs[] = {&c->partial_recip, &c->partial_real, &c->qsums, &c->stage_pos, &c->stage_q,
+    DevBuf *bufs[] = {&c->partial_recip, &c->partial_real, &c->qsums, &c->done, &c->stage_pos, &c->stage_q,
                       &c->stage_e, &c->stage_comp, &c->mv_walker, &c->mv_electron, &c->mv_newr,
                       &c->mv_de, &c->st_pos, &c->st_q, &c->st_rho, &c->st_qinfo};
     for (DevBuf *b : bufs) release(b);
@@ -842,13 +842,14 @@ static int real_min_cap(const ewald_ctx *c, bool ortho, bool uq)
 }
 
 template <typename T>
-static ewald_status launch_real(ewald_ctx *c, int W, int n, const T *pos, const T *q, int *n_tiles_out)
+static ewald_status launch_real(ewald_ctx *c, int W, int n, const T *pos, const T *q, int n_slabs, double *energies,
+                                double *components)
 {
     RealArgs<T> A;
     A.pos = pos; A.q = q; A.n = n; A.npad = ewald_padded_n(n);
     A.img = Tabs<T>::img(c); A.nimg = c->nimg;
     A.ion_pos = Tabs<T>::ion_pos(c); A.ion_q = Tabs<T>::ion_q(c); A.n_ion = c->t.n_ion;
-    fill_pair_tabs<T>(c, (const double *)c->qsums.p, &A.P);
+    fill_pair_tabs<T>(c, nullptr, &A.P); /* the kernel finds the all-equal flag of the charges itself */
     fill_geom(c->t, &A.g);
     const bool ortho = real_ortho(c);
     if (ortho) A.nimg = 0; /* the orthorhombic path does not read the image list */
@@ -869,7 +870,22 @@ static ewald_status launch_real(ewald_ctx *c, int W, int n, const T *pos, const 
     if (st != EWALD_OK) return st;
     A.partial = (double *)c->partial_real.p;
     A.n_tiles = (int)n_tiles;
+    /* [S6] folded into the kernel: per-walker arrival counters (zero between calls: the last CTA resets its own) */
+    if ((size_t)W * sizeof(int) > c->done.cap) {
+        if ((st = ensure(c, &c->done, (size_t)W * sizeof(int))) != EWALD_OK) return st;
+        CU_TRY(c, cudaMemsetAsync(c->done.p, 0, c->done.cap, c->stream));
+    }
+    A.done = (int *)c->done.p;
+    A.comb.recip_partial = (const double *)c->partial_recip.p; A.comb.n_recip = n_slabs;
+    A.comb.real_partial = A.partial; A.comb.n_real = (int)n_tiles;
+    A.comb.ion_q2 = c->t.ion_q2; A.comb.ion_qsum = c->t.ion_qsum; A.comb.ion_real = c->t.ion_real;
+    A.comb.xi_r = c->t.xi_r; A.comb.self_coef = c->t.self_coef; A.comb.bg_coef = c->t.bg_coef;
+    A.comb.energies = energies; A.comb.components = components; A.comb.n_walkers = W;
     const long long grid = (long long)W * n_tiles;
+    /* small batches (at most two waves of CTAs): [S6] inside the kernel, one launch less; large ones: combine_kernel */
+    const bool fold = grid <= 2LL * c->sm_count;
+    const CombineArgs comb = A.comb;
+    if (!fold) A.comb.energies = nullptr;
     if (grid > 0x7fffffffLL) return fail(c, EWALD_ERANGE, "grid too large");
 #define EWALD_LAUNCH_REAL(DIM, ORTHO, M)                                                          \
     do {                                                                                          \
@@ -892,7 +908,11 @@ static ewald_status launch_real(ewald_ctx *c, int W, int n, const T *pos, const 
     }
 #undef EWALD_LAUNCH_REAL
     CU_TRY(c, cudaGetLastError());
-    *n_tiles_out = (int)n_tiles;
+    if (!fold) {
+        ProfScope ps(c, 2);
+        combine_kernel<T><<<(W + 127) / 128, 128, 0, c->stream>>>(comb, q, n);
+        CU_TRY(c, cudaGetLastError());
+    }
     return EWALD_OK;
 }
 
@@ -924,31 +944,13 @@ template <typename T>
 static ewald_status energy_batch_t(ewald_ctx *c, int W, int n, const T *pos, const T *q,
                                    double *energies, double *components)
 {
-    int n_slabs = 0, n_tiles = 0;
-    {
-        ProfScope ps(c, 2);
-        charge_sums_kernel<T><<<1, 256, 0, c->stream>>>(q, n, (double *)c->qsums.p);
-    }
-    CU_TRY(c, cudaGetLastError());
+    /* two launches: [S1-S4] reciprocal, then [S5] real space with [S6] folded into the last CTA of every walker */
+    int n_slabs = 0;
     const bool oct = c->recip_variant != 1 && c->t.oct.valid;
     if (c->recip_variant >= 2 && !oct) return fail(c, EWALD_ESTATE, "octant kernel: no plan for this G set");
     ewald_status st = launch_recip_any<T>(c, oct, W, n, pos, q, &n_slabs);
     if (st != EWALD_OK) return st;
-    st = launch_real<T>(c, W, n, pos, q, &n_tiles);
-    if (st != EWALD_OK) return st;
-    CombineArgs A;
-    A.recip_partial = (const double *)c->partial_recip.p; A.n_recip = n_slabs;
-    A.real_partial = (const double *)c->partial_real.p; A.n_real = n_tiles;
-    A.qsums = (const double *)c->qsums.p;
-    A.ion_q2 = c->t.ion_q2; A.ion_qsum = c->t.ion_qsum; A.ion_real = c->t.ion_real;
-    A.xi_r = c->t.xi_r; A.self_coef = c->t.self_coef; A.bg_coef = c->t.bg_coef;
-    A.energies = energies; A.components = components; A.n_walkers = W;
-    {
-        ProfScope ps(c, 2);
-        combine_kernel<<<(W + 127) / 128, 128, 0, c->stream>>>(A);
-    }
-    CU_TRY(c, cudaGetLastError());
-    return EWALD_OK;
+    return launch_real<T>(c, W, n, pos, q, n_slabs, energies, components);
 }
 
 static ewald_status check_batch(ewald_ctx *c, int W, int n, ewald_prec prec, const void *pos, const void *q)

@@ -8,7 +8,8 @@
  *                           (The energy path uses recip_oct_kernel, ewald_recip_oct.cuh.)
  *   real_kernel    [S5]     sum_{i<j} q_i q_j sum_R erfc(kappa|r_ij-R|)/|r_ij-R| (real-lattice sum of
  *                           Eq. 3) plus mobile-ion pairs; machinery in ewald_realspace.cuh
- *   combine_kernel [S6]     adds partial sums and the constants of Eqs. 3-4; charge_sums_kernel gives
+ *   [S6] combine            folded into real_kernel: the last CTA of a walker adds the partial sums and the
+ *                           constants of Eqs. 3-4; charge_sums_kernel (stored populations) gives
  *                           sum q^2, sum q and the all-equal flag of the mobile charges
  *   move_kernel    [S7a-d]  single-particle moves, one warp per move: Delta E and patch of the stored rho(G)
  *   fma_probe_kernel   measurement helper (roofline denominator); dmma_probe_kernel in ewald_recip_mma.cuh
@@ -141,6 +142,15 @@ template <typename T> struct PairTabs {
     int capf_u, capf_g;              /* far-stack capacity per lane                                     */
 };
 
+/* [S6] what the combine needs (folded into the last CTA of a walker in real_kernel) */
+struct CombineArgs {
+    const double *recip_partial; int n_recip;
+    const double *real_partial; int n_real;
+    double ion_q2, ion_qsum, ion_real;
+    double xi_r, self_coef, bg_coef;
+    double *energies; double *components; int n_walkers;
+};
+
 template <typename T> struct RealArgs {
     const T *pos; const T *q;
     int n, npad;
@@ -150,6 +160,8 @@ template <typename T> struct RealArgs {
     double *partial;                              /* [W][n_tiles] */
     int n_tiles;
     RealGeom<T> g;
+    CombineArgs comb;                             /* energies == null: no combine */
+    int *done;                                    /* [W] CTAs of the walker that have finished (zero between calls) */
 };
 
 constexpr int REAL_MAX_THREADS = 512;
@@ -337,35 +349,67 @@ __global__ void __launch_bounds__(REAL_MAX_THREADS) real_kernel(RealArgs<T> A)
     tma_wait(bar, 0);
     __syncthreads();
 
-    const bool uq = A.P.qinfo[2] != 0.0 && A.P.ion_uniform;
-    const T q0 = (T)A.P.qinfo[3];
+    /* all mobile charges equal (the electron gas): the stacks then hold bare t (ewald_realspace.cuh) */
+    bool eq = true;
+    for (int t = tid; t < A.n; t += blockDim.x) eq = eq && sq[t] == sq[0];
+    const bool uq = __syncthreads_and(eq) && A.P.ion_uniform;
+    const T q0 = sq[0];
     double acc;
     if (uq) acc = real_body<T, DIM, ORTHO, M, true>(A, S, sp, sq, tile, q0);
     else acc = real_body<T, DIM, ORTHO, M, false>(A, S, sp, sq, tile, q0);
     acc = block_sum(acc, red);
     if (tid == 0) A.partial[(size_t)w * A.n_tiles + tile] = acc * A.g.kappa_d;
+
+    /* [S6] The CTA of a walker that finishes last adds the partial sums in fixed order and the constants of
+     * Eqs. 3-4: E = E_recip + E_real + E_self + E_bg (the reciprocal kernel ran before this one on the stream). */
+    if (A.comb.energies == nullptr) return;
+    int *last = reinterpret_cast<int *>(&red[40]); /* inside red[]: static shared memory stays a multiple of 128 bytes */
+    if (tid == 0) {
+        __threadfence();
+        *last = atomicAdd(&A.done[w], 1) == A.n_tiles - 1;
+    }
+    __syncthreads();
+    if (!*last) return;
+    double s2 = 0, s1 = 0;
+    for (int t = tid; t < A.n; t += blockDim.x) { const double v = (double)sq[t]; s2 += v * v; s1 += v; }
+    s2 = block_sum(s2, red);
+    s1 = block_sum(s1, red);
+    if (tid == 0) {
+        __threadfence();
+        const CombineArgs &C = A.comb;
+        double er = 0, ep = 0;
+        for (int k = 0; k < C.n_recip; k++) er += __ldcg(C.recip_partial + (size_t)w * C.n_recip + k);
+        for (int k = 0; k < A.n_tiles; k++) ep += __ldcg(A.partial + (size_t)w * A.n_tiles + k);
+        const double q2 = s2 + C.ion_q2, qs = s1 + C.ion_qsum;
+        const double e_real = ep + C.ion_real + 0.5 * q2 * C.xi_r;
+        const double e_self = -C.self_coef * q2;
+        const double e_bg = -0.5 * C.bg_coef * qs * qs;
+        C.energies[w] = er + e_real + e_self + e_bg;
+        if (C.components) {
+            C.components[4 * w + 0] = er;
+            C.components[4 * w + 1] = e_real;
+            C.components[4 * w + 2] = e_self;
+            C.components[4 * w + 3] = e_bg;
+        }
+        A.done[w] = 0;
+    }
 }
 
 /* ------------------------------------------------------------------------------------------ */
-/* [S6] combine.  One thread per walker. */
-
-struct CombineArgs {
-    const double *recip_partial; int n_recip;
-    const double *real_partial; int n_real;
-    const double *qsums;   /* [2] = sum q^2, sum q of the mobile particles */
-    double ion_q2, ion_qsum, ion_real;
-    double xi_r, self_coef, bg_coef;
-    double *energies; double *components; int n_walkers;
-};
-
-__global__ void combine_kernel(CombineArgs A)
+/* [S6] combine as a kernel of its own (large batches: the arrival counter of the folded form costs every CTA of
+ * real_kernel a fence and an atomic, ~1.5 % of a many-wave launch).  One thread per walker; every thread adds the
+ * charges itself (broadcast loads, the same order for every walker). */
+template <typename T>
+__global__ void combine_kernel(CombineArgs A, const T *q, int n)
 {
     const int w = blockIdx.x * blockDim.x + threadIdx.x;
     if (w >= A.n_walkers) return;
+    double s2 = 0, s1 = 0;
+    for (int i = 0; i < n; i++) { const double v = (double)__ldg(q + i); s2 += v * v; s1 += v; }
     double er = 0, ep = 0;
     for (int k = 0; k < A.n_recip; k++) er += A.recip_partial[(size_t)w * A.n_recip + k];
     for (int k = 0; k < A.n_real; k++) ep += A.real_partial[(size_t)w * A.n_real + k];
-    const double q2 = A.qsums[0] + A.ion_q2, qs = A.qsums[1] + A.ion_qsum;
+    const double q2 = s2 + A.ion_q2, qs = s1 + A.ion_qsum;
     const double e_real = ep + A.ion_real + 0.5 * q2 * A.xi_r;
     const double e_self = -A.self_coef * q2;
     const double e_bg = -0.5 * A.bg_coef * qs * qs;
@@ -377,6 +421,9 @@ __global__ void combine_kernel(CombineArgs A)
         A.components[4 * w + 3] = e_bg;
     }
 }
+
+/* ------------------------------------------------------------------------------------------ */
+/* Charge sums of a stored population (ewald_load_walkers): sum q^2, sum q, all-equal flag, q_0. */
 
 template <typename T>
 __global__ void charge_sums_kernel(const T *q, int n, double *out)
