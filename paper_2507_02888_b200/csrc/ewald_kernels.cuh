@@ -397,15 +397,21 @@ __global__ void __launch_bounds__(REAL_MAX_THREADS) real_kernel(RealArgs<T> A)
 
 /* ------------------------------------------------------------------------------------------ */
 /* [S6] combine as a kernel of its own (large batches: the arrival counter of the folded form costs every CTA of
- * real_kernel a fence and an atomic, ~1.5 % of a many-wave launch).  One thread per walker; every thread adds the
- * charges itself (broadcast loads, the same order for every walker). */
+ * real_kernel a fence and an atomic, ~1.5 % of a many-wave launch).  One thread per walker; every block adds the
+ * charges once (the same block size and order for every walker). */
 template <typename T>
 __global__ void combine_kernel(CombineArgs A, const T *q, int n)
 {
+    __shared__ double red[32], sums[2];
+    double s2 = 0, s1 = 0;
+    for (int i = threadIdx.x; i < n; i += blockDim.x) { const double v = (double)__ldg(q + i); s2 += v * v; s1 += v; }
+    s2 = block_sum(s2, red);
+    s1 = block_sum(s1, red);
+    if (threadIdx.x == 0) { sums[0] = s2; sums[1] = s1; }
+    __syncthreads();
+    s2 = sums[0]; s1 = sums[1];
     const int w = blockIdx.x * blockDim.x + threadIdx.x;
     if (w >= A.n_walkers) return;
-    double s2 = 0, s1 = 0;
-    for (int i = 0; i < n; i++) { const double v = (double)__ldg(q + i); s2 += v * v; s1 += v; }
     double er = 0, ep = 0;
     for (int k = 0; k < A.n_recip; k++) er += A.recip_partial[(size_t)w * A.n_recip + k];
     for (int k = 0; k < A.n_real; k++) ep += A.real_partial[(size_t)w * A.n_real + k];
