@@ -135,6 +135,7 @@ template <typename T> struct PairTabs {
     T t_safe;                        /* some t inside the table                                         */
     const float *far_tab; int n_far; /* FP64 kernels: [n_far][FarFmt::REP][4] far-shell cubics; 0 = none */
     int key_far;                     /* order key of the far shell's start, INT_MAX = none              */
+    int far_t0;                      /* t at which this kernel's far shell (and its staged table) starts */
     const double *qinfo;             /* device [4]: sum q^2, sum q, all-equal flag, q_0                  */
     int ion_uniform;                 /* at most 4 distinct fixed charges (species)                      */
     int n_species, sp_start[5];      /* ions [sp_start[s], sp_start[s+1]) carry one charge each         */
@@ -237,8 +238,8 @@ __device__ __forceinline__ void init_stacks(PairStacks<double, UQ, SIGNED> &st, 
     unsigned char *mem = S.stacks + (size_t)warp * RealSmem<double>::warp_stack_bytes(P);
     st.nr.init(mem, lane, UQ ? P.cap_u : P.cap_g, S.tab, bias, P.t_safe);
     st.key_far = P.key_far;
-    if (st.has_far()) st.fr.init(mem + (size_t)P.cap_u * 32 * sizeof(double), lane, UQ ? P.capf_u : P.capf_g, S.far);
-    else { st.fr.base_a = st.fr.top_a = 0; st.fr.cap_b = 0; st.fr.sum = 0; }
+    if (st.has_far()) st.fr.init(mem + (size_t)P.cap_u * 32 * sizeof(double), lane, UQ ? P.capf_u : P.capf_g, S.far, P.far_t0);
+    else { st.fr.base_a = st.fr.top_a = 0; st.fr.cap_b = 0; st.fr.sum = 0; st.fr.bin0 = 0; }
 }
 
 /* Pairs (i, j = i + k + 1 mod n), rows k = 0..H-1 (H = (n-1)/2) and, for even n, half of row H, dealt

@@ -264,21 +264,23 @@ struct FarFmt {
 #ifndef EWALD_FAR_T0
 #define EWALD_FAR_T0 13
 #endif
-    static constexpr int T0 = EWALD_FAR_T0; /* the far shell starts at t = T0                      */
+    static constexpr int T0 = EWALD_FAR_T0; /* the far table starts at t = T0 (a kernel may start its far shell later) */
 };
 __device__ __forceinline__ unsigned far_fixed(double t) { return (unsigned)__double2loint(t + 134217728.0 /* 2^27 */); }
 
 template <bool UQ, bool SIGNED> struct FarStack : StackBase<unsigned, float, UQ, FarStack<UQ, SIGNED>> {
     typedef float Acc;
     const float4 *tab; /* [bin][REP] cubic in u = (fraction of the bin) - 1/2; this lane's copy pre-selected */
-    __device__ __forceinline__ void init(void *warp_mem, int lane, int cap, const float *table)
+    int bin0;          /* first bin of the staged table = (t at which this kernel's far shell starts) << KB */
+    __device__ __forceinline__ void init(void *warp_mem, int lane, int cap, const float *table, int t0)
     {
         tab = reinterpret_cast<const float4 *>(table) + (lane & (FarFmt::REP - 1));
-        this->init_base(warp_mem, lane, cap, (unsigned)FarFmt::T0 << FarFmt::S);
+        bin0 = t0 << FarFmt::KB;
+        this->init_base(warp_mem, lane, cap, (unsigned)t0 << FarFmt::S);
     }
     __device__ __forceinline__ float term(unsigned x, float w) const
     {
-        const int idx = (int)((x & 0x7fffffffu) >> FarFmt::MB) - (FarFmt::T0 << FarFmt::KB);
+        const int idx = (int)((x & 0x7fffffffu) >> FarFmt::MB) - bin0;
         /* the MB bits inside the bin become the mantissa of a float in [1, 2) */
         const float u = __uint_as_float(((x << (23 - FarFmt::MB)) & 0x7fffffu) | 0x3f800000u) - 1.5f;
         const float4 c = tab[idx * FarFmt::REP];
