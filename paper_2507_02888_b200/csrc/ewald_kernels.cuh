@@ -239,7 +239,7 @@ __device__ __forceinline__ void init_stacks(PairStacks<double, UQ, SIGNED> &st, 
     st.nr.init(mem, lane, UQ ? P.cap_u : P.cap_g, S.tab, bias, P.t_safe);
     st.key_far = P.key_far;
     if (st.has_far()) st.fr.init(mem + (size_t)P.cap_u * 32 * sizeof(double), lane, UQ ? P.capf_u : P.capf_g, S.far, P.far_t0);
-    else { st.fr.base_a = st.fr.top_a = 0; st.fr.cap_b = 0; st.fr.sum = 0; st.fr.bin0 = 0; }
+    else { st.fr.base_a = st.fr.top_a = 0; st.fr.cap_b = 0; st.fr.sum = 0; }
 }
 
 /* Pairs (i, j = i + k + 1 mod n), rows k = 0..H-1 (H = (n-1)/2) and, for even n, half of row H, dealt
@@ -522,9 +522,13 @@ __device__ __forceinline__ double move_real(const MoveArgs<T> &A, RealSmem<T> &S
 }
 
 constexpr int MOVE_MAX_THREADS = 512;
+#ifndef EWALD_MOVE_G_BATCH
+#define EWALD_MOVE_G_BATCH 4
+#endif
+constexpr int MOVE_G_BATCH = EWALD_MOVE_G_BATCH; /* rho(G) vectors a lane loads ahead in [S7b] */
 
 template <typename T, int DIM, bool ORTHO, int M>
-__global__ void __launch_bounds__(MOVE_MAX_THREADS) move_kernel(MoveArgs<T> A)
+__global__ void __launch_bounds__(MOVE_MAX_THREADS, sizeof(T) == 4 ? 2 : 1) move_kernel(MoveArgs<T> A)
 {
     typedef typename Num<T>::T2 T2;
     extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -559,36 +563,50 @@ __global__ void __launch_bounds__(MOVE_MAX_THREADS) move_kernel(MoveArgs<T> A)
         }
         __syncwarp();
 
-        /* [S7b] Delta E_recip and the patch of rho(G) */
+        /* [S7b] Delta E_recip and the patch of rho(G).  The walker's rho comes from HBM and nothing else of the
+         * warp's work can cover that latency, so the loads of MOVE_G_BATCH vectors per lane are issued before the
+         * first of them is used (one load in flight per lane ran at 1.1 TB/s over the whole GPU). */
         T *rr = A.rho + (size_t)w * 2 * A.ngp_pad;
         double acc = 0;
-#pragma unroll 2
-        for (int g = lane; g < A.ngp; g += 32) {
-            const short4 nn = A.gn[g];
-            const T re = rr[g], im = rr[A.ngp_pad + g];
-            T2 ph[2];
+        for (int g0 = lane; g0 < A.ngp; g0 += 32 * MOVE_G_BATCH) {
+            short4 nn[MOVE_G_BATCH];
+            T re[MOVE_G_BATCH], im[MOVE_G_BATCH], wg[MOVE_G_BATCH];
 #pragma unroll
-            for (int which = 0; which < 2; which++) {
-                const T2 *row = tab + which * A.rowlen;
-                T2 e1 = row[A.off[0] + nn.x];
-                T2 e2 = row[A.off[1] + (nn.y < 0 ? -nn.y : nn.y)];
-                if (nn.y < 0) e2.y = -e2.y;
-                T2 e;
-                e.x = e1.x * e2.x - e1.y * e2.y;
-                e.y = e1.x * e2.y + e1.y * e2.x;
-                if (DIM == 3) {
-                    T2 e3 = row[A.off[2] + (nn.z < 0 ? -nn.z : nn.z)];
-                    if (nn.z < 0) e3.y = -e3.y;
-                    T2 f;
-                    f.x = e.x * e3.x - e.y * e3.y;
-                    f.y = e.x * e3.y + e.y * e3.x;
-                    e = f;
-                }
-                ph[which] = e;
+            for (int u = 0; u < MOVE_G_BATCH; u++) {
+                const int g = g0 + 32 * u;
+                const bool in = g < A.ngp;
+                nn[u] = in ? __ldg(A.gn + g) : make_short4(0, 0, 0, 0);
+                re[u] = in ? rr[g] : T(0);
+                im[u] = in ? rr[A.ngp_pad + g] : T(0);
+                wg[u] = in ? __ldg(A.w2 + g) : T(0);
             }
-            const T dr = ph[1].x - ph[0].x, di = ph[1].y - ph[0].y;
-            acc += (double)(A.w2[g] * (2 * qk * (re * dr + im * di) + qk * qk * (dr * dr + di * di)));
-            if (A.commit) { rr[g] = re + qk * dr; rr[A.ngp_pad + g] = im + qk * di; }
+#pragma unroll
+            for (int u = 0; u < MOVE_G_BATCH; u++) {
+                const int g = g0 + 32 * u;
+                T2 ph[2];
+#pragma unroll
+                for (int which = 0; which < 2; which++) {
+                    const T2 *row = tab + which * A.rowlen;
+                    T2 e1 = row[A.off[0] + nn[u].x];
+                    T2 e2 = row[A.off[1] + (nn[u].y < 0 ? -nn[u].y : nn[u].y)];
+                    if (nn[u].y < 0) e2.y = -e2.y;
+                    T2 e;
+                    e.x = e1.x * e2.x - e1.y * e2.y;
+                    e.y = e1.x * e2.y + e1.y * e2.x;
+                    if (DIM == 3) {
+                        T2 e3 = row[A.off[2] + (nn[u].z < 0 ? -nn[u].z : nn[u].z)];
+                        if (nn[u].z < 0) e3.y = -e3.y;
+                        T2 f;
+                        f.x = e.x * e3.x - e.y * e3.y;
+                        f.y = e.x * e3.y + e.y * e3.x;
+                        e = f;
+                    }
+                    ph[which] = e;
+                }
+                const T dr = ph[1].x - ph[0].x, di = ph[1].y - ph[0].y;
+                acc += (double)(wg[u] * (2 * qk * (re[u] * dr + im[u] * di) + qk * qk * (dr * dr + di * di)));
+                if (A.commit && g < A.ngp) { rr[g] = re[u] + qk * dr; rr[A.ngp_pad + g] = im[u] + qk * di; }
+            }
         }
 
         /* [S7c] Delta E_real = q_k sum_{j != k} q_j [psi(r'-r_j) - psi(r-r_j)] */

@@ -271,16 +271,16 @@ __device__ __forceinline__ unsigned far_fixed(double t) { return (unsigned)__dou
 template <bool UQ, bool SIGNED> struct FarStack : StackBase<unsigned, float, UQ, FarStack<UQ, SIGNED>> {
     typedef float Acc;
     const float4 *tab; /* [bin][REP] cubic in u = (fraction of the bin) - 1/2; this lane's copy pre-selected */
-    int bin0;          /* first bin of the staged table = (t at which this kernel's far shell starts) << KB */
+    /* the staged table starts at bin t0 << KB (t0 = where this kernel's far shell starts): the pointer is biased
+     * by that many bins, so that the bin index cut from x addresses it directly */
     __device__ __forceinline__ void init(void *warp_mem, int lane, int cap, const float *table, int t0)
     {
-        tab = reinterpret_cast<const float4 *>(table) + (lane & (FarFmt::REP - 1));
-        bin0 = t0 << FarFmt::KB;
+        tab = reinterpret_cast<const float4 *>(table) + (lane & (FarFmt::REP - 1)) - (ptrdiff_t)(t0 << FarFmt::KB) * FarFmt::REP;
         this->init_base(warp_mem, lane, cap, (unsigned)t0 << FarFmt::S);
     }
     __device__ __forceinline__ float term(unsigned x, float w) const
     {
-        const int idx = (int)((x & 0x7fffffffu) >> FarFmt::MB) - bin0;
+        const int idx = (int)((x & 0x7fffffffu) >> FarFmt::MB);
         /* the MB bits inside the bin become the mantissa of a float in [1, 2) */
         const float u = __uint_as_float(((x << (23 - FarFmt::MB)) & 0x7fffffu) | 0x3f800000u) - 1.5f;
         const float4 c = tab[idx * FarFmt::REP];
