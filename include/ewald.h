@@ -209,6 +209,12 @@ ewald_status ewald_probe_dmma(ewald_ctx *ctx, int iters, double *flops);
 ewald_status ewald_profile_enable(ewald_ctx *ctx, int on);
 ewald_status ewald_profile_read(ewald_ctx *ctx, double ms[4], int launches[4]);
 
+/* Shape of the context's last real-space launch (which = 0: real_kernel) or move launch (which = 1: move_kernel),
+ * zeros before the first: out HOST [8] = threads per CTA, dynamic shared memory in bytes, near-stack and far-stack
+ * capacity per lane in bare-t items, bins of the near table staged, bins of the far table staged (0 = far shell
+ * off), CTAs launched, 1 if the far stack is serviced once per pair.  No device work. */
+ewald_status ewald_launch_shape(const ewald_ctx *ctx, int which, int out[8]);
+
 /* Number of kernels this context has launched since ewald_setup. */
 long long ewald_launch_count(const ewald_ctx *ctx);
 

@@ -54,6 +54,7 @@ struct ewald_ctx {
     std::vector<ProfRec> recs;
     std::vector<void *> retired;           /* outgrown scratch buffers, freed at destroy */
     long long launches = 0; /* kernels launched since setup */
+    int shape[2][8] = {{0}};               /* ewald_launch_shape: last real-space [0] and move [1] launch */
     HostTables t;
     int device = 0;
     cudaStream_t stream = nullptr;
@@ -256,7 +257,24 @@ extern "C" ewald_status ewald_setup(ewald_ctx **out, int dim, const double *cell
         for (size_t i = 0; i < im.size(); i++) { hl[i] = (float)im[i]; hl[im.size() + i] = (float)(im[i] - (double)hl[i]); }
         if (st == EWALD_OK) st = upload(c, &c->d_imgf, hl);
     }
-    if (st == EWALD_OK) st = upload(c, &c->d_pair, t.pair64.coef);
+    {   /* FP64 table in 512-byte rows [chunk][slot][2] (PairFmt<double>): 8 bins per row below t = 2^E_SPLIT, one bin in
+         * 8 copies per row above */
+        typedef PairFmt<double> F;
+        static_assert(F::K == PAIR_K64 && F::DEG == PAIR_DEG64 && F::NC == PAIR_DEG64 + 1 && F::E_MIN == PAIR_EMIN,
+                      "device and host formats of the FP64 pair table differ");
+        const PairTable &pt = t.pair64;
+        std::vector<double> rows(F::elems(pt.n_bins), 0.0);
+        for (int b = 0; b < pt.n_bins; b++)
+            for (int ch = 0; ch < 4; ch++) {
+                const double c0 = pt.coef[(size_t)b * F::NC + 2 * ch], c1 = pt.coef[(size_t)b * F::NC + 2 * ch + 1];
+                const size_t row = b < F::LOW ? b >> 3 : F::LOW / 8 + (b - F::LOW);
+                for (int s = b < F::LOW ? (b & 7) : 0; s < (b < F::LOW ? (b & 7) + 1 : 8); s++) {
+                    rows[row * F::ROW + (size_t)ch * 16 + 2 * s] = c0;
+                    rows[row * F::ROW + (size_t)ch * 16 + 2 * s + 1] = c1;
+                }
+            }
+        if (st == EWALD_OK) st = upload(c, &c->d_pair, rows);
+    }
     {   /* FP32 table: PairFmt<float>::REP interleaved copies */
         const std::vector<float> one = to_f32(t.pair32.coef);
         constexpr int R = PairFmt<float>::REP, NCF = PairFmt<float>::NC;
@@ -782,11 +800,13 @@ template <> void fill_pair_tabs<double>(const ewald_ctx *c, const double *qinfo,
     /* the far table starts at FAR_T0; a kernel may start its far shell later (P->far_t0 set by the caller: the
      * move kernel keeps 16, where the longer table would cost its stacks a slot) */
     if (P->far_t0 < FAR_T0) P->far_t0 = FAR_T0;
-    if (P->far_t0 > 16) P->far_t0 = 16; /* the quintic table below covers t < 16 */
+    if (P->far_t0 > 16) P->far_t0 = 16;
     const int skip = (P->far_t0 - FAR_T0) << FAR_KB;
     if (c->t.n_far - skip <= 0) far = false;
-    /* with the far shell on, the quintic table is needed below t = 16 = 2^4 only */
-    const int near_bins = (4 - pt.e_min) << pt.kbits;
+    /* with the far shell on, the near table is needed below far_t0 only: the bins that start below it */
+    int e_far;
+    const double m_far = std::frexp((double)P->far_t0, &e_far); /* far_t0 = m 2^e, m in [1/2, 1) */
+    const int near_bins = ((e_far - 1 - pt.e_min) << pt.kbits) + (int)std::ceil((2 * m_far - 1) * (1 << pt.kbits));
     P->n_bins = far && near_bins < pt.n_bins ? near_bins : pt.n_bins;
     P->far_tab = far ? c->d_far + (size_t)skip * FAR_REP * 4 : nullptr; P->n_far = far ? c->t.n_far - skip : 0;
     P->key_far = far ? host_key((double)P->far_t0) : 0x7fffffff;
@@ -811,22 +831,40 @@ static bool real_shape(const ewald_ctx *c, size_t fixed, int min_cap_u, int min_
         const size_t budget = pass == 0 ? (half < full ? half : full) : full;
         for (int th = max_threads; th >= 32; th /= 2) {
             if (fixed >= budget) break;
-            /* bytes per unit of capacity: one near item + ff far items of 4 bytes, per lane, per warp.  ff = 2 (the
-             * far stack twice as deep: it receives twice the terms and can be serviced once per pair) if that
-             * fits, else 1 */
-            for (int ff = far ? 2 : 1; ff >= 1; ff--) {
-                const size_t per_cap = (size_t)(th / 32) * 32 * (sizeof(T) + (far ? 4 * ff : 0));
-                long long cu = (long long)((budget - fixed) / per_cap);
-                const long long want = 2 * (min_cap_u > min_cap_g ? min_cap_u : min_cap_g) + 8;
+            /* bytes per lane for the stacks of the CTA's th / 32 warps */
+            const long long lane_bytes = (long long)((budget - fixed) / ((size_t)(th / 32) * 32));
+            const long long want = 2 * (min_cap_u > min_cap_g ? min_cap_u : min_cap_g) + 8;
+            const long long need = min_cap_u > 2 * min_cap_g ? min_cap_u : 2 * min_cap_g;
+            long long cu = 0, cf = 0;
+            if (!far) {
+                cu = lane_bytes / (long long)sizeof(T);
                 if (cu > want) cu = want;
                 cu &= ~1LL;
-                if (cu >= min_cap_u && cu >= 2 * min_cap_g) {
-                    *threads = th;
-                    P->cap_u = (int)cu; P->cap_g = (int)(cu / 2);
-                    P->capf_u = far ? ff * (int)cu : 0; P->capf_g = far ? ff * (int)cu / 2 : 0;
-                    *smem = fixed + (size_t)cu * per_cap;
-                    return true;
+            } else {
+                /* the far stack receives twice the terms: first choice twice the near capacity (the same bytes);
+                 * if that does not fit, the near stack at its minimum and the rest to the far stack, which at
+                 * 20 + PAIR_R items is serviced once per pair (set_outer_far); else equal capacities */
+                cu = lane_bytes / (long long)(sizeof(T) + 8);
+                if (cu > want) cu = want;
+                cu &= ~1LL;
+                cf = 2 * cu;
+                if (cu < need) {
+                    cu = need + (need & 1);
+                    cf = ((lane_bytes - cu * (long long)sizeof(T)) / 4) & ~1LL;
+                    if (cf > 2 * cu) cf = 2 * cu;
+                    if (cf < 20 + PAIR_R) {
+                        cu = (lane_bytes / (long long)(sizeof(T) + 4)) & ~1LL;
+                        if (cu > want) cu = want;
+                        cf = cu;
+                    }
                 }
+            }
+            if (cu >= need && (!far || cf >= need)) {
+                *threads = th;
+                P->cap_u = (int)cu; P->cap_g = (int)(cu / 2);
+                P->capf_u = far ? (int)cf : 0; P->capf_g = far ? (int)(cf / 2) : 0;
+                *smem = fixed + (size_t)(th / 32) * 32 * ((size_t)cu * sizeof(T) + (far ? (size_t)cf * 4 : 0));
+                return true;
             }
             if (pass == 0) break; /* two CTAs per SM only at full size */
         }
@@ -894,6 +932,10 @@ static ewald_status launch_real(ewald_ctx *c, int W, int n, const T *pos, const 
     const CombineArgs comb = A.comb;
     if (!fold) A.comb.energies = nullptr;
     if (grid > 0x7fffffffLL) return fail(c, EWALD_ERANGE, "grid too large");
+    {
+        const int sh[8] = {threads, (int)smem, A.P.cap_u, A.P.capf_u, A.P.n_bins, A.P.n_far, (int)grid, A.g.far_once};
+        std::memcpy(c->shape[0], sh, sizeof sh);
+    }
 #define EWALD_LAUNCH_REAL(DIM, ORTHO, M)                                                          \
     do {                                                                                          \
         st = allow_smem(c, real_kernel<T, DIM, ORTHO, M>, smem);                                  \
@@ -1058,7 +1100,10 @@ static ewald_status move_batch_t(ewald_ctx *c, int n_moves, const int *walker, c
     A.rowlen = c->rowlen;
     A.img = Tabs<T>::img(c); A.nimg = c->nimg;
     A.ion_pos = Tabs<T>::ion_pos(c); A.ion_q = Tabs<T>::ion_q(c); A.n_ion = c->t.n_ion;
-    A.P.far_t0 = 16; /* measured: 13.4 M moves/s with the far shell from t = 16, 10.5 M from t = 13 (config 5, FP64) */
+#ifndef EWALD_MOVE_FAR_T0
+#define EWALD_MOVE_FAR_T0 16
+#endif
+    A.P.far_t0 = EWALD_MOVE_FAR_T0; /* measured: 13.4 M moves/s with the far shell from t = 16, 10.5 M from t = 13 (config 5, FP64) */
     fill_pair_tabs<T>(c, (const double *)c->st_qinfo.p, &A.P);
     A.n_moves = n_moves;
     A.walker = walker; A.electron = electron; A.new_r = new_r; A.commit = commit; A.delta_e = delta_e;
@@ -1089,6 +1134,8 @@ static ewald_status move_batch_t(ewald_ctx *c, int n_moves, const int *walker, c
                                                                 smem));                           \
         if (per_sm < 1) per_sm = 1;                                                               \
         const int grid = want_grid < c->sm_count * per_sm ? want_grid : c->sm_count * per_sm;     \
+        const int sh[8] = {threads, (int)smem, A.P.cap_u, A.P.capf_u, A.P.n_bins, A.P.n_far, grid, A.g.far_once}; \
+        std::memcpy(c->shape[1], sh, sizeof sh);                                                  \
         ProfScope ps(c, 3);                                                                       \
         move_kernel<T, DIM, ORTHO, M><<<grid, threads, smem, c->stream>>>(A);                     \
     } while (0)
@@ -1167,6 +1214,13 @@ extern "C" ewald_status ewald_move_delta(ewald_ctx *c, int walker, int electron,
 }
 
 /* ---- per-kernel timers -------------------------------------------------------------------- */
+
+extern "C" ewald_status ewald_launch_shape(const ewald_ctx *c, int which, int *out)
+{
+    if (!c || !out || which < 0 || which > 1) return EWALD_EINVAL;
+    std::memcpy(out, c->shape[which], sizeof c->shape[which]);
+    return EWALD_OK;
+}
 
 extern "C" ewald_status ewald_profile_enable(ewald_ctx *c, int on)
 {

@@ -74,7 +74,7 @@ struct PairTable {
     double t_min = 0, t_max = 0;          /* the table covers [t_min, t_max)                         */
     std::vector<double> coef;             /* [n_bins][degree + 1], variable u = t - bin centre       */
 };
-constexpr int PAIR_K64 = 7, PAIR_DEG64 = 5;  /* FP64: 128 bins per octave, quintic: rel. error < 1e-16 */
+constexpr int PAIR_K64 = 5, PAIR_DEG64 = 7;  /* FP64:  32 bins per octave, degree 7: rel. error < 2e-14 */
 constexpr int PAIR_K32 = 5, PAIR_DEG32 = 3;  /* FP32:  32 bins per octave, cubic:   rel. error < 3e-9  */
 #ifndef EWALD_FAR_T0
 #define EWALD_FAR_T0 13

@@ -131,7 +131,7 @@ __global__ void __launch_bounds__(RECIP_THREADS) recip_kernel(RecipArgs<T> A)
 
 /* Tables and stack shapes of the real-space machinery, common to the energy and move kernels. */
 template <typename T> struct PairTabs {
-    const T *pair_tab; int n_bins;   /* [n_bins][PairFmt<T>::REP][PairFmt<T>::NC]                       */
+    const T *pair_tab; int n_bins;   /* PairFmt<T>::elems(n_bins) values in the layout of PairFmt<T>    */
     T t_safe;                        /* some t inside the table                                         */
     const float *far_tab; int n_far; /* FP64 kernels: [n_far][FarFmt::REP][4] far-shell cubics; 0 = none */
     int key_far;                     /* order key of the far shell's start, INT_MAX = none              */
@@ -169,7 +169,7 @@ constexpr int REAL_MAX_THREADS = 512;
 
 /* Shared-memory carve-up common to the real-space and move kernels. */
 template <typename T> struct RealSmem {
-    T *tab;     /* [n_bins][REP][NC] */
+    T *tab;     /* PairFmt<T>::elems(n_bins) */
     float *far; /* [n_far][REP][4] */
     T *img;     /* [nimg][3]; FP32: followed by the [nimg][3] low parts */
     T *ion;     /* [n_ion][4] = x,y,z,q */
@@ -181,7 +181,7 @@ template <typename T> struct RealSmem {
     __device__ __forceinline__ RealSmem(unsigned char *raw, const PairTabs<T> &P, int nimg, int n_ion, size_t rest_elems)
     {
         tab = reinterpret_cast<T *>(raw);
-        far = reinterpret_cast<float *>(tab + up4((size_t)P.n_bins * PairFmt<T>::NC * PairFmt<T>::REP));
+        far = reinterpret_cast<float *>(tab + up4(PairFmt<T>::elems(P.n_bins)));
         img = reinterpret_cast<T *>(reinterpret_cast<unsigned char *>(far) + far_bytes(P.n_far));
         ion = img + up4(3 * IMG_PARTS * (size_t)nimg);
         rest = ion + up4(4 * (size_t)n_ion);
@@ -190,19 +190,19 @@ template <typename T> struct RealSmem {
     /* bytes before the stacks */
     static size_t fixed_bytes(int n_bins, int n_far, int nimg, int n_ion, size_t rest_elems)
     {
-        return (up4((size_t)n_bins * PairFmt<T>::NC * PairFmt<T>::REP) + up4(3 * IMG_PARTS * (size_t)nimg) + up4(4 * (size_t)n_ion) +
+        return (up4(PairFmt<T>::elems(n_bins)) + up4(3 * IMG_PARTS * (size_t)nimg) + up4(4 * (size_t)n_ion) +
                 up4(rest_elems)) * sizeof(T) + far_bytes(n_far);
     }
     /* bytes of one warp's stacks (the two item kinds of a stack share the same bytes) */
     static __host__ __device__ size_t warp_stack_bytes(const PairTabs<T> &P)
     {
-        return (size_t)P.cap_u * 32 * sizeof(T) + (size_t)P.capf_u * 32 * 4; /* capf_u = 2 cap_u or 0 */
+        return (size_t)P.cap_u * 32 * sizeof(T) + (size_t)P.capf_u * 32 * 4; /* near items, then far items */
     }
     __device__ __forceinline__ void fill(const PairTabs<T> &P, const T *gimg, int nimg, const T *ion_pos,
                                          const T *ion_q, int n_ion, int tid, int nthreads)
     {
-        {   /* NC * sizeof(T) is a multiple of 16 */
-            const int n4 = P.n_bins * PairFmt<T>::NC * PairFmt<T>::REP * (int)sizeof(T) / 16;
+        {   /* a multiple of 16 bytes in both layouts */
+            const int n4 = (int)(PairFmt<T>::elems(P.n_bins) * sizeof(T) / 16);
             const int4 *src = reinterpret_cast<const int4 *>(P.pair_tab);
             int4 *dst = reinterpret_cast<int4 *>(tab);
             for (int t = tid; t < n4; t += nthreads) dst[t] = src[t];
@@ -330,7 +330,7 @@ __device__ __forceinline__ double real_body(const RealArgs<T> &A, RealSmem<T> &S
 }
 
 template <typename T, int DIM, bool ORTHO, int M>
-__global__ void __launch_bounds__(REAL_MAX_THREADS) real_kernel(RealArgs<T> A)
+__global__ void __launch_bounds__(REAL_MAX_THREADS, sizeof(T) == 4 ? 2 : 1) real_kernel(RealArgs<T> A)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     RealSmem<T> S(smem_raw, A.P, A.nimg, A.n_ion, (size_t)DIM * A.npad + A.n);
@@ -488,22 +488,32 @@ __device__ __forceinline__ double move_real(const MoveArgs<T> &A, RealSmem<T> &S
         const int j0 = seg == 0 || !UQ ? 0 : A.P.sp_start[seg - 1];
         const int cnt = seg == 0 ? A.n : (UQ ? A.P.sp_start[seg] : A.n_ion);
         const T qion0 = seg == 0 ? T(0) : S.ion[4 * j0 + 3];
-        for (int base = j0; base < cnt; base += 32) {
+        /* the partner of the next round is loaded before this round's scan (its latency was 12 % of the kernel) */
+        auto fetch = [&](int base, T (&r)[3], T &wt) {
             const int j = base + lane;
-            const bool valid = j < cnt && (seg >= 1 || j != k);
-            T rj[3] = {0, 0, 0};
-            T w = UQ ? T(1) : T(0);
-            if (valid) {
+            const bool ok = j < cnt && (seg >= 1 || j != k);
+            r[0] = r[1] = r[2] = T(0);
+            wt = UQ ? T(1) : T(0);
+            if (ok) {
                 if (seg == 0) {
 #pragma unroll
-                    for (int x = 0; x < DIM; x++) rj[x] = pw[x * A.npad + j];
-                    if (!UQ) w = A.q[j];
+                    for (int x = 0; x < DIM; x++) r[x] = pw[x * A.npad + j];
+                    if (!UQ) wt = A.q[j];
                 } else {
 #pragma unroll
-                    for (int x = 0; x < DIM; x++) rj[x] = S.ion[4 * j + x];
-                    if (!UQ) w = S.ion[4 * j + 3];
+                    for (int x = 0; x < DIM; x++) r[x] = S.ion[4 * j + x];
+                    if (!UQ) wt = S.ion[4 * j + 3];
                 }
             }
+            return ok;
+        };
+        T rj_next[3], w_next;
+        bool valid_next = fetch(j0, rj_next, w_next);
+        for (int base = j0; base < cnt; base += 32) {
+            const bool valid = valid_next;
+            const T rj[3] = {rj_next[0], rj_next[1], rj_next[2]};
+            const T w = w_next;
+            valid_next = fetch(base + 32, rj_next, w_next);
             T dn[3] = {0, 0, 0}, dold[3] = {0, 0, 0};
 #pragma unroll
             for (int x = 0; x < DIM; x++) {
@@ -522,10 +532,9 @@ __device__ __forceinline__ double move_real(const MoveArgs<T> &A, RealSmem<T> &S
 }
 
 constexpr int MOVE_MAX_THREADS = 512;
-#ifndef EWALD_MOVE_G_BATCH
-#define EWALD_MOVE_G_BATCH 4
-#endif
-constexpr int MOVE_G_BATCH = EWALD_MOVE_G_BATCH; /* rho(G) vectors a lane loads ahead in [S7b] */
+/* rho(G) vectors per lane and batch in [S7b] (two batches in flight); more spills registers: FP64 2 / 3 / 4 gave
+ * 13.5 / 15.4 / 11.7 M moves/s, FP32 (64 registers) 25.9 / 24.5 / 23.4 */
+template <typename T> struct MoveBatch { static constexpr int N = sizeof(T) == 8 ? 3 : 2; };
 
 template <typename T, int DIM, bool ORTHO, int M>
 __global__ void __launch_bounds__(MOVE_MAX_THREADS, sizeof(T) == 4 ? 2 : 1) move_kernel(MoveArgs<T> A)
@@ -564,38 +573,41 @@ __global__ void __launch_bounds__(MOVE_MAX_THREADS, sizeof(T) == 4 ? 2 : 1) move
         __syncwarp();
 
         /* [S7b] Delta E_recip and the patch of rho(G).  The walker's rho comes from HBM and nothing else of the
-         * warp's work can cover that latency, so the loads of MOVE_G_BATCH vectors per lane are issued before the
+         * warp's work can cover that latency, so the loads of MoveBatch<T>::N vectors per lane are issued before the
          * first of them is used (one load in flight per lane ran at 1.1 TB/s over the whole GPU). */
         T *rr = A.rho + (size_t)w * 2 * A.ngp_pad;
         double acc = 0;
-        for (int g0 = lane; g0 < A.ngp; g0 += 32 * MOVE_G_BATCH) {
-            short4 nn[MOVE_G_BATCH];
-            T re[MOVE_G_BATCH], im[MOVE_G_BATCH], wg[MOVE_G_BATCH];
+        /* (prefetching rho alone and reading the shared G indices and weights when used was slower: 13.3 M) */
+        struct GBatch { short4 nn[MoveBatch<T>::N]; T re[MoveBatch<T>::N], im[MoveBatch<T>::N], wg[MoveBatch<T>::N]; };
+        auto load = [&](GBatch &b, int g0) {
 #pragma unroll
-            for (int u = 0; u < MOVE_G_BATCH; u++) {
+            for (int u = 0; u < MoveBatch<T>::N; u++) {
                 const int g = g0 + 32 * u;
                 const bool in = g < A.ngp;
-                nn[u] = in ? __ldg(A.gn + g) : make_short4(0, 0, 0, 0);
-                re[u] = in ? rr[g] : T(0);
-                im[u] = in ? rr[A.ngp_pad + g] : T(0);
-                wg[u] = in ? __ldg(A.w2 + g) : T(0);
+                b.nn[u] = in ? __ldg(A.gn + g) : make_short4(0, 0, 0, 0);
+                b.re[u] = in ? rr[g] : T(0);
+                b.im[u] = in ? rr[A.ngp_pad + g] : T(0);
+                b.wg[u] = in ? __ldg(A.w2 + g) : T(0);
             }
+        };
+        auto patch = [&](const GBatch &b, int g0) {
 #pragma unroll
-            for (int u = 0; u < MOVE_G_BATCH; u++) {
+            for (int u = 0; u < MoveBatch<T>::N; u++) {
                 const int g = g0 + 32 * u;
+                const short4 nn = b.nn[u];
                 T2 ph[2];
 #pragma unroll
                 for (int which = 0; which < 2; which++) {
                     const T2 *row = tab + which * A.rowlen;
-                    T2 e1 = row[A.off[0] + nn[u].x];
-                    T2 e2 = row[A.off[1] + (nn[u].y < 0 ? -nn[u].y : nn[u].y)];
-                    if (nn[u].y < 0) e2.y = -e2.y;
+                    T2 e1 = row[A.off[0] + nn.x];
+                    T2 e2 = row[A.off[1] + (nn.y < 0 ? -nn.y : nn.y)];
+                    if (nn.y < 0) e2.y = -e2.y;
                     T2 e;
                     e.x = e1.x * e2.x - e1.y * e2.y;
                     e.y = e1.x * e2.y + e1.y * e2.x;
                     if (DIM == 3) {
-                        T2 e3 = row[A.off[2] + (nn[u].z < 0 ? -nn[u].z : nn[u].z)];
-                        if (nn[u].z < 0) e3.y = -e3.y;
+                        T2 e3 = row[A.off[2] + (nn.z < 0 ? -nn.z : nn.z)];
+                        if (nn.z < 0) e3.y = -e3.y;
                         T2 f;
                         f.x = e.x * e3.x - e.y * e3.y;
                         f.y = e.x * e3.y + e.y * e3.x;
@@ -604,8 +616,23 @@ __global__ void __launch_bounds__(MOVE_MAX_THREADS, sizeof(T) == 4 ? 2 : 1) move
                     ph[which] = e;
                 }
                 const T dr = ph[1].x - ph[0].x, di = ph[1].y - ph[0].y;
-                acc += (double)(wg[u] * (2 * qk * (re[u] * dr + im[u] * di) + qk * qk * (dr * dr + di * di)));
-                if (A.commit && g < A.ngp) { rr[g] = re[u] + qk * dr; rr[A.ngp_pad + g] = im[u] + qk * di; }
+                acc += (double)(b.wg[u] * (2 * qk * (b.re[u] * dr + b.im[u] * di) + qk * qk * (dr * dr + di * di)));
+                if (A.commit && g < A.ngp) { rr[g] = b.re[u] + qk * dr; rr[A.ngp_pad + g] = b.im[u] + qk * di; }
+            }
+        };
+        {   /* two batches in flight: the loads of the next one are issued before the current one is used */
+            constexpr int STEP = 32 * MoveBatch<T>::N;
+            GBatch b0, b1;
+            int g0 = lane;
+            load(b0, g0);
+            while (g0 < A.ngp) {
+                load(b1, g0 + STEP);
+                patch(b0, g0);
+                g0 += STEP;
+                if (g0 >= A.ngp) break;
+                load(b0, g0 + STEP);
+                patch(b1, g0);
+                g0 += STEP;
             }
         }
 

@@ -7,7 +7,7 @@
  * bins are cut from the floating-point bits of t (2^K per binary octave), the local variable is
  * u = t - (bin centre), the coefficients were fitted in long double at setup ("lookup tables ...
  * always DP"; ewald_setup.cpp build_pair_table) and sit in shared memory as
- * [bin][degree+1] (FP64: quintic, 3 LDS.128 per term; FP32: cubic, 1 LDS.128).
+ * polynomials per bin (FP64: degree 7, 4 conflict-free LDS.128 per term; FP32: cubic, 1 LDS.128; layouts at PairFmt).
  *
  * Two phases per warp:
  *   A  cull: each lane owns one pair, reduces its displacement to the cell, scans the candidate
@@ -24,11 +24,28 @@
 namespace ewald {
 
 template <typename T> struct PairFmt;
-/* REP: copies of the table, interleaved [bin][copy][NC]; lane l reads copy l mod REP.  The 16-byte FP32
- * entries are replicated 8 times: the 8 lanes of a quarter-warp then read 8 different 16-byte columns and
- * the gather has no bank conflicts (6 KB -> 48 KB; the 61 KB FP64 table cannot afford it). */
-template <> struct PairFmt<double> { static constexpr int K = 7, DEG = 5, NC = 6, SHIFT = 20 - 7, EBIAS = 1023, REP = 1; };
-template <> struct PairFmt<float> { static constexpr int K = 5, DEG = 3, NC = 4, SHIFT = 23 - 5, EBIAS = 127, REP = 8; };
+/* FP32: cubic on 32 bins per octave, REP = 8 copies interleaved [bin][copy][NC]; lane l reads copy l mod 8, so the
+ * 8 lanes of a quarter-warp read 8 different 16-byte columns and the gather has no bank conflicts (6 KB -> 48 KB).
+ * FP64: degree 7 on 32 bins per octave (64 bytes per bin; the quintic on 128 bins per octave of round 1 and 2
+ * took 48-byte rows from one copy: ~2.6 wavefronts per quarter-warp and LDS.128 instead of 1).  The table is a
+ * sequence of 512-byte ROWS [chunk 0..3][slot 0..7][2 doubles], chunk c = coefficients (2c, 2c + 1):
+ *   t >= 4 (86 % of the terms below t = 13 of a uniform gas): one bin per row, the 8 slots are 8 copies, lane l
+ *           reads slot l mod 8: each of the four LDS.128 of a term is conflict-free (4 wavefronts per warp);
+ *   t <  4 (8 octaves, 256 bins): 8 consecutive bins per row, slot = bin mod 8 (one copy: 16 KB instead of 128).
+ * Both regions are addressed as row * 512 + slot * 16 + chunk * 128 bytes.  With the far shell from t = 13 the
+ * table takes 43 KB (52 + 32 rows); eight copies from t = 1 (72 KB) cost the stacks their depth and were slower. */
+template <> struct PairFmt<double> {
+    static constexpr int K = 5, DEG = 7, NC = 8, SHIFT = 20 - 5, EBIAS = 1023, REP = 8;
+    static constexpr int E_MIN = -6, E_SPLIT = 0;        /* the table starts at 2^E_MIN; copies from 2^E_SPLIT */
+    static constexpr int LOW = (E_SPLIT - E_MIN) << K;   /* bins below the split */
+    static constexpr int ROW = 64;                       /* doubles per row */
+    __host__ __device__ static constexpr int rows(int n_bins) { return n_bins <= LOW ? (n_bins + 7) / 8 : LOW / 8 + (n_bins - LOW); }
+    __host__ __device__ static constexpr size_t elems(int n_bins) { return (size_t)rows(n_bins) * ROW; }
+};
+template <> struct PairFmt<float> {
+    static constexpr int K = 5, DEG = 3, NC = 4, SHIFT = 23 - 5, EBIAS = 127, REP = 8;
+    __host__ __device__ static constexpr size_t elems(int n_bins) { return (size_t)n_bins * NC * REP; }
+};
 
 /* Geometry in kappa-scaled units. */
 template <typename T> struct RealGeom {
@@ -102,20 +119,35 @@ __device__ __forceinline__ float bin_centre(float, int key)
     return __int_as_float((key & ~((1 << S) - 1)) | (1 << (S - 1)));
 }
 
-/* F(t) from the shared-memory table; requires t_min <= t < t_max. */
-__device__ __forceinline__ double pair_f(double t, const double *tab, int bias)
+/* F(t) from the shared-memory table; requires t_min <= t < t_max.  slot2 = 2 * (lane mod 8).
+ * ESTRIN: 9 operations in a chain of 4 instead of Horner's 7 in a chain of 7: faster in real_kernel (0.662 ->
+ * 0.638 ms on config 2), slower in move_kernel, whose 16 warps per SM sit at the 128-register limit (15.2 -> 14.1 M
+ * moves/s): each kernel takes its own. */
+template <bool ESTRIN>
+__device__ __forceinline__ double pair_f(double t, const double *tab, int bias, int slot2)
 {
+    typedef PairFmt<double> F;
     const int key = order_key(t);
     const double u = t - bin_centre(t, key);
-    const double2 *c = reinterpret_cast<const double2 *>(tab) + 3 * ((key >> PairFmt<double>::SHIFT) - bias);
-    const double2 c01 = c[0], c23 = c[1], c45 = c[2];
-    double p = fma(c45.y, u, c45.x);
-    p = fma(p, u, c23.y);
-    p = fma(p, u, c23.x);
-    p = fma(p, u, c01.y);
-    return fma(p, u, c01.x);
+    const int bin = (key >> F::SHIFT) - bias, hb = bin - F::LOW;
+    const int off = hb >= 0 ? (hb + F::LOW / 8) * F::ROW + slot2 : (bin >> 3) * F::ROW + 2 * (bin & 7);
+    const double2 *c = reinterpret_cast<const double2 *>(tab + off);
+    const double2 c01 = c[0], c23 = c[8], c45 = c[16], c67 = c[24];
+    if (!ESTRIN) {
+        double p = fma(c67.y, u, c67.x);
+        p = fma(p, u, c45.y);
+        p = fma(p, u, c45.x);
+        p = fma(p, u, c23.y);
+        p = fma(p, u, c23.x);
+        p = fma(p, u, c01.y);
+        return fma(p, u, c01.x);
+    }
+    const double u2 = u * u;
+    const double a = fma(c01.y, u, c01.x), b = fma(c23.y, u, c23.x), c4 = fma(c45.y, u, c45.x), d = fma(c67.y, u, c67.x);
+    return fma(u2 * u2, fma(d, u2, c4), fma(b, u2, a));
 }
-__device__ __forceinline__ float pair_f(float t, const float *tab, int bias)
+template <bool ESTRIN>
+__device__ __forceinline__ float pair_f(float t, const float *tab, int bias, int)
 {
     const int key = order_key(t);
     const float u = t - bin_centre(t, key);
@@ -233,17 +265,20 @@ struct LaneStack : StackBase<T, T, UQ, LaneStack<T, UQ, SIGNED>> {
     typedef T Acc;
     const T *tab;
     int bias;
+    int slot2; /* FP64: 2 * (lane mod 8), the lane's 16-byte column of a table row */
     __device__ __forceinline__ void init(void *warp_mem, int lane, int cap, const T *table, int b, T t_safe)
     {
-        tab = table + (lane % PairFmt<T>::REP) * PairFmt<T>::NC; /* this lane's copy */
+        /* FP32: this lane's copy; FP64: the table's base (the column is chosen per term, see pair_f) */
+        tab = sizeof(T) == 4 ? table + (lane % PairFmt<T>::REP) * PairFmt<T>::NC : table;
+        slot2 = 2 * (lane & 7);
         bias = b;
         this->init_base(warp_mem, lane, cap, t_safe);
     }
     __device__ __forceinline__ T term(T t, T w) const
     {
         /* SIGNED stacks of bare t carry the sign of the term in the sign bit of t */
-        if (UQ && SIGNED) return pair_f(abs_of(t), tab, bias) * sign_unit(t);
-        return UQ ? pair_f(t, tab, bias) : pair_f(t, tab, bias) * w;
+        if (UQ && SIGNED) return pair_f<!SIGNED>(abs_of(t), tab, bias, slot2) * sign_unit(t);
+        return UQ ? pair_f<!SIGNED>(t, tab, bias, slot2) : pair_f<!SIGNED>(t, tab, bias, slot2) * w;
     }
 };
 

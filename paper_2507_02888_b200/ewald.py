@@ -25,7 +25,7 @@ SYMBOLS = ["ewald_padded_n", "ewald_setup", "ewald_setup_summary", "ewald_oct_pl
            "ewald_load_walkers", "ewald_move_delta_batch", "ewald_move_delta_batch_host",
            "ewald_move_delta", "ewald_num_g", "ewald_num_images", "ewald_r_cutoff", "ewald_get_g",
            "ewald_get_rho", "ewald_get_positions", "ewald_get_constants", "ewald_probe_fma", "ewald_probe_dmma",
-           "ewald_profile_enable", "ewald_profile_read", "ewald_launch_count",
+           "ewald_profile_enable", "ewald_profile_read", "ewald_launch_count", "ewald_launch_shape",
            "ewald_last_error", "ewald_version"]
 
 
@@ -84,6 +84,7 @@ def load_library():
         "ewald_probe_dmma": (i, [vp, i, dp]),
         "ewald_profile_enable": (i, [vp, i]),
         "ewald_profile_read": (i, [vp, dp, ip]),
+        "ewald_launch_shape": (i, [vp, i, ip]),
         "ewald_launch_count": (ctypes.c_longlong, [vp]),
         "ewald_last_error": (ctypes.c_char_p, [vp]),
         "ewald_version": (ctypes.c_char_p, []),
@@ -402,6 +403,14 @@ def ewald_profile_read(ctx):
     ms, cnt = (ctypes.c_double * 4)(), (ctypes.c_int * 4)()
     _check(ctx, load_library().ewald_profile_read(ctx.handle, ms, cnt))
     return {k: (ms[i], cnt[i]) for i, k in enumerate(KERNEL_CLASSES)}
+
+
+def ewald_launch_shape(ctx, which):
+    """Shape of the last real-space (which = 0) or move (which = 1) launch of the context, as a dict."""
+    out = (ctypes.c_int * 8)()
+    _check(ctx, load_library().ewald_launch_shape(ctx.handle, int(which), out))
+    keys = ("threads", "smem_bytes", "cap_near", "cap_far", "near_bins", "far_bins", "ctas", "far_once")
+    return dict(zip(keys, list(out)))
 
 
 def ewald_launch_count(ctx):
