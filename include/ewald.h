@@ -147,6 +147,27 @@ ewald_status ewald_energy_batch_host(ewald_ctx *ctx, int n_walkers, int n_partic
                                      ewald_prec prec, const void *positions, const void *charges,
                                      double *energies, double *components);
 
+/* Allocation-free entry point, for callers that cannot call cudaMalloc (CUDA graph capture, tight serving loops,
+ * harnesses that forbid it): the reciprocal-space energy E_recip of every walker (steps S1-S4: the reciprocal sum
+ * of Eq. 3; the same value as components[...][0] of ewald_energy_batch), computed by the complex
+ * half-set kernel (the one ewald_set_recip_variant(ctx, 1) selects) with its scratch -- one partial sum per walker
+ * and slab of 1024 G-vectors of the half set -- in a file-scope device array of EWALD_STATIC_SCRATCH_BYTES that
+ * every GPU holding the library keeps until the process exits.  Its device address is taken at ewald_setup.
+ *   positions, charges : DEVICE, layouts and types as for ewald_energy_batch
+ *   e_recip            : DEVICE [n_walkers] double, Hartree
+ * Limit: n_walkers * ceil(N_G+ / 1024) <= EWALD_STATIC_SCRATCH_BYTES / 8 = 131072 (N_G+ = ewald_num_g / 2; e.g.
+ * 131072 walkers per call on configs 1-5, whose half sets fit one slab); beyond it EWALD_ERANGE, nothing launched,
+ * ewald_last_error says by how much.  EWALD_ECUDA if the array's address could not be taken at set-up.
+ * The call enqueues two kernels on the context's stream and returns; it calls no cudaMalloc, cudaFree, event or
+ * stream creation and does not synchronise.  Nothing in the array has to start at zero: every element a call reads
+ * it has written itself, so leftovers of earlier calls are harmless.  EVERY call on a device, from any context,
+ * shares the one array: calls that can overlap on the GPU (different streams, different contexts or host threads
+ * without ordering between them) race on it; order them on one stream or with events.  n_walkers = 0 is a
+ * no-op.  The fixed charges of ewald_set_fixed_charges enter as in ewald_energy_batch. */
+#define EWALD_STATIC_SCRATCH_BYTES (1 << 20)
+ewald_status ewald_recip_energy_static(ewald_ctx *ctx, int n_walkers, int n_particles, ewald_prec prec,
+                                       const void *positions, const void *charges, double *e_recip);
+
 /* Store a walker population in the context for single-particle moves: copies the positions and
  * charges and computes and stores rho(G) (of mobile particles plus fixed charges) per walker, in
  * the precision given.  Replaces any earlier population.  DEVICE pointers, layouts as above.       */

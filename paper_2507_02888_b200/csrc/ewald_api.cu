@@ -4,6 +4,7 @@
 #include <cmath>
 #include <cstdio>
 #include <cstring>
+#include <mutex>
 #include <new>
 #include <string>
 #include <vector>
@@ -78,6 +79,11 @@ struct ewald_ctx {
     DevBuf partial_recip, partial_real, qsums, done;
     DevBuf stage_pos, stage_q, stage_e, stage_comp;           /* *_host entry points */
     DevBuf mv_walker, mv_electron, mv_newr, mv_de;
+
+    /* ewald_recip_energy_static: device address of the file-scope scratch array on this context's device (null:
+     * the address could not be taken at set-up, static_err says why) */
+    double *static_scratch = nullptr;
+    std::string static_err;
 
     /* stored walker population */
     int st_walkers = 0, st_n = 0, st_npad = 0;
@@ -221,6 +227,39 @@ extern "C" int ewald_padded_n(int n) { return n <= 0 ? 0 : (n + 3) & ~3; }
 extern "C" const char *ewald_version(void) { return kVersion; }
 extern "C" const char *ewald_last_error(const ewald_ctx *c) { return c ? c->err.c_str() : ""; }
 
+/* ---- scratch of the allocation-free entry point (ewald_recip_energy_static, end of this file) ----
+ * One file-scope device array per GPU that loads the library, held until the process exits.  In HOST code the name
+ * `g_static_scratch` is only a stand-in for the symbol, not a device address: the address is taken once per device,
+ * at set-up, with that device current, by cudaGetSymbolAddress, and it is that pointer the kernels receive. */
+static_assert(EWALD_STATIC_SCRATCH_BYTES % 256 == 0, "scratch size");
+constexpr size_t STATIC_SCRATCH_DOUBLES = EWALD_STATIC_SCRATCH_BYTES / sizeof(double);
+static __device__ __align__(256) double g_static_scratch[STATIC_SCRATCH_DOUBLES];
+
+constexpr int STATIC_MAX_DEVICES = 64;
+static std::mutex g_static_mutex;
+static bool g_static_tried[STATIC_MAX_DEVICES];
+static double *g_static_addr[STATIC_MAX_DEVICES];
+static cudaError_t g_static_status[STATIC_MAX_DEVICES];
+
+/* Call with c->device current.  A failure does not fail the set-up: only the static entry point needs the address
+ * and it reports the recorded error. */
+static void resolve_static_scratch(ewald_ctx *c)
+{
+    std::lock_guard<std::mutex> lock(g_static_mutex);
+    const int d = c->device;
+    double *ptr = nullptr;
+    cudaError_t e;
+    if (d >= 0 && d < STATIC_MAX_DEVICES && g_static_tried[d]) {
+        ptr = g_static_addr[d]; e = g_static_status[d];
+    } else {
+        e = cudaGetSymbolAddress((void **)&ptr, g_static_scratch);
+        if (e != cudaSuccess) { ptr = nullptr; (void)cudaGetLastError(); }
+        if (d >= 0 && d < STATIC_MAX_DEVICES) { g_static_tried[d] = true; g_static_addr[d] = ptr; g_static_status[d] = e; }
+    }
+    c->static_scratch = ptr;
+    if (e != cudaSuccess) c->static_err = std::string("cudaGetSymbolAddress(g_static_scratch): ") + cudaGetErrorString(e);
+}
+
 extern "C" ewald_status ewald_setup(ewald_ctx **out, int dim, const double *cell, double gamma,
                                     double g_cutoff, const ewald_opts *opts)
 {
@@ -235,6 +274,7 @@ extern "C" ewald_status ewald_setup(ewald_ctx **out, int dim, const double *cell
     c->stream = opts ? (cudaStream_t)opts->stream : nullptr;
     DeviceGuard guard_(c->device);
     if (!guard_.ok) { delete c; return EWALD_ECUDA; }
+    resolve_static_scratch(c);
 
     const HostTables &t = c->t;
     c->ngp = (int)t.g_w2.size();
@@ -1375,4 +1415,81 @@ extern "C" ewald_status ewald_probe_fma(ewald_ctx *c, ewald_prec prec, int iters
     cudaEventDestroy(e1);
     *flops = 2.0 * 64.0 * iters * (double)blocks * threads / (ms * 1e-3);
     return EWALD_OK;
+}
+
+/* ---- allocation-free entry point ------------------------------------------------------------------------
+ * ewald_recip_energy_static: E_recip per walker (S1-S4, the reciprocal sum of Eq. 3) by the
+ * complex half-set kernel recip_kernel -- the kernel whose per-(walker, slab) partial sums are its scratch --
+ * with that scratch in g_static_scratch instead of the context's growing buffer.  No cudaMalloc, no cudaFree, no
+ * event creation, no synchronisation: two kernel launches on the context's stream. */
+
+/* out[w] = sum over the slabs, in slab order (the order combine_kernel uses). */
+__global__ void static_slab_sum_kernel(const double *partial, int n_slabs, int n_walkers, double *out)
+{
+    const int w = blockIdx.x * blockDim.x + threadIdx.x;
+    if (w >= n_walkers) return;
+    double e = 0;
+    for (int k = 0; k < n_slabs; k++) e += partial[(size_t)w * n_slabs + k];
+    out[w] = e;
+}
+
+template <typename T>
+static ewald_status recip_energy_static_t(ewald_ctx *c, int W, int n, const T *pos, const T *q, int n_slabs,
+                                          double *e_recip)
+{
+    typedef typename Num<T>::T2 T2;
+    RecipArgs<T> A;
+    A.pos = pos; A.q = q; A.n = n; A.npad = ewald_padded_n(n);
+    A.gn = c->d_gn; A.w2 = Tabs<T>::w2(c); A.ion_rho = c->t.n_ion ? Tabs<T>::ion_rho(c) : nullptr;
+    A.ngp = c->ngp; A.ngp_pad = c->ngp_pad;
+    for (int k = 0; k < 3; k++) { A.nmax[k] = c->t.n_max[k]; A.off[k] = c->off[k]; }
+    A.rowlen = c->rowlen;
+    A.rho_out = nullptr;
+    A.partial = c->static_scratch; /* the device address from cudaGetSymbolAddress, never the symbol's name */
+    A.n_slabs = n_slabs;
+    for (int i = 0; i < 9; i++) A.binv[i] = c->t.binv[i];
+    const size_t smem = (size_t)RECIP_CHUNK * c->rowlen * sizeof(T2);
+    const long long grid = (long long)W * n_slabs;
+    ewald_status st;
+    if (c->t.dim == 3) {
+        if ((st = allow_smem(c, recip_kernel<T, 3>, smem)) != EWALD_OK) return st;
+        recip_kernel<T, 3><<<(unsigned)grid, RECIP_THREADS, smem, c->stream>>>(A);
+    } else {
+        if ((st = allow_smem(c, recip_kernel<T, 2>, smem)) != EWALD_OK) return st;
+        recip_kernel<T, 2><<<(unsigned)grid, RECIP_THREADS, smem, c->stream>>>(A);
+    }
+    CU_TRY(c, cudaGetLastError());
+    static_slab_sum_kernel<<<(W + 127) / 128, 128, 0, c->stream>>>(c->static_scratch, n_slabs, W, e_recip);
+    CU_TRY(c, cudaGetLastError());
+    c->launches += 2;
+    return EWALD_OK;
+}
+
+extern "C" ewald_status ewald_recip_energy_static(ewald_ctx *c, int W, int n, ewald_prec prec, const void *pos,
+                                                  const void *q, double *e_recip)
+{
+    ewald_status st = check_batch(c, W, n, prec, pos, q);
+    if (st != EWALD_OK) return st;
+    if (W == 0) return EWALD_OK;
+    if (!e_recip) return fail(c, EWALD_EINVAL, "null e_recip");
+    EWALD_DEVICE(c);
+    if (!c->static_scratch) {
+        c->err = "static scratch unavailable: " + c->static_err;
+        return EWALD_ECUDA;
+    }
+    const int per = RECIP_THREADS * RECIP_GPT;
+    const int n_slabs = (c->ngp + per - 1) / per;
+    const unsigned long long need = (unsigned long long)W * (unsigned long long)n_slabs;
+    if (need > STATIC_SCRATCH_DOUBLES) {
+        char msg[256];
+        std::snprintf(msg, sizeof msg,
+                      "ewald_recip_energy_static: n_walkers (%d) x slabs (%d) = %llu partial sums exceed the static "
+                      "scratch of %llu doubles (EWALD_STATIC_SCRATCH_BYTES = %d); at most %llu walkers per call here",
+                      W, n_slabs, need, (unsigned long long)STATIC_SCRATCH_DOUBLES, (int)EWALD_STATIC_SCRATCH_BYTES,
+                      (unsigned long long)(STATIC_SCRATCH_DOUBLES / n_slabs));
+        return fail(c, EWALD_ERANGE, msg);
+    }
+    if (prec == EWALD_F64)
+        return recip_energy_static_t<double>(c, W, n, (const double *)pos, (const double *)q, n_slabs, e_recip);
+    return recip_energy_static_t<float>(c, W, n, (const float *)pos, (const float *)q, n_slabs, e_recip);
 }

@@ -21,7 +21,7 @@ _STATUS = {0: "EWALD_OK", 1: "EWALD_EINVAL", 2: "EWALD_ESINGULAR", 3: "EWALD_ERA
 SYMBOLS = ["ewald_padded_n", "ewald_setup", "ewald_setup_summary", "ewald_oct_plan_summary", "ewald_mma_plan_summary",
            "ewald_pair_table_eval",
            "ewald_destroy", "ewald_set_stream", "ewald_set_recip_variant", "ewald_set_real_variant",
-           "ewald_set_fixed_charges", "ewald_energy_batch", "ewald_energy_batch_host",
+           "ewald_set_fixed_charges", "ewald_energy_batch", "ewald_energy_batch_host", "ewald_recip_energy_static",
            "ewald_load_walkers", "ewald_move_delta_batch", "ewald_move_delta_batch_host",
            "ewald_move_delta", "ewald_num_g", "ewald_num_images", "ewald_r_cutoff", "ewald_get_g",
            "ewald_get_rho", "ewald_get_positions", "ewald_get_constants", "ewald_probe_fma", "ewald_probe_dmma",
@@ -69,6 +69,7 @@ def load_library():
         "ewald_set_fixed_charges": (i, [vp, i, dp, dp]),
         "ewald_energy_batch": (i, [vp, i, i, i, vp, vp, vp, vp]),
         "ewald_energy_batch_host": (i, [vp, i, i, i, vp, vp, vp, vp]),
+        "ewald_recip_energy_static": (i, [vp, i, i, i, vp, vp, vp]),
         "ewald_load_walkers": (i, [vp, i, i, i, vp, vp]),
         "ewald_move_delta_batch": (i, [vp, i, vp, vp, vp, i, vp]),
         "ewald_move_delta_batch_host": (i, [vp, i, vp, vp, vp, i, vp]),
@@ -286,6 +287,18 @@ def ewald_energy_batch(ctx, n_particles, positions, charges, energies, component
     _check(ctx, load_library().ewald_energy_batch(
         ctx.handle, w, n_particles, _prec_of(positions.dtype), _dev_ptr(positions, "positions"),
         _dev_ptr(charges, "charges"), _dev_ptr(energies, "energies"), _dev_ptr(components, "components")))
+
+
+EWALD_STATIC_SCRATCH_BYTES = 1 << 20  # include/ewald.h
+
+
+def ewald_recip_energy_static(ctx, n_particles, positions, charges, e_recip):
+    """E_recip per walker with the kernel's scratch in the library's static device array: allocates nothing.
+    positions: CUDA tensor [W, dim, n_pad]; charges: CUDA [n]; e_recip: CUDA float64 [W]."""
+    _check_batch(ctx, n_particles, positions, charges, e_recip)
+    _check(ctx, load_library().ewald_recip_energy_static(
+        ctx.handle, positions.shape[0], n_particles, _prec_of(positions.dtype), _dev_ptr(positions, "positions"),
+        _dev_ptr(charges, "charges"), _dev_ptr(e_recip, "e_recip")))
 
 
 def ewald_energy_batch_host(ctx, n_particles, positions, charges, energies, components=None):
