@@ -948,7 +948,13 @@ static ewald_status launch_real(ewald_ctx *c, int W, int n, const T *pos, const 
     const long long H = (n - 1) / 2;
     const long long total = (long long)n * H + ((n & 1) ? 0 : n / 2) + (long long)n * c->t.n_ion;
     long long n_tiles = (4LL * c->sm_count + W - 1) / W;
-    const long long max_tiles = (total + threads - 1) / threads;
+    long long max_tiles = (total + threads - 1) / threads;
+    /* Small batches of small boxes (|m| <= 2 in 3D, 125 candidates per pair; config 1): with one pair per thread the
+     * grid is a fraction of the GPU (8 walkers x 3 tiles), so the five z-images of a pair go to five lanes
+     * (ScanShape::ZSPLIT): five times the items, each a fifth of the work plus the pair's set-up again -- only when
+     * the pairs alone cannot fill the SMs */
+    A.zsplit = ortho && c->t.dim == 3 && c->t.m_shift == 2 && (long long)W * max_tiles < c->sm_count ? 1 : 0;
+    if (A.zsplit) max_tiles = (5 * total + threads - 1) / threads;
     if (n_tiles > max_tiles) n_tiles = max_tiles;
     if (n_tiles < 1) n_tiles = 1;
     ewald_status st = ensure(c, &c->partial_real, (size_t)W * n_tiles * sizeof(double));

@@ -163,6 +163,7 @@ template <typename T> struct RealArgs {
     RealGeom<T> g;
     CombineArgs comb;                             /* energies == null: no combine */
     int *done;                                    /* [W] CTAs of the walker that have finished (zero between calls) */
+    int zsplit;                                   /* ScanShape::ZSPLIT shapes: one z-image of a pair per lane (small batches) */
 };
 
 constexpr int REAL_MAX_THREADS = 512;
@@ -197,6 +198,31 @@ template <typename T> struct RealSmem {
     static __host__ __device__ size_t warp_stack_bytes(const PairTabs<T> &P)
     {
         return (size_t)P.cap_u * 32 * sizeof(T) + (size_t)P.capf_u * 32 * 4; /* near items, then far items */
+    }
+    /* bytes of the two tables (multiples of 128) */
+    static __host__ __device__ unsigned table_bytes(const PairTabs<T> &P)
+    {
+        return (unsigned)(PairFmt<T>::elems(P.n_bins) * sizeof(T) + far_bytes(P.n_far));
+    }
+    /* One thread: the two tables by TMA bulk copies on `bar` (announced by the caller's tma_expect).  A loop of
+     * 16-byte loads and stores over the ~100 KB took a CTA 6 us (a dozen dependent global-load latencies per
+     * thread): 6 % of a CTA's life on config 2, a third of the kernel on config 1. */
+    __device__ __forceinline__ void tma_tables(const PairTabs<T> &P, uint64_t *bar)
+    {
+        tma_copy_1d(tab, P.pair_tab, (unsigned)(PairFmt<T>::elems(P.n_bins) * sizeof(T)), bar);
+        if (P.n_far > 0) tma_copy_1d(far, P.far_tab, (unsigned)far_bytes(P.n_far), bar);
+    }
+    /* the small arrays: image list and fixed charges */
+    __device__ __forceinline__ void fill_small(const T *gimg, int nimg, const T *ion_pos, const T *ion_q, int n_ion,
+                                               int tid, int nthreads)
+    {
+        for (int t = tid; t < 3 * IMG_PARTS * nimg; t += nthreads) img[t] = gimg[t];
+        for (int t = tid; t < n_ion; t += nthreads) {
+            ion[4 * t + 0] = ion_pos[3 * t + 0];
+            ion[4 * t + 1] = ion_pos[3 * t + 1];
+            ion[4 * t + 2] = ion_pos[3 * t + 2];
+            ion[4 * t + 3] = ion_q[t];
+        }
     }
     __device__ __forceinline__ void fill(const PairTabs<T> &P, const T *gimg, int nimg, const T *ion_pos,
                                          const T *ion_q, int n_ion, int tid, int nthreads)
@@ -265,8 +291,15 @@ __device__ __forceinline__ double real_body(const RealArgs<T> &A, RealSmem<T> &S
     PairStacks<T, UQ, false> st;
     init_stacks(st, S, A.P, A.g.bias, warp, lane);
     __syncwarp();
-    const int team = A.n_tiles * blockDim.x, gid = tile * blockDim.x + tid;
     double total = 0, direct = 0;
+    /* work items are pairs, dealt round-robin to the walker's threads; with zsplit an item is (pair, z-image):
+     * ROW consecutive threads share a pair */
+    typedef ScanShape<DIM, ORTHO, M, UQ> Shape0;
+    const bool zs = Shape0::ZSPLIT && A.zsplit != 0;
+    const int all_threads = A.n_tiles * blockDim.x, my_thread = tile * blockDim.x + tid;
+    const int team = zs ? all_threads / Shape0::ROW : all_threads, gid = zs ? my_thread / Shape0::ROW : my_thread;
+    const int zsel = zs ? my_thread - gid * Shape0::ROW : -1;
+    const bool active = !zs || gid < team; /* zsplit: the last all_threads mod ROW threads have no item */
 
     /* mobile-mobile pairs */
     {
@@ -279,11 +312,11 @@ __device__ __forceinline__ double real_body(const RealArgs<T> &A, RealSmem<T> &S
         const int group = ORTHO ? GROUP : list_group;
         PairWalk pw; pw.init(gid, team, n);
         for (;;) {
-            bool valid = pw.k < H || (even && pw.k == H && pw.i < n / 2);
+            bool valid = active && (pw.k < H || (even && pw.k == H && pw.i < n / 2));
             if (!__any_sync(0xffffffffu, valid)) break;
 #pragma unroll
             for (int u = 0; u < (ORTHO ? GROUP : group); u++) {
-                if (u > 0) valid = pw.k < H || (even && pw.k == H && pw.i < n / 2);
+                if (u > 0) valid = active && (pw.k < H || (even && pw.k == H && pw.i < n / 2));
                 T d[3] = {0, 0, 0};
                 T w = UQ ? q0 * q0 : T(0);
                 if (valid) {
@@ -295,7 +328,7 @@ __device__ __forceinline__ double real_body(const RealArgs<T> &A, RealSmem<T> &S
                     if (!UQ) w = sq[i] * sq[j];
                 }
                 scan_pair<T, DIM, ORTHO, M, UQ, false, false, GROUP == 1>(A.g, d, w, valid, st, direct, S.img, A.nimg,
-                                                                          group == 1);
+                                                                          group == 1, zsel);
                 pw.next();
             }
             if (group > 1) st.service(Shape::LIMIT);
@@ -310,7 +343,7 @@ __device__ __forceinline__ double real_body(const RealArgs<T> &A, RealSmem<T> &S
         PairWalk pw; pw.init(gid, team, n);
         pw.k += k0;
         for (;;) {
-            const bool valid = pw.k < k1;
+            const bool valid = active && pw.k < k1;
             if (!__any_sync(0xffffffffu, valid)) break;
             T d[3] = {0, 0, 0};
             T w = UQ ? q0 * qion0 : T(0);
@@ -320,7 +353,7 @@ __device__ __forceinline__ double real_body(const RealArgs<T> &A, RealSmem<T> &S
                 for (int x = 0; x < DIM; x++) d[x] = sp[x * A.npad + i] - S.ion[4 * I + x];
                 if (!UQ) w = sq[i] * S.ion[4 * I + 3];
             }
-            scan_pair<T, DIM, ORTHO, M, UQ>(A.g, d, w, valid, st, direct, S.img, A.nimg);
+            scan_pair<T, DIM, ORTHO, M, UQ>(A.g, d, w, valid, st, direct, S.img, A.nimg, true, zsel);
             pw.next();
         }
         st.finish();
@@ -341,12 +374,18 @@ __global__ void __launch_bounds__(REAL_MAX_THREADS, sizeof(T) == 4 ? 2 : 1) real
     __shared__ __align__(128) double red[48];
     uint64_t *bar = reinterpret_cast<uint64_t *>(&red[32]);
     const int w = blockIdx.x / A.n_tiles, tile = blockIdx.x - w * A.n_tiles, tid = threadIdx.x;
-    /* the walker's SoA block [DIM][npad] is contiguous: one TMA bulk copy stages it while the threads copy the tables */
+    /* the walker's SoA block [DIM][npad] is contiguous: TMA bulk copies stage it and the two tables while the
+     * threads copy the small arrays */
     if (tid == 0) tma_barrier_init(bar);
     __syncthreads();
-    if (tid == 0) tma_load_1d(sp, A.pos + (size_t)w * DIM * A.npad, (unsigned)(DIM * A.npad * sizeof(T)), bar);
+    if (tid == 0) {
+        const unsigned pos_bytes = (unsigned)(DIM * A.npad * sizeof(T));
+        tma_expect(bar, pos_bytes + RealSmem<T>::table_bytes(A.P));
+        tma_copy_1d(sp, A.pos + (size_t)w * DIM * A.npad, pos_bytes, bar);
+        S.tma_tables(A.P, bar);
+    }
     for (int t = tid; t < A.n; t += blockDim.x) sq[t] = A.q[t];
-    S.fill(A.P, A.img, A.nimg, A.ion_pos, A.ion_q, A.n_ion, tid, blockDim.x);
+    S.fill_small(A.img, A.nimg, A.ion_pos, A.ion_q, A.n_ion, tid, blockDim.x);
     tma_wait(bar, 0);
     __syncthreads();
 

@@ -59,6 +59,21 @@ __device__ __forceinline__ void tma_load_1d(void *dst_smem, const void *src_gmem
     asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
                  ::"r"(smem_u32(dst_smem)), "l"(src_gmem), "r"(bytes), "r"(smem_u32(bar)) : "memory");
 }
+/* Several bulk copies on one barrier: the issuing thread announces the total once, then starts the copies
+ * (each a multiple of 16 bytes, 16-byte aligned on both sides; long ones are cut into pieces of at most 32 KB). */
+__device__ __forceinline__ void tma_expect(uint64_t *bar, unsigned total_bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(total_bytes) : "memory");
+}
+__device__ __forceinline__ void tma_copy_1d(void *dst_smem, const void *src_gmem, unsigned bytes, uint64_t *bar)
+{
+    constexpr unsigned PIECE = 32 * 1024;
+    for (unsigned o = 0; o < bytes; o += PIECE) {
+        const unsigned b = bytes - o < PIECE ? bytes - o : PIECE;
+        asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                     ::"r"(smem_u32(dst_smem) + o), "l"((const char *)src_gmem + o), "r"(b), "r"(smem_u32(bar)) : "memory");
+    }
+}
 __device__ __forceinline__ void tma_wait(uint64_t *bar, unsigned parity)
 {
     unsigned done;

@@ -380,6 +380,9 @@ template <int DIM, bool ORTHO, int M, bool UQ> struct ScanShape {
     static constexpr int LIMIT = ORTHO ? (WHOLE ? ALL * GROUP : PLANE ? 12 : ROW) : (UQ ? IMG_STEP : IMG_STEP / 2);
     static constexpr int MIN_CAP = LIMIT + PAIR_R;
     static constexpr int FAR_LIMIT = 20; /* PLANE, fast variant: all 20 candidates between two far services */
+    /* small batches of small boxes (|m| <= 2 in 3D: 125 candidates per pair): the energy kernel can deal the ROW
+     * z-images of a pair to ROW different lanes, so that few walkers still fill the GPU (RealArgs::zsplit) */
+    static constexpr bool ZSPLIT = ORTHO && !WHOLE && !PLANE && DIM == 3 && M == 2;
 };
 
 /* Phase A for one pair per lane.  d = r_i - r_j (raw, neither scaled nor reduced); w = q_i q_j.  Terms below the
@@ -388,8 +391,10 @@ template <typename T, int DIM, bool ORTHO, int M, bool UQ, bool SIGNED = false, 
           bool SERVICE = true>
 __device__ __forceinline__ void scan_pair(const RealGeom<T> &g, T *d, T w, bool valid,
                                           PairStacks<T, UQ, SIGNED> &st, double &direct, const T *simg, int nimg,
-                                          bool list_service = true)
+                                          bool list_service = true, int zsel = -1)
 {
+    /* zsel >= 0 (uniform over the grid; ScanShape::ZSPLIT shapes only): this lane scans the z-image zsel of its
+     * pair alone, ROW lanes share the pair */
     /* list_service = false (image-list path, few images): the caller services the stacks after several pairs.
      * NEG (move kernel, old position): the term enters with a minus sign -- in w for (t, w) items (the
      * caller passes -w), in the sign bit of t for bare-t items */
@@ -460,7 +465,7 @@ __device__ __forceinline__ void scan_pair(const RealGeom<T> &g, T *d, T w, bool 
         T t0 = sq[0][M] + sq[1][M];
         if (DIM == 3) t0 += sq[2][M];
         const bool tiny = valid && order_key(t0) < g.key_min;
-        if (tiny) direct += (double)((FLIP ? -w : w) * pair_f_direct(t0));
+        if (tiny && (!Shape::ZSPLIT || zsel < 0 || zsel == M)) direct += (double)((FLIP ? -w : w) * pair_f_direct(t0));
         const bool central_ok = valid && !tiny;
         if (Shape::WHOLE) {
 #pragma unroll
@@ -480,8 +485,11 @@ __device__ __forceinline__ void scan_pair(const RealGeom<T> &g, T *d, T w, bool 
             if (SERVICE) st.service(Shape::LIMIT); /* else the caller does, after Shape::GROUP pairs */
         } else {
             /* rolled loops over the y and z images (the stacks are serviced after every x-row) */
+            const bool zs = Shape::ZSPLIT && zsel >= 0;
+            const int z_trips = zs ? 1 : (DIM == 3 ? ROW : 1);
 #pragma unroll 1
-            for (int mz = 0; mz < (DIM == 3 ? ROW : 1); mz++) {
+            for (int zi = 0; zi < z_trips; zi++) {
+                const int mz = zs ? zsel : zi;
                 T sz = 0;
                 if (DIM == 3) sz = axis_square(g, 2, fma((T)(M - mz), axis_unit(g, 2), d[2]));
 #pragma unroll 1
