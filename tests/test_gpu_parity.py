@@ -260,6 +260,34 @@ def test_orthorhombic_noncubic_cells_all_image_ranges(torch_cuda, dim):
         assert (np.abs(c32 - c_ref32) / np.abs(c_ref32).max(axis=1)[:, None]).max() <= TOL32, (kappa, rc)
 
 
+@pytest.mark.parametrize("with_ions", [False, True])
+def test_small_batch_z_split_agrees_with_large_batch(torch_cuda, with_ions):
+    """Boxes that need |m| <= 2 images per axis in 3D (config 1: r_c = 2.2 L, 125 candidates per pair): a batch too
+    small to fill the SMs deals the five z-images of a pair to five lanes (ScanShape::ZSPLIT, chosen by the launch),
+    a large batch does not.  Both must give the oracle's energies, and the same walker the same energy (up to the
+    order of the tile sums) in either batch; ewald_launch_shape shows that the two launches differed."""
+    torch = torch_cuda
+    w = workloads.config(1)
+    rng = np.random.default_rng(11)
+    ions = (rng.random((5, 3)) * w.L, np.array([2.0, 2.0, 3.0, 3.0, 2.0])) if with_ions else (None, None)
+    ctx = E.ewald_setup(w.dim, w.cell, w.kappa, w.g_cutoff, w.r_cutoff)
+    if with_ions:
+        E.ewald_set_fixed_charges(ctx, *ions)
+    pos = w.positions(400)
+    e_small, c_small = _gpu_energy(torch, ctx, pos[:6], w.charges, "f64")
+    shape_small = E.ewald_launch_shape(ctx, 0)
+    e_big, c_big = _gpu_energy(torch, ctx, pos, w.charges, "f64")
+    shape_big = E.ewald_launch_shape(ctx, 0)
+    assert shape_small["threads"] == shape_big["threads"] == 512
+    assert shape_small["ctas"] > 6 * 3            # more tiles per walker than the pairs alone would give
+    assert shape_big["ctas"] == 400 * 2           # (4 x 148 + 399) / 400 tiles per walker
+    e_ref, c_ref = ref.energy_batch(w.dim, w.cell, w.kappa, w.g_cutoff, w.r_cutoff, pos[:6], w.charges, *ions)
+    _assert_energy(e_small, c_small, e_ref, c_ref, TOL64)
+    _assert_energy(e_big[:6], c_big[:6], e_ref, c_ref, TOL64)
+    assert (np.abs(e_small - e_big[:6]) / np.abs(e_ref)).max() <= 1e-13
+
+
+
 def test_uniform_charges_cutoff_reaching_two_far_images(torch_cuda):
     """Equal charges (bare-t stacks, candidate images enumerated as core / one far image / two or more far
     images) in cubic and orthorhombic cells whose cut-off r_c = 1.46 L_min exceeds sqrt(2) L_min: the branch
