@@ -144,10 +144,13 @@ def run_reference(args, rank):
         "gpu_launches": 0}))
 
 
+FAR_T0 = 13.0  # start of the FP32 far shell of the FP64 energy kernel
+
+
 def count_pair_terms(w, pos):
     """Pairs and pair-image terms (|r_ij - R| < r_c) per walker of an orthorhombic workload, counted with
     numpy on a few walkers: the unit count of the real-space kernel's roofline.
-    Returns pairs, terms, terms of the far shell (kappa^2 r^2 >= 16, evaluated in FP32 by the FP64 kernel),
+    Returns pairs, terms, terms of the far shell (kappa^2 r^2 >= 13, evaluated in FP32 by the FP64 energy kernel),
     images per axis."""
     sides = np.diag(w.cell)[:w.dim]
     m = int(math.floor(w.r_cutoff / sides.min() + 0.5 - 1e-12))
@@ -161,7 +164,7 @@ def count_pair_terms(w, pos):
             d -= np.rint(d / sides) * sides
             r2 = ((d[:, :, None, :] - shifts[None, None, :, :]) ** 2).sum(-1)
             inside = r2 < w.r_cutoff ** 2
-            outer = inside & (r2 * w.kappa ** 2 >= 16.0)
+            outer = inside & (r2 * w.kappa ** 2 >= FAR_T0)
             if k == 0:
                 iu = np.triu_indices(len(p), 1)
                 cnt += int(inside[iu].sum()); cnt_far += int(outer[iu].sum())
@@ -177,7 +180,7 @@ def real_space_work(w, pos, n_images):
     """Algorithmic work of the real-space kernel per walker: pairs, pair-image terms, and a
     flop count in FP64 equivalents -- per pair 12 (displacement and reduction to the cell) + 5 per axis image
     square + 2 per enumerated candidate (20 in 3D with one image per side, else (2M+1)^dim); per near term
-    (kappa^2 r^2 < 16) 12 FP64 flops (u, quintic Horner, accumulate); per far term 8 FP32 flops = 4 FP64
+    (kappa^2 r^2 < 13) 12 FP64 flops (u, degree-7 polynomial, accumulate); per far term 8 FP32 flops = 4 FP64
     equivalents (the FP64 kernel evaluates the far shell by an FP32 cubic; FP32 peak = 2 x FP64 peak)."""
     n_ion = 0 if w.ion_q is None else len(w.ion_q)
     if np.count_nonzero(w.cell - np.diag(np.diag(w.cell))) == 0:

@@ -1146,10 +1146,7 @@ static ewald_status move_batch_t(ewald_ctx *c, int n_moves, const int *walker, c
     A.rowlen = c->rowlen;
     A.img = Tabs<T>::img(c); A.nimg = c->nimg;
     A.ion_pos = Tabs<T>::ion_pos(c); A.ion_q = Tabs<T>::ion_q(c); A.n_ion = c->t.n_ion;
-#ifndef EWALD_MOVE_FAR_T0
-#define EWALD_MOVE_FAR_T0 16
-#endif
-    A.P.far_t0 = EWALD_MOVE_FAR_T0; /* measured: 13.4 M moves/s with the far shell from t = 16, 10.5 M from t = 13 (config 5, FP64) */
+    A.P.far_t0 = 16; /* the move kernel's far shell starts later than the energy kernels' */
     fill_pair_tabs<T>(c, (const double *)c->st_qinfo.p, &A.P);
     A.n_moves = n_moves;
     A.walker = walker; A.electron = electron; A.new_r = new_r; A.commit = commit; A.delta_e = delta_e;

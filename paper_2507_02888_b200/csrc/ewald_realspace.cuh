@@ -259,7 +259,7 @@ template <typename K, typename W, bool UQ, typename Derived> struct StackBase {
     }
 };
 
-/* Near stack: t in the kernel's precision, F from the quintic (FP32: cubic) table. */
+/* Near stack: t in the kernel's precision, F from the degree-7 (FP32: cubic) table. */
 template <typename T, bool UQ, bool SIGNED = false>
 struct LaneStack : StackBase<T, T, UQ, LaneStack<T, UQ, SIGNED>> {
     typedef T Acc;
