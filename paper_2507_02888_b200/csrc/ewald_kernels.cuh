@@ -186,13 +186,17 @@ template <typename T> struct RealSmem {
         img = reinterpret_cast<T *>(reinterpret_cast<unsigned char *>(far) + far_bytes(P.n_far));
         ion = img + up4(3 * IMG_PARTS * (size_t)nimg);
         rest = ion + up4(4 * (size_t)n_ion);
-        stacks = reinterpret_cast<unsigned char *>(rest + up4(rest_elems));
+        /* the lane stacks' rows are 128 or 256 bytes: they start on a 128-byte boundary of the window (the kernels
+         * keep their static shared memory a multiple of 128 bytes), else every push and pop touches two lines */
+        const size_t off = reinterpret_cast<unsigned char *>(rest + up4(rest_elems)) - raw;
+        stacks = raw + ((off + 127) & ~(size_t)127);
     }
     /* bytes before the stacks */
     static size_t fixed_bytes(int n_bins, int n_far, int nimg, int n_ion, size_t rest_elems)
     {
-        return (up4(PairFmt<T>::elems(n_bins)) + up4(3 * IMG_PARTS * (size_t)nimg) + up4(4 * (size_t)n_ion) +
-                up4(rest_elems)) * sizeof(T) + far_bytes(n_far);
+        const size_t b = (up4(PairFmt<T>::elems(n_bins)) + up4(3 * IMG_PARTS * (size_t)nimg) + up4(4 * (size_t)n_ion) +
+                          up4(rest_elems)) * sizeof(T) + far_bytes(n_far);
+        return (b + 127) & ~(size_t)127;
     }
     /* bytes of one warp's stacks (the two item kinds of a stack share the same bytes) */
     static __host__ __device__ size_t warp_stack_bytes(const PairTabs<T> &P)
