@@ -19,8 +19,10 @@ HEADERS = [os.path.join(ROOT, "include", "ewald.h"), os.path.join(ROOT, "include
            os.path.join(CSRC, "ewald_kernels_common.cuh"), os.path.join(CSRC, "ewald_realspace.cuh"),
            os.path.join(CSRC, "ewald_recip_oct.cuh")]
 
+# --split-compile is pinned: with =0 (one piece per host core) the register allocation of the big kernels, and with
+# it 4-13 % of their speed, depended on the core count of the machine that built the library
 NVCC_FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
-              "-Xcompiler", "-fPIC", "-shared", "-cudart", "static", "--split-compile=0"]
+              "-Xcompiler", "-fPIC", "-shared", "-cudart", "static", "--split-compile=1"]
 
 
 def _nvcc():
