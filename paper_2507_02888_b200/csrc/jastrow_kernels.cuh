@@ -81,9 +81,13 @@ template <typename T2> __device__ __forceinline__ T2 jas_pick(const T2 *row, int
     return e;
 }
 
-/* u(r), u'(r)/r and u''(r) of Eq. 6 for r < L_u, Horner in (poly, poly', poly'') */
+__device__ __forceinline__ double jas_rsqrt(double x) { return rsqrt(x); }
+__device__ __forceinline__ float jas_rsqrt(float x) { return rsqrtf(x); }
+
+/* u(r), u'(r)/r and u''(r) of Eq. 6 for r < L_u, Horner in (poly, poly', poly''); inv_r = 1/r from the caller's
+ * reciprocal square root (no division, no square root here; 0 where u'/r is not wanted or r = 0) */
 template <typename T>
-__device__ __forceinline__ void jas_u(const JasTabs &t, T r, T *u, T *du_over_r, T *d2u)
+__device__ __forceinline__ void jas_u(const JasTabs &t, T r, T inv_r, T *u, T *du_over_r, T *d2u)
 {
     T p = 0, dp = 0, d2p = 0;
     for (int l = t.n_u; l >= 0; l--) {
@@ -100,7 +104,7 @@ __device__ __forceinline__ void jas_u(const JasTabs &t, T r, T *u, T *du_over_r,
     const T d1 = t.c_exp >= 1 ? c * sc1 : T(0), d2 = t.c_exp >= 2 ? c * (c - 1) * sc2 : T(0);
     *u = p * sc;
     const T du = dp * sc + p * d1;
-    *du_over_r = du / r;
+    *du_over_r = du * inv_r;
     *d2u = d2p * sc + 2 * dp * d1 + p * d2;
 }
 
@@ -108,6 +112,11 @@ __device__ __forceinline__ void jas_u(const JasTabs &t, T r, T *u, T *du_over_r,
 template <typename T, int DIM>
 __device__ __forceinline__ void jas_min_image(const JasTabs &t, T (&d)[3])
 {
+    if (t.ortho) { /* diagonal cell: one rounding and one FMA per axis */
+#pragma unroll
+        for (int x = 0; x < DIM; x++) d[x] -= (T)t.a[4 * x] * Num<T>::rint_(d[x] * (T)t.binv[4 * x]);
+        return;
+    }
     T f[3] = {0, 0, 0};
 #pragma unroll
     for (int k = 0; k < DIM; k++) {
@@ -238,9 +247,10 @@ __global__ void __launch_bounds__(JAS_THREADS) jastrow_kernel(JasArgs<T> A)
                 jas_min_image<T, DIM>(t, d);
                 const T r2 = d[0] * d[0] + d[1] * d[1] + d[2] * d[2];
                 if (j != i && r2 < lu2) {
-                    const T r = sqrt(r2);
+                    /* coincident particles (r = 0): u(0) counts, the gradient term does not (as in the oracle) */
+                    const T inv_r = r2 > 0 ? jas_rsqrt(r2) : T(0), r = r2 * inv_r;
                     T u, dur, d2u;
-                    jas_u<T>(t, r, &u, &dur, &d2u);
+                    jas_u<T>(t, r, inv_r, &u, &dur, &d2u);
                     uv += u;
 #pragma unroll
                     for (int x = 0; x < DIM; x++) ug[x] += dur * d[x];
@@ -334,7 +344,7 @@ __global__ void __launch_bounds__(JAS_MOVE_THREADS) jastrow_move_kernel(JasMoveA
                 const T r2 = d[0] * d[0] + d[1] * d[1] + d[2] * d[2];
                 if (r2 < lu2) {
                     T u, dur, d2u;
-                    jas_u<T>(t, sqrt(r2), &u, &dur, &d2u);
+                    jas_u<T>(t, sqrt(r2), T(0), &u, &dur, &d2u);
                     part += which ? u : -u;
                 }
             }
