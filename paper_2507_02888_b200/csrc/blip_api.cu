@@ -46,11 +46,17 @@ template <typename T>
 __global__ void __launch_bounds__(BLIP_THREADS) blip_kernel(BlipArgs<T> A)
 {
     const int lane = threadIdx.x & 31, warps = (gridDim.x * blockDim.x) >> 5;
+    /* The 36 one-dimensional blip values of a position (Theta, Theta', Theta'' x 3 axes x 4 neighbours) are the same
+     * for the whole warp and are indexed by the loop counters below: as per-thread arrays they sat in LOCAL memory
+     * (288 bytes per thread, more than L1 holds for 2048 threads), whose traffic competed in L2 with the
+     * coefficient gather (FP64: 2.5 to 5.7 ms per launch depending on how ptxas scheduled the reloads).  Lane k < 3
+     * computes axis k; the warp reads them from shared memory (one broadcast wavefront per read). */
+    __shared__ T s1d[BLIP_THREADS / 32][3][3][4]; /* [warp][f, d1, d2][axis][neighbour] */
+    T (*f)[4] = s1d[threadIdx.x >> 5][0], (*d1)[4] = s1d[threadIdx.x >> 5][1], (*d2)[4] = s1d[threadIdx.x >> 5][2];
     for (int p = (blockIdx.x * blockDim.x + threadIdx.x) >> 5; p < A.n_points; p += warps) {
-        T f[3][4], d1[3][4], d2[3][4];
         int i0[3];
-#pragma unroll
-        for (int k = 0; k < 3; k++) {
+        {
+            const int k = lane < 3 ? lane : 0;
             double s = 0;
 #pragma unroll
             for (int x = 0; x < 3; x++) s += (double)A.points[x * A.n_pad + p] * A.binv[3 * k + x];
@@ -58,34 +64,60 @@ __global__ void __launch_bounds__(BLIP_THREADS) blip_kernel(BlipArgs<T> A)
             const double u = s * A.grid[k];
             int i = (int)floor(u);
             if (i >= A.grid[k]) i = A.grid[k] - 1; /* s rounded up to 1 */
-            i0[k] = i;
-            blip_1d<T>((T)(u - i), f[k], d1[k], d2[k]);
+            T tf[4], td1[4], td2[4];
+            blip_1d<T>((T)(u - i), tf, td1, td2);
+            __syncwarp(); /* the previous position's reads are done */
+            if (lane < 3) {
+#pragma unroll
+                for (int a = 0; a < 4; a++) { f[k][a] = tf[a]; d1[k][a] = td1[a]; d2[k][a] = td2[a]; }
+            }
+#pragma unroll
+            for (int kk = 0; kk < 3; kk++) i0[kk] = __shfl_sync(0xffffffffu, i, kk);
+            __syncwarp();
         }
+        /* FP32: the values of axis 2 (indexed by the unrolled innermost loop) and those of the current a and b are
+         * kept in registers (1.74 -> 1.35 ms); FP64 reads all of them from shared memory where they are used (in
+         * registers the kernel needs 178 of them: 1.90 -> 3.34 ms, or 2.53 ms bounded to 128 with spills) */
+        constexpr bool HOIST = sizeof(T) == 4;
+        T f2[4], d12[4], d22[4];
+#pragma unroll
+        for (int c = 0; c < 4; c++) { f2[c] = HOIST ? f[2][c] : T(0); d12[c] = HOIST ? d1[2][c] : T(0); d22[c] = HOIST ? d2[2][c] : T(0); }
+#define F2(c) (HOIST ? f2[c] : f[2][c])
+#define D12(c) (HOIST ? d12[c] : d1[2][c])
+#define D22(c) (HOIST ? d22[c] : d2[2][c])
         for (int ob = 0; ob < A.n_orb; ob += 32 * BLIP_OPL) {
             T v[BLIP_OPL], gx[BLIP_OPL], gy[BLIP_OPL], gz[BLIP_OPL], lp[BLIP_OPL];
 #pragma unroll
             for (int q = 0; q < BLIP_OPL; q++) v[q] = gx[q] = gy[q] = gz[q] = lp[q] = 0;
             for (int a = 0; a < 4; a++) {
                 int ia = i0[0] + a - 1; ia += ia < 0 ? A.grid[0] : 0; ia -= ia >= A.grid[0] ? A.grid[0] : 0;
+                const T f0a = HOIST ? f[0][a] : T(0), d10a = HOIST ? d1[0][a] : T(0), d20a = HOIST ? d2[0][a] : T(0);
                 for (int b = 0; b < 4; b++) {
                     int ib = i0[1] + b - 1; ib += ib < 0 ? A.grid[1] : 0; ib -= ib >= A.grid[1] ? A.grid[1] : 0;
-                    const T f01 = f[0][a] * f[1][b], g0 = d1[0][a] * f[1][b], g1 = f[0][a] * d1[1][b];
-                    const T h00 = d2[0][a] * f[1][b], h11 = f[0][a] * d2[1][b], h01 = d1[0][a] * d1[1][b];
+                    T f01, g0, g1, h00, h11, h01;
+                    if (HOIST) {
+                        const T f1b = f[1][b], d11b = d1[1][b], d21b = d2[1][b];
+                        f01 = f0a * f1b; g0 = d10a * f1b; g1 = f0a * d11b;
+                        h00 = d20a * f1b; h11 = f0a * d21b; h01 = d10a * d11b;
+                    } else {
+                        f01 = f[0][a] * f[1][b]; g0 = d1[0][a] * f[1][b]; g1 = f[0][a] * d1[1][b];
+                        h00 = d2[0][a] * f[1][b]; h11 = f[0][a] * d2[1][b]; h01 = d1[0][a] * d1[1][b];
+                    }
 #pragma unroll
                     for (int c = 0; c < 4; c++) {
                         int ic = i0[2] + c - 1; ic += ic < 0 ? A.grid[2] : 0; ic -= ic >= A.grid[2] ? A.grid[2] : 0;
-                        const T w = f01 * f[2][c];
-                        const T u0 = g0 * f[2][c], u1 = g1 * f[2][c], u2 = f01 * d1[2][c]; /* fractional gradient */
+                        const T w = f01 * F2(c);
+                        const T u0 = g0 * F2(c), u1 = g1 * F2(c), u2 = f01 * D12(c); /* fractional gradient */
                         const T wx = u0 * (T)A.gm[0] + u1 * (T)A.gm[3] + u2 * (T)A.gm[6];
                         const T wy = u0 * (T)A.gm[1] + u1 * (T)A.gm[4] + u2 * (T)A.gm[7];
                         const T wz = u0 * (T)A.gm[2] + u1 * (T)A.gm[5] + u2 * (T)A.gm[8];
-                        const T wl = (T)A.metric[0] * h00 * f[2][c] + (T)A.metric[1] * h11 * f[2][c] + (T)A.metric[2] * f01 * d2[2][c] +
-                                     2 * ((T)A.metric[3] * h01 * f[2][c] + (T)A.metric[4] * g0 * d1[2][c] + (T)A.metric[5] * g1 * d1[2][c]);
+                        const T wl = (T)A.metric[0] * h00 * F2(c) + (T)A.metric[1] * h11 * F2(c) + (T)A.metric[2] * f01 * D22(c) +
+                                     2 * ((T)A.metric[3] * h01 * F2(c) + (T)A.metric[4] * g0 * D12(c) + (T)A.metric[5] * g1 * D12(c));
                         const T *cp = A.coef + ((size_t)(ia * A.grid[1] + ib) * A.grid[2] + ic) * A.no_pad + ob + lane;
 #pragma unroll
                         for (int q = 0; q < BLIP_OPL; q++) {
                             if (ob + 32 * q < A.no_pad) { /* uniform */
-                                const T cc = cp[32 * q];
+                                const T cc = __ldg(cp + 32 * q);
                                 v[q] += cc * w; gx[q] += cc * wx; gy[q] += cc * wy; gz[q] += cc * wz; lp[q] += cc * wl;
                             }
                         }
@@ -96,18 +128,24 @@ __global__ void __launch_bounds__(BLIP_THREADS) blip_kernel(BlipArgs<T> A)
             for (int q = 0; q < BLIP_OPL; q++) {
                 const int o = ob + 32 * q + lane;
                 if (o < A.n_orb) {
-                    A.psi[(size_t)p * A.n_orb + o] = v[q];
+                    /* streaming stores: the 1.3 GB of outputs of a launch must not push the coefficient table
+                     * (14 MB, re-read 64 times per position) out of L2 */
+                    __stcs(A.psi + (size_t)p * A.n_orb + o, (double)v[q]);
                     if (A.grad) {
-                        A.grad[((size_t)p * 3 + 0) * A.n_orb + o] = gx[q];
-                        A.grad[((size_t)p * 3 + 1) * A.n_orb + o] = gy[q];
-                        A.grad[((size_t)p * 3 + 2) * A.n_orb + o] = gz[q];
+                        __stcs(A.grad + ((size_t)p * 3 + 0) * A.n_orb + o, (double)gx[q]);
+                        __stcs(A.grad + ((size_t)p * 3 + 1) * A.n_orb + o, (double)gy[q]);
+                        __stcs(A.grad + ((size_t)p * 3 + 2) * A.n_orb + o, (double)gz[q]);
                     }
-                    if (A.lap) A.lap[(size_t)p * A.n_orb + o] = lp[q];
+                    if (A.lap) __stcs(A.lap + (size_t)p * A.n_orb + o, (double)lp[q]);
                 }
             }
         }
     }
 }
+
+#undef F2
+#undef D12
+#undef D22
 
 struct blip_ctx {
     int device = 0;
