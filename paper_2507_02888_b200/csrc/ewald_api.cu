@@ -800,7 +800,7 @@ template <typename T> static void set_outer_far(const ewald_ctx *c, const PairTa
     g->outer_far = 1;
     /* ... and if the far stack holds all 20 candidates of a pair plus a round, it is serviced once per pair
      * (call after real_shape has fixed the capacities) */
-    g->far_once = !g->multi_far && P.capf_u >= 20 + PAIR_R;
+    g->far_once = !g->multi_far && P.capf_u >= 20 + P.round_items;
 }
 
 /* The orthorhombic image scan needs boxes that reach the cut-off within +-2 images and that are wide enough
@@ -857,7 +857,7 @@ template <> void fill_pair_tabs<double>(const ewald_ctx *c, const double *qinfo,
 
 /* CTA size and per-lane stack capacities that fit the shared memory left after `fixed` bytes of tables.
  * The two item kinds of a stack (bare t / (t, qq)) share the same bytes, so the (t, qq) capacity is half.
- * min_cap = ScanShape::MIN_CAP of the kernel variant. */
+ * min_cap = ScanShape::min_cap(P->round_items) of the kernel variant. */
 template <typename T>
 static bool real_shape(const ewald_ctx *c, size_t fixed, int min_cap_u, int min_cap_g, int max_threads,
                        PairTabs<T> *P, int *threads, size_t *smem, bool allow_two = true)
@@ -883,7 +883,7 @@ static bool real_shape(const ewald_ctx *c, size_t fixed, int min_cap_u, int min_
             } else {
                 /* the far stack receives twice the terms: first choice twice the near capacity (the same bytes);
                  * if that does not fit, the near stack at its minimum and the rest to the far stack, which at
-                 * 20 + PAIR_R items is serviced once per pair (set_outer_far); else equal capacities */
+                 * 20 + round_items items is serviced once per pair (set_outer_far); else equal capacities */
                 cu = lane_bytes / (long long)(sizeof(T) + 8);
                 if (cu > want) cu = want;
                 cu &= ~1LL;
@@ -892,7 +892,7 @@ static bool real_shape(const ewald_ctx *c, size_t fixed, int min_cap_u, int min_
                     cu = need + (need & 1);
                     cf = ((lane_bytes - cu * (long long)sizeof(T)) / 4) & ~1LL;
                     if (cf > 2 * cu) cf = 2 * cu;
-                    if (cf < 20 + PAIR_R) {
+                    if (cf < 20 + P->round_items) {
                         cu = (lane_bytes / (long long)(sizeof(T) + 4)) & ~1LL;
                         if (cu > want) cu = want;
                         cf = cu;
@@ -912,17 +912,17 @@ static bool real_shape(const ewald_ctx *c, size_t fixed, int min_cap_u, int min_
     return false;
 }
 
-template <int DIM, bool ORTHO, int M> static int scan_min_cap(bool uq)
+template <int DIM, bool ORTHO, int M> static int scan_min_cap(bool uq, int r)
 {
-    return uq ? ScanShape<DIM, ORTHO, M, true>::MIN_CAP : ScanShape<DIM, ORTHO, M, false>::MIN_CAP;
+    return uq ? ScanShape<DIM, ORTHO, M, true>::min_cap(r) : ScanShape<DIM, ORTHO, M, false>::min_cap(r);
 }
-static int real_min_cap(const ewald_ctx *c, bool ortho, bool uq)
+static int real_min_cap(const ewald_ctx *c, bool ortho, bool uq, int r)
 {
     const int m = c->t.m_shift;
-    if (c->t.dim == 3) return !ortho ? scan_min_cap<3, false, 0>(uq) : m == 0 ? scan_min_cap<3, true, 0>(uq)
-                            : m == 1 ? scan_min_cap<3, true, 1>(uq) : scan_min_cap<3, true, 2>(uq);
-    return !ortho ? scan_min_cap<2, false, 0>(uq) : m == 0 ? scan_min_cap<2, true, 0>(uq)
-         : m == 1 ? scan_min_cap<2, true, 1>(uq) : scan_min_cap<2, true, 2>(uq);
+    if (c->t.dim == 3) return !ortho ? scan_min_cap<3, false, 0>(uq, r) : m == 0 ? scan_min_cap<3, true, 0>(uq, r)
+                            : m == 1 ? scan_min_cap<3, true, 1>(uq, r) : scan_min_cap<3, true, 2>(uq, r);
+    return !ortho ? scan_min_cap<2, false, 0>(uq, r) : m == 0 ? scan_min_cap<2, true, 0>(uq, r)
+         : m == 1 ? scan_min_cap<2, true, 1>(uq, r) : scan_min_cap<2, true, 2>(uq, r);
 }
 
 template <typename T>
@@ -934,13 +934,14 @@ static ewald_status launch_real(ewald_ctx *c, int W, int n, const T *pos, const 
     A.img = Tabs<T>::img(c); A.nimg = c->nimg;
     A.ion_pos = Tabs<T>::ion_pos(c); A.ion_q = Tabs<T>::ion_q(c); A.n_ion = c->t.n_ion;
     A.P.far_t0 = FAR_T0;
+    A.P.round_items = RoundSize<T, false>::R;
     fill_pair_tabs<T>(c, nullptr, &A.P); /* the kernel finds the all-equal flag of the charges itself */
     fill_geom(c->t, &A.g);
     const bool ortho = real_ortho(c);
     if (ortho) A.nimg = 0; /* the orthorhombic path does not read the image list */
     const size_t fixed = RealSmem<T>::fixed_bytes(A.P.n_bins, A.P.n_far, A.nimg, A.n_ion, (size_t)c->t.dim * ewald_padded_n(n) + n);
     int threads = 0; size_t smem = 0;
-    if (!real_shape<T>(c, fixed, real_min_cap(c, ortho, true), real_min_cap(c, ortho, false), REAL_MAX_THREADS, &A.P,
+    if (!real_shape<T>(c, fixed, real_min_cap(c, ortho, true, A.P.round_items), real_min_cap(c, ortho, false, A.P.round_items), REAL_MAX_THREADS, &A.P,
                        &threads, &smem))
         return fail(c, EWALD_ERANGE, "real-space kernel: problem too large for shared memory");
     set_outer_far(c, A.P, &A.g);
@@ -1146,6 +1147,7 @@ static ewald_status move_batch_t(ewald_ctx *c, int n_moves, const int *walker, c
     A.rowlen = c->rowlen;
     A.img = Tabs<T>::img(c); A.nimg = c->nimg;
     A.ion_pos = Tabs<T>::ion_pos(c); A.ion_q = Tabs<T>::ion_q(c); A.n_ion = c->t.n_ion;
+    A.P.round_items = RoundSize<T, true>::R;
     A.P.far_t0 = 16; /* the move kernel's far shell starts later than the energy kernels' */
     fill_pair_tabs<T>(c, (const double *)c->st_qinfo.p, &A.P);
     A.n_moves = n_moves;
@@ -1160,7 +1162,7 @@ static ewald_status move_batch_t(ewald_ctx *c, int n_moves, const int *walker, c
     for (int th = MOVE_MAX_THREADS; th >= 32 && !fits; th /= 2) {
         const size_t fixed = RealSmem<T>::fixed_bytes(A.P.n_bins, A.P.n_far, A.nimg, A.n_ion,
                                                       4 * (size_t)c->rowlen * (th / 32));
-        fits = real_shape<T>(c, fixed, real_min_cap(c, ortho, true), real_min_cap(c, ortho, false), th, &A.P, &threads,
+        fits = real_shape<T>(c, fixed, real_min_cap(c, ortho, true, A.P.round_items), real_min_cap(c, ortho, false, A.P.round_items), th, &A.P, &threads,
                              &smem) && threads == th;
     }
     if (!fits) return fail(c, EWALD_ERANGE, "move kernel: tables too large for shared memory");

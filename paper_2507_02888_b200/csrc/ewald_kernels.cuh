@@ -141,6 +141,7 @@ template <typename T> struct PairTabs {
     int n_species, sp_start[5];      /* ions [sp_start[s], sp_start[s+1]) carry one charge each         */
     int cap_u, cap_g;                /* near-stack capacity per lane: bare t items / (t, qq) items      */
     int capf_u, capf_g;              /* far-stack capacity per lane                                     */
+    int round_items;                 /* host only: RoundSize<T, SIGNED>::R of the kernel these shapes are for */
 };
 
 /* [S6] what the combine needs (folded into the last CTA of a walker in real_kernel) */

@@ -206,11 +206,16 @@ template <typename K, typename W> struct StackItem<K, W, false> {
     __device__ __forceinline__ static void load(unsigned a, K &t, W &w) { ld_s(a, t, w); }
 };
 
-constexpr int PAIR_R = 4; /* items per lane per evaluation round (independent FMA chains) */
+/* Items per lane per evaluation round (independent FMA chains), chosen per kernel (measured in one call, config 2 /
+ * 3 / 4 real space in ms with 4, 5, 6 items: 0.626 / 0.490 / 3.40; 0.617 / 0.450 / 3.40; 0.613 / 0.449 / 3.38): the
+ * FP64 energy kernel takes 5 (with 6 config 1's stacks do not fit 512 threads), the FP32 energy kernel and the move
+ * kernels 4 (FP32 energy 0.366 -> 0.370 ms with 5; moves 15.6 -> 15.4 M / 26.9 -> 22.1 M).  The capacities are sized
+ * for the kernel's own value (ScanShape::min_cap, PairTabs::round_items). */
+template <typename T, bool SIGNED> struct RoundSize { static constexpr int R = !SIGNED && sizeof(T) == 8 ? 5 : 4; };
 
 /* Per-lane stack in shared memory, layout [slot][lane] per warp, kept as byte addresses; all control flow
  * that touches it is warp-uniform, the contents are lane-private.  Derived classes supply term(). */
-template <typename K, typename W, bool UQ, typename Derived> struct StackBase {
+template <typename K, typename W, bool UQ, int R, typename Derived> struct StackBase {
     typedef StackItem<K, W, UQ> Item;
     static constexpr int SLOT = 32 * Item::BYTES;  /* bytes between two slots of a lane */
     unsigned base_a;  /* this lane's slot 0 */
@@ -233,7 +238,7 @@ template <typename K, typename W, bool UQ, typename Derived> struct StackBase {
     {
         typename Derived::Acc part = 0;
 #pragma unroll
-        for (int r = 0; r < PAIR_R; r++) {
+        for (int r = 0; r < R; r++) {
             const unsigned a = top_a - SLOT * (r + 1);
             const bool have = !MASKED || (int)(a - base_a) >= 0;
             K t; W w;
@@ -241,27 +246,27 @@ template <typename K, typename W, bool UQ, typename Derived> struct StackBase {
             const typename Derived::Acc f = static_cast<Derived *>(this)->term(t, w);
             part += MASKED ? (have ? f : typename Derived::Acc(0)) : f;
         }
-        top_a = MASKED ? base_a + max((int)(top_a - base_a) - SLOT * PAIR_R, 0) : top_a - SLOT * PAIR_R;
+        top_a = MASKED ? base_a + max((int)(top_a - base_a) - SLOT * R, 0) : top_a - SLOT * R;
         sum += (double)part;
     }
     /* Called by the whole warp after each group of at most `limit` pushes per lane. */
     __device__ __forceinline__ void service(int limit)
     {
         int mn = __reduce_min_sync(0xffffffffu, (int)(top_a - base_a));
-        while (mn >= SLOT * PAIR_R) { round<false>(); mn -= SLOT * PAIR_R; }
+        while (mn >= SLOT * R) { round<false>(); mn -= SLOT * R; }
         int mx = __reduce_max_sync(0xffffffffu, (int)(top_a - base_a));
-        while (mx > cap_b - SLOT * limit) { round<true>(); mx -= SLOT * PAIR_R; }
+        while (mx > cap_b - SLOT * limit) { round<true>(); mx -= SLOT * R; }
     }
     __device__ __forceinline__ void finish()
     {
         int mx = __reduce_max_sync(0xffffffffu, (int)(top_a - base_a));
-        while (mx > 0) { round<true>(); mx -= SLOT * PAIR_R; }
+        while (mx > 0) { round<true>(); mx -= SLOT * R; }
     }
 };
 
 /* Near stack: t in the kernel's precision, F from the degree-7 (FP32: cubic) table. */
 template <typename T, bool UQ, bool SIGNED = false>
-struct LaneStack : StackBase<T, T, UQ, LaneStack<T, UQ, SIGNED>> {
+struct LaneStack : StackBase<T, T, UQ, RoundSize<T, SIGNED>::R, LaneStack<T, UQ, SIGNED>> {
     typedef T Acc;
     const T *tab;
     int bias;
@@ -303,7 +308,7 @@ struct FarFmt {
 };
 __device__ __forceinline__ unsigned far_fixed(double t) { return (unsigned)__double2loint(t + 134217728.0 /* 2^27 */); }
 
-template <bool UQ, bool SIGNED> struct FarStack : StackBase<unsigned, float, UQ, FarStack<UQ, SIGNED>> {
+template <bool UQ, bool SIGNED> struct FarStack : StackBase<unsigned, float, UQ, RoundSize<double, SIGNED>::R, FarStack<UQ, SIGNED>> {
     typedef float Acc;
     const float4 *tab; /* [bin][REP] cubic in u = (fraction of the bin) - 1/2; this lane's copy pre-selected */
     /* the staged table starts at bin t0 << KB (t0 = where this kernel's far shell starts): the pointer is biased
@@ -378,7 +383,7 @@ template <int DIM, bool ORTHO, int M, bool UQ> struct ScanShape {
     static constexpr int GROUP = UQ && ORTHO && WHOLE && ALL <= 4 ? 8 / ALL : 1;
     /* image-list path: (t, qq) items have half the capacity, so half the images between two services */
     static constexpr int LIMIT = ORTHO ? (WHOLE ? ALL * GROUP : PLANE ? 12 : ROW) : (UQ ? IMG_STEP : IMG_STEP / 2);
-    static constexpr int MIN_CAP = LIMIT + PAIR_R;
+    static constexpr int min_cap(int round_items) { return LIMIT + round_items; }
     static constexpr int FAR_LIMIT = 20; /* PLANE, fast variant: all 20 candidates between two far services */
     /* small batches of small boxes (|m| <= 2 in 3D: 125 candidates per pair): the energy kernel can deal the ROW
      * z-images of a pair to ROW different lanes, so that few walkers still fill the GPU (RealArgs::zsplit) */
